@@ -1,0 +1,149 @@
+/* galario_b200.h — C ABI of the B200-native GALARIO hot path (arXiv:1709.06999).
+ *
+ * What the library computes (citations are lines of the paper text, PAPER.md):
+ *   model image (or radial profile swept into an inclined image)
+ *     -> centre shift + 2-D real-to-complex FFT + shift along v
+ *     -> rotation of the (u, v) points by PA                                (Eq. 11-12)
+ *     -> bilinear interpolation of the half-plane spectrum
+ *     -> phase ramp for (dRA, dDec)
+ *     -> weighted chi-square against observed visibilities                  (Eq. 10, 718)
+ * The executable definition followed is the paper's Appendix D listing;
+ * the readings taken where it is silent or garbled are listed in DESIGN.md (A1..A17).
+ *
+ * Conventions
+ *   - Every array pointer is a DEVICE pointer unless the function name ends in `_host_*`, in which case
+ *     every array pointer is a HOST pointer (pinned or pageable) and the call copies in, computes, copies
+ *     the result out and synchronises the stream before returning (the paper's own calling convention:
+ *     inputs start in host memory).
+ *   - The caller owns every buffer.  Inputs are const and never modified.  The plan owns its twiddle
+ *     tables, the half-plane spectrum workspace, the reduction scratch and (for `_host_` calls) its
+ *     device staging buffers.
+ *   - Device-pointer calls are asynchronous on `stream` (a cudaStream_t passed as void*, NULL = the
+ *     legacy default stream), never synchronise the host, and leave their results in device memory.
+ *   - A plan is bound to one device and is not safe for concurrent use from several streams/threads.
+ *   - Suffix _f64 / _f32 = storage and FFT precision of every array.  In _f32 the index and phase
+ *     arithmetic of the sampling stage is still carried in double (reading A14).
+ *   - Units: dxy, dRA, dDec, Rmin, dR, inc, PA in radians; u, v in wavelengths; images in Jy/pixel;
+ *     profiles in Jy/sr.  dRA > 0 moves the source East, dDec > 0 North, PA is
+ *     measured East of North.
+ *   - Image layout: row-major [nxy][nxy], row 0 = North, column 0 = East, origin at pixel
+ *     [nxy/2][nxy/2].  nxy must be a power of two in [8, 4096].
+ *   - Visibilities out: complex interleaved (re, im), 2*M reals.  Observations in:
+ *     separate re_obs[M], im_obs[M], w[M].
+ *   - (u, v) points whose interpolation cell leaves the half-plane grid are NOT clamped: the spectrum is
+ *     extended to the whole plane by its own periodicity and Hermitian symmetry (reading A6); the number
+ *     of such points in the last call is available from gal_last_oob_count().
+ *   - Return value: 0 = GAL_OK, negative = error (see below).  No exception crosses this boundary.
+ *     M == 0 is valid: chi2 = 0, nothing written to vis_out.
+ */
+#ifndef GALARIO_B200_H
+#define GALARIO_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GAL_OK 0
+#define GAL_ERR_INVALID_ARGUMENT (-1) /* null pointer, bad nxy, M < 0, nr < 2, dR <= 0, dxy <= 0, |inc| >= pi/2, C > plan batch, wrong precision */
+#define GAL_ERR_ALLOC (-2)            /* device or host allocation failed */
+#define GAL_ERR_CUDA (-3)             /* a CUDA call failed; see gal_last_cuda_error() */
+#define GAL_ERR_UNSUPPORTED (-4)      /* valid in the paper but not built here (nxy > 4096) */
+
+typedef struct gal_plan gal_plan;
+
+/* Create a plan for images of nxy x nxy pixels, up to `batch` images per call (1 for everything but
+ * the batched cube), precision_bits = 64 or 32, on CUDA device `device`.  Allocates the twiddle table
+ * and the workspace (batch * nxy * (nxy/2+1) complex numbers + reduction scratch). */
+int gal_plan_create(gal_plan** out, int nxy, int batch, int precision_bits, int device);
+int gal_plan_destroy(gal_plan* plan);
+/* Bytes of device memory the plan owns (workspace + tables + staging). */
+size_t gal_plan_workspace_bytes(const gal_plan* plan);
+/* Points of the most recent sample/chi2 call that fell outside the half-plane grid (synchronises the
+ * stream of that call).  Returns -1 on error. */
+int64_t gal_last_oob_count(gal_plan* plan);
+/* cudaError_t of the most recent failing CUDA call made through this plan (0 if none). */
+int gal_last_cuda_error(const gal_plan* plan);
+const char* gal_strerror(int code);
+/* Number of kernels the plan has launched since it was created (for launch accounting). */
+int64_t gal_plan_launch_count(const gal_plan* plan);
+
+/* ---- sweep: image_out[nxy][nxy] = dxy^2 * lerp(I, (r - Rmin)/dR),
+ *      r = sqrt((x/cos inc)^2 + y^2), 0 outside [Rmin, Rmin + (nr-1) dR]. ---- */
+int gal_sweep_f64(gal_plan* plan, const double* I, int nr, double Rmin, double dR, double dxy, double inc,
+                  double* image_out, void* stream);
+int gal_sweep_f32(gal_plan* plan, const float* I, int nr, double Rmin, double dR, double dxy, double inc,
+                  float* image_out, void* stream);
+
+/* ---- the transform alone: spectrum_out[nxy][nxy/2+1] complex interleaved =
+ *      fftshift(rfft2(fftshift(image)), axes=0), in the paper's layout (for tests and inspection;
+ *      the sampling calls use an internal u-major copy and never materialise this one). ---- */
+int gal_fft2_shifted_f64(gal_plan* plan, const double* image, double* spectrum_out, void* stream);
+int gal_fft2_shifted_f32(gal_plan* plan, const float* image, float* spectrum_out, void* stream);
+
+/* ---- sampleImage: vis_out[2M]. ---- */
+int gal_sample_image_f64(gal_plan* plan, const double* image, double dxy, const double* u, const double* v,
+                         int64_t M, double dRA, double dDec, double PA, double* vis_out, void* stream);
+int gal_sample_image_f32(gal_plan* plan, const float* image, double dxy, const float* u, const float* v,
+                         int64_t M, double dRA, double dDec, double PA, float* vis_out, void* stream);
+
+/* ---- chi2Image: chi2_out[1] (device, always double). ---- */
+int gal_chi2_image_f64(gal_plan* plan, const double* image, double dxy, const double* u, const double* v,
+                       const double* re_obs, const double* im_obs, const double* w, int64_t M, double dRA,
+                       double dDec, double PA, double* chi2_out, void* stream);
+int gal_chi2_image_f32(gal_plan* plan, const float* image, double dxy, const float* u, const float* v,
+                       const float* re_obs, const float* im_obs, const float* w, int64_t M, double dRA,
+                       double dDec, double PA, double* chi2_out, void* stream);
+
+/* ---- sampleProfile / chi2Profile: the image is swept from the profile
+ *      inside the first FFT pass and never written to memory; nxy comes from the plan. ---- */
+int gal_sample_profile_f64(gal_plan* plan, const double* I, int nr, double Rmin, double dR, double dxy,
+                           const double* u, const double* v, int64_t M, double dRA, double dDec, double PA,
+                           double inc, double* vis_out, void* stream);
+int gal_sample_profile_f32(gal_plan* plan, const float* I, int nr, double Rmin, double dR, double dxy,
+                           const float* u, const float* v, int64_t M, double dRA, double dDec, double PA,
+                           double inc, float* vis_out, void* stream);
+int gal_chi2_profile_f64(gal_plan* plan, const double* I, int nr, double Rmin, double dR, double dxy,
+                         const double* u, const double* v, const double* re_obs, const double* im_obs,
+                         const double* w, int64_t M, double dRA, double dDec, double PA, double inc,
+                         double* chi2_out, void* stream);
+int gal_chi2_profile_f32(gal_plan* plan, const float* I, int nr, double Rmin, double dR, double dxy,
+                         const float* u, const float* v, const float* re_obs, const float* im_obs,
+                         const float* w, int64_t M, double dRA, double dDec, double PA, double inc,
+                         double* chi2_out, void* stream);
+
+/* ---- batched spectral cube (not in the paper; motivated at PAPER.md:45; reading A17):
+ *      C <= plan batch independent chi2Image problems sharing (nxy, dxy, dRA, dDec, PA, M).
+ *      images [C][nxy][nxy]; u, v, re_obs, im_obs, w each [C][M]; chi2_per_channel[C] and
+ *      chi2_total[1] (device, double; the total is summed in channel order). ---- */
+int gal_chi2_image_batch_f64(gal_plan* plan, const double* images, int C, double dxy, const double* u,
+                             const double* v, const double* re_obs, const double* im_obs, const double* w,
+                             int64_t M, double dRA, double dDec, double PA, double* chi2_per_channel,
+                             double* chi2_total, void* stream);
+int gal_chi2_image_batch_f32(gal_plan* plan, const float* images, int C, double dxy, const float* u,
+                             const float* v, const float* re_obs, const float* im_obs, const float* w,
+                             int64_t M, double dRA, double dDec, double PA, double* chi2_per_channel,
+                             double* chi2_total, void* stream);
+
+/* ---- HOST-pointer entry points (the paper's calling convention): every array is in
+ *      host memory; the call stages it through plan-owned device buffers on `stream`, runs the same
+ *      kernels, copies the result back and synchronises `stream`.  chi2_out / vis_out are host. ---- */
+int gal_chi2_image_host_f64(gal_plan* plan, const double* image, double dxy, const double* u, const double* v,
+                            const double* re_obs, const double* im_obs, const double* w, int64_t M, double dRA,
+                            double dDec, double PA, double* chi2_out, void* stream);
+int gal_chi2_image_host_f32(gal_plan* plan, const float* image, double dxy, const float* u, const float* v,
+                            const float* re_obs, const float* im_obs, const float* w, int64_t M, double dRA,
+                            double dDec, double PA, double* chi2_out, void* stream);
+int gal_sample_image_host_f64(gal_plan* plan, const double* image, double dxy, const double* u, const double* v,
+                              int64_t M, double dRA, double dDec, double PA, double* vis_out, void* stream);
+int gal_chi2_profile_host_f64(gal_plan* plan, const double* I, int nr, double Rmin, double dR, double dxy,
+                              const double* u, const double* v, const double* re_obs, const double* im_obs,
+                              const double* w, int64_t M, double dRA, double dDec, double PA, double inc,
+                              double* chi2_out, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GALARIO_B200_H */

@@ -1,0 +1,249 @@
+"""ctypes binding of include/galario_b200.h (same names, argument marshalling only)."""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+from typing import Optional
+
+import numpy as np
+import torch
+
+_HERE = Path(__file__).resolve().parent
+_LIB_PATH = _HERE / "libgalario_b200.so"
+_lib: Optional[ctypes.CDLL] = None
+
+_vp, _i, _d, _i64 = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_int64
+
+
+class GalarioError(RuntimeError):
+    pass
+
+
+def library_path() -> Path:
+    return _LIB_PATH
+
+
+def load_library() -> ctypes.CDLL:
+    """Load the C-ABI library.  Fails loudly when it has not been built (no fallback exists)."""
+    global _lib
+    if _lib is None:
+        if not _LIB_PATH.exists():
+            raise GalarioError(f"{_LIB_PATH} is missing: run `python -m paper_1709_06999_b200.build` "
+                               "(or __graft_entry__.build()).  There is no CPU fallback.")
+        lib = ctypes.CDLL(str(_LIB_PATH))
+        lib.gal_strerror.restype = ctypes.c_char_p
+        lib.gal_plan_workspace_bytes.restype = ctypes.c_size_t
+        lib.gal_last_oob_count.restype = _i64
+        lib.gal_plan_launch_count.restype = _i64
+        lib.gal_plan_create.argtypes = [ctypes.POINTER(_vp), _i, _i, _i, _i]
+        for name in ("gal_plan_destroy", "gal_plan_workspace_bytes", "gal_last_oob_count", "gal_last_cuda_error",
+                     "gal_plan_launch_count"):
+            getattr(lib, name).argtypes = [_vp]
+        for s in ("f64", "f32"):
+            getattr(lib, f"gal_sweep_{s}").argtypes = [_vp, _vp, _i, _d, _d, _d, _d, _vp, _vp]
+            getattr(lib, f"gal_fft2_shifted_{s}").argtypes = [_vp, _vp, _vp, _vp]
+            getattr(lib, f"gal_sample_image_{s}").argtypes = [_vp, _vp, _d, _vp, _vp, _i64, _d, _d, _d, _vp, _vp]
+            getattr(lib, f"gal_chi2_image_{s}").argtypes = [_vp, _vp, _d, _vp, _vp, _vp, _vp, _vp, _i64, _d, _d, _d,
+                                                            _vp, _vp]
+            getattr(lib, f"gal_chi2_image_host_{s}").argtypes = [_vp, _vp, _d, _vp, _vp, _vp, _vp, _vp, _i64, _d, _d,
+                                                                 _d, _vp, _vp]
+            getattr(lib, f"gal_sample_profile_{s}").argtypes = [_vp, _vp, _i, _d, _d, _d, _vp, _vp, _i64, _d, _d, _d,
+                                                                _d, _vp, _vp]
+            getattr(lib, f"gal_chi2_profile_{s}").argtypes = [_vp, _vp, _i, _d, _d, _d, _vp, _vp, _vp, _vp, _vp, _i64,
+                                                              _d, _d, _d, _d, _vp, _vp]
+            getattr(lib, f"gal_chi2_image_batch_{s}").argtypes = [_vp, _vp, _i, _d, _vp, _vp, _vp, _vp, _vp, _i64, _d,
+                                                                  _d, _d, _vp, _vp, _vp]
+        lib.gal_sample_image_host_f64.argtypes = [_vp, _vp, _d, _vp, _vp, _i64, _d, _d, _d, _vp, _vp]
+        lib.gal_chi2_profile_host_f64.argtypes = [_vp, _vp, _i, _d, _d, _d, _vp, _vp, _vp, _vp, _vp, _i64, _d, _d, _d,
+                                                  _d, _vp, _vp]
+        _lib = lib
+    return _lib
+
+
+def _check(rc: int, what: str, plan: "Plan" = None) -> None:
+    if rc != 0:
+        msg = load_library().gal_strerror(rc).decode()
+        extra = f" (cudaError {load_library().gal_last_cuda_error(plan._h)})" if plan is not None and rc == -3 else ""
+        raise GalarioError(f"{what}: {msg}{extra}")
+
+
+def _stream() -> int:
+    return torch.cuda.current_stream().cuda_stream
+
+
+class Plan:
+    """gal_plan: owns the twiddle table, the half-plane spectrum workspace and the reduction scratch."""
+
+    def __init__(self, nxy: int, batch: int = 1, dtype: torch.dtype = torch.float64, device: int = 0):
+        if dtype not in (torch.float64, torch.float32):
+            raise GalarioError("dtype must be torch.float64 or torch.float32")
+        if not torch.cuda.is_available():
+            raise GalarioError("no CUDA device: the galario-b200 path has no CPU fallback")
+        self.nxy, self.batch, self.dtype, self.device = int(nxy), int(batch), dtype, int(device)
+        self._sfx = "f64" if dtype == torch.float64 else "f32"
+        self._cdtype = torch.complex128 if dtype == torch.float64 else torch.complex64
+        self._lib = load_library()
+        h = _vp()
+        _check(self._lib.gal_plan_create(ctypes.byref(h), self.nxy, self.batch, 64 if dtype == torch.float64 else 32,
+                                         self.device), "gal_plan_create")
+        self._h = h
+
+    def __del__(self):
+        h = getattr(self, "_h", None)
+        if h:
+            self._lib.gal_plan_destroy(h)
+            self._h = None
+
+    # -- helpers ---------------------------------------------------------------------------
+    def _fn(self, name):
+        return getattr(self._lib, f"gal_{name}_{self._sfx}")
+
+    def _dev(self, t: torch.Tensor, what: str) -> int:
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == self.dtype and t.is_contiguous()):
+            raise GalarioError(f"{what} must be a contiguous CUDA tensor of dtype {self.dtype}")
+        return t.data_ptr()
+
+    def workspace_bytes(self) -> int:
+        return int(self._lib.gal_plan_workspace_bytes(self._h))
+
+    def last_oob_count(self) -> int:
+        return int(self._lib.gal_last_oob_count(self._h))
+
+    def launch_count(self) -> int:
+        return int(self._lib.gal_plan_launch_count(self._h))
+
+    # -- the paper's calls ---------------------------------------------------------------------
+    def sweep(self, I, Rmin, dR, dxy, inc=0.0, out=None):
+        out = torch.empty((self.nxy, self.nxy), dtype=self.dtype, device=I.device) if out is None else out
+        _check(self._fn("sweep")(self._h, self._dev(I, "I"), I.numel(), Rmin, dR, dxy, inc, self._dev(out, "out"),
+                                 _stream()), "gal_sweep", self)
+        return out
+
+    def fft2_shifted(self, image, out=None):
+        if out is None:
+            out = torch.empty((self.nxy, self.nxy // 2 + 1), dtype=self._cdtype, device=image.device)
+        _check(self._fn("fft2_shifted")(self._h, self._dev(image, "image"), out.data_ptr(), _stream()),
+               "gal_fft2_shifted", self)
+        return out
+
+    def sampleImage(self, image, dxy, u, v, PA=0.0, dRA=0.0, dDec=0.0, out=None):
+        M = u.numel()
+        out = torch.empty(M, dtype=self._cdtype, device=u.device) if out is None else out
+        _check(self._fn("sample_image")(self._h, self._dev(image, "image"), dxy, self._dev(u, "u"), self._dev(v, "v"),
+                                        M, dRA, dDec, PA, out.data_ptr(), _stream()), "gal_sample_image", self)
+        return out
+
+    def chi2Image(self, image, dxy, u, v, re_obs, im_obs, w, dRA=0.0, dDec=0.0, PA=0.0, out=None):
+        out = torch.empty(1, dtype=torch.float64, device=u.device) if out is None else out
+        _check(self._fn("chi2_image")(self._h, self._dev(image, "image"), dxy, self._dev(u, "u"), self._dev(v, "v"),
+                                      self._dev(re_obs, "re_obs"), self._dev(im_obs, "im_obs"), self._dev(w, "w"),
+                                      u.numel(), dRA, dDec, PA, out.data_ptr(), _stream()), "gal_chi2_image", self)
+        return out
+
+    def sampleProfile(self, I, Rmin, dR, dxy, u, v, inc=0.0, PA=0.0, dRA=0.0, dDec=0.0, out=None):
+        M = u.numel()
+        out = torch.empty(M, dtype=self._cdtype, device=u.device) if out is None else out
+        _check(self._fn("sample_profile")(self._h, self._dev(I, "I"), I.numel(), Rmin, dR, dxy, self._dev(u, "u"),
+                                          self._dev(v, "v"), M, dRA, dDec, PA, inc, out.data_ptr(), _stream()),
+               "gal_sample_profile", self)
+        return out
+
+    def chi2Profile(self, I, Rmin, dR, dxy, u, v, re_obs, im_obs, w, dRA=0.0, dDec=0.0, PA=0.0, inc=0.0, out=None):
+        out = torch.empty(1, dtype=torch.float64, device=u.device) if out is None else out
+        _check(self._fn("chi2_profile")(self._h, self._dev(I, "I"), I.numel(), Rmin, dR, dxy, self._dev(u, "u"),
+                                        self._dev(v, "v"), self._dev(re_obs, "re_obs"), self._dev(im_obs, "im_obs"),
+                                        self._dev(w, "w"), u.numel(), dRA, dDec, PA, inc, out.data_ptr(), _stream()),
+               "gal_chi2_profile", self)
+        return out
+
+    def chi2ImageBatch(self, images, dxy, u, v, re_obs, im_obs, w, dRA=0.0, dDec=0.0, PA=0.0, out=None):
+        """images [C][n][n]; u, v, re_obs, im_obs, w [C][M].  Returns (chi2[C], total[1]) on the device."""
+        C, M = images.shape[0], u.shape[1]
+        if out is None:
+            out = torch.empty(C + 1, dtype=torch.float64, device=u.device)
+        _check(self._fn("chi2_image_batch")(self._h, self._dev(images, "images"), C, dxy, self._dev(u, "u"),
+                                            self._dev(v, "v"), self._dev(re_obs, "re_obs"), self._dev(im_obs, "im_obs"),
+                                            self._dev(w, "w"), M, dRA, dDec, PA, out.data_ptr(),
+                                            out.data_ptr() + 8 * C, _stream()), "gal_chi2_image_batch", self)
+        return out[:C], out[C:]
+
+    # -- host-pointer calls (numpy / CPU tensors in, Python float or numpy out) ------------------
+    def _host(self, a, what):
+        a = a.numpy() if isinstance(a, torch.Tensor) else a
+        want = np.float64 if self.dtype == torch.float64 else np.float32
+        if not (isinstance(a, np.ndarray) and a.dtype == want and a.flags.c_contiguous):
+            raise GalarioError(f"{what} must be a C-contiguous host array of dtype {want.__name__}")
+        return a.ctypes.data
+
+    def chi2Image_host(self, image, dxy, u, v, re_obs, im_obs, w, dRA=0.0, dDec=0.0, PA=0.0) -> float:
+        out = ctypes.c_double(0.0)
+        _check(self._fn("chi2_image_host")(self._h, self._host(image, "image"), dxy, self._host(u, "u"),
+                                           self._host(v, "v"), self._host(re_obs, "re_obs"),
+                                           self._host(im_obs, "im_obs"), self._host(w, "w"), u.size if isinstance(u, np.ndarray) else u.numel(),
+                                           dRA, dDec, PA, ctypes.addressof(out), _stream()), "gal_chi2_image_host", self)
+        return out.value
+
+    def sampleImage_host(self, image, dxy, u, v, PA=0.0, dRA=0.0, dDec=0.0) -> np.ndarray:
+        M = u.size if isinstance(u, np.ndarray) else u.numel()
+        out = np.empty(M, dtype=np.complex128)
+        _check(self._lib.gal_sample_image_host_f64(self._h, self._host(image, "image"), dxy, self._host(u, "u"),
+                                                   self._host(v, "v"), M, dRA, dDec, PA, out.ctypes.data, _stream()),
+               "gal_sample_image_host", self)
+        return out
+
+    def chi2Profile_host(self, I, Rmin, dR, dxy, u, v, re_obs, im_obs, w, dRA=0.0, dDec=0.0, PA=0.0, inc=0.0) -> float:
+        out = ctypes.c_double(0.0)
+        n = I.size if isinstance(I, np.ndarray) else I.numel()
+        M = u.size if isinstance(u, np.ndarray) else u.numel()
+        _check(self._lib.gal_chi2_profile_host_f64(self._h, self._host(I, "I"), n, Rmin, dR, dxy, self._host(u, "u"),
+                                                   self._host(v, "v"), self._host(re_obs, "re_obs"),
+                                                   self._host(im_obs, "im_obs"), self._host(w, "w"), M, dRA, dDec, PA,
+                                                   inc, ctypes.addressof(out), _stream()), "gal_chi2_profile_host", self)
+        return out.value
+
+
+# -- module-level calls in the paper's style, with a plan cache -------------------------------------
+_plans: dict = {}
+
+
+def get_plan(nxy: int, batch: int = 1, dtype: torch.dtype = torch.float64, device: Optional[int] = None) -> Plan:
+    device = torch.cuda.current_device() if device is None else device
+    key = (int(nxy), int(batch), dtype, int(device))
+    if key not in _plans:
+        _plans[key] = Plan(nxy, batch, dtype, device)
+    return _plans[key]
+
+
+def _plan_for(t: torch.Tensor, nxy: int, batch: int = 1) -> Plan:
+    if not (isinstance(t, torch.Tensor) and t.is_cuda):
+        raise GalarioError("inputs must be CUDA tensors (there is no CPU path)")
+    return get_plan(nxy, batch, t.dtype, t.device.index)
+
+
+def sampleImage(image, dxy, u, v, PA=0.0, dRA=0.0, dDec=0.0):
+    return _plan_for(image, image.shape[-1]).sampleImage(image, dxy, u, v, PA, dRA, dDec)
+
+
+def chi2Image(image, dxy, u, v, re_obs, im_obs, w, dRA=0.0, dDec=0.0, PA=0.0):
+    return _plan_for(image, image.shape[-1]).chi2Image(image, dxy, u, v, re_obs, im_obs, w, dRA, dDec, PA)
+
+
+def sampleProfile(I, Rmin, dR, nxy, dxy, u, v, inc=0.0, PA=0.0, dRA=0.0, dDec=0.0):
+    return _plan_for(I, nxy).sampleProfile(I, Rmin, dR, dxy, u, v, inc, PA, dRA, dDec)
+
+
+def chi2Profile(I, Rmin, dR, nxy, dxy, u, v, re_obs, im_obs, w, dRA=0.0, dDec=0.0, PA=0.0, inc=0.0):
+    return _plan_for(I, nxy).chi2Profile(I, Rmin, dR, dxy, u, v, re_obs, im_obs, w, dRA, dDec, PA, inc)
+
+
+def sweep(I, Rmin, dR, nxy, dxy, inc=0.0):
+    return _plan_for(I, nxy).sweep(I, Rmin, dR, dxy, inc)
+
+
+def chi2ImageBatch(images, dxy, u, v, re_obs, im_obs, w, dRA=0.0, dDec=0.0, PA=0.0):
+    return _plan_for(images, images.shape[-1], images.shape[0]).chi2ImageBatch(images, dxy, u, v, re_obs, im_obs, w,
+                                                                              dRA, dDec, PA)
+
+
+def fft2_shifted(image):
+    return _plan_for(image, image.shape[-1]).fft2_shifted(image)

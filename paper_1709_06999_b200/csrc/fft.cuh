@@ -1,0 +1,362 @@
+// fft.cuh — hand-written 2-D real-to-complex FFT for sm_100a (no cuFFT).
+//
+// Computes F = rfft2(fftshift(image)) followed by fftshift along axis 0,
+// stored u-major: spec[b][ku][kvs], ku = 0..N/2, kvs = (kv + N/2) mod N, complex<T>.
+//   * S2 (centre shift of the image) is never a pass: for even N it equals multiplying the
+//     spectrum by (-1)^(ku+kv), applied in the last store of the column pass.
+//   * S4 (shift along v) is an index fold in that same store.
+//   * Row pass: one real row of N samples is read as N/2 complex numbers z[n] = x[2n] + i x[2n+1],
+//     transformed with an (N/2)-point complex FFT in shared memory and untangled into the N/2+1
+//     half-spectrum values; F rows per CTA are written TRANSPOSED (F*16 B contiguous per ku) so the
+//     column pass reads and writes contiguous 16*N-byte columns.  L2 merges the partial lines.
+//   * Column pass: in place, one column per FFT, three radix passes through shared memory.
+//   * With SWEEP the row loader evaluates the swept profile instead of reading an
+//     image, so *Profile calls never materialise the image.
+//
+// The 1-D FFT of length L = R1*R2*R3 is a three-step Cooley-Tukey decomposition, all steps in
+// registers with radix-R butterflies, exchanging through a padded shared-memory cube:
+//   n = R2R3*n1 + R3*a + b,   k = k1 + R1*(c + R2*d)
+//   step 1: DFT_R1 over n1, twiddle W_L^(n2*k1)           (n2 = R3*a + b)
+//   step 2: DFT_R2 over a,  twiddle W_(R2R3)^(b*c)        (in place per work item)
+//   step 3: DFT_R3 over b                                 (in place, or straight to global memory)
+// Shared-memory address of element (k1, a|c, b|d): k1*P1 + (a|c)*R3 + (b|d), P1 = R2*R3 + 1 (odd),
+// which makes every access pattern of the three steps bank-conflict free for 8/16-byte elements.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace galb {
+
+template <typename T> struct Vec2;
+template <> struct Vec2<double> { using type = double2; };
+template <> struct Vec2<float> { using type = float2; };
+template <typename T> using cx = typename Vec2<T>::type;
+
+template <typename T> __device__ __forceinline__ cx<T> mk(T x, T y) { cx<T> r; r.x = x; r.y = y; return r; }
+template <typename V> __device__ __forceinline__ V cadd(V a, V b) { a.x += b.x; a.y += b.y; return a; }
+template <typename V> __device__ __forceinline__ V csub(V a, V b) { a.x -= b.x; a.y -= b.y; return a; }
+template <typename V> __device__ __forceinline__ V cmul(V a, V b) {
+    V r; r.x = a.x * b.x - a.y * b.y; r.y = a.x * b.y + a.y * b.x; return r;
+}
+template <typename V> __device__ __forceinline__ V mul_mi(V a) { V r; r.x = a.y; r.y = -a.x; return r; }  // * (-i)
+
+// ------------------------------------------------------------------------------------------
+// Radix-R DFTs on register arrays, forward kernel exp(-2 pi i nk/R), natural-order output.
+// ------------------------------------------------------------------------------------------
+template <typename T, int R> struct Dft;
+
+template <typename T> struct Dft<T, 1> { static __device__ __forceinline__ void run(cx<T>*) {} };
+
+template <typename T> struct Dft<T, 2> {
+    static __device__ __forceinline__ void run(cx<T>* a) {
+        cx<T> t = a[0];
+        a[0] = cadd(t, a[1]);
+        a[1] = csub(t, a[1]);
+    }
+};
+
+template <typename T> struct Dft<T, 4> {
+    static __device__ __forceinline__ void run(cx<T>* a) {
+        cx<T> s02 = cadd(a[0], a[2]), d02 = csub(a[0], a[2]);
+        cx<T> s13 = cadd(a[1], a[3]), d13 = mul_mi(csub(a[1], a[3]));
+        a[0] = cadd(s02, s13);
+        a[2] = csub(s02, s13);
+        a[1] = cadd(d02, d13);
+        a[3] = csub(d02, d13);
+    }
+};
+
+template <typename T> struct Dft<T, 8> {
+    static __device__ __forceinline__ void run(cx<T>* a) {
+        const T h = (T)0.70710678118654752440;
+        cx<T> e[4] = {a[0], a[2], a[4], a[6]};
+        cx<T> o[4] = {a[1], a[3], a[5], a[7]};
+        Dft<T, 4>::run(e);
+        Dft<T, 4>::run(o);
+        // o[k] *= exp(-2 pi i k / 8)
+        o[1] = mk<T>((o[1].x + o[1].y) * h, (o[1].y - o[1].x) * h);
+        o[2] = mul_mi(o[2]);
+        o[3] = mk<T>((o[3].y - o[3].x) * h, -(o[3].x + o[3].y) * h);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            a[k] = cadd(e[k], o[k]);
+            a[k + 4] = csub(e[k], o[k]);
+        }
+    }
+};
+
+template <typename T> struct Dft<T, 16> {
+    static __device__ __forceinline__ void run(cx<T>* a) {
+        const T h = (T)0.70710678118654752440;
+        const T c1 = (T)0.92387953251128675613;  // cos(pi/8)
+        const T s1 = (T)0.38268343236508977173;  // sin(pi/8)
+        cx<T> e[8], o[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) { e[k] = a[2 * k]; o[k] = a[2 * k + 1]; }
+        Dft<T, 8>::run(e);
+        Dft<T, 8>::run(o);
+        // o[k] *= exp(-2 pi i k / 16) = (cos(pi k/8), -sin(pi k/8))
+        o[1] = cmul(o[1], mk<T>(c1, -s1));
+        o[2] = mk<T>((o[2].x + o[2].y) * h, (o[2].y - o[2].x) * h);
+        o[3] = cmul(o[3], mk<T>(s1, -c1));
+        o[4] = mul_mi(o[4]);
+        o[5] = cmul(o[5], mk<T>(-s1, -c1));
+        o[6] = mk<T>((o[6].y - o[6].x) * h, -(o[6].x + o[6].y) * h);
+        o[7] = cmul(o[7], mk<T>(-c1, -s1));
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            a[k] = cadd(e[k], o[k]);
+            a[k + 8] = csub(e[k], o[k]);
+        }
+    }
+};
+
+// ------------------------------------------------------------------------------------------
+// Geometry of one L-point FFT in shared memory.
+// ------------------------------------------------------------------------------------------
+constexpr int cmax(int a, int b) { return a > b ? a : b; }
+
+template <typename T, int R1, int R2, int R3, int F> struct Geom {
+    static constexpr int L = R1 * R2 * R3;
+    static constexpr int RMAX = cmax(R1, cmax(R2, R3));
+    static constexpr int TPF = L / RMAX;                                // threads per FFT
+    static constexpr int NT = TPF * F;                                  // threads per CTA
+    static constexpr int P1 = (R2 * R3 > 1) ? R2 * R3 + 1 : 1;          // k1 stride (odd)
+    static constexpr int BG = 128 / (int)sizeof(cx<T>);                 // elements per 128 B of banks
+    static constexpr int SKEW = (F >= BG) ? 1 : BG / F;                 // region stride mod BG
+    static constexpr int BASE = R1 * P1;
+    static constexpr int REGION = BASE + ((SKEW - BASE % BG) % BG + BG) % BG;
+    static constexpr size_t SMEM = (size_t)REGION * F * sizeof(cx<T>);
+    static __device__ __forceinline__ int zaddr(int k) {                // where X[k] sits after step 3
+        return (k % R1) * P1 + ((k / R1) % R2) * R3 + k / (R1 * R2);
+    }
+};
+
+// Steps 1 and 2.  S = this FFT's shared-memory region, t = thread index inside the FFT,
+// tw[m * tws] = exp(-2 pi i m / L), load(n) returns input element n.  Ends with a barrier.
+template <typename T, int R1, int R2, int R3, int TPF, typename LoadFn>
+__device__ __forceinline__ void fft_steps12(cx<T>* S, int t, const cx<T>* __restrict__ tw, int tws, LoadFn load) {
+    constexpr int L = R1 * R2 * R3;
+    constexpr int P1 = (R2 * R3 > 1) ? R2 * R3 + 1 : 1;
+    constexpr int N2 = R2 * R3;
+    for (int n2 = t; n2 < N2; n2 += TPF) {
+        cx<T> a[R1];
+#pragma unroll
+        for (int n1 = 0; n1 < R1; ++n1) a[n1] = load(N2 * n1 + n2);
+        Dft<T, R1>::run(a);
+        S[n2] = a[0];
+#pragma unroll
+        for (int k1 = 1; k1 < R1; ++k1) {
+            if (N2 > 1) a[k1] = cmul(a[k1], tw[(n2 * k1) * tws]);
+            S[k1 * P1 + n2] = a[k1];
+        }
+    }
+    __syncthreads();
+    if (R2 > 1) {
+        for (int it = t; it < R1 * R3; it += TPF) {
+            const int b = it % R3, k1 = it / R3;
+            cx<T>* base = S + k1 * P1 + b;
+            cx<T> a[R2];
+#pragma unroll
+            for (int i = 0; i < R2; ++i) a[i] = base[i * R3];
+            Dft<T, R2>::run(a);
+            base[0] = a[0];
+#pragma unroll
+            for (int c = 1; c < R2; ++c) {
+                if (R3 > 1) a[c] = cmul(a[c], tw[(b * c) * (R1 * tws)]);
+                base[c * R3] = a[c];
+            }
+        }
+        __syncthreads();
+    }
+    (void)L;
+}
+
+// ------------------------------------------------------------------------------------------
+// Sweep: pixel value of the swept profile, every operation in the order of the
+// listing and individually rounded (no FMA contraction) so that the hard-edge decisions
+// r < Rmin, r > Rmax agree with a plain IEEE evaluation.
+// ------------------------------------------------------------------------------------------
+struct SweepParams {
+    const void* I;      // profile, T[nr]
+    int nr;
+    double Rmin, dR, Rmax, dxy, inc_cos;
+};
+
+template <typename T>
+__device__ __forceinline__ double sweep_pixel(const SweepParams& sp, int N, int i, int j) {
+    const double fN = (double)N;
+    const double y = __dmul_rn(__dmul_rn(__dsub_rn(0.5, __ddiv_rn((double)i, fN)), sp.dxy), fN);
+    const double x = __dmul_rn(__dmul_rn(__dsub_rn(0.5, __ddiv_rn((double)j, fN)), sp.dxy), fN);
+    const double xs = __ddiv_rn(x, sp.inc_cos);
+    const double r = __dsqrt_rn(__dadd_rn(__dmul_rn(xs, xs), __dmul_rn(y, y)));
+    if (!(r >= sp.Rmin && r <= sp.Rmax)) return 0.0;
+    const double pos = __ddiv_rn(__dsub_rn(r, sp.Rmin), sp.dR);
+    long long k = (long long)floor(pos);
+    if (k >= sp.nr - 1) k = sp.nr - 2;
+    if (k < 0) k = 0;
+    const double t = __dsub_rn(pos, (double)k);
+    const T* I = (const T*)sp.I;
+    const double i0 = (double)__ldg(I + k), i1 = (double)__ldg(I + k + 1);
+    const double val = __dadd_rn(i0, __dmul_rn(t, __dsub_rn(i1, i0)));
+    return __dmul_rn(__dmul_rn(val, sp.dxy), sp.dxy);
+}
+
+// ------------------------------------------------------------------------------------------
+// Row pass.
+// ------------------------------------------------------------------------------------------
+template <typename T> struct RowParams {
+    const T* image;        // [rows_total][N] (unused with SWEEP)
+    cx<T>* spec;           // [batch][N/2+1][N]
+    const cx<T>* tw;       // exp(-2 pi i m / N), m = 0..N-1
+    int N;
+    int rows_total;        // batch * N
+    SweepParams sweep;
+};
+
+template <typename T, int R1, int R2, int R3, int F, bool SWEEP>
+__global__ void __launch_bounds__(Geom<T, R1, R2, R3, F>::NT)
+row_pass_kernel(const RowParams<T> p) {
+    using G = Geom<T, R1, R2, R3, F>;
+    constexpr int L = G::L;                    // = N / 2
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cx<T>* smem = reinterpret_cast<cx<T>*>(smem_raw);
+    const int tid = threadIdx.x;
+    const int f = tid / G::TPF, t = tid % G::TPF;
+    const int N = p.N;
+    const long long row0 = (long long)blockIdx.x * F;
+    const long long row = row0 + f;
+    const bool valid = row < p.rows_total;
+    cx<T>* S = smem + f * G::REGION;
+
+    if (SWEEP) {
+        const int i = (int)(row % N);
+        fft_steps12<T, R1, R2, R3, G::TPF>(S, t, p.tw, 2, [&](int n) -> cx<T> {
+            if (!valid) return mk<T>(0, 0);
+            return mk<T>((T)sweep_pixel<T>(p.sweep, N, i, 2 * n), (T)sweep_pixel<T>(p.sweep, N, i, 2 * n + 1));
+        });
+    } else {
+        const cx<T>* z = reinterpret_cast<const cx<T>*>(p.image + (valid ? row : 0) * (long long)N);
+        fft_steps12<T, R1, R2, R3, G::TPF>(S, t, p.tw, 2, [&](int n) -> cx<T> {
+            return valid ? __ldcs(z + n) : mk<T>(0, 0);
+        });
+    }
+    // step 3, in place: X[k1 + R1*(c + R2*d)] -> S[k1*P1 + c*R3 + d]
+    if (R3 > 1) {
+        for (int it = t; it < R1 * R2; it += G::TPF) {
+            const int k1 = it % R1, c = it / R1;
+            cx<T>* base = S + k1 * G::P1 + c * R3;
+            cx<T> a[R3];
+#pragma unroll
+            for (int b = 0; b < R3; ++b) a[b] = base[b];
+            Dft<T, R3>::run(a);
+#pragma unroll
+            for (int d = 0; d < R3; ++d) base[d] = a[d];
+        }
+        __syncthreads();
+    }
+    // Untangle the packed real FFT and write F rows transposed.
+    //   E = (Z[k] + conj Z[L-k]) / 2,  O = -i (Z[k] - conj Z[L-k]) / 2,  W = exp(-2 pi i k / N)
+    //   X[k] = E + W O,   X[L-k] = conj(E - W O)     (k = 0 gives X[0] and X[L])
+    const int NU = N / 2 + 1;
+    const long long b_img = row0 / N;
+    const int i0 = (int)(row0 % N);
+    cx<T>* out = p.spec + b_img * (long long)NU * N + i0;
+    const int rows_here = (int)((p.rows_total - row0) < F ? (p.rows_total - row0) : F);
+    for (int idx = tid; idx < F * (L / 2 + 1); idx += G::NT) {
+        const int ff = idx % F, k = idx / F;
+        if (ff >= rows_here) continue;
+        const cx<T>* Sf = smem + ff * G::REGION;
+        const cx<T> zk = Sf[G::zaddr(k)];
+        const cx<T> zm = Sf[G::zaddr((L - k) % L)];
+        const cx<T> E = mk<T>((T)0.5 * (zk.x + zm.x), (T)0.5 * (zk.y - zm.y));
+        const cx<T> O = mk<T>((T)0.5 * (zk.y + zm.y), (T)-0.5 * (zk.x - zm.x));
+        const cx<T> WO = cmul(__ldg(p.tw + k), O);
+        const cx<T> xk = cadd(E, WO);
+        cx<T> xm = csub(E, WO);
+        xm.y = -xm.y;
+        out[(long long)k * N + ff] = xk;
+        out[(long long)(L - k) * N + ff] = xm;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// Column pass (in place).
+// ------------------------------------------------------------------------------------------
+template <typename T> struct ColParams {
+    cx<T>* spec;           // [batch][N/2+1][N]
+    const cx<T>* tw;
+    int N;
+    long long cols_total;  // batch * (N/2+1)
+};
+
+template <typename T, int R1, int R2, int R3, int F>
+__global__ void __launch_bounds__(Geom<T, R1, R2, R3, F>::NT)
+col_pass_kernel(const ColParams<T> p) {
+    using G = Geom<T, R1, R2, R3, F>;
+    constexpr int L = G::L;                    // = N
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cx<T>* smem = reinterpret_cast<cx<T>*>(smem_raw);
+    const int tid = threadIdx.x;
+    const int f = tid / G::TPF, t = tid % G::TPF;
+    const long long g = (long long)blockIdx.x * F + f;
+    const bool valid = g < p.cols_total;
+    const int NU = L / 2 + 1;
+    const int ku = (int)(g % NU);
+    cx<T>* col = p.spec + (valid ? g : 0) * (long long)L;
+    cx<T>* S = smem + f * G::REGION;
+
+    fft_steps12<T, R1, R2, R3, G::TPF>(S, t, p.tw, 1, [&](int n) -> cx<T> {
+        return valid ? col[n] : mk<T>(0, 0);
+    });
+    // step 3 straight to global memory: kv = k1 + R1*(c + R2*d); sign (-1)^(ku+kv) folds the image
+    // centre shift, row (kv + N/2) mod N folds the shift along v.
+    for (int it = t; it < R1 * R2; it += G::TPF) {
+        const int k1 = it % R1, c = it / R1;
+        const cx<T>* base = S + k1 * G::P1 + c * R3;
+        cx<T> a[R3];
+#pragma unroll
+        for (int b = 0; b < R3; ++b) a[b] = base[b];
+        Dft<T, R3>::run(a);
+        if (valid) {
+#pragma unroll
+            for (int d = 0; d < R3; ++d) {
+                const int kv = k1 + R1 * (c + R2 * d);
+                const T sgn = ((ku + kv) & 1) ? (T)-1 : (T)1;
+                col[(kv + L / 2) & (L - 1)] = mk<T>(sgn * a[d].x, sgn * a[d].y);
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// Standalone sweep (image written to memory) and the u-major -> paper-layout transpose.
+// ------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void sweep_kernel(SweepParams sp, int N, T* __restrict__ image) {
+    const long long total = (long long)N * N;
+    for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
+         idx += (long long)gridDim.x * blockDim.x) {
+        const int i = (int)(idx / N), j = (int)(idx % N);
+        image[idx] = (T)sweep_pixel<T>(sp, N, i, j);
+    }
+}
+
+// out[kvs][ku] = spec[ku][kvs]   (paper layout [N][N/2+1])
+template <typename T>
+__global__ void transpose_to_paper_layout_kernel(const cx<T>* __restrict__ spec, cx<T>* __restrict__ out, int N) {
+    __shared__ cx<T> tile[32][33];
+    const int NU = N / 2 + 1;
+    const int kv0 = blockIdx.x * 32, ku0 = blockIdx.y * 32;
+    for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+        const int ku = ku0 + r, kv = kv0 + threadIdx.x;
+        if (ku < NU && kv < N) tile[r][threadIdx.x] = spec[(long long)ku * N + kv];
+    }
+    __syncthreads();
+    for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+        const int kv = kv0 + r, ku = ku0 + threadIdx.x;
+        if (ku < NU && kv < N) out[(long long)kv * NU + ku] = tile[threadIdx.x][r];
+    }
+}
+
+}  // namespace galb

@@ -1,0 +1,458 @@
+// galario_b200.cu — plan object, kernel dispatch and the C ABI declared in include/galario_b200.h.
+// Everything on the path runs in the kernels of fft.cuh and sample.cuh; this file only validates
+// arguments, picks the launch geometry and launches on the caller's stream.
+#include "../../include/galario_b200.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "fft.cuh"
+#include "sample.cuh"
+
+using namespace galb;
+
+struct gal_plan {
+    int nxy = 0, batch = 0, bits = 0, device = 0;
+    int sm_count = 148;
+    void* spec = nullptr;            // cx<T>[batch][nxy/2+1][nxy]
+    void* tw = nullptr;              // cx<T>[nxy]
+    double* partials = nullptr;      // [batch][max_gx]
+    unsigned int* tickets = nullptr; // [batch + 1]
+    double* chi2_scratch = nullptr;  // [batch]
+    unsigned long long* oob = nullptr;
+    int max_gx = 0;
+    size_t owned_bytes = 0;
+    int last_cuda = 0;
+    int64_t launches = 0;
+    cudaStream_t last_stream = nullptr;
+    // staging for the _host_ entry points (grown on demand)
+    void* st_image = nullptr; size_t st_image_bytes = 0;
+    void* st_pts = nullptr;   size_t st_pts_bytes = 0;
+    void* st_out = nullptr;   size_t st_out_bytes = 0;
+    double* st_chi2 = nullptr;
+};
+
+namespace {
+
+inline bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+
+#define GAL_CUDA(plan, call)                                   \
+    do {                                                       \
+        cudaError_t e__ = (call);                              \
+        if (e__ != cudaSuccess) {                              \
+            (plan)->last_cuda = (int)e__;                      \
+            return e__ == cudaErrorMemoryAllocation ? GAL_ERR_ALLOC : GAL_ERR_CUDA; \
+        }                                                      \
+    } while (0)
+
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(int dev) { cudaGetDevice(&prev); if (prev != dev) cudaSetDevice(dev); else prev = -1; }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+template <typename K> int set_smem(gal_plan* p, K kernel, size_t bytes) {
+    if (bytes > 48 * 1024) GAL_CUDA(p, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    return GAL_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// FFT launchers
+// ---------------------------------------------------------------------------------------------
+template <typename T, int R1, int R2, int R3, int F>
+int launch_row(gal_plan* p, const T* image, const SweepParams* sw, int batch, cudaStream_t st) {
+    using G = Geom<T, R1, R2, R3, F>;
+    RowParams<T> rp;
+    rp.image = image;
+    rp.spec = (cx<T>*)p->spec;
+    rp.tw = (const cx<T>*)p->tw;
+    rp.N = p->nxy;
+    rp.rows_total = batch * p->nxy;
+    if (sw) rp.sweep = *sw; else memset(&rp.sweep, 0, sizeof(rp.sweep));
+    const unsigned grid = (unsigned)((rp.rows_total + F - 1) / F);
+    if (sw) {
+        auto k = row_pass_kernel<T, R1, R2, R3, F, true>;
+        int rc = set_smem(p, k, G::SMEM); if (rc) return rc;
+        k<<<grid, G::NT, G::SMEM, st>>>(rp);
+    } else {
+        auto k = row_pass_kernel<T, R1, R2, R3, F, false>;
+        int rc = set_smem(p, k, G::SMEM); if (rc) return rc;
+        k<<<grid, G::NT, G::SMEM, st>>>(rp);
+    }
+    p->launches++;
+    GAL_CUDA(p, cudaGetLastError());
+    return GAL_OK;
+}
+
+template <typename T, int R1, int R2, int R3, int F>
+int launch_col(gal_plan* p, int batch, cudaStream_t st) {
+    using G = Geom<T, R1, R2, R3, F>;
+    ColParams<T> cp;
+    cp.spec = (cx<T>*)p->spec;
+    cp.tw = (const cx<T>*)p->tw;
+    cp.N = p->nxy;
+    cp.cols_total = (long long)batch * (p->nxy / 2 + 1);
+    const unsigned grid = (unsigned)((cp.cols_total + F - 1) / F);
+    auto k = col_pass_kernel<T, R1, R2, R3, F>;
+    int rc = set_smem(p, k, G::SMEM); if (rc) return rc;
+    k<<<grid, G::NT, G::SMEM, st>>>(cp);
+    p->launches++;
+    GAL_CUDA(p, cudaGetLastError());
+    return GAL_OK;
+}
+
+// Radix plans.  Row FFT length is nxy/2, column FFT length is nxy.
+template <typename T>
+int fft2(gal_plan* p, const T* image, const SweepParams* sw, int batch, cudaStream_t st) {
+    int rc;
+    switch (p->nxy) {
+#define GAL_FFT_CASE(NXY, ROW, COL)                                         \
+    case NXY:                                                               \
+        rc = launch_row<T, ROW>(p, image, sw, batch, st); if (rc) return rc; \
+        return launch_col<T, COL>(p, batch, st);
+#define RR(...) __VA_ARGS__
+        GAL_FFT_CASE(8, RR(4, 1, 1, 8), RR(8, 1, 1, 8))
+        GAL_FFT_CASE(16, RR(8, 1, 1, 16), RR(16, 1, 1, 16))
+        GAL_FFT_CASE(32, RR(16, 1, 1, 16), RR(8, 4, 1, 16))
+        GAL_FFT_CASE(64, RR(8, 4, 1, 16), RR(8, 8, 1, 16))
+        GAL_FFT_CASE(128, RR(8, 8, 1, 16), RR(16, 8, 1, 16))
+        GAL_FFT_CASE(256, RR(16, 8, 1, 16), RR(16, 16, 1, 8))
+        GAL_FFT_CASE(512, RR(16, 16, 1, 8), RR(8, 8, 8, 4))
+        GAL_FFT_CASE(1024, RR(8, 8, 8, 4), RR(16, 8, 8, 4))
+        GAL_FFT_CASE(2048, RR(16, 8, 8, 4), RR(16, 16, 8, 2))
+        GAL_FFT_CASE(4096, RR(16, 16, 8, 2), RR(16, 16, 16, 1))
+#undef RR
+#undef GAL_FFT_CASE
+        default:
+            return GAL_ERR_UNSUPPORTED;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// sampling launcher
+// ---------------------------------------------------------------------------------------------
+template <typename T>
+int launch_sample(gal_plan* p, int C, double dxy, const T* u, const T* v, const T* re, const T* im, const T* w,
+                  int64_t M, double dRA, double dDec, double PA, T* vis, double* chi2_pc, double* chi2_tot,
+                  cudaStream_t st) {
+    const bool do_chi2 = (vis == nullptr);
+    GAL_CUDA(p, cudaMemsetAsync(p->oob, 0, sizeof(unsigned long long), st));
+    if (M == 0) {
+        if (chi2_pc) GAL_CUDA(p, cudaMemsetAsync(chi2_pc, 0, sizeof(double) * C, st));
+        if (chi2_tot) GAL_CUDA(p, cudaMemsetAsync(chi2_tot, 0, sizeof(double), st));
+        return GAL_OK;
+    }
+    SampleParams<T> sp;
+    sp.spec = (const cx<T>*)p->spec;
+    sp.N = p->nxy;
+    sp.M = M;
+    sp.u = u; sp.v = v; sp.re_obs = re; sp.im_obs = im; sp.w = w; sp.vis = vis;
+    // host-side scalars, plain double arithmetic in the listing's order
+    const double two_pi = 2.0 * 3.14159265358979323846;
+    const double dRA2 = dRA * 2.0 * 3.14159265358979323846;
+    const double dDec2 = dDec * 2.0 * 3.14159265358979323846;
+    (void)two_pi;
+    sp.du = 1.0 / ((double)p->nxy * dxy);
+    sp.rdu = 1.0 / sp.du;
+    {   // Markstein's shortcut needs a divisor whose significand is not all ones
+        uint64_t bits; memcpy(&bits, &sp.du, 8);
+        sp.du_exact_div = ((bits & 0xFFFFFFFFFFFFFull) == 0xFFFFFFFFFFFFFull) || !std::isnormal(sp.du) || !std::isnormal(sp.rdu);
+    }
+    sp.cos_PA = std::cos(PA);
+    sp.sin_PA = std::sin(PA);
+    sp.dRArot = dRA2 * sp.cos_PA - dDec2 * sp.sin_PA;
+    sp.dDecrot = dRA2 * sp.sin_PA + dDec2 * sp.cos_PA;
+    sp.has_phase = !(sp.dRArot == 0.0 && sp.dDecrot == 0.0);
+    sp.partials = p->partials;
+    sp.tickets = p->tickets;
+    sp.chi2_per_channel = chi2_pc;
+    sp.chi2_total = chi2_tot;
+    sp.oob = p->oob;
+    long long need = (M + 255) / 256;
+    long long cap = p->max_gx;
+    if (C > 1) { cap = (2LL * p->max_gx + C - 1) / C; if (cap > p->max_gx) cap = p->max_gx; }
+    long long gx = need < cap ? need : cap;
+    if (gx < 1) gx = 1;
+    dim3 grid((unsigned)gx, (unsigned)C);
+    if (do_chi2) sample_kernel<T, false, true><<<grid, 256, 0, st>>>(sp);
+    else sample_kernel<T, true, false><<<grid, 256, 0, st>>>(sp);
+    p->launches++;
+    GAL_CUDA(p, cudaGetLastError());
+    return GAL_OK;
+}
+
+template <typename T> bool prec_ok(const gal_plan* p) { return p && p->bits == (int)(8 * sizeof(T)); }
+
+bool sweep_args(const gal_plan* p, const void* I, int nr, double Rmin, double dR, double dxy, double inc,
+                SweepParams* sw) {
+    if (!I || nr < 2 || !(dR > 0) || !(dxy > 0) || !std::isfinite(Rmin) || !std::isfinite(inc)) return false;
+    const double c = std::cos(inc);
+    if (!(std::fabs(inc) < 1.5707963267948966) || !(c > 0)) return false;
+    sw->I = I; sw->nr = nr; sw->Rmin = Rmin; sw->dR = dR; sw->dxy = dxy; sw->inc_cos = c;
+    sw->Rmax = Rmin + dR * (double)(nr - 1);
+    (void)p;
+    return true;
+}
+
+template <typename T>
+int do_sample_image(gal_plan* p, const T* image, const SweepParams* sw, int C, double dxy, const T* u, const T* v,
+                    const T* re, const T* im, const T* w, int64_t M, double dRA, double dDec, double PA, T* vis,
+                    double* chi2_pc, double* chi2_tot, void* stream) {
+    if (!prec_ok<T>(p) || (!image && !sw) || !(dxy > 0) || M < 0 || C < 1 || C > p->batch) return GAL_ERR_INVALID_ARGUMENT;
+    if (M > 0 && (!u || !v)) return GAL_ERR_INVALID_ARGUMENT;
+    const bool chi2 = (vis == nullptr);
+    if (chi2 && (!chi2_pc && !chi2_tot)) return GAL_ERR_INVALID_ARGUMENT;
+    if (chi2 && M > 0 && (!re || !im || !w)) return GAL_ERR_INVALID_ARGUMENT;
+    if (!std::isfinite(dRA) || !std::isfinite(dDec) || !std::isfinite(PA)) return GAL_ERR_INVALID_ARGUMENT;
+    DeviceGuard g(p->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    p->last_stream = st;
+    int rc = fft2<T>(p, image, sw, C, st);
+    if (rc) return rc;
+    return launch_sample<T>(p, C, dxy, u, v, re, im, w, M, dRA, dDec, PA, vis, chi2_pc, chi2_tot, st);
+}
+
+template <typename T>
+int do_sweep(gal_plan* p, const T* I, int nr, double Rmin, double dR, double dxy, double inc, T* out, void* stream) {
+    SweepParams sw;
+    if (!prec_ok<T>(p) || !out || !sweep_args(p, I, nr, Rmin, dR, dxy, inc, &sw)) return GAL_ERR_INVALID_ARGUMENT;
+    DeviceGuard g(p->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    p->last_stream = st;
+    const long long total = (long long)p->nxy * p->nxy;
+    long long blocks = (total + 255) / 256;
+    if (blocks > p->sm_count * 16) blocks = p->sm_count * 16;
+    sweep_kernel<T><<<(unsigned)blocks, 256, 0, st>>>(sw, p->nxy, out);
+    p->launches++;
+    GAL_CUDA(p, cudaGetLastError());
+    return GAL_OK;
+}
+
+template <typename T>
+int do_fft2_shifted(gal_plan* p, const T* image, T* out, void* stream) {
+    if (!prec_ok<T>(p) || !image || !out) return GAL_ERR_INVALID_ARGUMENT;
+    DeviceGuard g(p->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    p->last_stream = st;
+    int rc = fft2<T>(p, image, nullptr, 1, st);
+    if (rc) return rc;
+    dim3 grid((p->nxy + 31) / 32, (p->nxy / 2 + 1 + 31) / 32), block(32, 8);
+    transpose_to_paper_layout_kernel<T><<<grid, block, 0, st>>>((const cx<T>*)p->spec, (cx<T>*)out, p->nxy);
+    p->launches++;
+    GAL_CUDA(p, cudaGetLastError());
+    return GAL_OK;
+}
+
+int grow(gal_plan* p, void** buf, size_t* have, size_t want) {
+    if (*have >= want) return GAL_OK;
+    if (*buf) { cudaFree(*buf); p->owned_bytes -= *have; *buf = nullptr; *have = 0; }
+    GAL_CUDA(p, cudaMalloc(buf, want));
+    *have = want;
+    p->owned_bytes += want;
+    return GAL_OK;
+}
+
+// Host-pointer variant: stage everything through plan-owned device buffers on `stream`.
+template <typename T>
+int do_host_call(gal_plan* p, const T* image, const T* I, int nr, double Rmin, double dR, double inc, double dxy,
+                 const T* u, const T* v, const T* re, const T* im, const T* w, int64_t M, double dRA, double dDec,
+                 double PA, T* vis_out, double* chi2_out, void* stream) {
+    if (!prec_ok<T>(p) || M < 0 || (!image && !I)) return GAL_ERR_INVALID_ARGUMENT;
+    if (!vis_out && !chi2_out) return GAL_ERR_INVALID_ARGUMENT;
+    if (M > 0 && (!u || !v || (chi2_out && (!re || !im || !w)))) return GAL_ERR_INVALID_ARGUMENT;
+    DeviceGuard g(p->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t n2 = (size_t)p->nxy * p->nxy;
+    const size_t img_bytes = image ? n2 * sizeof(T) : (size_t)nr * sizeof(T);
+    const int narr = chi2_out ? 5 : 2;
+    int rc;
+    if ((rc = grow(p, &p->st_image, &p->st_image_bytes, img_bytes))) return rc;
+    if ((rc = grow(p, &p->st_pts, &p->st_pts_bytes, (size_t)narr * (size_t)(M > 0 ? M : 1) * sizeof(T)))) return rc;
+    if (vis_out && (rc = grow(p, &p->st_out, &p->st_out_bytes, (size_t)2 * (size_t)(M > 0 ? M : 1) * sizeof(T)))) return rc;
+    GAL_CUDA(p, cudaMemcpyAsync(p->st_image, image ? (const void*)image : (const void*)I, img_bytes, cudaMemcpyHostToDevice, st));
+    T* d = (T*)p->st_pts;
+    const T* src[5] = {u, v, re, im, w};
+    for (int a = 0; a < narr && M > 0; ++a)
+        GAL_CUDA(p, cudaMemcpyAsync(d + (size_t)a * M, src[a], (size_t)M * sizeof(T), cudaMemcpyHostToDevice, st));
+    SweepParams sw;
+    const SweepParams* swp = nullptr;
+    if (!image) {
+        if (!sweep_args(p, p->st_image, nr, Rmin, dR, dxy, inc, &sw)) return GAL_ERR_INVALID_ARGUMENT;
+        swp = &sw;
+    }
+    rc = do_sample_image<T>(p, image ? (const T*)p->st_image : nullptr, swp, 1, dxy, d, d + M, d + 2 * M, d + 3 * M,
+                            d + 4 * M, M, dRA, dDec, PA, vis_out ? (T*)p->st_out : nullptr,
+                            chi2_out ? p->st_chi2 : nullptr, nullptr, stream);
+    if (rc) return rc;
+    if (vis_out && M > 0)
+        GAL_CUDA(p, cudaMemcpyAsync(vis_out, p->st_out, (size_t)2 * M * sizeof(T), cudaMemcpyDeviceToHost, st));
+    if (chi2_out) GAL_CUDA(p, cudaMemcpyAsync(chi2_out, p->st_chi2, sizeof(double), cudaMemcpyDeviceToHost, st));
+    GAL_CUDA(p, cudaStreamSynchronize(st));
+    return GAL_OK;
+}
+
+}  // namespace
+
+// =============================================================================================
+// C ABI
+// =============================================================================================
+extern "C" {
+
+const char* gal_strerror(int code) {
+    switch (code) {
+        case GAL_OK: return "ok";
+        case GAL_ERR_INVALID_ARGUMENT: return "invalid argument";
+        case GAL_ERR_ALLOC: return "allocation failed";
+        case GAL_ERR_CUDA: return "CUDA error (see gal_last_cuda_error)";
+        case GAL_ERR_UNSUPPORTED: return "unsupported size";
+        default: return "unknown error";
+    }
+}
+
+int gal_plan_create(gal_plan** out, int nxy, int batch, int precision_bits, int device) {
+    if (!out) return GAL_ERR_INVALID_ARGUMENT;
+    *out = nullptr;
+    if (!is_pow2(nxy) || nxy < 8 || batch < 1 || (precision_bits != 64 && precision_bits != 32) || device < 0)
+        return GAL_ERR_INVALID_ARGUMENT;
+    if (nxy > 4096) return GAL_ERR_UNSUPPORTED;
+    gal_plan* p = new (std::nothrow) gal_plan();
+    if (!p) return GAL_ERR_ALLOC;
+    p->nxy = nxy; p->batch = batch; p->bits = precision_bits; p->device = device;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device >= ndev) { delete p; return GAL_ERR_CUDA; }
+    DeviceGuard g(device);
+    cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, device);
+    p->max_gx = p->sm_count * 8;
+    const size_t esz = precision_bits == 64 ? sizeof(double2) : sizeof(float2);
+    const size_t spec_bytes = (size_t)batch * (nxy / 2 + 1) * nxy * esz;
+    auto fail = [&](int code, cudaError_t e) { p->last_cuda = (int)e; gal_plan_destroy(p); return code; };
+    cudaError_t e;
+    if ((e = cudaMalloc(&p->spec, spec_bytes)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
+    if ((e = cudaMalloc(&p->tw, (size_t)nxy * esz)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
+    if ((e = cudaMalloc((void**)&p->partials, sizeof(double) * (size_t)batch * p->max_gx)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
+    if ((e = cudaMalloc((void**)&p->tickets, sizeof(unsigned int) * (batch + 1))) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
+    if ((e = cudaMalloc((void**)&p->chi2_scratch, sizeof(double) * batch)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
+    if ((e = cudaMalloc((void**)&p->oob, sizeof(unsigned long long))) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
+    if ((e = cudaMalloc((void**)&p->st_chi2, sizeof(double))) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
+    p->owned_bytes = spec_bytes + (size_t)nxy * esz + sizeof(double) * (size_t)batch * p->max_gx +
+                     sizeof(unsigned int) * (batch + 1) + sizeof(double) * batch + 16;
+    if ((e = cudaMemset(p->tickets, 0, sizeof(unsigned int) * (batch + 1))) != cudaSuccess) return fail(GAL_ERR_CUDA, e);
+    if ((e = cudaMemset(p->oob, 0, sizeof(unsigned long long))) != cudaSuccess) return fail(GAL_ERR_CUDA, e);
+    // twiddle table exp(-2 pi i m / nxy): evaluated in long double on the host, octant-exact
+    std::vector<double> twd((size_t)2 * nxy);
+    const long double PI = 3.14159265358979323846264338327950288L;
+    for (int m = 0; m < nxy; ++m) {
+        long double a = -2.0L * PI * (long double)m / (long double)nxy;
+        twd[2 * m] = (double)cosl(a);
+        twd[2 * m + 1] = (double)sinl(a);
+    }
+    if (precision_bits == 64) {
+        e = cudaMemcpy(p->tw, twd.data(), sizeof(double) * 2 * nxy, cudaMemcpyHostToDevice);
+    } else {
+        std::vector<float> twf((size_t)2 * nxy);
+        for (size_t i = 0; i < twf.size(); ++i) twf[i] = (float)twd[i];
+        e = cudaMemcpy(p->tw, twf.data(), sizeof(float) * 2 * nxy, cudaMemcpyHostToDevice);
+    }
+    if (e != cudaSuccess) return fail(GAL_ERR_CUDA, e);
+    *out = p;
+    return GAL_OK;
+}
+
+int gal_plan_destroy(gal_plan* p) {
+    if (!p) return GAL_ERR_INVALID_ARGUMENT;
+    DeviceGuard g(p->device);
+    cudaFree(p->spec); cudaFree(p->tw); cudaFree(p->partials); cudaFree(p->tickets); cudaFree(p->chi2_scratch);
+    cudaFree(p->oob); cudaFree(p->st_image); cudaFree(p->st_pts); cudaFree(p->st_out); cudaFree(p->st_chi2);
+    delete p;
+    return GAL_OK;
+}
+
+size_t gal_plan_workspace_bytes(const gal_plan* p) { return p ? p->owned_bytes : 0; }
+int gal_last_cuda_error(const gal_plan* p) { return p ? p->last_cuda : 0; }
+int64_t gal_plan_launch_count(const gal_plan* p) { return p ? p->launches : -1; }
+
+int64_t gal_last_oob_count(gal_plan* p) {
+    if (!p) return -1;
+    DeviceGuard g(p->device);
+    unsigned long long h = 0;
+    if (cudaStreamSynchronize(p->last_stream) != cudaSuccess) return -1;
+    if (cudaMemcpy(&h, p->oob, sizeof(h), cudaMemcpyDeviceToHost) != cudaSuccess) return -1;
+    return (int64_t)h;
+}
+
+#define GAL_DEFINE_PRECISION(SFX, T)                                                                                  \
+    int gal_sweep_##SFX(gal_plan* p, const T* I, int nr, double Rmin, double dR, double dxy, double inc, T* out,      \
+                        void* stream) {                                                                               \
+        return do_sweep<T>(p, I, nr, Rmin, dR, dxy, inc, out, stream);                                                \
+    }                                                                                                                 \
+    int gal_fft2_shifted_##SFX(gal_plan* p, const T* image, T* out, void* stream) {                                   \
+        return do_fft2_shifted<T>(p, image, out, stream);                                                             \
+    }                                                                                                                 \
+    int gal_sample_image_##SFX(gal_plan* p, const T* image, double dxy, const T* u, const T* v, int64_t M,            \
+                               double dRA, double dDec, double PA, T* vis, void* stream) {                            \
+        if (!image || (M > 0 && !vis)) return GAL_ERR_INVALID_ARGUMENT;                                               \
+        if (M == 0) return GAL_OK;                                                                                    \
+        return do_sample_image<T>(p, image, nullptr, 1, dxy, u, v, nullptr, nullptr, nullptr, M, dRA, dDec, PA, vis,  \
+                                  nullptr, nullptr, stream);                                                          \
+    }                                                                                                                 \
+    int gal_chi2_image_##SFX(gal_plan* p, const T* image, double dxy, const T* u, const T* v, const T* re,            \
+                             const T* im, const T* w, int64_t M, double dRA, double dDec, double PA, double* chi2,    \
+                             void* stream) {                                                                          \
+        if (!image || !chi2) return GAL_ERR_INVALID_ARGUMENT;                                                         \
+        return do_sample_image<T>(p, image, nullptr, 1, dxy, u, v, re, im, w, M, dRA, dDec, PA, nullptr, chi2,        \
+                                  nullptr, stream);                                                                   \
+    }                                                                                                                 \
+    int gal_sample_profile_##SFX(gal_plan* p, const T* I, int nr, double Rmin, double dR, double dxy, const T* u,     \
+                                 const T* v, int64_t M, double dRA, double dDec, double PA, double inc, T* vis,       \
+                                 void* stream) {                                                                      \
+        SweepParams sw;                                                                                               \
+        if (!sweep_args(p, I, nr, Rmin, dR, dxy, inc, &sw) || (M > 0 && !vis)) return GAL_ERR_INVALID_ARGUMENT;       \
+        if (M == 0) return GAL_OK;                                                                                    \
+        return do_sample_image<T>(p, nullptr, &sw, 1, dxy, u, v, nullptr, nullptr, nullptr, M, dRA, dDec, PA, vis,    \
+                                  nullptr, nullptr, stream);                                                          \
+    }                                                                                                                 \
+    int gal_chi2_profile_##SFX(gal_plan* p, const T* I, int nr, double Rmin, double dR, double dxy, const T* u,       \
+                               const T* v, const T* re, const T* im, const T* w, int64_t M, double dRA, double dDec,  \
+                               double PA, double inc, double* chi2, void* stream) {                                   \
+        SweepParams sw;                                                                                               \
+        if (!sweep_args(p, I, nr, Rmin, dR, dxy, inc, &sw) || !chi2) return GAL_ERR_INVALID_ARGUMENT;                 \
+        return do_sample_image<T>(p, nullptr, &sw, 1, dxy, u, v, re, im, w, M, dRA, dDec, PA, nullptr, chi2, nullptr, \
+                                  stream);                                                                            \
+    }                                                                                                                 \
+    int gal_chi2_image_batch_##SFX(gal_plan* p, const T* images, int C, double dxy, const T* u, const T* v,           \
+                                   const T* re, const T* im, const T* w, int64_t M, double dRA, double dDec,          \
+                                   double PA, double* chi2_pc, double* chi2_tot, void* stream) {                      \
+        if (!p || !images || !chi2_pc || C < 1) return GAL_ERR_INVALID_ARGUMENT;                                      \
+        return do_sample_image<T>(p, images, nullptr, C, dxy, u, v, re, im, w, M, dRA, dDec, PA, nullptr, chi2_pc,    \
+                                  chi2_tot, stream);                                                                  \
+    }                                                                                                                 \
+    int gal_chi2_image_host_##SFX(gal_plan* p, const T* image, double dxy, const T* u, const T* v, const T* re,       \
+                                  const T* im, const T* w, int64_t M, double dRA, double dDec, double PA,             \
+                                  double* chi2, void* stream) {                                                       \
+        if (!image || !chi2) return GAL_ERR_INVALID_ARGUMENT;                                                         \
+        return do_host_call<T>(p, image, nullptr, 0, 0, 0, 0, dxy, u, v, re, im, w, M, dRA, dDec, PA, nullptr, chi2,  \
+                               stream);                                                                               \
+    }
+
+GAL_DEFINE_PRECISION(f64, double)
+GAL_DEFINE_PRECISION(f32, float)
+
+int gal_sample_image_host_f64(gal_plan* p, const double* image, double dxy, const double* u, const double* v,
+                              int64_t M, double dRA, double dDec, double PA, double* vis, void* stream) {
+    if (!image || !vis) return GAL_ERR_INVALID_ARGUMENT;
+    return do_host_call<double>(p, image, nullptr, 0, 0, 0, 0, dxy, u, v, nullptr, nullptr, nullptr, M, dRA, dDec, PA,
+                                vis, nullptr, stream);
+}
+
+int gal_chi2_profile_host_f64(gal_plan* p, const double* I, int nr, double Rmin, double dR, double dxy,
+                              const double* u, const double* v, const double* re, const double* im, const double* w,
+                              int64_t M, double dRA, double dDec, double PA, double inc, double* chi2, void* stream) {
+    if (!I || !chi2 || nr < 2) return GAL_ERR_INVALID_ARGUMENT;
+    return do_host_call<double>(p, nullptr, I, nr, Rmin, dR, inc, dxy, u, v, re, im, w, M, dRA, dDec, PA, nullptr,
+                                chi2, stream);
+}
+
+}  // extern "C"

@@ -1,0 +1,399 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs.  Run on the B200 box with ``-m gpu``.
+
+Tolerances (BASELINE.json north_star; reading A13 for "relative"):
+  fp64: per visibility  |dV| / max(|V_oracle|, 1e-6 peak) <= 1e-9;   chi2 relative <= 1e-10
+  fp32: per visibility  |dV| <= 1e-4 peak;                           chi2 relative <= 1e-4
+  FFT stage alone (fp64): <= 1e-12 of the spectrum's peak.
+Integer decisions (the cell a point falls in, the out-of-grid count, the sweep's hard edge) are
+taken by both sides in double with the listing's operation order, so they are compared exactly.
+"""
+import numpy as np
+import pytest
+import torch
+
+from paper_1709_06999_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+ARCSEC = np.pi / 648000.0
+TOL_VIS_F64, TOL_CHI2_F64 = 1e-9, 1e-10
+TOL_VIS_F32, TOL_CHI2_F32 = 1e-4, 1e-4
+
+
+@pytest.fixture(scope="module")
+def g():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_1709_06999_b200 as pkg
+    pkg.load_library()          # fails loudly if the extension is missing
+    return pkg
+
+
+def dev(a, dtype=None):
+    t = torch.as_tensor(np.ascontiguousarray(a), device="cuda")
+    return t if dtype is None else t.to(dtype)
+
+
+def rel_err(vis, ref):
+    peak = np.abs(ref).max()
+    return (np.abs(vis - ref) / np.maximum(np.abs(ref), 1e-6 * peak)).max()
+
+
+def threads(orc):
+    return orc.host_threads()
+
+
+# ---------------------------------------------------------------------------------------------
+# S2+S3+S4: the transform alone, every supported size (several tiles, both FFT code paths)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n", [8, 16, 32, 64, 128, 256, 512, 1024, 2048, 4096])
+def test_fft2_shifted_matches_oracle_f64(g, orc, n):
+    rng = np.random.default_rng(n)
+    img = rng.standard_normal((n, n))
+    img[n // 2, n // 2] += 5.0
+    ref = orc.spectrum(img, nthreads=threads(orc))
+    out = g.Plan(n).fft2_shifted(dev(img)).cpu().numpy()
+    assert out.shape == ref.shape
+    assert np.abs(out - ref).max() <= 1e-12 * np.abs(ref).max()
+
+
+@pytest.mark.parametrize("n", [8, 64, 512, 4096])
+def test_fft2_shifted_matches_oracle_f32(g, orc, n):
+    rng = np.random.default_rng(n + 1)
+    img = rng.random((n, n)).astype(np.float32)
+    ref = orc.spectrum(img.astype(np.float64), nthreads=threads(orc))
+    out = g.Plan(n, dtype=torch.float32).fft2_shifted(dev(img)).cpu().numpy()
+    assert np.abs(out - ref).max() <= 2e-6 * np.abs(ref).max()
+
+
+def test_fft_delta_and_sign_fold(g):
+    """Delta a px East / b px North of the centre -> exp(+2 pi i (ku a + kv b)/n): pins the (-1)^(ku+kv)
+    fold of the centre shift and the row fold of the v shift directly on the GPU."""
+    n, a, b = 256, 3, -5
+    img = np.zeros((n, n))
+    img[n // 2 - b, n // 2 - a] = 1.0
+    out = g.Plan(n).fft2_shifted(dev(img)).cpu().numpy()
+    ku = np.arange(n // 2 + 1)[None, :]
+    kv = (np.arange(n) - n // 2)[:, None]
+    assert np.abs(out - np.exp(2j * np.pi * (ku * a + kv * b) / n)).max() <= 1e-13
+
+
+# ---------------------------------------------------------------------------------------------
+# S1: sweep
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n,inc", [(64, 0.0), (256, 0.6), (1024, np.deg2rad(45.0))])
+def test_sweep_matches_oracle(g, orc, n, inc):
+    w = W.config(1, nxy=n, M=10, nr=700)
+    ref = orc.sweep(w.profile, w.Rmin, w.dR, n, w.dxy, inc)
+    out = g.Plan(n).sweep(dev(w.profile), w.Rmin, w.dR, w.dxy, inc).cpu().numpy()
+    assert np.array_equal(out == 0, ref == 0)                 # hard edge and zero centre decided identically
+    assert np.array_equal(out, ref)                           # same operations, same rounding
+    out32 = g.Plan(n, dtype=torch.float32).sweep(dev(w.profile.astype(np.float32)), w.Rmin, w.dR, w.dxy, inc)
+    ref32 = orc.sweep(w.profile.astype(np.float32).astype(np.float64), w.Rmin, w.dR, n, w.dxy, inc)
+    assert np.array_equal(out32.cpu().numpy(), ref32.astype(np.float32))
+
+
+# ---------------------------------------------------------------------------------------------
+# the five configs, reduced (oracle in seconds, several tiles, ragged tails) ...
+# ---------------------------------------------------------------------------------------------
+REDUCED = [
+    (0, dict(nxy=256, M=10_000)),                     # config 0 is already small: run it as written
+    (1, dict(nxy=512, M=50_001, nr=1000)),
+    (2, dict(nxy=1024, M=200_003)),
+    (3, dict(nxy=2048, M=300_007, n_src=120)),
+]
+
+
+def run_gpu(g, w, dtype=torch.float64):
+    plan = g.Plan(w.nxy, 1, dtype)
+    t = lambda a: dev(a)
+    if w.entry == "chi2Profile":
+        vis = plan.sampleProfile(t(w.profile), w.Rmin, w.dR, w.dxy, t(w.u), t(w.v), w.inc, w.PA, w.dRA, w.dDec)
+        oob = plan.last_oob_count()
+        chi2 = plan.chi2Profile(t(w.profile), w.Rmin, w.dR, w.dxy, t(w.u), t(w.v), t(w.re_obs), t(w.im_obs), t(w.w),
+                                w.dRA, w.dDec, w.PA, w.inc)
+    else:
+        vis = plan.sampleImage(t(w.image), w.dxy, t(w.u), t(w.v), w.PA, w.dRA, w.dDec)
+        oob = plan.last_oob_count()
+        chi2 = plan.chi2Image(t(w.image), w.dxy, t(w.u), t(w.v), t(w.re_obs), t(w.im_obs), t(w.w), w.dRA, w.dDec, w.PA)
+    return vis.cpu().numpy(), float(chi2.cpu()[0]), oob
+
+
+def run_oracle(orc, w):
+    f = lambda a: np.asarray(a, dtype=np.float64)
+    nt = threads(orc)
+    if w.entry == "chi2Profile":
+        image = orc.sweep(f(w.profile), w.Rmin, w.dR, w.nxy, w.dxy, w.inc)
+    else:
+        image = f(w.image)
+    vis, oob = orc.sampleImage(image, w.dxy, f(w.u), f(w.v), w.PA, w.dRA, w.dDec, nthreads=nt, return_oob=True)
+    chi2 = orc.chi2(vis, f(w.re_obs), f(w.im_obs), f(w.w))
+    return vis, chi2, oob
+
+
+@pytest.mark.parametrize("idx,kw", REDUCED)
+def test_configs_reduced_f64(g, orc, idx, kw):
+    w = W.config(idx, **kw)
+    vis, chi2, oob = run_gpu(g, w)
+    ref, ref_chi2, ref_oob = run_oracle(orc, w)
+    assert oob == ref_oob
+    assert rel_err(vis, ref) <= TOL_VIS_F64
+    assert abs(chi2 - ref_chi2) <= TOL_CHI2_F64 * abs(ref_chi2)
+
+
+@pytest.mark.parametrize("idx,kw", REDUCED)
+def test_configs_reduced_f32(g, orc, idx, kw):
+    w = W.config(idx, **kw).as_f32()
+    vis, chi2, oob = run_gpu(g, w, torch.float32)
+    ref, ref_chi2, ref_oob = run_oracle(orc, w)              # fp64 oracle on the fp32-rounded inputs (A14)
+    assert oob == ref_oob
+    assert np.abs(vis - ref).max() <= TOL_VIS_F32 * np.abs(ref).max()
+    assert abs(chi2 - ref_chi2) <= TOL_CHI2_F32 * abs(ref_chi2)
+
+
+def test_config4_reduced_batch(g, orc):
+    w = W.config(4, nxy=256, M=20_011, C=5)
+    plan = g.Plan(w.nxy, 5)
+    per, tot = plan.chi2ImageBatch(dev(w.image), w.dxy, dev(w.u), dev(w.v), dev(w.re_obs), dev(w.im_obs), dev(w.w),
+                                   w.dRA, w.dDec, w.PA)
+    rper, rtot = orc.chi2ImageBatch(w.image, w.dxy, w.u, w.v, w.re_obs, w.im_obs, w.w, w.dRA, w.dDec, w.PA,
+                                    nthreads=threads(orc))
+    per, tot = per.cpu().numpy(), float(tot.cpu()[0])
+    assert np.abs(per - rper).max() <= TOL_CHI2_F64 * np.abs(rper).max()
+    assert abs(tot - rtot) <= TOL_CHI2_F64 * abs(rtot)
+    # a batch of C is exactly C single calls (same kernels, same reduction geometry per channel is not
+    # promised, so compare at the chi2 tolerance) and a smaller C on a larger plan works
+    p1 = g.Plan(w.nxy, 1)
+    for c in (0, 4):
+        one = p1.chi2Image(dev(w.image[c]), w.dxy, dev(w.u[c]), dev(w.v[c]), dev(w.re_obs[c]), dev(w.im_obs[c]),
+                           dev(w.w[c]), w.dRA, w.dDec, w.PA)
+        assert abs(float(one.cpu()[0]) - rper[c]) <= TOL_CHI2_F64 * abs(rper[c])
+    per3, tot3 = plan.chi2ImageBatch(dev(w.image[:3]), w.dxy, dev(w.u[:3]), dev(w.v[:3]), dev(w.re_obs[:3]),
+                                     dev(w.im_obs[:3]), dev(w.w[:3]), w.dRA, w.dDec, w.PA)
+    assert np.abs(per3.cpu().numpy() - rper[:3]).max() <= TOL_CHI2_F64 * np.abs(rper).max()
+    assert abs(float(tot3.cpu()[0]) - rper[:3].sum()) <= TOL_CHI2_F64 * rper[:3].sum()
+
+
+# ---------------------------------------------------------------------------------------------
+# ... and at BASELINE.json's full sizes, in the launch configuration bench.py times
+# ---------------------------------------------------------------------------------------------
+def test_config1_full(g, orc):
+    w = W.config(1)
+    vis, chi2, oob = run_gpu(g, w)
+    ref, ref_chi2, ref_oob = run_oracle(orc, w)
+    assert oob == ref_oob
+    assert rel_err(vis, ref) <= TOL_VIS_F64
+    assert abs(chi2 - ref_chi2) <= TOL_CHI2_F64 * abs(ref_chi2)
+
+
+def test_config2_full(g, orc):
+    w = W.config(2)
+    vis, chi2, oob = run_gpu(g, w)
+    ref, ref_chi2, ref_oob = run_oracle(orc, w)
+    assert oob == ref_oob
+    assert rel_err(vis, ref) <= TOL_VIS_F64
+    assert abs(chi2 - ref_chi2) <= TOL_CHI2_F64 * abs(ref_chi2)
+
+
+@pytest.fixture(scope="module")
+def cfg3_full():
+    return W.config(3)
+
+
+def test_config3_full_f64(g, orc, cfg3_full):
+    w = cfg3_full
+    vis, chi2, oob = run_gpu(g, w)
+    ref, ref_chi2, ref_oob = run_oracle(orc, w)
+    assert oob == ref_oob
+    assert rel_err(vis, ref) <= TOL_VIS_F64
+    assert abs(chi2 - ref_chi2) <= TOL_CHI2_F64 * abs(ref_chi2)
+    # determinism: fixed reduction tree, no floating-point atomics
+    _, chi2b, _ = run_gpu(g, w)
+    assert chi2b == chi2
+
+
+def test_config3_full_f32(g, orc, cfg3_full):
+    w = cfg3_full.as_f32()
+    vis, chi2, oob = run_gpu(g, w, torch.float32)
+    ref, ref_chi2, ref_oob = run_oracle(orc, w)
+    assert oob == ref_oob
+    assert np.abs(vis - ref).max() <= TOL_VIS_F32 * np.abs(ref).max()
+    assert abs(chi2 - ref_chi2) <= TOL_CHI2_F32 * abs(ref_chi2)
+
+
+def test_config4_full(g, orc):
+    w = W.config(4)
+    C = w.image.shape[0]
+    plan = g.Plan(w.nxy, C)
+    per, tot = plan.chi2ImageBatch(dev(w.image), w.dxy, dev(w.u), dev(w.v), dev(w.re_obs), dev(w.im_obs), dev(w.w),
+                                   w.dRA, w.dDec, w.PA)
+    oob = plan.last_oob_count()
+    per, tot = per.cpu().numpy(), float(tot.cpu()[0])
+    # the oracle computes sampled channels one by one; the total is checked by its definition
+    for c in (0, 1, 37, 63, 64, 100, 127):
+        r = orc.chi2Image(w.image[c], w.dxy, w.u[c], w.v[c], w.re_obs[c], w.im_obs[c], w.w[c], w.dRA, w.dDec, w.PA,
+                          nthreads=threads(orc))
+        assert abs(per[c] - r) <= TOL_CHI2_F64 * abs(r), c
+    import math
+    assert abs(tot - math.fsum(per)) <= 1e-13 * tot
+    assert oob > 0          # 16 km at 230 GHz reaches index 609 > 512: some points wrap (reading A6)
+
+
+# ---------------------------------------------------------------------------------------------
+# identities that hold at any size, on the GPU itself
+# ---------------------------------------------------------------------------------------------
+def test_sampleProfile_is_sampleImage_of_sweep_bit_for_bit(g):
+    """PAPER.md:402.  The fused row loader and the standalone sweep kernel share one device function."""
+    w = W.config(1, nxy=512, M=30_000, nr=1000)
+    plan = g.Plan(w.nxy)
+    a = plan.sampleProfile(dev(w.profile), w.Rmin, w.dR, w.dxy, dev(w.u), dev(w.v), w.inc, w.PA, 1e-7, -2e-7)
+    img = plan.sweep(dev(w.profile), w.Rmin, w.dR, w.dxy, w.inc)
+    b = plan.sampleImage(img, w.dxy, dev(w.u), dev(w.v), w.PA, 1e-7, -2e-7)
+    assert torch.equal(a, b)
+
+
+def test_point_source_closed_form_on_gpu(g):
+    n, dxy = 1024, 0.01 * ARCSEC
+    img = np.zeros((n, n))
+    img[n // 2, n // 2] = 1.0
+    rng = np.random.default_rng(3)
+    du = 1.0 / (n * dxy)
+    q, az = rng.uniform(0, 0.45 * n, 100_000) * du, rng.uniform(0, 2 * np.pi, 100_000)
+    u, v = q * np.cos(az), q * np.sin(az)
+    dRA, dDec = 0.4 * ARCSEC, -0.25 * ARCSEC
+    vis = g.Plan(n).sampleImage(dev(img), dxy, dev(u), dev(v), 0.9, dRA, dDec).cpu().numpy()
+    assert np.abs(vis - np.exp(2j * np.pi * (u * dRA + v * dDec))).max() <= 1e-12
+
+
+def test_chi2_properties_on_gpu(g):
+    w = W.config(0)
+    plan = g.Plan(w.nxy)
+    t = dev
+    vis = plan.sampleImage(t(w.image), w.dxy, t(w.u), t(w.v), w.PA, w.dRA, w.dDec)
+    vr, vi = vis.real.contiguous(), vis.imag.contiguous()
+    zero = plan.chi2Image(t(w.image), w.dxy, t(w.u), t(w.v), vr, vi, t(w.w), w.dRA, w.dDec, w.PA)
+    assert float(zero.cpu()[0]) == 0.0                       # V_obs = V exactly -> 0 exactly
+    z = torch.zeros_like(vr)
+    c0 = float(plan.chi2Image(t(w.image), w.dxy, t(w.u), t(w.v), z, z, t(w.w), w.dRA, w.dDec, w.PA).cpu()[0])
+    expect = float((t(w.w) * (vr * vr + vi * vi)).sum().cpu())
+    assert abs(c0 - expect) <= 1e-12 * expect
+    c3 = float(plan.chi2Image(t(w.image), w.dxy, t(w.u), t(w.v), z, z, 3.0 * t(w.w), w.dRA, w.dDec, w.PA).cpu()[0])
+    assert abs(c3 - 3.0 * c0) <= 1e-13 * c3
+
+
+# ---------------------------------------------------------------------------------------------
+# edge cases
+# ---------------------------------------------------------------------------------------------
+def test_edge_points_and_wrap(g, orc):
+    """Exact nodes, u' = 0 and -0.0, the top row, the Nyquist column, and points beyond the grid."""
+    n, dxy = 64, 0.05 * ARCSEC
+    du = 1.0 / (n * dxy)
+    img = np.random.default_rng(0).random((n, n))
+    u = np.array([0.0, -0.0, 2.0, -3.0, 0.0, n / 2.0, -n / 2.0, n / 2 + 0.5, -(n / 2 + 2.0), 3.0, 3.0, 2.0, 1e-300,
+                  n / 2 - 1e-9, 75.3, -140.7]) * du
+    v = np.array([0.0, 1.5, 1.0, 4.0, n / 2 - 1.0, 2.5, -1.0, 0.0, 1.0, n / 2 - 0.5, -n / 2 - 0.25, n / 2 - 1.0, -0.0,
+                  -n / 2, 99.1, -64.0]) * du
+    plan = g.Plan(n)
+    for PA, dRA, dDec in ((0.0, 0.0, 0.0), (0.0, 1e-7, 2e-7), (1.1, -3e-7, 1e-7)):
+        vis = plan.sampleImage(dev(img), dxy, dev(u), dev(v), PA, dRA, dDec).cpu().numpy()
+        oob = plan.last_oob_count()
+        ref, ref_oob = orc.sampleImage(img, dxy, u, v, PA, dRA, dDec, return_oob=True)
+        assert oob == ref_oob
+        assert rel_err(vis, ref) <= TOL_VIS_F64
+
+
+def test_empty_single_and_ragged_M(g, orc):
+    w = W.config(0)
+    plan = g.Plan(w.nxy)
+    t = dev
+    e = torch.empty(0, dtype=torch.float64, device="cuda")
+    assert plan.sampleImage(t(w.image), w.dxy, e, e).numel() == 0
+    assert float(plan.chi2Image(t(w.image), w.dxy, e, e, e, e, e).cpu()[0]) == 0.0
+    for M in (1, 31, 257, 9_999):
+        s = slice(0, M)
+        vis = plan.sampleImage(t(w.image), w.dxy, t(w.u[s]), t(w.v[s]), w.PA, w.dRA, w.dDec).cpu().numpy()
+        ref = orc.sampleImage(w.image, w.dxy, w.u[s], w.v[s], w.PA, w.dRA, w.dDec)
+        assert rel_err(vis, ref) <= TOL_VIS_F64
+        c = float(plan.chi2Image(t(w.image), w.dxy, t(w.u[s]), t(w.v[s]), t(w.re_obs[s]), t(w.im_obs[s]), t(w.w[s]),
+                                 w.dRA, w.dDec, w.PA).cpu()[0])
+        r = orc.chi2(ref, w.re_obs[s], w.im_obs[s], w.w[s])
+        assert abs(c - r) <= TOL_CHI2_F64 * abs(r)
+
+
+def test_smallest_and_largest_nxy_end_to_end(g, orc):
+    for n, M in ((8, 100), (4096, 1000)):
+        rng = np.random.default_rng(n)
+        dxy = 0.01 * ARCSEC
+        du = 1.0 / (n * dxy)
+        img = rng.random((n, n))
+        u, v = rng.uniform(-0.45 * n, 0.45 * n, M) * du, rng.uniform(-0.45 * n, 0.45 * n, M) * du
+        vis = g.Plan(n).sampleImage(dev(img), dxy, dev(u), dev(v), 0.3, 1e-7, 1e-7).cpu().numpy()
+        ref = orc.sampleImage(img, dxy, u, v, 0.3, 1e-7, 1e-7, nthreads=threads(orc))
+        assert rel_err(vis, ref) <= TOL_VIS_F64
+
+
+def test_error_codes(g):
+    lib = g.load_library()
+    import ctypes
+    h = ctypes.c_void_p()
+    assert lib.gal_plan_create(ctypes.byref(h), 100, 1, 64, 0) == -1        # not a power of two
+    assert lib.gal_plan_create(ctypes.byref(h), 256, 0, 64, 0) == -1        # batch < 1
+    assert lib.gal_plan_create(ctypes.byref(h), 256, 1, 16, 0) == -1        # precision
+    assert lib.gal_plan_create(ctypes.byref(h), 8192, 1, 64, 0) == -4       # unsupported size
+    assert lib.gal_plan_create(None, 256, 1, 64, 0) == -1
+    plan = g.Plan(64)
+    img = torch.zeros(64, 64, dtype=torch.float64, device="cuda")
+    x = torch.zeros(10, dtype=torch.float64, device="cuda")
+    out = torch.zeros(1, dtype=torch.float64, device="cuda")
+    f = lib.gal_chi2_image_f64
+    ok = (plan._h, img.data_ptr(), 1e-7, x.data_ptr(), x.data_ptr(), x.data_ptr(), x.data_ptr(), x.data_ptr(), 10,
+          0.0, 0.0, 0.0, out.data_ptr(), None)
+    assert f(*ok) == 0
+    bad = lambda i, val: f(*[val if j == i else a for j, a in enumerate(ok)])
+    assert bad(1, None) == -1 and bad(3, None) == -1 and bad(7, None) == -1 and bad(12, None) == -1
+    assert bad(2, 0.0) == -1 and bad(2, -1.0) == -1 and bad(8, -5) == -1 and bad(9, float("nan")) == -1
+    assert lib.gal_chi2_image_f32(*ok) == -1                                 # plan precision mismatch
+    prof = torch.ones(10, dtype=torch.float64, device="cuda")
+    sw = lib.gal_sweep_f64
+    assert sw(plan._h, prof.data_ptr(), 10, 0.0, 1e-7, 1e-7, 0.0, img.data_ptr(), None) == 0
+    assert sw(plan._h, prof.data_ptr(), 1, 0.0, 1e-7, 1e-7, 0.0, img.data_ptr(), None) == -1     # nr < 2
+    assert sw(plan._h, prof.data_ptr(), 10, 0.0, 0.0, 1e-7, 0.0, img.data_ptr(), None) == -1     # dR <= 0
+    assert sw(plan._h, prof.data_ptr(), 10, 0.0, 1e-7, 1e-7, 1.6, img.data_ptr(), None) == -1    # |inc| >= pi/2
+    with pytest.raises(g.GalarioError):
+        g.Plan(64, 2).chi2ImageBatch(torch.zeros(3, 64, 64, dtype=torch.float64, device="cuda"), 1e-7,
+                                     torch.zeros(3, 4, dtype=torch.float64, device="cuda"),
+                                     torch.zeros(3, 4, dtype=torch.float64, device="cuda"),
+                                     torch.zeros(3, 4, dtype=torch.float64, device="cuda"),
+                                     torch.zeros(3, 4, dtype=torch.float64, device="cuda"),
+                                     torch.zeros(3, 4, dtype=torch.float64, device="cuda"))       # C > plan batch
+    torch.cuda.synchronize()
+
+
+def test_host_pointer_calls_match_device_calls(g, orc):
+    w = W.config(0)
+    plan = g.Plan(w.nxy)
+    c_host = plan.chi2Image_host(w.image, w.dxy, w.u, w.v, w.re_obs, w.im_obs, w.w, w.dRA, w.dDec, w.PA)
+    c_dev = float(plan.chi2Image(dev(w.image), w.dxy, dev(w.u), dev(w.v), dev(w.re_obs), dev(w.im_obs), dev(w.w),
+                                 w.dRA, w.dDec, w.PA).cpu()[0])
+    assert c_host == c_dev
+    v_host = plan.sampleImage_host(w.image, w.dxy, w.u, w.v, w.PA, w.dRA, w.dDec)
+    v_dev = plan.sampleImage(dev(w.image), w.dxy, dev(w.u), dev(w.v), w.PA, w.dRA, w.dDec).cpu().numpy()
+    assert np.array_equal(v_host, v_dev)
+    w1 = W.config(1, nxy=256, M=5000, nr=500)
+    p1 = g.Plan(w1.nxy)
+    ch = p1.chi2Profile_host(w1.profile, w1.Rmin, w1.dR, w1.dxy, w1.u, w1.v, w1.re_obs, w1.im_obs, w1.w, 0.0, 0.0,
+                             w1.PA, w1.inc)
+    r = orc.chi2Profile(w1.profile, w1.Rmin, w1.dR, w1.nxy, w1.dxy, w1.u, w1.v, w1.re_obs, w1.im_obs, w1.w, 0.0, 0.0,
+                        w1.PA, w1.inc)
+    assert abs(ch - r) <= TOL_CHI2_F64 * abs(r)
+
+
+def test_paper_style_module_calls(g, orc):
+    w = W.config(0)
+    vis = g.sampleImage(dev(w.image), w.dxy, dev(w.u), dev(w.v), PA=w.PA, dRA=w.dRA, dDec=w.dDec).cpu().numpy()
+    ref = orc.sampleImage(w.image, w.dxy, w.u, w.v, PA=w.PA, dRA=w.dRA, dDec=w.dDec)
+    assert rel_err(vis, ref) <= TOL_VIS_F64
+    c = g.chi2Image(dev(w.image), w.dxy, dev(w.u), dev(w.v), dev(w.re_obs), dev(w.im_obs), dev(w.w), w.dRA, w.dDec, w.PA)
+    r = orc.chi2(ref, w.re_obs, w.im_obs, w.w)
+    assert abs(float(c.cpu()[0]) - r) <= TOL_CHI2_F64 * abs(r)
