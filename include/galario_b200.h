@@ -70,6 +70,14 @@ const char* gal_strerror(int code);
 /* Number of kernels the plan has launched since it was created (for launch accounting). */
 int64_t gal_plan_launch_count(const gal_plan* plan);
 
+/* Diagnostic per-kernel timing.  After gal_plan_timing_enable(plan, n) the next n sample/chi2 calls record a
+ * CUDA event on their stream before the row pass, between the kernels and after the sampling kernel
+ * (n = 0 switches it off and frees the events).  gal_plan_timing_read synchronises those events and returns
+ * the average duration in milliseconds of the row pass, the column pass and the sampling kernel
+ * (ms_per_kernel[3]) over the calls recorded so far (*calls, may be null). */
+int gal_plan_timing_enable(gal_plan* plan, int max_calls);
+int gal_plan_timing_read(gal_plan* plan, double* ms_per_kernel, int64_t* calls);
+
 /* ---- sweep: image_out[nxy][nxy] = dxy^2 * lerp(I, (r - Rmin)/dR),
  *      r = sqrt((x/cos inc)^2 + y^2), 0 outside [Rmin, Rmin + (nr-1) dR]. ---- */
 int gal_sweep_f64(gal_plan* plan, const double* I, int nr, double Rmin, double dR, double dxy, double inc,

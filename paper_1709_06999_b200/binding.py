@@ -39,6 +39,8 @@ def load_library() -> ctypes.CDLL:
         for name in ("gal_plan_destroy", "gal_plan_workspace_bytes", "gal_last_oob_count", "gal_last_cuda_error",
                      "gal_plan_launch_count"):
             getattr(lib, name).argtypes = [_vp]
+        lib.gal_plan_timing_enable.argtypes = [_vp, _i]
+        lib.gal_plan_timing_read.argtypes = [_vp, _vp, _vp]
         for s in ("f64", "f32"):
             getattr(lib, f"gal_sweep_{s}").argtypes = [_vp, _vp, _i, _d, _d, _d, _d, _vp, _vp]
             getattr(lib, f"gal_fft2_shifted_{s}").argtypes = [_vp, _vp, _vp, _vp]
@@ -111,6 +113,17 @@ class Plan:
 
     def launch_count(self) -> int:
         return int(self._lib.gal_plan_launch_count(self._h))
+
+    def timing_enable(self, max_calls: int) -> None:
+        _check(self._lib.gal_plan_timing_enable(self._h, int(max_calls)), "gal_plan_timing_enable", self)
+
+    def timing_read(self):
+        """Average ms of (row pass, column pass, sampling kernel) over the recorded calls, and their number."""
+        ms = (ctypes.c_double * 3)()
+        n = ctypes.c_int64(0)
+        _check(self._lib.gal_plan_timing_read(self._h, ctypes.addressof(ms), ctypes.addressof(n)),
+               "gal_plan_timing_read", self)
+        return [ms[0], ms[1], ms[2]], n.value
 
     # -- the paper's calls ---------------------------------------------------------------------
     def sweep(self, I, Rmin, dR, dxy, inc=0.0, out=None):

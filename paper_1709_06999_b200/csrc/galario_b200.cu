@@ -33,6 +33,10 @@ struct gal_plan {
     void* st_pts = nullptr;   size_t st_pts_bytes = 0;
     void* st_out = nullptr;   size_t st_out_bytes = 0;
     double* st_chi2 = nullptr;
+    // optional per-kernel timing (gal_plan_timing_enable): 4 events per call
+    std::vector<cudaEvent_t> tev;
+    int t_max_calls = 0, t_calls = 0;
+    cudaEvent_t* t_split = nullptr;  // when set, the row launcher records t_split[1] after its kernel
 };
 
 namespace {
@@ -84,6 +88,7 @@ int launch_row(gal_plan* p, const T* image, const SweepParams* sw, int batch, cu
     }
     p->launches++;
     GAL_CUDA(p, cudaGetLastError());
+    if (p->t_split) GAL_CUDA(p, cudaEventRecord(p->t_split[1], st));
     return GAL_OK;
 }
 
@@ -184,6 +189,26 @@ int launch_sample(gal_plan* p, int C, double dxy, const T* u, const T* v, const 
     return GAL_OK;
 }
 
+// Same launches with a CUDA event between the kernels (diagnostic mode, gal_plan_timing_enable).
+template <typename T>
+int timed_call(gal_plan* p, const T* image, const SweepParams* sw, int C, double dxy, const T* u, const T* v,
+               const T* re, const T* im, const T* w, int64_t M, double dRA, double dDec, double PA, T* vis,
+               double* chi2_pc, double* chi2_tot, cudaStream_t st) {
+    cudaEvent_t* e = &p->tev[(size_t)4 * p->t_calls];
+    int rc;
+    GAL_CUDA(p, cudaEventRecord(e[0], st));
+    p->t_split = e;
+    rc = fft2<T>(p, image, sw, C, st);
+    p->t_split = nullptr;
+    if (rc) return rc;
+    GAL_CUDA(p, cudaEventRecord(e[2], st));
+    rc = launch_sample<T>(p, C, dxy, u, v, re, im, w, M, dRA, dDec, PA, vis, chi2_pc, chi2_tot, st);
+    if (rc) return rc;
+    GAL_CUDA(p, cudaEventRecord(e[3], st));
+    p->t_calls++;
+    return GAL_OK;
+}
+
 template <typename T> bool prec_ok(const gal_plan* p) { return p && p->bits == (int)(8 * sizeof(T)); }
 
 bool sweep_args(const gal_plan* p, const void* I, int nr, double Rmin, double dR, double dxy, double inc,
@@ -210,6 +235,7 @@ int do_sample_image(gal_plan* p, const T* image, const SweepParams* sw, int C, d
     DeviceGuard g(p->device);
     cudaStream_t st = (cudaStream_t)stream;
     p->last_stream = st;
+    if (p->t_calls < p->t_max_calls) return timed_call<T>(p, image, sw, C, dxy, u, v, re, im, w, M, dRA, dDec, PA, vis, chi2_pc, chi2_tot, st);
     int rc = fft2<T>(p, image, sw, C, st);
     if (rc) return rc;
     return launch_sample<T>(p, C, dxy, u, v, re, im, w, M, dRA, dDec, PA, vis, chi2_pc, chi2_tot, st);
@@ -365,8 +391,40 @@ int gal_plan_destroy(gal_plan* p) {
     if (!p) return GAL_ERR_INVALID_ARGUMENT;
     DeviceGuard g(p->device);
     cudaFree(p->spec); cudaFree(p->tw); cudaFree(p->partials); cudaFree(p->tickets); cudaFree(p->chi2_scratch);
+    for (cudaEvent_t e : p->tev) cudaEventDestroy(e);
     cudaFree(p->oob); cudaFree(p->st_image); cudaFree(p->st_pts); cudaFree(p->st_out); cudaFree(p->st_chi2);
     delete p;
+    return GAL_OK;
+}
+
+int gal_plan_timing_enable(gal_plan* p, int max_calls) {
+    if (!p || max_calls < 0 || max_calls > (1 << 20)) return GAL_ERR_INVALID_ARGUMENT;
+    DeviceGuard g(p->device);
+    for (cudaEvent_t e : p->tev) cudaEventDestroy(e);
+    p->tev.clear();
+    p->t_calls = 0;
+    p->t_max_calls = 0;
+    p->tev.resize((size_t)4 * max_calls);
+    for (auto& e : p->tev) GAL_CUDA(p, cudaEventCreate(&e));
+    p->t_max_calls = max_calls;
+    return GAL_OK;
+}
+
+int gal_plan_timing_read(gal_plan* p, double* ms_per_kernel, int64_t* calls) {
+    if (!p || !ms_per_kernel) return GAL_ERR_INVALID_ARGUMENT;
+    DeviceGuard g(p->device);
+    double acc[3] = {0, 0, 0};
+    for (int c = 0; c < p->t_calls; ++c) {
+        cudaEvent_t* e = &p->tev[(size_t)4 * c];
+        GAL_CUDA(p, cudaEventSynchronize(e[3]));
+        for (int k = 0; k < 3; ++k) {
+            float ms = 0;
+            GAL_CUDA(p, cudaEventElapsedTime(&ms, e[k], e[k + 1]));
+            acc[k] += ms;
+        }
+    }
+    for (int k = 0; k < 3; ++k) ms_per_kernel[k] = p->t_calls ? acc[k] / p->t_calls : 0.0;
+    if (calls) *calls = p->t_calls;
     return GAL_OK;
 }
 

@@ -1,0 +1,54 @@
+"""Host-side logic of bench.py that does not need a GPU: the algorithmic-byte table of
+SURVEY.md §8(d) and the max-over-ranks timing rule on a world_size-2 gloo group."""
+import os
+import sys
+
+import pytest
+import torch
+import torch.multiprocessing as mp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+sys.path.insert(0, ROOT)
+
+
+def test_algorithmic_bytes_match_survey_table():
+    import bench
+    B = bench.algorithmic_bytes(4096, 5_000_000, 8)
+    assert B["row_pass"] == 4096 * 4096 * 8 + 4096 * 2049 * 16
+    assert B["col_pass"] == 2 * 4096 * 2049 * 16
+    assert B["sample"] == 200_000_000
+    assert abs(B["step"] / 1e6 - 737.1) < 0.5            # 537.1 MB of FFT passes + 200 MB
+    S = bench.algorithmic_bytes(4096, 5_000_000, 8, "sampleImage")
+    assert S["sample"] == 160_000_000
+    F = bench.algorithmic_bytes(4096, 5_000_000, 4)
+    assert F["step"] * 2 == B["step"]
+
+
+def _worker(rank, world, port, q):
+    import torch.distributed as dist
+    import bench
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    ms = bench.max_over_ranks(10.0 + 5.0 * rank, world)
+    q.put((rank, ms))
+    dist.destroy_process_group()
+
+
+def test_max_over_ranks_gloo_world2():
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 29500 + os.getpid() % 1000
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = dict(q.get(timeout=120) for _ in range(2))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert res == {0: 15.0, 1: 15.0}
+
+
+def test_max_over_ranks_single():
+    import bench
+    assert bench.max_over_ranks(3.5, 1) == 3.5
