@@ -111,6 +111,16 @@ template <typename T> struct Dft<T, 16> {
     }
 };
 
+// w[k] = w1^k for k = 1..R-1 from one table value, by a product tree of depth <= log2(R)
+// (w[2j] = w[j]^2, w[2j+1] = w[j] w[j+1]): at most four roundings deep for R = 16.
+template <typename T, int R>
+__device__ __forceinline__ void twiddle_powers(cx<T> w1, cx<T>* w) {
+    w[0] = mk<T>(1, 0);
+    if (R > 1) w[1] = w1;
+#pragma unroll
+    for (int k = 2; k < R; ++k) w[k] = (k & 1) ? cmul(w[k / 2], w[k / 2 + 1]) : cmul(w[k / 2], w[k / 2]);
+}
+
 // ------------------------------------------------------------------------------------------
 // Geometry of one L-point FFT in shared memory.
 // ------------------------------------------------------------------------------------------
@@ -136,19 +146,28 @@ template <typename T, int R1, int R2, int R3, int F> struct Geom {
 // tw[m * tws] = exp(-2 pi i m / L), load(n) returns input element n.  Ends with a barrier.
 template <typename T, int R1, int R2, int R3, int TPF, typename LoadFn>
 __device__ __forceinline__ void fft_steps12(cx<T>* S, int t, const cx<T>* __restrict__ tw, int tws, LoadFn load) {
-    constexpr int L = R1 * R2 * R3;
     constexpr int P1 = (R2 * R3 > 1) ? R2 * R3 + 1 : 1;
     constexpr int N2 = R2 * R3;
+    // The only table reads: one base twiddle per work item and step, W_L^n2 and W_(R2R3)^b.  They are
+    // issued before the data loads so their latency hides behind them; the powers are formed in registers.
+    cx<T> wb1 = mk<T>(1, 0), wb2 = mk<T>(1, 0);
+    if (N2 > 1) wb1 = __ldg(tw + t * tws);
+    if (R2 > 1 && R3 > 1) wb2 = __ldg(tw + (t % R3) * (R1 * tws));
     for (int n2 = t; n2 < N2; n2 += TPF) {
         cx<T> a[R1];
 #pragma unroll
         for (int n1 = 0; n1 < R1; ++n1) a[n1] = load(N2 * n1 + n2);
+        if (N2 > 1 && n2 != t) wb1 = __ldg(tw + n2 * tws);
         Dft<T, R1>::run(a);
         S[n2] = a[0];
+        if (N2 > 1) {
+            cx<T> w[R1];
+            twiddle_powers<T, R1>(wb1, w);
 #pragma unroll
-        for (int k1 = 1; k1 < R1; ++k1) {
-            if (N2 > 1) a[k1] = cmul(a[k1], tw[(n2 * k1) * tws]);
-            S[k1 * P1 + n2] = a[k1];
+            for (int k1 = 1; k1 < R1; ++k1) S[k1 * P1 + n2] = cmul(a[k1], w[k1]);
+        } else {
+#pragma unroll
+            for (int k1 = 1; k1 < R1; ++k1) S[k1 * P1 + n2] = a[k1];
         }
     }
     __syncthreads();
@@ -159,17 +178,21 @@ __device__ __forceinline__ void fft_steps12(cx<T>* S, int t, const cx<T>* __rest
             cx<T> a[R2];
 #pragma unroll
             for (int i = 0; i < R2; ++i) a[i] = base[i * R3];
+            if (R3 > 1 && (TPF % R3) != 0 && it != t) wb2 = __ldg(tw + b * (R1 * tws));
             Dft<T, R2>::run(a);
             base[0] = a[0];
+            if (R3 > 1) {
+                cx<T> w[R2];
+                twiddle_powers<T, R2>(wb2, w);
 #pragma unroll
-            for (int c = 1; c < R2; ++c) {
-                if (R3 > 1) a[c] = cmul(a[c], tw[(b * c) * (R1 * tws)]);
-                base[c * R3] = a[c];
+                for (int c = 1; c < R2; ++c) base[c * R3] = cmul(a[c], w[c]);
+            } else {
+#pragma unroll
+                for (int c = 1; c < R2; ++c) base[c * R3] = a[c];
             }
         }
         __syncthreads();
     }
-    (void)L;
 }
 
 // ------------------------------------------------------------------------------------------

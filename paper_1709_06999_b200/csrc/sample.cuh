@@ -58,67 +58,102 @@ __device__ __forceinline__ cx<T> node_any(const cx<T>* __restrict__ spec, int N,
     return g;
 }
 
+// Points per thread and loop trip.  All streamed inputs of the U points are requested first, then the
+// 4U spectrum nodes, then the arithmetic: three dependent memory latencies per trip instead of per point.
+constexpr int SAMPLE_U = 2;
+
 template <typename T, bool WRITE_VIS, bool DO_CHI2>
 __global__ void __launch_bounds__(256) sample_kernel(const SampleParams<T> p) {
+    constexpr int U = SAMPLE_U;
     const int c = blockIdx.y;
     const int N = p.N, H = N >> 1;
     const long long M = p.M;
     const cx<T>* __restrict__ spec = p.spec + (long long)c * (H + 1) * N;
     const T* __restrict__ u = p.u + c * M;
     const T* __restrict__ v = p.v + c * M;
+    const T* __restrict__ re_obs = DO_CHI2 ? p.re_obs + c * M : nullptr;
+    const T* __restrict__ im_obs = DO_CHI2 ? p.im_obs + c * M : nullptr;
+    const T* __restrict__ wgt = DO_CHI2 ? p.w + c * M : nullptr;
     const double fH = (double)H;
 
     double acc = 0.0;
     unsigned int oob = 0;
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < M; k += stride) {
-        const double uk = (double)__ldcs(u + k), vk = (double)__ldcs(v + k);
-        // PAPER.md:667-668 (Eq. 11-12)
-        const double urot = __dsub_rn(__dmul_rn(uk, p.cos_PA), __dmul_rn(vk, p.sin_PA));
-        const double vrot = __dadd_rn(__dmul_rn(uk, p.sin_PA), __dmul_rn(vk, p.cos_PA));
-        // PAPER.md:676-683
-        const double urot_idx = div_by(fabs(urot), p.du, p.rdu, p.du_exact_div);
-        const bool uneg = urot < 0.0;
-        const double vq = div_by(vrot, p.du, p.rdu, p.du_exact_div);
-        const double vrot_idx = uneg ? __dsub_rn(fH, vq) : __dadd_rn(fH, vq);
-        if (urot_idx > fH || vrot_idx < 0.0 || vrot_idx > (double)(N - 1)) ++oob;
-        // bilinear interpolation
-        const double fx0 = floor(urot_idx), fy0 = floor(vrot_idx);
-        const long long ix = (long long)fx0, iy = (long long)fy0;
-        const double tx = __dsub_rn(urot_idx, fx0), ty = __dsub_rn(vrot_idx, fy0);
-        cx<T> g00, g01, g10, g11;   // g{row offset}{col offset}
-        if (ix + 1 <= H && iy >= 0 && iy + 1 <= N - 1) {
-            const cx<T>* b0 = spec + ix * N + iy;
-            g00 = __ldg(b0);
-            g10 = __ldg(b0 + 1);
-            g01 = __ldg(b0 + N);
-            g11 = __ldg(b0 + N + 1);
-        } else {
-            g00 = node_any<T>(spec, N, iy, ix);
-            g01 = node_any<T>(spec, N, iy, ix + 1);
-            g10 = node_any<T>(spec, N, iy + 1, ix);
-            g11 = node_any<T>(spec, N, iy + 1, ix + 1);
+    const long long stride = (long long)gridDim.x * blockDim.x * U;
+    for (long long k0 = (long long)blockIdx.x * blockDim.x * U + threadIdx.x; k0 < M; k0 += stride) {
+        double uk[U], vk[U], ro[U], io[U], wk[U];
+        bool live[U];
+#pragma unroll
+        for (int j = 0; j < U; ++j) {
+            const long long k = k0 + (long long)j * blockDim.x;
+            live[j] = k < M;
+            uk[j] = vk[j] = ro[j] = io[j] = wk[j] = 0.0;
+            if (live[j]) {
+                uk[j] = (double)__ldcs(u + k);
+                vk[j] = (double)__ldcs(v + k);
+                if (DO_CHI2) {
+                    ro[j] = (double)__ldcs(re_obs + k);
+                    io[j] = (double)__ldcs(im_obs + k);
+                    wk[j] = (double)__ldcs(wgt + k);
+                }
+            }
         }
-        const double ax = 1.0 - tx, ay = 1.0 - ty;
-        double ReInt = ay * (ax * (double)g00.x + tx * (double)g01.x) + ty * (ax * (double)g10.x + tx * (double)g11.x);
-        double ImInt = ay * (ax * (double)g00.y + tx * (double)g01.y) + ty * (ax * (double)g10.y + tx * (double)g11.y);
-        if (uneg) ImInt = -ImInt;
-        double vr = ReInt, vi = ImInt;
-        if (p.has_phase) {
-            const double theta = __dadd_rn(__dmul_rn(urot, p.dRArot), __dmul_rn(vrot, p.dDecrot));
-            double s, co;
-            sincos(theta, &s, &co);
-            vr = ReInt * co - ImInt * s;
-            vi = ReInt * s + ImInt * co;
+        double urot[U], vrot[U], tx[U], ty[U];
+        bool uneg[U];
+        cx<T> g00[U], g01[U], g10[U], g11[U];   // g{row offset}{col offset}
+#pragma unroll
+        for (int j = 0; j < U; ++j) {
+            // PAPER.md:667-668 (Eq. 11-12)
+            urot[j] = __dsub_rn(__dmul_rn(uk[j], p.cos_PA), __dmul_rn(vk[j], p.sin_PA));
+            vrot[j] = __dadd_rn(__dmul_rn(uk[j], p.sin_PA), __dmul_rn(vk[j], p.cos_PA));
+            // PAPER.md:676-683
+            const double urot_idx = div_by(fabs(urot[j]), p.du, p.rdu, p.du_exact_div);
+            uneg[j] = urot[j] < 0.0;
+            const double vq = div_by(vrot[j], p.du, p.rdu, p.du_exact_div);
+            const double vrot_idx = uneg[j] ? __dsub_rn(fH, vq) : __dadd_rn(fH, vq);
+            if (live[j] && (urot_idx > fH || vrot_idx < 0.0 || vrot_idx > (double)(N - 1))) ++oob;
+            // bilinear interpolation
+            const double fx0 = floor(urot_idx), fy0 = floor(vrot_idx);
+            const long long ix = (long long)fx0, iy = (long long)fy0;
+            tx[j] = __dsub_rn(urot_idx, fx0);
+            ty[j] = __dsub_rn(vrot_idx, fy0);
+            if (ix + 1 <= H && iy >= 0 && iy + 1 <= N - 1) {
+                const cx<T>* b0 = spec + ix * N + iy;
+                g00[j] = __ldg(b0);
+                g10[j] = __ldg(b0 + 1);
+                g01[j] = __ldg(b0 + N);
+                g11[j] = __ldg(b0 + N + 1);
+            } else {
+                g00[j] = node_any<T>(spec, N, iy, ix);
+                g01[j] = node_any<T>(spec, N, iy, ix + 1);
+                g10[j] = node_any<T>(spec, N, iy + 1, ix);
+                g11[j] = node_any<T>(spec, N, iy + 1, ix + 1);
+            }
         }
-        if (WRITE_VIS) {
-            cx<T>* out = reinterpret_cast<cx<T>*>(p.vis) + c * M + k;
-            __stcs(out, mk<T>((T)vr, (T)vi));
-        }
-        if (DO_CHI2) {                                          // PAPER.md:718 (Eq. 10)
-            const double dr = vr - (double)__ldcs(p.re_obs + c * M + k);
-            const double di = vi - (double)__ldcs(p.im_obs + c * M + k);
-            acc += (dr * dr + di * di) * (double)__ldcs(p.w + c * M + k);
+#pragma unroll
+        for (int j = 0; j < U; ++j) {
+            const double ax = 1.0 - tx[j], ay = 1.0 - ty[j];
+            double ReInt = ay * (ax * (double)g00[j].x + tx[j] * (double)g01[j].x) +
+                           ty[j] * (ax * (double)g10[j].x + tx[j] * (double)g11[j].x);
+            double ImInt = ay * (ax * (double)g00[j].y + tx[j] * (double)g01[j].y) +
+                           ty[j] * (ax * (double)g10[j].y + tx[j] * (double)g11[j].y);
+            if (uneg[j]) ImInt = -ImInt;
+            double vr = ReInt, vi = ImInt;
+            if (p.has_phase) {
+                const double theta = __dadd_rn(__dmul_rn(urot[j], p.dRArot), __dmul_rn(vrot[j], p.dDecrot));
+                double sn, co;
+                sincos(theta, &sn, &co);
+                vr = ReInt * co - ImInt * sn;
+                vi = ReInt * sn + ImInt * co;
+            }
+            if (WRITE_VIS && live[j]) {
+                cx<T>* out = reinterpret_cast<cx<T>*>(p.vis) + c * M + k0 + (long long)j * blockDim.x;
+                __stcs(out, mk<T>((T)vr, (T)vi));
+            }
+            if (DO_CHI2) {                                      // PAPER.md:718 (Eq. 10); wk = 0 for dead slots
+                const double dr = vr - ro[j];
+                const double di = vi - io[j];
+                acc += (dr * dr + di * di) * wk[j];
+            }
         }
     }
 
