@@ -8,8 +8,11 @@ from typing import Optional
 import numpy as np
 import torch
 
+import os
+
 _HERE = Path(__file__).resolve().parent
-_LIB_PATH = _HERE / "libgalario_b200.so"
+# GALARIO_B200_LIB points at another build of the same library (e.g. one compiled with different -D tuning flags).
+_LIB_PATH = Path(os.environ.get("GALARIO_B200_LIB", _HERE / "libgalario_b200.so"))
 _lib: Optional[ctypes.CDLL] = None
 
 _vp, _i, _d, _i64 = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_int64

@@ -42,9 +42,10 @@ __device__ __forceinline__ double div_by(double a, double b, double r, int exact
 }
 
 // Node (row = shifted v index, col = u index) of the spectrum extended to all integers by the
-// periodicity and Hermitian symmetry of the DFT of a real image (reading A6).
+// periodicity and Hermitian symmetry of the DFT of a real image (reading A6).  Rare path (points
+// beyond the half-plane grid), kept out of line.
 template <typename T>
-__device__ __forceinline__ cx<T> node_any(const cx<T>* __restrict__ spec, int N, long long row, long long col) {
+__device__ __noinline__ cx<T> node_any(const cx<T>* __restrict__ spec, int N, long long row, long long col) {
     const int H = N >> 1;
     long long kv = row - H;
     long long cu = col & (long long)(N - 1);          // N is a power of two: floor-mod
@@ -58,13 +59,47 @@ __device__ __forceinline__ cx<T> node_any(const cx<T>* __restrict__ spec, int N,
     return g;
 }
 
-// Points per thread and loop trip.  All streamed inputs of the U points are requested first, then the
-// 4U spectrum nodes, then the arithmetic: three dependent memory latencies per trip instead of per point.
-constexpr int SAMPLE_U = 2;
+// Points per thread and loop trip (U), and resident CTAs per SM the register budget is set for.
+// Per trip: the streamed inputs of the NEXT trip are requested first (register double buffer), then
+// the 4U spectrum nodes of this trip, then the arithmetic — so the DRAM latency of the per-point
+// arrays is off the critical path and only the (mostly L2-resident) gather latency is exposed.
+#ifndef GAL_SAMPLE_U
+#define GAL_SAMPLE_U 2
+#endif
+#ifndef GAL_SAMPLE_MINB
+#define GAL_SAMPLE_MINB 2
+#endif
 
+template <typename T, bool DO_CHI2> struct PointIn {
+    double u, v, ro, io, w;
+};
+
+template <typename T, bool DO_CHI2>
+__device__ __forceinline__ void load_point(PointIn<T, DO_CHI2>& q, const T* __restrict__ u, const T* __restrict__ v,
+                                           const T* __restrict__ re, const T* __restrict__ im,
+                                           const T* __restrict__ w, long long k, long long M) {
+    q.u = q.v = q.ro = q.io = q.w = 0.0;            // dead slots: index (0, N/2), weight 0
+    if (k < M) {
+        q.u = (double)__ldcs(u + k);
+        q.v = (double)__ldcs(v + k);
+        if (DO_CHI2) {
+            q.ro = (double)__ldcs(re + k);
+            q.io = (double)__ldcs(im + k);
+            q.w = (double)__ldcs(w + k);
+        }
+    }
+}
+
+// Gather by lane pairs.  The four nodes of a cell are two 32-byte runs (kvs, kvs+1 at ku and at ku+1) in
+// the u-major spectrum.  A warp-wide 16-byte load of 32 unrelated addresses costs the L1 32 tag look-ups,
+// and with four of them per point that look-up rate (one line per clock and SM) is what bounds the kernel,
+// not HBM.  So lanes 2i and 2i+1 fetch each other's cells together: in every load instruction the even
+// lane reads node kvs and the odd lane node kvs+1 of the SAME cell — one line per lane pair, 16-18 lines
+// per instruction instead of 32.  Each lane then forms the u-direction interpolation of its row for both
+// cells, one shuffle hands the row the partner needs across, and the owner finishes its own point.
 template <typename T, bool WRITE_VIS, bool DO_CHI2>
-__global__ void __launch_bounds__(256) sample_kernel(const SampleParams<T> p) {
-    constexpr int U = SAMPLE_U;
+__global__ void __launch_bounds__(256, GAL_SAMPLE_MINB) sample_kernel(const SampleParams<T> p) {
+    constexpr int U = GAL_SAMPLE_U;
     const int c = blockIdx.y;
     const int N = p.N, H = N >> 1;
     const long long M = p.M;
@@ -74,68 +109,77 @@ __global__ void __launch_bounds__(256) sample_kernel(const SampleParams<T> p) {
     const T* __restrict__ re_obs = DO_CHI2 ? p.re_obs + c * M : nullptr;
     const T* __restrict__ im_obs = DO_CHI2 ? p.im_obs + c * M : nullptr;
     const T* __restrict__ wgt = DO_CHI2 ? p.w + c * M : nullptr;
-    const double fH = (double)H;
+    const double fH = (double)H, fN1 = (double)(N - 1);
+    const int odd = threadIdx.x & 1;
 
     double acc = 0.0;
     unsigned int oob = 0;
     const long long stride = (long long)gridDim.x * blockDim.x * U;
-    for (long long k0 = (long long)blockIdx.x * blockDim.x * U + threadIdx.x; k0 < M; k0 += stride) {
-        double uk[U], vk[U], ro[U], io[U], wk[U];
-        bool live[U];
+    long long k0 = (long long)blockIdx.x * blockDim.x * U + threadIdx.x;
+    long long kw = k0 - (threadIdx.x & 31);                 // warp-uniform: every lane takes every trip
+    PointIn<T, DO_CHI2> nxt[U];
 #pragma unroll
-        for (int j = 0; j < U; ++j) {
-            const long long k = k0 + (long long)j * blockDim.x;
-            live[j] = k < M;
-            uk[j] = vk[j] = ro[j] = io[j] = wk[j] = 0.0;
-            if (live[j]) {
-                uk[j] = (double)__ldcs(u + k);
-                vk[j] = (double)__ldcs(v + k);
-                if (DO_CHI2) {
-                    ro[j] = (double)__ldcs(re_obs + k);
-                    io[j] = (double)__ldcs(im_obs + k);
-                    wk[j] = (double)__ldcs(wgt + k);
-                }
-            }
-        }
-        double urot[U], vrot[U], tx[U], ty[U];
-        bool uneg[U];
-        cx<T> g00[U], g01[U], g10[U], g11[U];   // g{row offset}{col offset}
+    for (int j = 0; j < U; ++j) load_point<T, DO_CHI2>(nxt[j], u, v, re_obs, im_obs, wgt, k0 + (long long)j * blockDim.x, M);
+    for (; kw < M; kw += stride, k0 += stride) {
+        PointIn<T, DO_CHI2> cur[U];
+#pragma unroll
+        for (int j = 0; j < U; ++j) cur[j] = nxt[j];
+#pragma unroll
+        for (int j = 0; j < U; ++j)
+            load_point<T, DO_CHI2>(nxt[j], u, v, re_obs, im_obs, wgt, k0 + stride + (long long)j * blockDim.x, M);
+
+        double urot[U], vrot[U], tx[U], ty[U], uidx[U], vidx[U];
+        bool uneg[U], inside[U];
+        cx<T> ga0[U], ga1[U], gb0[U], gb1[U];   // even lane's cell (a) / odd lane's cell (b); column ku+0 / ku+1
 #pragma unroll
         for (int j = 0; j < U; ++j) {
             // PAPER.md:667-668 (Eq. 11-12)
-            urot[j] = __dsub_rn(__dmul_rn(uk[j], p.cos_PA), __dmul_rn(vk[j], p.sin_PA));
-            vrot[j] = __dadd_rn(__dmul_rn(uk[j], p.sin_PA), __dmul_rn(vk[j], p.cos_PA));
+            urot[j] = __dsub_rn(__dmul_rn(cur[j].u, p.cos_PA), __dmul_rn(cur[j].v, p.sin_PA));
+            vrot[j] = __dadd_rn(__dmul_rn(cur[j].u, p.sin_PA), __dmul_rn(cur[j].v, p.cos_PA));
             // PAPER.md:676-683
-            const double urot_idx = div_by(fabs(urot[j]), p.du, p.rdu, p.du_exact_div);
+            uidx[j] = div_by(fabs(urot[j]), p.du, p.rdu, p.du_exact_div);
             uneg[j] = urot[j] < 0.0;
             const double vq = div_by(vrot[j], p.du, p.rdu, p.du_exact_div);
-            const double vrot_idx = uneg[j] ? __dsub_rn(fH, vq) : __dadd_rn(fH, vq);
-            if (live[j] && (urot_idx > fH || vrot_idx < 0.0 || vrot_idx > (double)(N - 1))) ++oob;
+            vidx[j] = uneg[j] ? __dsub_rn(fH, vq) : __dadd_rn(fH, vq);
             // bilinear interpolation
-            const double fx0 = floor(urot_idx), fy0 = floor(vrot_idx);
-            const long long ix = (long long)fx0, iy = (long long)fy0;
-            tx[j] = __dsub_rn(urot_idx, fx0);
-            ty[j] = __dsub_rn(vrot_idx, fy0);
-            if (ix + 1 <= H && iy >= 0 && iy + 1 <= N - 1) {
-                const cx<T>* b0 = spec + ix * N + iy;
-                g00[j] = __ldg(b0);
-                g10[j] = __ldg(b0 + 1);
-                g01[j] = __ldg(b0 + N);
-                g11[j] = __ldg(b0 + N + 1);
-            } else {
-                g00[j] = node_any<T>(spec, N, iy, ix);
-                g01[j] = node_any<T>(spec, N, iy, ix + 1);
-                g10[j] = node_any<T>(spec, N, iy + 1, ix);
-                g11[j] = node_any<T>(spec, N, iy + 1, ix + 1);
-            }
+            const double fx0 = floor(uidx[j]), fy0 = floor(vidx[j]);
+            tx[j] = __dsub_rn(uidx[j], fx0);
+            ty[j] = __dsub_rn(vidx[j], fy0);
+            inside[j] = uidx[j] <= fH - 1.0 && vidx[j] >= 0.0 && vidx[j] < fN1;     // cell fully inside the grid
+            const int off = inside[j] ? (int)fx0 * N + (int)fy0 : 0;
+            const int off_partner = __shfl_xor_sync(0xffffffffu, off, 1);
+            const cx<T>* pa = spec + ((odd ? off_partner : off) + odd);
+            const cx<T>* pb = spec + ((odd ? off : off_partner) + odd);
+            ga0[j] = __ldg(pa);
+            ga1[j] = __ldg(pa + N);
+            gb0[j] = __ldg(pb);
+            gb1[j] = __ldg(pb + N);
         }
 #pragma unroll
         for (int j = 0; j < U; ++j) {
-            const double ax = 1.0 - tx[j], ay = 1.0 - ty[j];
-            double ReInt = ay * (ax * (double)g00[j].x + tx[j] * (double)g01[j].x) +
-                           ty[j] * (ax * (double)g10[j].x + tx[j] * (double)g11[j].x);
-            double ImInt = ay * (ax * (double)g00[j].y + tx[j] * (double)g01[j].y) +
-                           ty[j] * (ax * (double)g10[j].y + tx[j] * (double)g11[j].y);
+            const double tx_partner = __shfl_xor_sync(0xffffffffu, tx[j], 1);
+            const double txa = odd ? tx_partner : tx[j], txb = odd ? tx[j] : tx_partner;
+            const double axa = 1.0 - txa, axb = 1.0 - txb;
+            // this lane's row (kvs + odd) of both cells, interpolated along u
+            const double ra_re = axa * (double)ga0[j].x + txa * (double)ga1[j].x;
+            const double ra_im = axa * (double)ga0[j].y + txa * (double)ga1[j].y;
+            const double rb_re = axb * (double)gb0[j].x + txb * (double)gb1[j].x;
+            const double rb_im = axb * (double)gb0[j].y + txb * (double)gb1[j].y;
+            // the even lane needs row kvs+1 of cell a, the odd lane row kvs of cell b
+            const double o_re = __shfl_xor_sync(0xffffffffu, odd ? ra_re : rb_re, 1);
+            const double o_im = __shfl_xor_sync(0xffffffffu, odd ? ra_im : rb_im, 1);
+            const double ay = 1.0 - ty[j];
+            double ReInt = odd ? ay * o_re + ty[j] * rb_re : ay * ra_re + ty[j] * o_re;
+            double ImInt = odd ? ay * o_im + ty[j] * rb_im : ay * ra_im + ty[j] * o_im;
+            if (!inside[j]) {           // rare: the cell leaves the half-plane grid (reading A6); dead slots never get here
+                const long long ix = (long long)floor(uidx[j]), iy = (long long)floor(vidx[j]);
+                if (uidx[j] > fH || vidx[j] < 0.0 || vidx[j] > fN1) ++oob;
+                const cx<T> g00 = node_any<T>(spec, N, iy, ix), g01 = node_any<T>(spec, N, iy, ix + 1);
+                const cx<T> g10 = node_any<T>(spec, N, iy + 1, ix), g11 = node_any<T>(spec, N, iy + 1, ix + 1);
+                const double ax = 1.0 - tx[j];
+                ReInt = ay * (ax * (double)g00.x + tx[j] * (double)g01.x) + ty[j] * (ax * (double)g10.x + tx[j] * (double)g11.x);
+                ImInt = ay * (ax * (double)g00.y + tx[j] * (double)g01.y) + ty[j] * (ax * (double)g10.y + tx[j] * (double)g11.y);
+            }
             if (uneg[j]) ImInt = -ImInt;
             double vr = ReInt, vi = ImInt;
             if (p.has_phase) {
@@ -145,14 +189,14 @@ __global__ void __launch_bounds__(256) sample_kernel(const SampleParams<T> p) {
                 vr = ReInt * co - ImInt * sn;
                 vi = ReInt * sn + ImInt * co;
             }
-            if (WRITE_VIS && live[j]) {
-                cx<T>* out = reinterpret_cast<cx<T>*>(p.vis) + c * M + k0 + (long long)j * blockDim.x;
-                __stcs(out, mk<T>((T)vr, (T)vi));
+            if (WRITE_VIS) {
+                const long long k = k0 + (long long)j * blockDim.x;
+                if (k < M) __stcs(reinterpret_cast<cx<T>*>(p.vis) + c * M + k, mk<T>((T)vr, (T)vi));
             }
-            if (DO_CHI2) {                                      // PAPER.md:718 (Eq. 10); wk = 0 for dead slots
-                const double dr = vr - ro[j];
-                const double di = vi - io[j];
-                acc += (dr * dr + di * di) * wk[j];
+            if (DO_CHI2) {                                      // PAPER.md:718 (Eq. 10); w = 0 for dead slots
+                const double dr = vr - cur[j].ro;
+                const double di = vi - cur[j].io;
+                acc += (dr * dr + di * di) * cur[j].w;
             }
         }
     }
