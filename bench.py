@@ -53,13 +53,20 @@ def measured_peaks():
 
 
 def ncu_traffic(kernel: str):
-    """DRAM bytes per launch from the committed ncu --set full summary, or None."""
-    path = os.path.join(ROOT, "profiles", "ncu_traffic.json")
-    try:
-        with open(path) as f:
-            return json.load(f).get(kernel)
-    except (OSError, ValueError):
-        return None
+    """DRAM bytes per launch (read + write) of `kernel` from the newest committed `ncu --set full` summary
+    (profiles/*_ncu_traffic.csv: kernel,dram_bytes_read,dram_bytes_write,gpu_time_us), or None."""
+    import csv
+    import glob
+    best = None
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_ncu_traffic.csv"))):
+        try:
+            with open(path) as f:
+                for row in csv.DictReader(f):
+                    if row["kernel"].startswith(kernel):
+                        best = int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
+        except (OSError, ValueError, KeyError):
+            continue
+    return best
 
 
 class ClockSampler:
