@@ -70,11 +70,24 @@ const char* gal_strerror(int code);
 /* Number of kernels the plan has launched since it was created (for launch accounting). */
 int64_t gal_plan_launch_count(const gal_plan* plan);
 
+/* Pruned transform (not in the paper, changes no result).  The bilinear gather only
+ * reads the part of the half plane the (u, v) set reaches (Eq. 19 of the paper, keeps it
+ * inside a quarter of the grid).  With pruning on, a call first reduces the point set to its extent
+ * {largest column ku, first and last shifted row kvs} with the sampler's own index arithmetic, and the FFT
+ * passes neither form nor write what lies outside it.  mode 0 = never, 1 = automatic (default: prune when
+ * re-reading u and v costs less than a quarter of the three spectrum passes it can save), 2 = always.
+ * A point whose cell leaves the grid (reading A6) makes the extent the whole half plane. */
+int gal_plan_set_pruning(gal_plan* plan, int mode);
+/* extent[3] (host) = {kumax, kvs_min, kvs_max} used by the most recent sample/chi2 call (the whole half plane
+ * {nxy/2, 0, nxy-1} if that call did not prune).  Synchronises the stream of that call. */
+int gal_last_uv_extent(gal_plan* plan, int* extent);
+
 /* Diagnostic per-kernel timing.  After gal_plan_timing_enable(plan, n) the next n sample/chi2 calls record a
- * CUDA event on their stream before the row pass, between the kernels and after the sampling kernel
+ * CUDA event on their stream before the first kernel, between the kernels and after the sampling kernel
  * (n = 0 switches it off and frees the events).  gal_plan_timing_read synchronises those events and returns
- * the average duration in milliseconds of the row pass, the column pass and the sampling kernel
- * (ms_per_kernel[3]) over the calls recorded so far (*calls, may be null). */
+ * the average duration in milliseconds of the uv-extent kernel (0 when the call did not prune), the row
+ * pass, the column pass and the sampling kernel (ms_per_kernel[4]) over the calls recorded so far (*calls,
+ * may be null). */
 int gal_plan_timing_enable(gal_plan* plan, int max_calls);
 int gal_plan_timing_read(gal_plan* plan, double* ms_per_kernel, int64_t* calls);
 

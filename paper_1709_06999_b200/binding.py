@@ -44,6 +44,8 @@ def load_library() -> ctypes.CDLL:
             getattr(lib, name).argtypes = [_vp]
         lib.gal_plan_timing_enable.argtypes = [_vp, _i]
         lib.gal_plan_timing_read.argtypes = [_vp, _vp, _vp]
+        lib.gal_plan_set_pruning.argtypes = [_vp, _i]
+        lib.gal_last_uv_extent.argtypes = [_vp, _vp]
         for s in ("f64", "f32"):
             getattr(lib, f"gal_sweep_{s}").argtypes = [_vp, _vp, _i, _d, _d, _d, _d, _vp, _vp]
             getattr(lib, f"gal_fft2_shifted_{s}").argtypes = [_vp, _vp, _vp, _vp]
@@ -121,12 +123,23 @@ class Plan:
         _check(self._lib.gal_plan_timing_enable(self._h, int(max_calls)), "gal_plan_timing_enable", self)
 
     def timing_read(self):
-        """Average ms of (row pass, column pass, sampling kernel) over the recorded calls, and their number."""
-        ms = (ctypes.c_double * 3)()
+        """Average ms of (uv-extent kernel, row pass, column pass, sampling kernel) over the recorded calls, and
+        their number."""
+        ms = (ctypes.c_double * 4)()
         n = ctypes.c_int64(0)
         _check(self._lib.gal_plan_timing_read(self._h, ctypes.addressof(ms), ctypes.addressof(n)),
                "gal_plan_timing_read", self)
-        return [ms[0], ms[1], ms[2]], n.value
+        return [ms[0], ms[1], ms[2], ms[3]], n.value
+
+    def set_pruning(self, mode: int) -> None:
+        """0 = never, 1 = automatic (default), 2 = always: see gal_plan_set_pruning."""
+        _check(self._lib.gal_plan_set_pruning(self._h, int(mode)), "gal_plan_set_pruning", self)
+
+    def last_uv_extent(self):
+        """(kumax, kvs_min, kvs_max) the most recent call's transform was pruned to."""
+        ext = (ctypes.c_int * 3)()
+        _check(self._lib.gal_last_uv_extent(self._h, ctypes.addressof(ext)), "gal_last_uv_extent", self)
+        return int(ext[0]), int(ext[1]), int(ext[2])
 
     # -- the paper's calls ---------------------------------------------------------------------
     def sweep(self, I, Rmin, dR, dxy, inc=0.0, out=None):

@@ -234,6 +234,7 @@ template <typename T> struct RowParams {
     const cx<T>* tw;       // exp(-2 pi i m / N), m = 0..N-1
     int N;
     int rows_total;        // batch * N
+    const int* ext;        // {largest column ku needed, first row kvs, last row kvs} (sample.cuh, uv extent)
     SweepParams sweep;
 };
 
@@ -286,7 +287,10 @@ row_pass_kernel(const RowParams<T> p) {
     const int i0 = (int)(row0 % N);
     cx<T>* out = p.spec + b_img * (long long)NU * N + i0;
     const int rows_here = (int)((p.rows_total - row0) < F ? (p.rows_total - row0) : F);
-    for (int idx = tid; idx < F * (L / 2 + 1); idx += G::NT) {
+    // columns beyond the uv extent are never sampled: neither formed nor written
+    const int kumax = __ldg(p.ext);
+    const int kend = kumax < L / 2 ? kumax : L / 2;
+    for (int idx = tid; idx < F * (kend + 1); idx += G::NT) {
         const int ff = idx % F, k = idx / F;
         if (ff >= rows_here) continue;
         const cx<T>* Sf = smem + ff * G::REGION;
@@ -299,7 +303,7 @@ row_pass_kernel(const RowParams<T> p) {
         cx<T> xm = csub(E, WO);
         xm.y = -xm.y;
         out[(long long)k * N + ff] = xk;
-        out[(long long)(L - k) * N + ff] = xm;
+        if (L - k <= kumax) out[(long long)(L - k) * N + ff] = xm;
     }
 }
 
@@ -311,6 +315,7 @@ template <typename T> struct ColParams {
     const cx<T>* tw;
     int N;
     long long cols_total;  // batch * (N/2+1)
+    const int* ext;        // as RowParams::ext
 };
 
 template <typename T, int R1, int R2, int R3, int F>
@@ -323,9 +328,20 @@ col_pass_kernel(const ColParams<T> p) {
     const int tid = threadIdx.x;
     const int f = tid / G::TPF, t = tid % G::TPF;
     const long long g = (long long)blockIdx.x * F + f;
-    const bool valid = g < p.cols_total;
     const int NU = L / 2 + 1;
     const int ku = (int)(g % NU);
+    // uv extent: columns beyond kumax are skipped, rows outside [rmin, rmax] are not written
+    const int kumax = __ldg(p.ext), rmin = __ldg(p.ext + 1), rmax = __ldg(p.ext + 2);
+    {
+        bool any = false;
+#pragma unroll
+        for (int ff = 0; ff < F; ++ff) {
+            const long long gg = (long long)blockIdx.x * F + ff;
+            any = any || (gg < p.cols_total && (int)(gg % NU) <= kumax);
+        }
+        if (!any) return;
+    }
+    const bool valid = g < p.cols_total && ku <= kumax;
     cx<T>* col = p.spec + (valid ? g : 0) * (long long)L;
     cx<T>* S = smem + f * G::REGION;
 
@@ -346,7 +362,8 @@ col_pass_kernel(const ColParams<T> p) {
             for (int d = 0; d < R3; ++d) {
                 const int kv = k1 + R1 * (c + R2 * d);
                 const T sgn = ((ku + kv) & 1) ? (T)-1 : (T)1;
-                col[(kv + L / 2) & (L - 1)] = mk<T>(sgn * a[d].x, sgn * a[d].y);
+                const int kvs = (kv + L / 2) & (L - 1);
+                if (kvs >= rmin && kvs <= rmax) col[kvs] = mk<T>(sgn * a[d].x, sgn * a[d].y);
             }
         }
     }

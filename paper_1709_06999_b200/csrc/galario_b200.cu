@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <set>
 #include <vector>
 
 #include "fft.cuh"
@@ -22,7 +23,14 @@ struct gal_plan {
     double* partials = nullptr;      // [batch][max_gx]
     unsigned int* tickets = nullptr; // [batch + 1]
     double* chi2_scratch = nullptr;  // [batch]
-    unsigned long long* oob = nullptr;
+    unsigned long long* oob = nullptr;   // call_state[0]; the uv extent follows it
+    int* ext = nullptr;                  // {kumax, rmin, rmax} of the current call (device)
+    int* ext_full = nullptr;             // constant {nxy/2, 0, nxy-1}: no pruning
+    void* call_state = nullptr;          // [oob (8 B) | ext (12 B) | pad] re-initialised per call from call_init
+    void* call_init = nullptr;
+    int prune_mode = 1;                  // 0 never, 1 auto, 2 always
+    bool last_pruned = false;            // did the most recent call compute a uv extent?
+    std::set<const void*> smem_set;      // kernels whose dynamic shared-memory limit has been raised
     int max_gx = 0;
     size_t owned_bytes = 0;
     int last_cuda = 0;
@@ -33,10 +41,10 @@ struct gal_plan {
     void* st_pts = nullptr;   size_t st_pts_bytes = 0;
     void* st_out = nullptr;   size_t st_out_bytes = 0;
     double* st_chi2 = nullptr;
-    // optional per-kernel timing (gal_plan_timing_enable): 4 events per call
+    // optional per-kernel timing (gal_plan_timing_enable): 5 events per call
     std::vector<cudaEvent_t> tev;
     int t_max_calls = 0, t_calls = 0;
-    cudaEvent_t* t_split = nullptr;  // when set, the row launcher records t_split[1] after its kernel
+    cudaEvent_t* t_split = nullptr;  // when set, the row launcher records t_split[2] after its kernel
 };
 
 namespace {
@@ -59,7 +67,10 @@ struct DeviceGuard {
 };
 
 template <typename K> int set_smem(gal_plan* p, K kernel, size_t bytes) {
-    if (bytes > 48 * 1024) GAL_CUDA(p, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    if (bytes > 48 * 1024 && !p->smem_set.count((const void*)kernel)) {
+        GAL_CUDA(p, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+        p->smem_set.insert((const void*)kernel);
+    }
     return GAL_OK;
 }
 
@@ -67,7 +78,7 @@ template <typename K> int set_smem(gal_plan* p, K kernel, size_t bytes) {
 // FFT launchers
 // ---------------------------------------------------------------------------------------------
 template <typename T, int R1, int R2, int R3, int F>
-int launch_row(gal_plan* p, const T* image, const SweepParams* sw, int batch, cudaStream_t st) {
+int launch_row(gal_plan* p, const T* image, const SweepParams* sw, int batch, const int* ext, cudaStream_t st) {
     using G = Geom<T, R1, R2, R3, F>;
     RowParams<T> rp;
     rp.image = image;
@@ -75,6 +86,7 @@ int launch_row(gal_plan* p, const T* image, const SweepParams* sw, int batch, cu
     rp.tw = (const cx<T>*)p->tw;
     rp.N = p->nxy;
     rp.rows_total = batch * p->nxy;
+    rp.ext = ext;
     if (sw) rp.sweep = *sw; else memset(&rp.sweep, 0, sizeof(rp.sweep));
     const unsigned grid = (unsigned)((rp.rows_total + F - 1) / F);
     if (sw) {
@@ -88,18 +100,19 @@ int launch_row(gal_plan* p, const T* image, const SweepParams* sw, int batch, cu
     }
     p->launches++;
     GAL_CUDA(p, cudaGetLastError());
-    if (p->t_split) GAL_CUDA(p, cudaEventRecord(p->t_split[1], st));
+    if (p->t_split) GAL_CUDA(p, cudaEventRecord(p->t_split[2], st));
     return GAL_OK;
 }
 
 template <typename T, int R1, int R2, int R3, int F>
-int launch_col(gal_plan* p, int batch, cudaStream_t st) {
+int launch_col(gal_plan* p, int batch, const int* ext, cudaStream_t st) {
     using G = Geom<T, R1, R2, R3, F>;
     ColParams<T> cp;
     cp.spec = (cx<T>*)p->spec;
     cp.tw = (const cx<T>*)p->tw;
     cp.N = p->nxy;
     cp.cols_total = (long long)batch * (p->nxy / 2 + 1);
+    cp.ext = ext;
     const unsigned grid = (unsigned)((cp.cols_total + F - 1) / F);
     auto k = col_pass_kernel<T, R1, R2, R3, F>;
     int rc = set_smem(p, k, G::SMEM); if (rc) return rc;
@@ -111,13 +124,13 @@ int launch_col(gal_plan* p, int batch, cudaStream_t st) {
 
 // Radix plans.  Row FFT length is nxy/2, column FFT length is nxy.
 template <typename T>
-int fft2(gal_plan* p, const T* image, const SweepParams* sw, int batch, cudaStream_t st) {
+int fft2(gal_plan* p, const T* image, const SweepParams* sw, int batch, const int* ext, cudaStream_t st) {
     int rc;
     switch (p->nxy) {
 #define GAL_FFT_CASE(NXY, ROW, COL)                                         \
     case NXY:                                                               \
-        rc = launch_row<T, ROW>(p, image, sw, batch, st); if (rc) return rc; \
-        return launch_col<T, COL>(p, batch, st);
+        rc = launch_row<T, ROW>(p, image, sw, batch, ext, st); if (rc) return rc; \
+        return launch_col<T, COL>(p, batch, ext, st);
 #define RR(...) __VA_ARGS__
         GAL_FFT_CASE(8, RR(4, 1, 1, 8), RR(8, 1, 1, 8))
         GAL_FFT_CASE(16, RR(8, 1, 1, 16), RR(16, 1, 1, 16))
@@ -137,14 +150,86 @@ int fft2(gal_plan* p, const T* image, const SweepParams* sw, int batch, cudaStre
 }
 
 // ---------------------------------------------------------------------------------------------
-// sampling launcher
+// per-call scalars, uv extent, sampling launcher
 // ---------------------------------------------------------------------------------------------
+struct CallScalars {
+    double du, rdu, cos_PA, sin_PA, dRA_turns, dDec_turns;
+    int du_exact_div, has_phase;
+};
+
+// host-side scalars, plain double arithmetic in the listing's order.  The
+// phase offsets are kept in turns (the listing's 2 pi factor is applied inside sincospi, exactly).
+CallScalars call_scalars(const gal_plan* p, double dxy, double dRA, double dDec, double PA) {
+    CallScalars cs;
+    cs.du = 1.0 / ((double)p->nxy * dxy);
+    cs.rdu = 1.0 / cs.du;
+    // Markstein's shortcut needs a divisor whose significand is not all ones
+    uint64_t bits; memcpy(&bits, &cs.du, 8);
+    cs.du_exact_div = ((bits & 0xFFFFFFFFFFFFFull) == 0xFFFFFFFFFFFFFull) || !std::isnormal(cs.du) || !std::isnormal(cs.rdu);
+    cs.cos_PA = std::cos(PA);
+    cs.sin_PA = std::sin(PA);
+    cs.dRA_turns = dRA * cs.cos_PA - dDec * cs.sin_PA;
+    cs.dDec_turns = dRA * cs.sin_PA + dDec * cs.cos_PA;
+    cs.has_phase = !(cs.dRA_turns == 0.0 && cs.dDec_turns == 0.0);
+    return cs;
+}
+
+// Re-arm the per-call device state: out-of-grid counter = 0, uv extent = the cell of the dead slots
+// (column 0..1, rows N/2..N/2+1), which the sampler reads with weight 0 for the points past the end.
+int reset_call_state(gal_plan* p, cudaStream_t st) {
+    GAL_CUDA(p, cudaMemcpyAsync(p->call_state, p->call_init, 32, cudaMemcpyDeviceToDevice, st));
+    return GAL_OK;
+}
+
+// Should this call compute the uv extent and prune the transform?  The extent pass re-reads u and v
+// (2 sizeof(T) M bytes per channel); pruning can save up to three passes over the spectrum.
 template <typename T>
-int launch_sample(gal_plan* p, int C, double dxy, const T* u, const T* v, const T* re, const T* im, const T* w,
-                  int64_t M, double dRA, double dDec, double PA, T* vis, double* chi2_pc, double* chi2_tot,
-                  cudaStream_t st) {
+bool want_prune(const gal_plan* p, int C, int64_t M) {
+    if (p->prune_mode == 0 || M <= 0) return false;
+    if (p->prune_mode == 2) return true;
+    const double ext_bytes = 2.0 * sizeof(T) * (double)M * C;
+    const double spec_bytes = 2.0 * sizeof(T) * (double)(p->nxy / 2 + 1) * p->nxy * C;
+    return ext_bytes <= 0.25 * 3.0 * spec_bytes;
+}
+
+template <typename T>
+int launch_extent(gal_plan* p, int C, const CallScalars& cs, const T* u, const T* v, int64_t M, cudaStream_t st) {
+    ExtentParams ep;
+    ep.N = p->nxy;
+    ep.total = (long long)C * M;
+    ep.du = cs.du; ep.rdu = cs.rdu; ep.du_exact_div = cs.du_exact_div;
+    ep.cos_PA = cs.cos_PA; ep.sin_PA = cs.sin_PA;
+    ep.ext = p->ext;
+    long long blocks = (ep.total + 1023) / 1024;
+    const long long cap = (long long)p->sm_count * 8;
+    if (blocks > cap) blocks = cap;
+    if (blocks < 1) blocks = 1;
+    uv_extent_kernel<T><<<(unsigned)blocks, 256, 0, st>>>(ep, u, v);
+    p->launches++;
+    GAL_CUDA(p, cudaGetLastError());
+    return GAL_OK;
+}
+
+inline bool aligned16(const void* q) { return ((uintptr_t)q & 15u) == 0; }
+
+template <typename T, bool WRITE_VIS, bool DO_CHI2>
+int launch_sample_kernel(gal_plan* p, const SampleParams<T>& sp, dim3 grid, bool tma, cudaStream_t st) {
+    using G = SampleGeom<T, DO_CHI2>;
+    if (tma) {
+        auto k = sample_kernel<T, WRITE_VIS, DO_CHI2, true>;
+        int rc = set_smem(p, k, G::SMEM); if (rc) return rc;
+        k<<<grid, 256, G::SMEM, st>>>(sp);
+    } else {
+        auto k = sample_kernel<T, WRITE_VIS, DO_CHI2, false>;
+        k<<<grid, 256, 0, st>>>(sp);
+    }
+    return GAL_OK;
+}
+
+template <typename T>
+int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T* v, const T* re, const T* im,
+                  const T* w, int64_t M, T* vis, double* chi2_pc, double* chi2_tot, cudaStream_t st) {
     const bool do_chi2 = (vis == nullptr);
-    GAL_CUDA(p, cudaMemsetAsync(p->oob, 0, sizeof(unsigned long long), st));
     if (M == 0) {
         if (chi2_pc) GAL_CUDA(p, cudaMemsetAsync(chi2_pc, 0, sizeof(double) * C, st));
         if (chi2_tot) GAL_CUDA(p, cudaMemsetAsync(chi2_tot, 0, sizeof(double), st));
@@ -155,57 +240,64 @@ int launch_sample(gal_plan* p, int C, double dxy, const T* u, const T* v, const 
     sp.N = p->nxy;
     sp.M = M;
     sp.u = u; sp.v = v; sp.re_obs = re; sp.im_obs = im; sp.w = w; sp.vis = vis;
-    // host-side scalars, plain double arithmetic in the listing's order
-    const double two_pi = 2.0 * 3.14159265358979323846;
-    const double dRA2 = dRA * 2.0 * 3.14159265358979323846;
-    const double dDec2 = dDec * 2.0 * 3.14159265358979323846;
-    (void)two_pi;
-    sp.du = 1.0 / ((double)p->nxy * dxy);
-    sp.rdu = 1.0 / sp.du;
-    {   // Markstein's shortcut needs a divisor whose significand is not all ones
-        uint64_t bits; memcpy(&bits, &sp.du, 8);
-        sp.du_exact_div = ((bits & 0xFFFFFFFFFFFFFull) == 0xFFFFFFFFFFFFFull) || !std::isnormal(sp.du) || !std::isnormal(sp.rdu);
-    }
-    sp.cos_PA = std::cos(PA);
-    sp.sin_PA = std::sin(PA);
-    sp.dRArot = dRA2 * sp.cos_PA - dDec2 * sp.sin_PA;
-    sp.dDecrot = dRA2 * sp.sin_PA + dDec2 * sp.cos_PA;
-    sp.has_phase = !(sp.dRArot == 0.0 && sp.dDecrot == 0.0);
+    sp.du = cs.du; sp.rdu = cs.rdu; sp.du_exact_div = cs.du_exact_div;
+    sp.cos_PA = cs.cos_PA; sp.sin_PA = cs.sin_PA;
+    sp.dRA_turns = cs.dRA_turns; sp.dDec_turns = cs.dDec_turns; sp.has_phase = cs.has_phase;
     sp.partials = p->partials;
     sp.tickets = p->tickets;
     sp.chi2_per_channel = chi2_pc;
     sp.chi2_total = chi2_tot;
     sp.oob = p->oob;
-    long long need = (M + 255) / 256;
-    long long cap = p->max_gx;
-    if (C > 1) { cap = (2LL * p->max_gx + C - 1) / C; if (cap > p->max_gx) cap = p->max_gx; }
-    long long gx = need < cap ? need : cap;
+    // one CTA works through tiles blockIdx.x, blockIdx.x + gridDim.x, ...: a whole number of CTAs per SM
+    const int tile = SampleGeom<T, true>::TILE;
+    const long long ntiles = (M + tile - 1) / tile;
+    long long cap = (long long)p->sm_count * GAL_SAMPLE_MINB;
+    if (C > 1) cap = (2 * cap + C - 1) / C;
+    if (cap > p->max_gx) cap = p->max_gx;
+    long long gx = ntiles < cap ? ntiles : cap;
     if (gx < 1) gx = 1;
     dim3 grid((unsigned)gx, (unsigned)C);
-    if (do_chi2) sample_kernel<T, false, true><<<grid, 256, 0, st>>>(sp);
-    else sample_kernel<T, true, false><<<grid, 256, 0, st>>>(sp);
+    // the TMA path needs 16-byte aligned tiles in every channel
+    bool tma = aligned16(u) && aligned16(v) && (C == 1 || ((size_t)M * sizeof(T)) % 16 == 0);
+    if (do_chi2) tma = tma && aligned16(re) && aligned16(im) && aligned16(w);
+    int rc = do_chi2 ? launch_sample_kernel<T, false, true>(p, sp, grid, tma, st)
+                     : launch_sample_kernel<T, true, false>(p, sp, grid, tma, st);
+    if (rc) return rc;
     p->launches++;
     GAL_CUDA(p, cudaGetLastError());
     return GAL_OK;
 }
 
-// Same launches with a CUDA event between the kernels (diagnostic mode, gal_plan_timing_enable).
+// One whole call: [uv extent] -> row pass -> column pass -> sampling, with (diagnostic mode,
+// gal_plan_timing_enable) a CUDA event between the kernels.
 template <typename T>
-int timed_call(gal_plan* p, const T* image, const SweepParams* sw, int C, double dxy, const T* u, const T* v,
-               const T* re, const T* im, const T* w, int64_t M, double dRA, double dDec, double PA, T* vis,
-               double* chi2_pc, double* chi2_tot, cudaStream_t st) {
-    cudaEvent_t* e = &p->tev[(size_t)4 * p->t_calls];
+int run_call(gal_plan* p, const T* image, const SweepParams* sw, int C, double dxy, const T* u, const T* v,
+             const T* re, const T* im, const T* w, int64_t M, double dRA, double dDec, double PA, T* vis,
+             double* chi2_pc, double* chi2_tot, cudaStream_t st) {
+    const CallScalars cs = call_scalars(p, dxy, dRA, dDec, PA);
+    const bool timed = p->t_calls < p->t_max_calls;
+    cudaEvent_t* e = timed ? &p->tev[(size_t)5 * p->t_calls] : nullptr;
     int rc;
-    GAL_CUDA(p, cudaEventRecord(e[0], st));
-    p->t_split = e;
-    rc = fft2<T>(p, image, sw, C, st);
-    p->t_split = nullptr;
-    if (rc) return rc;
-    GAL_CUDA(p, cudaEventRecord(e[2], st));
-    rc = launch_sample<T>(p, C, dxy, u, v, re, im, w, M, dRA, dDec, PA, vis, chi2_pc, chi2_tot, st);
-    if (rc) return rc;
-    GAL_CUDA(p, cudaEventRecord(e[3], st));
-    p->t_calls++;
+    if ((rc = reset_call_state(p, st))) return rc;
+    if (timed) GAL_CUDA(p, cudaEventRecord(e[0], st));
+    const int* ext = p->ext_full;
+    p->last_pruned = want_prune<T>(p, C, M);
+    if (p->last_pruned) {
+        if ((rc = launch_extent<T>(p, C, cs, u, v, M, st))) return rc;
+        ext = p->ext;
+    }
+    if (timed) GAL_CUDA(p, cudaEventRecord(e[1], st));
+    if (M > 0) {                                      // no points: nothing to transform for
+        p->t_split = e;
+        rc = fft2<T>(p, image, sw, C, ext, st);
+        p->t_split = nullptr;
+        if (rc) return rc;
+    } else if (timed) {
+        GAL_CUDA(p, cudaEventRecord(e[2], st));
+    }
+    if (timed) GAL_CUDA(p, cudaEventRecord(e[3], st));
+    if ((rc = launch_sample<T>(p, C, cs, u, v, re, im, w, M, vis, chi2_pc, chi2_tot, st))) return rc;
+    if (timed) { GAL_CUDA(p, cudaEventRecord(e[4], st)); p->t_calls++; }
     return GAL_OK;
 }
 
@@ -235,10 +327,7 @@ int do_sample_image(gal_plan* p, const T* image, const SweepParams* sw, int C, d
     DeviceGuard g(p->device);
     cudaStream_t st = (cudaStream_t)stream;
     p->last_stream = st;
-    if (p->t_calls < p->t_max_calls) return timed_call<T>(p, image, sw, C, dxy, u, v, re, im, w, M, dRA, dDec, PA, vis, chi2_pc, chi2_tot, st);
-    int rc = fft2<T>(p, image, sw, C, st);
-    if (rc) return rc;
-    return launch_sample<T>(p, C, dxy, u, v, re, im, w, M, dRA, dDec, PA, vis, chi2_pc, chi2_tot, st);
+    return run_call<T>(p, image, sw, C, dxy, u, v, re, im, w, M, dRA, dDec, PA, vis, chi2_pc, chi2_tot, st);
 }
 
 template <typename T>
@@ -263,7 +352,7 @@ int do_fft2_shifted(gal_plan* p, const T* image, T* out, void* stream) {
     DeviceGuard g(p->device);
     cudaStream_t st = (cudaStream_t)stream;
     p->last_stream = st;
-    int rc = fft2<T>(p, image, nullptr, 1, st);
+    int rc = fft2<T>(p, image, nullptr, 1, p->ext_full, st);
     if (rc) return rc;
     dim3 grid((p->nxy + 31) / 32, (p->nxy / 2 + 1 + 31) / 32), block(32, 8);
     transpose_to_paper_layout_kernel<T><<<grid, block, 0, st>>>((const cx<T>*)p->spec, (cx<T>*)out, p->nxy);
@@ -361,12 +450,24 @@ int gal_plan_create(gal_plan** out, int nxy, int batch, int precision_bits, int 
     if ((e = cudaMalloc((void**)&p->partials, sizeof(double) * (size_t)batch * p->max_gx)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     if ((e = cudaMalloc((void**)&p->tickets, sizeof(unsigned int) * (batch + 1))) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     if ((e = cudaMalloc((void**)&p->chi2_scratch, sizeof(double) * batch)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
-    if ((e = cudaMalloc((void**)&p->oob, sizeof(unsigned long long))) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
+    if ((e = cudaMalloc(&p->call_state, 32)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
+    if ((e = cudaMalloc(&p->call_init, 32)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
+    if ((e = cudaMalloc((void**)&p->ext_full, 16)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
+    p->oob = (unsigned long long*)p->call_state;
+    p->ext = (int*)((char*)p->call_state + 8);
+    {
+        int init[8] = {0, 0, /* ext: */ 1, nxy / 2, nxy / 2 + 1, 0, 0, 0};
+        int full[4] = {nxy / 2, 0, nxy - 1, 0};
+        if ((e = cudaMemcpy(p->call_init, init, 32, cudaMemcpyHostToDevice)) != cudaSuccess) return fail(GAL_ERR_CUDA, e);
+        if ((e = cudaMemcpy(p->call_state, init, 32, cudaMemcpyHostToDevice)) != cudaSuccess) return fail(GAL_ERR_CUDA, e);
+        if ((e = cudaMemcpy(p->ext_full, full, 16, cudaMemcpyHostToDevice)) != cudaSuccess) return fail(GAL_ERR_CUDA, e);
+    }
     if ((e = cudaMalloc((void**)&p->st_chi2, sizeof(double))) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     p->owned_bytes = spec_bytes + (size_t)nxy * esz + sizeof(double) * (size_t)batch * p->max_gx +
                      sizeof(unsigned int) * (batch + 1) + sizeof(double) * batch + 16;
     if ((e = cudaMemset(p->tickets, 0, sizeof(unsigned int) * (batch + 1))) != cudaSuccess) return fail(GAL_ERR_CUDA, e);
-    if ((e = cudaMemset(p->oob, 0, sizeof(unsigned long long))) != cudaSuccess) return fail(GAL_ERR_CUDA, e);
+    // the workspace starts as zeros (pruned calls leave parts of it unwritten; they are never sampled)
+    if ((e = cudaMemset(p->spec, 0, spec_bytes)) != cudaSuccess) return fail(GAL_ERR_CUDA, e);
     // twiddle table exp(-2 pi i m / nxy): evaluated in long double on the host, octant-exact
     std::vector<double> twd((size_t)2 * nxy);
     const long double PI = 3.14159265358979323846264338327950288L;
@@ -392,7 +493,7 @@ int gal_plan_destroy(gal_plan* p) {
     DeviceGuard g(p->device);
     cudaFree(p->spec); cudaFree(p->tw); cudaFree(p->partials); cudaFree(p->tickets); cudaFree(p->chi2_scratch);
     for (cudaEvent_t e : p->tev) cudaEventDestroy(e);
-    cudaFree(p->oob); cudaFree(p->st_image); cudaFree(p->st_pts); cudaFree(p->st_out); cudaFree(p->st_chi2);
+    cudaFree(p->call_state); cudaFree(p->call_init); cudaFree(p->ext_full); cudaFree(p->st_image); cudaFree(p->st_pts); cudaFree(p->st_out); cudaFree(p->st_chi2);
     delete p;
     return GAL_OK;
 }
@@ -404,7 +505,7 @@ int gal_plan_timing_enable(gal_plan* p, int max_calls) {
     p->tev.clear();
     p->t_calls = 0;
     p->t_max_calls = 0;
-    p->tev.resize((size_t)4 * max_calls);
+    p->tev.resize((size_t)5 * max_calls);
     for (auto& e : p->tev) GAL_CUDA(p, cudaEventCreate(&e));
     p->t_max_calls = max_calls;
     return GAL_OK;
@@ -413,18 +514,32 @@ int gal_plan_timing_enable(gal_plan* p, int max_calls) {
 int gal_plan_timing_read(gal_plan* p, double* ms_per_kernel, int64_t* calls) {
     if (!p || !ms_per_kernel) return GAL_ERR_INVALID_ARGUMENT;
     DeviceGuard g(p->device);
-    double acc[3] = {0, 0, 0};
+    double acc[4] = {0, 0, 0, 0};
     for (int c = 0; c < p->t_calls; ++c) {
-        cudaEvent_t* e = &p->tev[(size_t)4 * c];
-        GAL_CUDA(p, cudaEventSynchronize(e[3]));
-        for (int k = 0; k < 3; ++k) {
+        cudaEvent_t* e = &p->tev[(size_t)5 * c];
+        GAL_CUDA(p, cudaEventSynchronize(e[4]));
+        for (int k = 0; k < 4; ++k) {
             float ms = 0;
             GAL_CUDA(p, cudaEventElapsedTime(&ms, e[k], e[k + 1]));
             acc[k] += ms;
         }
     }
-    for (int k = 0; k < 3; ++k) ms_per_kernel[k] = p->t_calls ? acc[k] / p->t_calls : 0.0;
+    for (int k = 0; k < 4; ++k) ms_per_kernel[k] = p->t_calls ? acc[k] / p->t_calls : 0.0;
     if (calls) *calls = p->t_calls;
+    return GAL_OK;
+}
+
+int gal_plan_set_pruning(gal_plan* p, int mode) {
+    if (!p || mode < 0 || mode > 2) return GAL_ERR_INVALID_ARGUMENT;
+    p->prune_mode = mode;
+    return GAL_OK;
+}
+
+int gal_last_uv_extent(gal_plan* p, int* extent) {
+    if (!p || !extent) return GAL_ERR_INVALID_ARGUMENT;
+    DeviceGuard g(p->device);
+    GAL_CUDA(p, cudaStreamSynchronize(p->last_stream));
+    GAL_CUDA(p, cudaMemcpy(extent, p->last_pruned ? p->ext : p->ext_full, 3 * sizeof(int), cudaMemcpyDeviceToHost));
     return GAL_OK;
 }
 

@@ -283,6 +283,104 @@ def test_chi2_properties_on_gpu(g):
 
 
 # ---------------------------------------------------------------------------------------------
+# pruned transform and the two streaming paths of the sampler
+# ---------------------------------------------------------------------------------------------
+def numpy_extent(w, n):
+    """The listing's index arithmetic, operation by operation in numpy doubles."""
+    c, s = np.cos(w.PA), np.sin(w.PA)
+    du = 1.0 / (n * w.dxy)
+    urot, vrot = w.u * c - w.v * s, w.u * s + w.v * c
+    uidx = np.abs(urot) / du
+    vidx = np.where(urot < 0, n / 2 - vrot / du, n / 2 + vrot / du)
+    inside = (uidx <= n / 2 - 1.0) & (vidx >= 0.0) & (vidx < n - 1)
+    if not inside.all():
+        return (n // 2, 0, n - 1)
+    ix, iy = np.floor(uidx).astype(int), np.floor(vidx).astype(int)
+    # the cell of the dead slots (column 0..1, rows n/2..n/2+1) is always part of the extent
+    return (max(ix.max() + 1, 1), min(iy.min(), n // 2), max(iy.max() + 1, n // 2 + 1))
+
+
+@pytest.mark.parametrize("idx,kw", [(1, dict(nxy=512, M=50_001, nr=1000)), (2, dict(nxy=1024, M=200_003)),
+                                    (3, dict(nxy=2048, M=300_007, n_src=120)), (0, dict(nxy=256, M=10_000))])
+def test_pruned_transform_changes_nothing(g, idx, kw):
+    """The same call with the transform pruned to the uv extent and with the full transform: bit-identical
+    visibilities and chi2, and the extent is exactly what the index arithmetic of the listing gives."""
+    w = W.config(idx, **kw)
+    plan = g.Plan(w.nxy)
+    # poison the workspace with the spectrum of another image first
+    other = np.random.default_rng(5).standard_normal((w.nxy, w.nxy)) * 1e6
+    plan.set_pruning(0)
+    plan.sampleImage(dev(other), w.dxy, dev(w.u), dev(w.v), w.PA, w.dRA, w.dDec)
+    assert plan.last_uv_extent() == (w.nxy // 2, 0, w.nxy - 1)
+    res = {}
+    for mode in (2, 0, 1):
+        plan.set_pruning(mode)
+        res[mode] = run_gpu_on(plan, w)
+        if mode == 2:
+            assert plan.last_uv_extent() == numpy_extent(w, w.nxy)
+    for mode in (0, 1):
+        assert np.array_equal(res[2][0], res[mode][0])
+        assert res[2][1] == res[mode][1]
+        assert res[2][2] == res[mode][2]
+
+
+def run_gpu_on(plan, w):
+    t = dev
+    if w.entry == "chi2Profile":
+        vis = plan.sampleProfile(t(w.profile), w.Rmin, w.dR, w.dxy, t(w.u), t(w.v), w.inc, w.PA, w.dRA, w.dDec)
+        oob = plan.last_oob_count()
+        chi2 = plan.chi2Profile(t(w.profile), w.Rmin, w.dR, w.dxy, t(w.u), t(w.v), t(w.re_obs), t(w.im_obs), t(w.w),
+                                w.dRA, w.dDec, w.PA, w.inc)
+    else:
+        vis = plan.sampleImage(t(w.image), w.dxy, t(w.u), t(w.v), w.PA, w.dRA, w.dDec)
+        oob = plan.last_oob_count()
+        chi2 = plan.chi2Image(t(w.image), w.dxy, t(w.u), t(w.v), t(w.re_obs), t(w.im_obs), t(w.w), w.dRA, w.dDec, w.PA)
+    return vis.cpu().numpy(), float(chi2.cpu()[0]), oob
+
+
+def test_pruned_batch_and_f32(g):
+    w = W.config(4, nxy=256, M=20_000, C=4)
+    plan = g.Plan(w.nxy, 4)
+    out = {}
+    for mode in (0, 2):
+        plan.set_pruning(mode)
+        per, tot = plan.chi2ImageBatch(dev(w.image), w.dxy, dev(w.u), dev(w.v), dev(w.re_obs), dev(w.im_obs),
+                                       dev(w.w), w.dRA, w.dDec, w.PA)
+        out[mode] = (per.cpu().numpy(), float(tot.cpu()[0]))
+    assert np.array_equal(out[0][0], out[2][0]) and out[0][1] == out[2][1]
+    w3 = W.config(3, nxy=1024, M=100_003, n_src=50).as_f32()
+    p32 = g.Plan(w3.nxy, 1, torch.float32)
+    r = {}
+    for mode in (0, 2):
+        p32.set_pruning(mode)
+        r[mode] = run_gpu_on(p32, w3)
+    assert np.array_equal(r[0][0], r[2][0]) and r[0][1] == r[2][1]
+    ext = p32.last_uv_extent()
+    assert ext[0] < w3.nxy // 2 and ext[1] > 0 and ext[2] < w3.nxy - 1
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+def test_unaligned_arrays_take_the_plain_load_path(g, dtype):
+    """Tiles are streamed by TMA bulk copies when every per-point array is 16-byte aligned, by plain loads
+    otherwise; both give the same bits."""
+    w = W.config(3, nxy=512, M=70_001, n_src=30)
+    if dtype == torch.float32:
+        w = w.as_f32()
+    plan = g.Plan(w.nxy, 1, dtype)
+    arrs = [w.u, w.v, w.re_obs, w.im_obs, w.w]
+    al = [dev(a) for a in arrs]
+    un = [dev(np.concatenate([a[:1], a]))[1:] for a in arrs]              # data_ptr offset by one element
+    assert all(x.data_ptr() % 16 == 0 for x in al) and all(x.data_ptr() % 16 != 0 for x in un)
+    img = dev(w.image)
+    va = plan.sampleImage(img, w.dxy, al[0], al[1], w.PA, w.dRA, w.dDec)
+    vu = plan.sampleImage(img, w.dxy, un[0], un[1], w.PA, w.dRA, w.dDec)
+    assert torch.equal(va, vu)
+    ca = plan.chi2Image(img, w.dxy, *al, w.dRA, w.dDec, w.PA)
+    cu = plan.chi2Image(img, w.dxy, *un, w.dRA, w.dDec, w.PA)
+    assert float(ca.cpu()[0]) == float(cu.cpu()[0])
+
+
+# ---------------------------------------------------------------------------------------------
 # edge cases
 # ---------------------------------------------------------------------------------------------
 def test_edge_points_and_wrap(g, orc):
