@@ -1,7 +1,12 @@
 // fft.cuh — hand-written 2-D real-to-complex FFT for sm_100a (no cuFFT).
 //
 // Computes F = rfft2(fftshift(image)) followed by fftshift along axis 0,
-// stored u-major: spec[b][ku][kvs], ku = 0..N/2, kvs = (kv + N/2) mod N, complex<T>.
+// stored u-major as column pairs: pair[b][ku][kvs] = {F[ku][kvs], F[ku+1][kvs]}, ku = 0..N/2,
+// kvs = (kv + N/2) mod N — every value is stored twice (as .a of its own column and .b of the
+// column before), so the four nodes of an interpolation cell are two adjacent, sector-aligned
+// entries (64 contiguous bytes in fp64): exactly two 32-byte L2 sectors per sampled point instead
+// of three, and one 128-byte line instead of two (sample.cuh).  The row pass writes its
+// intermediate (the row-transformed image, transposed) to a separate u-major array work[b][ku][i].
 //   * S2 (centre shift of the image) is never a pass: for even N it equals multiplying the
 //     spectrum by (-1)^(ku+kv), applied in the last store of the column pass.
 //   * S4 (shift along v) is an index fold in that same store.
@@ -9,7 +14,7 @@
 //     transformed with an (N/2)-point complex FFT in shared memory and untangled into the N/2+1
 //     half-spectrum values; F rows per CTA are written TRANSPOSED (F*16 B contiguous per ku) so the
 //     column pass reads and writes contiguous 16*N-byte columns.  L2 merges the partial lines.
-//   * Column pass: in place, one column per FFT, three radix passes through shared memory.
+//   * Column pass: work -> pair, one column per FFT, three radix passes through shared memory.
 //   * With SWEEP the row loader evaluates the swept profile instead of reading an
 //     image, so *Profile calls never materialise the image.
 //
@@ -31,6 +36,9 @@ template <typename T> struct Vec2;
 template <> struct Vec2<double> { using type = double2; };
 template <> struct Vec2<float> { using type = float2; };
 template <typename T> using cx = typename Vec2<T>::type;
+
+// one entry of the sampled spectrum: the node of this column (.a) and of the next one (.b)
+template <typename T> struct __align__(2 * sizeof(cx<T>)) NodePair { cx<T> a, b; };
 
 template <typename T> __device__ __forceinline__ cx<T> mk(T x, T y) { cx<T> r; r.x = x; r.y = y; return r; }
 template <typename V> __device__ __forceinline__ V cadd(V a, V b) { a.x += b.x; a.y += b.y; return a; }
@@ -230,7 +238,7 @@ __device__ __forceinline__ double sweep_pixel(const SweepParams& sp, int N, int 
 // ------------------------------------------------------------------------------------------
 template <typename T> struct RowParams {
     const T* image;        // [rows_total][N] (unused with SWEEP)
-    cx<T>* spec;           // [batch][N/2+1][N]
+    cx<T>* spec;           // work[batch][N/2+1][N]: the row-transformed image, transposed
     const cx<T>* tw;       // exp(-2 pi i m / N), m = 0..N-1
     int N;
     int rows_total;        // batch * N
@@ -311,7 +319,8 @@ row_pass_kernel(const RowParams<T> p) {
 // Column pass (in place).
 // ------------------------------------------------------------------------------------------
 template <typename T> struct ColParams {
-    cx<T>* spec;           // [batch][N/2+1][N]
+    const cx<T>* work;     // [batch][N/2+1][N], written by the row pass
+    NodePair<T>* pair;     // [batch][N/2+1][N], the sampled spectrum
     const cx<T>* tw;
     int N;
     long long cols_total;  // batch * (N/2+1)
@@ -342,14 +351,17 @@ col_pass_kernel(const ColParams<T> p) {
         if (!any) return;
     }
     const bool valid = g < p.cols_total && ku <= kumax;
-    cx<T>* col = p.spec + (valid ? g : 0) * (long long)L;
+    const cx<T>* col = p.work + (valid ? g : 0) * (long long)L;
+    NodePair<T>* own = p.pair + (valid ? g : 0) * (long long)L;          // .a of this column's entries
+    NodePair<T>* prev = own - (ku > 0 ? L : 0);                          // .b of the entries one column down
     cx<T>* S = smem + f * G::REGION;
 
     fft_steps12<T, R1, R2, R3, G::TPF>(S, t, p.tw, 1, [&](int n) -> cx<T> {
         return valid ? col[n] : mk<T>(0, 0);
     });
     // step 3 straight to global memory: kv = k1 + R1*(c + R2*d); sign (-1)^(ku+kv) folds the image
-    // centre shift, row (kv + N/2) mod N folds the shift along v.
+    // centre shift, row (kv + N/2) mod N folds the shift along v.  Each value goes to its own entry (.a)
+    // and to the entry of the column before (.b).
     for (int it = t; it < R1 * R2; it += G::TPF) {
         const int k1 = it % R1, c = it / R1;
         const cx<T>* base = S + k1 * G::P1 + c * R3;
@@ -363,7 +375,11 @@ col_pass_kernel(const ColParams<T> p) {
                 const int kv = k1 + R1 * (c + R2 * d);
                 const T sgn = ((ku + kv) & 1) ? (T)-1 : (T)1;
                 const int kvs = (kv + L / 2) & (L - 1);
-                if (kvs >= rmin && kvs <= rmax) col[kvs] = mk<T>(sgn * a[d].x, sgn * a[d].y);
+                if (kvs >= rmin && kvs <= rmax) {
+                    const cx<T> val = mk<T>(sgn * a[d].x, sgn * a[d].y);
+                    own[kvs].a = val;
+                    if (ku > 0) prev[kvs].b = val;
+                }
             }
         }
     }
@@ -382,15 +398,15 @@ __global__ void sweep_kernel(SweepParams sp, int N, T* __restrict__ image) {
     }
 }
 
-// out[kvs][ku] = spec[ku][kvs]   (paper layout [N][N/2+1])
+// out[kvs][ku] = pair[ku][kvs].a   (paper layout [N][N/2+1])
 template <typename T>
-__global__ void transpose_to_paper_layout_kernel(const cx<T>* __restrict__ spec, cx<T>* __restrict__ out, int N) {
+__global__ void transpose_to_paper_layout_kernel(const NodePair<T>* __restrict__ spec, cx<T>* __restrict__ out, int N) {
     __shared__ cx<T> tile[32][33];
     const int NU = N / 2 + 1;
     const int kv0 = blockIdx.x * 32, ku0 = blockIdx.y * 32;
     for (int r = threadIdx.y; r < 32; r += blockDim.y) {
         const int ku = ku0 + r, kv = kv0 + threadIdx.x;
-        if (ku < NU && kv < N) tile[r][threadIdx.x] = spec[(long long)ku * N + kv];
+        if (ku < NU && kv < N) tile[r][threadIdx.x] = spec[(long long)ku * N + kv].a;
     }
     __syncthreads();
     for (int r = threadIdx.y; r < 32; r += blockDim.y) {

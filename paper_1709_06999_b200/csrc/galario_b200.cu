@@ -18,7 +18,8 @@ using namespace galb;
 struct gal_plan {
     int nxy = 0, batch = 0, bits = 0, device = 0;
     int sm_count = 148;
-    void* spec = nullptr;            // cx<T>[batch][nxy/2+1][nxy]
+    void* spec = nullptr;            // NodePair<T>[batch][nxy/2+1][nxy]: the sampled spectrum (column pairs)
+    void* work = nullptr;            // cx<T>[batch][nxy/2+1][nxy]: row-pass output
     void* tw = nullptr;              // cx<T>[nxy]
     double* partials = nullptr;      // [batch][max_gx]
     unsigned int* tickets = nullptr; // [batch + 1]
@@ -82,7 +83,7 @@ int launch_row(gal_plan* p, const T* image, const SweepParams* sw, int batch, co
     using G = Geom<T, R1, R2, R3, F>;
     RowParams<T> rp;
     rp.image = image;
-    rp.spec = (cx<T>*)p->spec;
+    rp.spec = (cx<T>*)p->work;
     rp.tw = (const cx<T>*)p->tw;
     rp.N = p->nxy;
     rp.rows_total = batch * p->nxy;
@@ -108,7 +109,8 @@ template <typename T, int R1, int R2, int R3, int F>
 int launch_col(gal_plan* p, int batch, const int* ext, cudaStream_t st) {
     using G = Geom<T, R1, R2, R3, F>;
     ColParams<T> cp;
-    cp.spec = (cx<T>*)p->spec;
+    cp.work = (const cx<T>*)p->work;
+    cp.pair = (NodePair<T>*)p->spec;
     cp.tw = (const cx<T>*)p->tw;
     cp.N = p->nxy;
     cp.cols_total = (long long)batch * (p->nxy / 2 + 1);
@@ -153,23 +155,28 @@ int fft2(gal_plan* p, const T* image, const SweepParams* sw, int batch, const in
 // per-call scalars, uv extent, sampling launcher
 // ---------------------------------------------------------------------------------------------
 struct CallScalars {
-    double du, rdu, cos_PA, sin_PA, dRA_turns, dDec_turns;
-    int du_exact_div, has_phase;
+    IndexScalars ix;
+    double dRA_turns, dDec_turns;
+    int has_phase;
 };
 
 // host-side scalars, plain double arithmetic in the listing's order.  The
 // phase offsets are kept in turns (the listing's 2 pi factor is applied inside sincospi, exactly).
 CallScalars call_scalars(const gal_plan* p, double dxy, double dRA, double dDec, double PA) {
     CallScalars cs;
-    cs.du = 1.0 / ((double)p->nxy * dxy);
-    cs.rdu = 1.0 / cs.du;
+    IndexScalars& ix = cs.ix;
+    ix.du = 1.0 / ((double)p->nxy * dxy);
+    ix.rdu = 1.0 / ix.du;
     // Markstein's shortcut needs a divisor whose significand is not all ones
-    uint64_t bits; memcpy(&bits, &cs.du, 8);
-    cs.du_exact_div = ((bits & 0xFFFFFFFFFFFFFull) == 0xFFFFFFFFFFFFFull) || !std::isnormal(cs.du) || !std::isnormal(cs.rdu);
-    cs.cos_PA = std::cos(PA);
-    cs.sin_PA = std::sin(PA);
-    cs.dRA_turns = dRA * cs.cos_PA - dDec * cs.sin_PA;
-    cs.dDec_turns = dRA * cs.sin_PA + dDec * cs.cos_PA;
+    uint64_t bits; memcpy(&bits, &ix.du, 8);
+    ix.du_exact_div = ((bits & 0xFFFFFFFFFFFFFull) == 0xFFFFFFFFFFFFFull) || !std::isnormal(ix.du) || !std::isnormal(ix.rdu);
+    ix.cos_PA = std::cos(PA);
+    ix.sin_PA = std::sin(PA);
+    ix.fH = (double)(p->nxy / 2);
+    ix.fHm1 = ix.fH - 1.0;
+    ix.fN1 = (double)(p->nxy - 1);
+    cs.dRA_turns = dRA * ix.cos_PA - dDec * ix.sin_PA;
+    cs.dDec_turns = dRA * ix.sin_PA + dDec * ix.cos_PA;
     cs.has_phase = !(cs.dRA_turns == 0.0 && cs.dDec_turns == 0.0);
     return cs;
 }
@@ -197,10 +204,9 @@ int launch_extent(gal_plan* p, int C, const CallScalars& cs, const T* u, const T
     ExtentParams ep;
     ep.N = p->nxy;
     ep.total = (long long)C * M;
-    ep.du = cs.du; ep.rdu = cs.rdu; ep.du_exact_div = cs.du_exact_div;
-    ep.cos_PA = cs.cos_PA; ep.sin_PA = cs.sin_PA;
+    ep.ix = cs.ix;
     ep.ext = p->ext;
-    long long blocks = (ep.total + 1023) / 1024;
+    long long blocks = (ep.total + 2047) / 2048;
     const long long cap = (long long)p->sm_count * 8;
     if (blocks > cap) blocks = cap;
     if (blocks < 1) blocks = 1;
@@ -216,12 +222,11 @@ template <typename T, bool WRITE_VIS, bool DO_CHI2>
 int launch_sample_kernel(gal_plan* p, const SampleParams<T>& sp, dim3 grid, bool tma, cudaStream_t st) {
     using G = SampleGeom<T, DO_CHI2>;
     if (tma) {
-        auto k = sample_kernel<T, WRITE_VIS, DO_CHI2, true>;
+        auto k = sample_kernel_tma<T, WRITE_VIS, DO_CHI2>;
         int rc = set_smem(p, k, G::SMEM); if (rc) return rc;
         k<<<grid, 256, G::SMEM, st>>>(sp);
     } else {
-        auto k = sample_kernel<T, WRITE_VIS, DO_CHI2, false>;
-        k<<<grid, 256, 0, st>>>(sp);
+        sample_kernel_plain<T, WRITE_VIS, DO_CHI2><<<grid, 256, 0, st>>>(sp);
     }
     return GAL_OK;
 }
@@ -236,12 +241,11 @@ int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T
         return GAL_OK;
     }
     SampleParams<T> sp;
-    sp.spec = (const cx<T>*)p->spec;
+    sp.spec = (const NodePair<T>*)p->spec;
     sp.N = p->nxy;
     sp.M = M;
     sp.u = u; sp.v = v; sp.re_obs = re; sp.im_obs = im; sp.w = w; sp.vis = vis;
-    sp.du = cs.du; sp.rdu = cs.rdu; sp.du_exact_div = cs.du_exact_div;
-    sp.cos_PA = cs.cos_PA; sp.sin_PA = cs.sin_PA;
+    sp.ix = cs.ix;
     sp.dRA_turns = cs.dRA_turns; sp.dDec_turns = cs.dDec_turns; sp.has_phase = cs.has_phase;
     sp.partials = p->partials;
     sp.tickets = p->tickets;
@@ -257,8 +261,8 @@ int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T
     long long gx = ntiles < cap ? ntiles : cap;
     if (gx < 1) gx = 1;
     dim3 grid((unsigned)gx, (unsigned)C);
-    // the TMA path needs 16-byte aligned tiles in every channel
-    bool tma = aligned16(u) && aligned16(v) && (C == 1 || ((size_t)M * sizeof(T)) % 16 == 0);
+    // the TMA path needs 16-byte aligned tiles in every channel (and a du fit for the division shortcut)
+    bool tma = !cs.ix.du_exact_div && aligned16(u) && aligned16(v) && (C == 1 || ((size_t)M * sizeof(T)) % 16 == 0);
     if (do_chi2) tma = tma && aligned16(re) && aligned16(im) && aligned16(w);
     int rc = do_chi2 ? launch_sample_kernel<T, false, true>(p, sp, grid, tma, st)
                      : launch_sample_kernel<T, true, false>(p, sp, grid, tma, st);
@@ -355,7 +359,7 @@ int do_fft2_shifted(gal_plan* p, const T* image, T* out, void* stream) {
     int rc = fft2<T>(p, image, nullptr, 1, p->ext_full, st);
     if (rc) return rc;
     dim3 grid((p->nxy + 31) / 32, (p->nxy / 2 + 1 + 31) / 32), block(32, 8);
-    transpose_to_paper_layout_kernel<T><<<grid, block, 0, st>>>((const cx<T>*)p->spec, (cx<T>*)out, p->nxy);
+    transpose_to_paper_layout_kernel<T><<<grid, block, 0, st>>>((const NodePair<T>*)p->spec, (cx<T>*)out, p->nxy);
     p->launches++;
     GAL_CUDA(p, cudaGetLastError());
     return GAL_OK;
@@ -442,10 +446,12 @@ int gal_plan_create(gal_plan** out, int nxy, int batch, int precision_bits, int 
     cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, device);
     p->max_gx = p->sm_count * 8;
     const size_t esz = precision_bits == 64 ? sizeof(double2) : sizeof(float2);
-    const size_t spec_bytes = (size_t)batch * (nxy / 2 + 1) * nxy * esz;
+    const size_t work_bytes = (size_t)batch * (nxy / 2 + 1) * nxy * esz;
+    const size_t spec_bytes = 2 * work_bytes;
     auto fail = [&](int code, cudaError_t e) { p->last_cuda = (int)e; gal_plan_destroy(p); return code; };
     cudaError_t e;
     if ((e = cudaMalloc(&p->spec, spec_bytes)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
+    if ((e = cudaMalloc(&p->work, work_bytes)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     if ((e = cudaMalloc(&p->tw, (size_t)nxy * esz)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     if ((e = cudaMalloc((void**)&p->partials, sizeof(double) * (size_t)batch * p->max_gx)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     if ((e = cudaMalloc((void**)&p->tickets, sizeof(unsigned int) * (batch + 1))) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
@@ -463,7 +469,7 @@ int gal_plan_create(gal_plan** out, int nxy, int batch, int precision_bits, int 
         if ((e = cudaMemcpy(p->ext_full, full, 16, cudaMemcpyHostToDevice)) != cudaSuccess) return fail(GAL_ERR_CUDA, e);
     }
     if ((e = cudaMalloc((void**)&p->st_chi2, sizeof(double))) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
-    p->owned_bytes = spec_bytes + (size_t)nxy * esz + sizeof(double) * (size_t)batch * p->max_gx +
+    p->owned_bytes = spec_bytes + work_bytes + (size_t)nxy * esz + sizeof(double) * (size_t)batch * p->max_gx +
                      sizeof(unsigned int) * (batch + 1) + sizeof(double) * batch + 16;
     if ((e = cudaMemset(p->tickets, 0, sizeof(unsigned int) * (batch + 1))) != cudaSuccess) return fail(GAL_ERR_CUDA, e);
     // the workspace starts as zeros (pruned calls leave parts of it unwritten; they are never sampled)
@@ -491,7 +497,7 @@ int gal_plan_create(gal_plan** out, int nxy, int batch, int precision_bits, int 
 int gal_plan_destroy(gal_plan* p) {
     if (!p) return GAL_ERR_INVALID_ARGUMENT;
     DeviceGuard g(p->device);
-    cudaFree(p->spec); cudaFree(p->tw); cudaFree(p->partials); cudaFree(p->tickets); cudaFree(p->chi2_scratch);
+    cudaFree(p->spec); cudaFree(p->work); cudaFree(p->tw); cudaFree(p->partials); cudaFree(p->tickets); cudaFree(p->chi2_scratch);
     for (cudaEvent_t e : p->tev) cudaEventDestroy(e);
     cudaFree(p->call_state); cudaFree(p->call_init); cudaFree(p->ext_full); cudaFree(p->st_image); cudaFree(p->st_pts); cudaFree(p->st_out); cudaFree(p->st_chi2);
     delete p;

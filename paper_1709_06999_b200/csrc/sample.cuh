@@ -6,7 +6,7 @@
 // operation by operation, each one individually rounded in double (no FMA contraction), so the
 // cell an (u, v) point falls in and its weights are decided exactly as a plain IEEE evaluation of
 // the listing decides them — in _f32 as well (reading A14).
-// The spectrum is the u-major array written by fft.cuh: spec[ku][kvs].
+// The spectrum is the u-major array of column pairs written by fft.cuh: pair[ku][kvs] = {F[ku][kvs], F[ku+1][kvs]}.
 //
 // Data movement (sm_100a):
 //   * the per-point arrays u, v, re_obs, im_obs, w are streamed by the TMA engine: one elected
@@ -14,23 +14,30 @@
 //     of shared-memory stages, completion signalled on an mbarrier.  The loads cost no registers,
 //     no LSU wavefronts and are always STAGES-1 tiles ahead of the arithmetic;
 //   * the four spectrum nodes of a point are gathered by lane pairs through the L1 (see below);
-//     that gather — one L1 wavefront per 128-byte line touched — is what bounds the kernel once
-//     the streams are off the LSU, so everything else is arranged to overlap with it.
+//     that gather is bounded by the L2 -> SM path and by the L1's one line per clock, so it is
+//     shaped to move the fewest sectors and lines, and everything else overlaps with it.
 #pragma once
 #include "fft.cuh"
 
 namespace galb {
 
+// Scalars of one call that the index arithmetic needs (host-computed).  They sit
+// in the kernel parameter block so the compiler reads them as constant-bank operands, not registers.
+struct IndexScalars {
+    double du, rdu;        // du = 1/(N dxy); rdu = RN(1/du) for the exact-division shortcut
+    double cos_PA, sin_PA;
+    double fH, fHm1, fN1;  // N/2, N/2 - 1, N - 1 as doubles
+    int du_exact_div;      // 1: rdu is not usable, take a true division
+};
+
 template <typename T> struct SampleParams {
-    const cx<T>* spec;     // [C][N/2+1][N]
+    const NodePair<T>* spec;   // [C][N/2+1][N] column pairs (fft.cuh)
     int N;
     long long M;           // points per channel
     const T* u; const T* v;                       // [C][M]
     const T* re_obs; const T* im_obs; const T* w; // [C][M] (chi2 only)
     T* vis;                                       // [C][2M] (sample only)
-    double du, rdu;        // du = 1/(N dxy); rdu = RN(1/du) for the exact-division shortcut
-    int du_exact_div;      // 1: use a true division (rdu not usable)
-    double cos_PA, sin_PA;
+    IndexScalars ix;
     double dRA_turns, dDec_turns;  // rotated offsets in turns: theta / 2 pi = u' dRA_turns + v' dDec_turns
     int has_phase;         // 0 when both rotated offsets are 0 (theta == 0 exactly)
     double* partials;      // [C][gridDim.x]
@@ -43,12 +50,13 @@ template <typename T> struct SampleParams {
 // Correctly rounded a / b from r = RN(1/b) (Markstein): q0 = RN(a r); rem = a - q0 b (exact in an
 // FMA); q = RN(q0 + rem r).  Bit-identical to __ddiv_rn for the operand ranges met here (finite,
 // normal, b without an all-ones significand — the host checks b and otherwise asks for a true
-// division).
-__device__ __forceinline__ double div_by(double a, double b, double r, int exact) {
-    if (exact) return __ddiv_rn(a, b);
-    const double q0 = __dmul_rn(a, r);
-    const double rem = __fma_rn(-q0, b, a);
-    return __fma_rn(rem, r, q0);
+// division, EXACT).
+template <bool EXACT>
+__device__ __forceinline__ double div_by(double a, const IndexScalars& s) {
+    if (EXACT) return s.du_exact_div ? __ddiv_rn(a, s.du) : __fma_rn(__fma_rn(-__dmul_rn(a, s.rdu), s.du, a), s.rdu, __dmul_rn(a, s.rdu));
+    const double q0 = __dmul_rn(a, s.rdu);
+    const double rem = __fma_rn(-q0, s.du, a);
+    return __fma_rn(rem, s.rdu, q0);
 }
 
 // The listing's index arithmetic for one point (Eq. 11-12, 676-683), shared by the
@@ -57,32 +65,36 @@ struct PointIndex {
     double urot, vrot, uidx, vidx;
     bool uneg;
 };
-template <typename P>
-__device__ __forceinline__ PointIndex point_index(const P& p, double u, double v, double fH) {
+template <bool EXACT>
+__device__ __forceinline__ PointIndex point_index(const IndexScalars& s, double u, double v) {
     PointIndex q;
-    q.urot = __dsub_rn(__dmul_rn(u, p.cos_PA), __dmul_rn(v, p.sin_PA));
-    q.vrot = __dadd_rn(__dmul_rn(u, p.sin_PA), __dmul_rn(v, p.cos_PA));
-    q.uidx = div_by(fabs(q.urot), p.du, p.rdu, p.du_exact_div);
+    q.urot = __dsub_rn(__dmul_rn(u, s.cos_PA), __dmul_rn(v, s.sin_PA));
+    q.vrot = __dadd_rn(__dmul_rn(u, s.sin_PA), __dmul_rn(v, s.cos_PA));
+    q.uidx = div_by<EXACT>(fabs(q.urot), s);
     q.uneg = q.urot < 0.0;
-    const double vq = div_by(q.vrot, p.du, p.rdu, p.du_exact_div);
-    q.vidx = q.uneg ? __dsub_rn(fH, vq) : __dadd_rn(fH, vq);
+    const double vq = div_by<EXACT>(q.vrot, s);
+    q.vidx = q.uneg ? __dsub_rn(s.fH, vq) : __dadd_rn(s.fH, vq);
     return q;
+}
+// the interpolation cell lies fully inside the stored half-plane grid
+__device__ __forceinline__ bool cell_inside(const IndexScalars& s, const PointIndex& q) {
+    return q.uidx <= s.fHm1 && q.vidx >= 0.0 && q.vidx < s.fN1;
 }
 
 // Node (row = shifted v index, col = u index) of the spectrum extended to all integers by the
 // periodicity and Hermitian symmetry of the DFT of a real image (reading A6).  Rare path (points
 // beyond the half-plane grid), kept out of line.
 template <typename T>
-__device__ __noinline__ cx<T> node_any(const cx<T>* __restrict__ spec, int N, long long row, long long col) {
+__device__ __noinline__ cx<T> node_any(const NodePair<T>* __restrict__ spec, int N, long long row, long long col) {
     const int H = N >> 1;
     long long kv = row - H;
     long long cu = col & (long long)(N - 1);          // N is a power of two: floor-mod
     if (cu <= H) {
         const long long r = ((kv & (N - 1)) + H) & (N - 1);
-        return __ldg(spec + cu * N + r);
+        return __ldg(&spec[cu * N + r].a);
     }
     const long long r = (((-kv) & (N - 1)) + H) & (N - 1);
-    cx<T> g = __ldg(spec + (N - cu) * N + r);
+    cx<T> g = __ldg(&spec[(N - cu) * N + r].a);
     g.y = -g.y;
     return g;
 }
@@ -93,33 +105,42 @@ __device__ __noinline__ cx<T> node_any(const cx<T>* __restrict__ spec, int N, lo
 // shifted row kvs; a point whose cell leaves the grid (reading A6: the wrap can reach anything)
 // sets the full extent.  Integer max/min only, so the result does not depend on the order.
 // The FFT passes skip what lies outside (fft.cuh), which changes no result.
+// Pure streaming (16 B per point): EU points per thread are requested before any arithmetic.
 // ------------------------------------------------------------------------------------------
 struct ExtentParams {
     int N;
     long long total;       // C * M
-    double du, rdu;
-    int du_exact_div;
-    double cos_PA, sin_PA;
-    int* ext;              // [3], initialised to {0, N-1, 0} by the host
+    IndexScalars ix;
+    int* ext;              // [3], initialised by the host to the cell of the sampler's dead slots
 };
 
 template <typename T>
 __global__ void __launch_bounds__(256) uv_extent_kernel(const ExtentParams p, const T* __restrict__ u,
                                                         const T* __restrict__ v) {
+    constexpr int EU = 8;
     const int N = p.N, H = N >> 1;
-    const double fH = (double)H, fN1 = (double)(N - 1);
     int cmax = 0, rmin = N - 1, rmax = 0;
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < p.total; k += stride) {
-        const PointIndex q = point_index(p, (double)__ldcs(u + k), (double)__ldcs(v + k), fH);
-        const bool inside = q.uidx <= fH - 1.0 && q.vidx >= 0.0 && q.vidx < fN1;
-        if (inside) {
-            const int ix = (int)q.uidx, iy = (int)q.vidx;      // both >= 0: truncation == floor
-            cmax = max(cmax, ix + 1);
-            rmin = min(rmin, iy);
-            rmax = max(rmax, iy + 1);
-        } else {
-            cmax = H; rmin = 0; rmax = N - 1;
+    const long long stride = (long long)gridDim.x * blockDim.x * EU;
+    for (long long k0 = (long long)blockIdx.x * blockDim.x * EU + threadIdx.x; k0 < p.total; k0 += stride) {
+        double pu[EU], pv[EU];
+#pragma unroll
+        for (int j = 0; j < EU; ++j) {
+            const long long k = k0 + j * 256;
+            const bool ok = k < p.total;
+            pu[j] = ok ? (double)__ldcs(u + k) : 0.0;
+            pv[j] = ok ? (double)__ldcs(v + k) : 0.0;      // (0, 0) is the dead-slot cell, already in the extent
+        }
+#pragma unroll
+        for (int j = 0; j < EU; ++j) {
+            const PointIndex q = point_index<true>(p.ix, pu[j], pv[j]);
+            if (cell_inside(p.ix, q)) {
+                const int ix = (int)q.uidx, iy = (int)q.vidx;      // both >= 0: truncation == floor
+                cmax = max(cmax, ix + 1);
+                rmin = min(rmin, iy);
+                rmax = max(rmax, iy + 1);
+            } else {
+                cmax = H; rmin = 0; rmax = N - 1;
+            }
         }
     }
 #pragma unroll
@@ -192,153 +213,127 @@ template <typename T, bool DO_CHI2> struct SampleGeom {
     static constexpr size_t SMEM = (size_t)S * STAGE_BYTES + 8 * S;
 };
 
-// Gather by lane pairs.  The four nodes of a cell are two 32-byte runs (kvs, kvs+1 at ku and at ku+1) in
-// the u-major spectrum.  The L1 serves about one 128-byte line per clock, whatever the width of the access
-// (measured: 0.8-1.0 clk per line touched by an LDG), and a point needs 2.25 lines, so a warp-wide 16-byte
-// load of 32 unrelated nodes would spend 32 clocks for 32 nodes.  Lanes 2i and 2i+1 therefore fetch each
-// other's cells together: in every load instruction the even lane reads node kvs and the odd lane node
-// kvs+1 of the SAME cell — one line per lane pair.  Each lane then forms the u-direction interpolation of
-// its row for both cells, one shuffle hands the row the partner needs across, and the owner finishes its
+// One column-pair entry through the read-only path: a single 256-bit load in fp64 (sm_100), 128-bit in fp32.
+__device__ __forceinline__ NodePair<double> load_pair(const NodePair<double>* p) {
+    NodePair<double> e;
+    asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(e.a.x), "=d"(e.a.y), "=d"(e.b.x), "=d"(e.b.y) : "l"(p));
+    return e;
+}
+__device__ __forceinline__ NodePair<float> load_pair(const NodePair<float>* p) {
+    const float4 q = __ldg(reinterpret_cast<const float4*>(p));
+    NodePair<float> e;
+    e.a.x = q.x; e.a.y = q.y; e.b.x = q.z; e.b.y = q.w;
+    return e;
+}
+
+// What every variant of the kernel needs per CTA.
+template <typename T> struct SampleCtx {
+    const NodePair<T>* spec;   // this channel's spectrum
+    int N;
+    int odd;               // lane parity
+    double acc;            // chi2 partial of this thread
+    unsigned int oob;      // points of this thread beyond the half-plane grid
+};
+
+// U points of one thread: rotate, index, gather, interpolate, phase, chi2 / store.
+//   ld(a, j): value a (0 = u, 1 = v, 2 = re_obs, 3 = im_obs, 4 = w) of this thread's j-th point, as double;
+//             points past the end read as u = v = 0 with weight 0 (cell (0, N/2), always inside).
+//   kpt(j):   global index of that point (only used to store the visibility).
+//
+// Gather by lane pairs.  The four nodes of a cell are two adjacent column-pair entries, (ku, kvs) and
+// (ku, kvs+1): 64 contiguous bytes in fp64.  What bounds the gather is the L2 -> SM path (about 43 bytes
+// per clock and SM, measured) and the L1's one line per clock, so the access is shaped to move the fewest
+// sectors and lines: lanes 2i and 2i+1 fetch each other's cells together — in each of the two load
+// instructions the even lane reads entry kvs and the odd lane entry kvs+1 of the SAME cell with one
+// 256-bit load (two sectors, 1.25 lines per cell; measured 45 clk per 32 points against 72 for the
+// single-copy layout and 126 for one 16-byte load per node and lane).  Each lane then interpolates its row
+// along u for both cells, one shuffle hands the row the partner needs across, and the owner finishes its
 // own point.
-template <typename T, bool WRITE_VIS, bool DO_CHI2, bool TMA>
-__global__ void __launch_bounds__(256, GAL_SAMPLE_MINB) sample_kernel(const SampleParams<T> p) {
-    using G = SampleGeom<T, DO_CHI2>;
-    constexpr int U = G::U, TILE = G::TILE, S = G::S;
-    extern __shared__ __align__(128) unsigned char sample_smem[];
-    const int tid = threadIdx.x;
-    const int c = blockIdx.y;
-    const int N = p.N, H = N >> 1;
-    const long long M = p.M;
-    const cx<T>* __restrict__ spec = p.spec + (long long)c * (H + 1) * N;
-    const T* __restrict__ gsrc[5] = {p.u + c * M, p.v + c * M, DO_CHI2 ? p.re_obs + c * M : nullptr,
-                                     DO_CHI2 ? p.im_obs + c * M : nullptr, DO_CHI2 ? p.w + c * M : nullptr};
-    const double fH = (double)H, fN1 = (double)(N - 1);
-    const int odd = tid & 1;
-    const long long ntiles = (M + TILE - 1) / TILE, nfull = M / TILE;
-
-    // ---- TMA producer: thread 0 keeps S-1 tiles in flight ----
-    const uint32_t bar0 = smem_u32(sample_smem + (size_t)S * G::STAGE_BYTES);
-    uint64_t pol = 0;
-    auto issue = [&](long long tile, int s) {
-        if (tile >= nfull) return;                       // the ragged last tile is read with plain loads
-        const uint32_t mb = bar0 + 8 * s;
-        const uint32_t dst = smem_u32(sample_smem + (size_t)s * G::STAGE_BYTES);
-        mbar_expect_tx(mb, G::STAGE_BYTES);
+template <typename T, bool WRITE_VIS, bool DO_CHI2, bool EXACT, int U, typename LD, typename KP>
+__device__ __forceinline__ void sample_points(const SampleParams<T>& p, SampleCtx<T>& cx_, LD ld, KP kpt, long long M,
+                                              int c) {
+    const int N = cx_.N, odd = cx_.odd;
+    const NodePair<T>* __restrict__ spec = cx_.spec;
+    double tx[U], ty[U], turns[U];
+    bool uneg[U], inside[U];
+    cx<T> ga0[U], ga1[U], gb0[U], gb1[U];   // even lane's cell (a) / odd lane's cell (b); column ku+0 / ku+1
 #pragma unroll
-        for (int a = 0; a < G::NARR; ++a) tma_load_1d(dst + a * G::ARR_BYTES, gsrc[a] + tile * TILE, G::ARR_BYTES, mb, pol);
-    };
-    if (TMA) {
-        if (tid == 0) {
-            for (int s = 0; s < S; ++s) mbar_init(bar0 + 8 * s, 1);
-            mbar_fence_init();
-            pol = l2_policy_evict_first();
-            for (int s = 0; s < S - 1; ++s) issue(blockIdx.x + (long long)s * gridDim.x, s);
+    for (int j = 0; j < U; ++j) {
+        const PointIndex q = point_index<EXACT>(p.ix, ld(0, j), ld(1, j));
+        // bilinear interpolation
+        const double fx0 = floor(q.uidx), fy0 = floor(q.vidx);
+        tx[j] = __dsub_rn(q.uidx, fx0);
+        ty[j] = __dsub_rn(q.vidx, fy0);
+        uneg[j] = q.uneg;
+        inside[j] = cell_inside(p.ix, q);
+        // theta / 2 pi in turns (exact range reduction in sincospi)
+        turns[j] = fma(q.urot, p.dRA_turns, q.vrot * p.dDec_turns);
+#ifdef GAL_DBG_NOGATHER
+        const int off = inside[j] ? ((int)fx0 * N + (int)fy0) & 7 : 0;
+#else
+        const int off = inside[j] ? (int)fx0 * N + (int)fy0 : 0;
+#endif
+        const int off_partner = __shfl_xor_sync(0xffffffffu, off, 1);
+        const NodePair<T> ea = load_pair(spec + ((odd ? off_partner : off) + odd));
+        const NodePair<T> eb = load_pair(spec + ((odd ? off : off_partner) + odd));
+        ga0[j] = ea.a; ga1[j] = ea.b;
+        gb0[j] = eb.a; gb1[j] = eb.b;
+    }
+#pragma unroll
+    for (int j = 0; j < U; ++j) {
+        const double tx_partner = __shfl_xor_sync(0xffffffffu, tx[j], 1);
+        const double txa = odd ? tx_partner : tx[j], txb = odd ? tx[j] : tx_partner;
+        // this lane's row (kvs + odd) of both cells, interpolated along u: g0 + t (g1 - g0)
+        const double ra_re = fma(txa, (double)ga1[j].x - (double)ga0[j].x, (double)ga0[j].x);
+        const double ra_im = fma(txa, (double)ga1[j].y - (double)ga0[j].y, (double)ga0[j].y);
+        const double rb_re = fma(txb, (double)gb1[j].x - (double)gb0[j].x, (double)gb0[j].x);
+        const double rb_im = fma(txb, (double)gb1[j].y - (double)gb0[j].y, (double)gb0[j].y);
+        // the even lane keeps row kvs of cell a and needs row kvs+1 of it; the odd lane keeps row kvs+1 of
+        // cell b and needs row kvs: mine + w (other - mine), w = ty (even) or 1 - ty (odd)
+        const double o_re = __shfl_xor_sync(0xffffffffu, odd ? ra_re : rb_re, 1);
+        const double o_im = __shfl_xor_sync(0xffffffffu, odd ? ra_im : rb_im, 1);
+        const double m_re = odd ? rb_re : ra_re, m_im = odd ? rb_im : ra_im;
+        const double wy = odd ? 1.0 - ty[j] : ty[j];
+        double ReInt = fma(wy, o_re - m_re, m_re);
+        double ImInt = fma(wy, o_im - m_im, m_im);
+        if (!inside[j]) {           // rare: the cell leaves the half-plane grid (reading A6); dead slots never get here
+            const PointIndex q = point_index<EXACT>(p.ix, ld(0, j), ld(1, j));
+            const long long ix = (long long)floor(q.uidx), iy = (long long)floor(q.vidx);
+            if (q.uidx > p.ix.fH || q.vidx < 0.0 || q.vidx > p.ix.fN1) ++cx_.oob;
+            const cx<T> g00 = node_any<T>(spec, N, iy, ix), g01 = node_any<T>(spec, N, iy, ix + 1);
+            const cx<T> g10 = node_any<T>(spec, N, iy + 1, ix), g11 = node_any<T>(spec, N, iy + 1, ix + 1);
+            const double ax = 1.0 - tx[j], ay = 1.0 - ty[j];
+            ReInt = ay * (ax * (double)g00.x + tx[j] * (double)g01.x) + ty[j] * (ax * (double)g10.x + tx[j] * (double)g11.x);
+            ImInt = ay * (ax * (double)g00.y + tx[j] * (double)g01.y) + ty[j] * (ax * (double)g10.y + tx[j] * (double)g11.y);
+        }
+        if (uneg[j]) ImInt = -ImInt;
+        double vr = ReInt, vi = ImInt;
+#ifdef GAL_DBG_NOPHASE
+        if (false) {
+#else
+        if (p.has_phase) {
+#endif
+            double sn, co;
+            sincospi(2.0 * turns[j], &sn, &co);
+            vr = ReInt * co - ImInt * sn;
+            vi = ReInt * sn + ImInt * co;
+        }
+        if (WRITE_VIS) {
+            const long long k = kpt(j);
+            if (k < M) __stcs(reinterpret_cast<cx<T>*>(p.vis) + c * M + k, mk<T>((T)vr, (T)vi));
+        }
+        if (DO_CHI2) {                                      // PAPER.md:718 (Eq. 10); w = 0 for dead slots
+            const double dr = vr - ld(2, j);
+            const double di = vi - ld(3, j);
+            cx_.acc = fma(fma(dr, dr, di * di), ld(4, j), cx_.acc);
         }
     }
+}
 
-    double acc = 0.0;
-    unsigned int oob = 0;
-    int it = 0;
-    for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
-        const int s = it % S;
-        const bool staged = TMA && tile < nfull;
-        if (TMA) {
-            __syncthreads();                             // stage (it-1) % S has been consumed by everyone
-            if (tid == 0) issue(tile + (long long)(S - 1) * gridDim.x, (it + S - 1) % S);
-            if (staged) mbar_wait(bar0 + 8 * s, (uint32_t)(it / S) & 1u);
-        }
-        const T* st = reinterpret_cast<const T*>(sample_smem + (size_t)s * G::STAGE_BYTES);
-        const long long k0 = tile * TILE + tid;
-
-        double tx[U], ty[U], ro[U], io[U], wt[U];
-        PointIndex q[U];
-        bool inside[U];
-        cx<T> ga0[U], ga1[U], gb0[U], gb1[U];   // even lane's cell (a) / odd lane's cell (b); column ku+0 / ku+1
-#pragma unroll
-        for (int j = 0; j < U; ++j) {
-            double pu = 0.0, pv = 0.0;                   // dead slots: index (0, N/2), weight 0
-            ro[j] = io[j] = wt[j] = 0.0;
-            if (staged) {
-                pu = (double)st[0 * TILE + j * 256 + tid];
-                pv = (double)st[1 * TILE + j * 256 + tid];
-                if (DO_CHI2) {
-                    ro[j] = (double)st[2 * TILE + j * 256 + tid];
-                    io[j] = (double)st[3 * TILE + j * 256 + tid];
-                    wt[j] = (double)st[4 * TILE + j * 256 + tid];
-                }
-            } else if (k0 + j * 256 < M) {
-                const long long k = k0 + j * 256;
-                pu = (double)__ldcs(gsrc[0] + k);
-                pv = (double)__ldcs(gsrc[1] + k);
-                if (DO_CHI2) {
-                    ro[j] = (double)__ldcs(gsrc[2] + k);
-                    io[j] = (double)__ldcs(gsrc[3] + k);
-                    wt[j] = (double)__ldcs(gsrc[4] + k);
-                }
-            }
-            q[j] = point_index(p, pu, pv, fH);
-            // bilinear interpolation
-            const double fx0 = floor(q[j].uidx), fy0 = floor(q[j].vidx);
-            tx[j] = __dsub_rn(q[j].uidx, fx0);
-            ty[j] = __dsub_rn(q[j].vidx, fy0);
-            inside[j] = q[j].uidx <= fH - 1.0 && q[j].vidx >= 0.0 && q[j].vidx < fN1;   // cell fully inside the grid
-            const int off = inside[j] ? (int)fx0 * N + (int)fy0 : 0;
-            const int off_partner = __shfl_xor_sync(0xffffffffu, off, 1);
-            const cx<T>* pa = spec + ((odd ? off_partner : off) + odd);
-            const cx<T>* pb = spec + ((odd ? off : off_partner) + odd);
-            ga0[j] = __ldg(pa);
-            ga1[j] = __ldg(pa + N);
-            gb0[j] = __ldg(pb);
-            gb1[j] = __ldg(pb + N);
-        }
-#pragma unroll
-        for (int j = 0; j < U; ++j) {
-            const double tx_partner = __shfl_xor_sync(0xffffffffu, tx[j], 1);
-            const double txa = odd ? tx_partner : tx[j], txb = odd ? tx[j] : tx_partner;
-            // this lane's row (kvs + odd) of both cells, interpolated along u: g0 + t (g1 - g0)
-            const double ra_re = fma(txa, (double)ga1[j].x - (double)ga0[j].x, (double)ga0[j].x);
-            const double ra_im = fma(txa, (double)ga1[j].y - (double)ga0[j].y, (double)ga0[j].y);
-            const double rb_re = fma(txb, (double)gb1[j].x - (double)gb0[j].x, (double)gb0[j].x);
-            const double rb_im = fma(txb, (double)gb1[j].y - (double)gb0[j].y, (double)gb0[j].y);
-            // the even lane needs row kvs+1 of cell a, the odd lane row kvs of cell b
-            const double o_re = __shfl_xor_sync(0xffffffffu, odd ? ra_re : rb_re, 1);
-            const double o_im = __shfl_xor_sync(0xffffffffu, odd ? ra_im : rb_im, 1);
-            const double lo_re = odd ? o_re : ra_re, hi_re = odd ? rb_re : o_re;
-            const double lo_im = odd ? o_im : ra_im, hi_im = odd ? rb_im : o_im;
-            double ReInt = fma(ty[j], hi_re - lo_re, lo_re);
-            double ImInt = fma(ty[j], hi_im - lo_im, lo_im);
-            if (!inside[j]) {           // rare: the cell leaves the half-plane grid (reading A6); dead slots never get here
-                const double uidx = q[j].uidx, vidx = q[j].vidx;
-                const long long ix = (long long)floor(uidx), iy = (long long)floor(vidx);
-                if (uidx > fH || vidx < 0.0 || vidx > fN1) ++oob;
-                const cx<T> g00 = node_any<T>(spec, N, iy, ix), g01 = node_any<T>(spec, N, iy, ix + 1);
-                const cx<T> g10 = node_any<T>(spec, N, iy + 1, ix), g11 = node_any<T>(spec, N, iy + 1, ix + 1);
-                const double ax = 1.0 - tx[j], ay = 1.0 - ty[j];
-                ReInt = ay * (ax * (double)g00.x + tx[j] * (double)g01.x) + ty[j] * (ax * (double)g10.x + tx[j] * (double)g11.x);
-                ImInt = ay * (ax * (double)g00.y + tx[j] * (double)g01.y) + ty[j] * (ax * (double)g10.y + tx[j] * (double)g11.y);
-            }
-            if (q[j].uneg) ImInt = -ImInt;
-            double vr = ReInt, vi = ImInt;
-            if (p.has_phase) {                                  // PAPER.md:712-713, theta in turns: exact range reduction
-                const double turns = fma(q[j].urot, p.dRA_turns, q[j].vrot * p.dDec_turns);
-                double sn, co;
-                sincospi(2.0 * turns, &sn, &co);
-                vr = ReInt * co - ImInt * sn;
-                vi = ReInt * sn + ImInt * co;
-            }
-            if (WRITE_VIS) {
-                const long long k = k0 + j * 256;
-                if (k < M) __stcs(reinterpret_cast<cx<T>*>(p.vis) + c * M + k, mk<T>((T)vr, (T)vi));
-            }
-            if (DO_CHI2) {                                      // PAPER.md:718 (Eq. 10); w = 0 for dead slots
-                const double dr = vr - ro[j];
-                const double di = vi - io[j];
-                acc = fma(fma(dr, dr, di * di), wt[j], acc);
-            }
-        }
-    }
-
-    // ---- deterministic reduction: warp shuffle -> block -> per-block partial -> last block ----
+// Deterministic reduction: warp shuffle -> block -> per-block partial -> last block (ticket), fixed order,
+// no floating-point atomics.  Also adds this CTA's out-of-grid count.
+template <typename T, bool DO_CHI2>
+__device__ __forceinline__ void sample_finish(const SampleParams<T>& p, int c, double acc, unsigned int oob) {
     __shared__ double wsum[8];
     __shared__ unsigned int woob[8];
     __shared__ bool is_last;
@@ -397,6 +392,109 @@ __global__ void __launch_bounds__(256, GAL_SAMPLE_MINB) sample_kernel(const Samp
             }
         }
     }
+}
+
+// One tile by plain (guarded) loads straight from global memory.
+template <typename T, bool WRITE_VIS, bool DO_CHI2, bool EXACT>
+__device__ __forceinline__ void sample_tile_plain(const SampleParams<T>& p, SampleCtx<T>& cx_, long long tile, long long M,
+                                                  int c) {
+    constexpr int U = SampleGeom<T, DO_CHI2>::U, TILE = SampleGeom<T, DO_CHI2>::TILE;
+    const long long k0 = tile * TILE + threadIdx.x;
+    const T* __restrict__ g0 = p.u + c * M;
+    const T* __restrict__ g1 = p.v + c * M;
+    const T* __restrict__ g2 = DO_CHI2 ? p.re_obs + c * M : nullptr;
+    const T* __restrict__ g3 = DO_CHI2 ? p.im_obs + c * M : nullptr;
+    const T* __restrict__ g4 = DO_CHI2 ? p.w + c * M : nullptr;
+    auto ld = [&](int a, int j) -> double {
+        const long long k = k0 + j * 256;
+        if (k >= M) return 0.0;
+        const T* g = a == 0 ? g0 : a == 1 ? g1 : a == 2 ? g2 : a == 3 ? g3 : g4;
+        return (double)__ldcs(g + k);
+    };
+    auto kpt = [&](int j) -> long long { return k0 + j * 256; };
+    sample_points<T, WRITE_VIS, DO_CHI2, EXACT, U>(p, cx_, ld, kpt, M, c);
+}
+
+// General kernel: any alignment, any du (takes the true division when the shortcut is not valid).
+template <typename T, bool WRITE_VIS, bool DO_CHI2>
+__global__ void __launch_bounds__(256, GAL_SAMPLE_MINB) sample_kernel_plain(const SampleParams<T> p) {
+    constexpr int TILE = SampleGeom<T, DO_CHI2>::TILE;
+    const int c = blockIdx.y;
+    const long long M = p.M;
+    SampleCtx<T> cx_;
+    cx_.N = p.N;
+    cx_.spec = p.spec + (long long)c * (p.N / 2 + 1) * p.N;
+    cx_.odd = threadIdx.x & 1;
+    cx_.acc = 0.0;
+    cx_.oob = 0;
+    const long long ntiles = (M + TILE - 1) / TILE;
+    for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x)
+        sample_tile_plain<T, WRITE_VIS, DO_CHI2, true>(p, cx_, tile, M, c);
+    sample_finish<T, DO_CHI2>(p, c, cx_.acc, cx_.oob);
+}
+
+// Fast kernel: every per-point array 16-byte aligned in every channel, du fit for the division shortcut.
+// Thread 0 is the TMA producer: it keeps S-1 whole tiles in flight in a ring of shared-memory stages; the
+// ragged last tile (if any) is read with plain loads by the CTA whose turn it would have been.
+template <typename T, bool WRITE_VIS, bool DO_CHI2>
+__global__ void __launch_bounds__(256, GAL_SAMPLE_MINB) sample_kernel_tma(const SampleParams<T> p) {
+    using G = SampleGeom<T, DO_CHI2>;
+    constexpr int U = G::U, TILE = G::TILE, S = G::S;
+    extern __shared__ __align__(128) unsigned char sample_smem[];
+    const int tid = threadIdx.x;
+    const int c = blockIdx.y;
+    const long long M = p.M;
+    SampleCtx<T> cx_;
+    cx_.N = p.N;
+    cx_.spec = p.spec + (long long)c * (p.N / 2 + 1) * p.N;
+    cx_.odd = tid & 1;
+    cx_.acc = 0.0;
+    cx_.oob = 0;
+    const long long nfull = M / TILE;
+    const uint32_t stage0 = smem_u32(sample_smem);
+    const uint32_t bar0 = stage0 + S * G::STAGE_BYTES;
+
+    // producer state (thread 0 only)
+    uint64_t pol = 0;
+    long long ptile = blockIdx.x;            // next tile to request
+    uint32_t pstage = 0;
+    auto produce = [&]() {
+        if (ptile < nfull) {
+            const uint32_t mb = bar0 + 8 * pstage, dst = stage0 + pstage * G::STAGE_BYTES;
+            const long long k = ptile * TILE + c * M;
+            mbar_expect_tx(mb, G::STAGE_BYTES);
+            tma_load_1d(dst, p.u + k, G::ARR_BYTES, mb, pol);
+            tma_load_1d(dst + G::ARR_BYTES, p.v + k, G::ARR_BYTES, mb, pol);
+            if (DO_CHI2) {
+                tma_load_1d(dst + 2 * G::ARR_BYTES, p.re_obs + k, G::ARR_BYTES, mb, pol);
+                tma_load_1d(dst + 3 * G::ARR_BYTES, p.im_obs + k, G::ARR_BYTES, mb, pol);
+                tma_load_1d(dst + 4 * G::ARR_BYTES, p.w + k, G::ARR_BYTES, mb, pol);
+            }
+        }
+        ptile += gridDim.x;
+        pstage = (pstage + 1 == S) ? 0 : pstage + 1;
+    };
+    if (tid == 0) {
+        for (int s = 0; s < S; ++s) mbar_init(bar0 + 8 * s, 1);
+        mbar_fence_init();
+        pol = l2_policy_evict_first();
+        for (int s = 0; s < S - 1; ++s) produce();
+    }
+
+    uint32_t cstage = 0, cparity = 0;
+    for (long long tile = blockIdx.x; tile < nfull; tile += gridDim.x) {
+        __syncthreads();                                 // the stage consumed one trip ago is free again
+        if (tid == 0) produce();
+        mbar_wait(bar0 + 8 * cstage, cparity);
+        const T* st = reinterpret_cast<const T*>(sample_smem + cstage * G::STAGE_BYTES) + tid;
+        auto ld = [&](int a, int j) -> double { return (double)st[a * TILE + j * 256]; };
+        auto kpt = [&](int j) -> long long { return tile * TILE + j * 256 + tid; };
+        sample_points<T, WRITE_VIS, DO_CHI2, false, U>(p, cx_, ld, kpt, M, c);
+        if (++cstage == S) { cstage = 0; cparity ^= 1u; }
+    }
+    if (nfull * TILE < M && (long long)blockIdx.x == nfull % gridDim.x)
+        sample_tile_plain<T, WRITE_VIS, DO_CHI2, false>(p, cx_, nfull, M, c);
+    sample_finish<T, DO_CHI2>(p, c, cx_.acc, cx_.oob);
 }
 
 }  // namespace galb
