@@ -206,8 +206,8 @@ int launch_extent(gal_plan* p, int C, const CallScalars& cs, const T* u, const T
     ep.total = (long long)C * M;
     ep.ix = cs.ix;
     ep.ext = p->ext;
-    long long blocks = (ep.total + 2047) / 2048;
-    const long long cap = (long long)p->sm_count * 8;
+    long long blocks = (ep.total + 1023) / 1024;
+    const long long cap = (long long)p->sm_count * 4;
     if (blocks > cap) blocks = cap;
     if (blocks < 1) blocks = 1;
     uv_extent_kernel<T><<<(unsigned)blocks, 256, 0, st>>>(ep, u, v);
@@ -224,9 +224,9 @@ int launch_sample_kernel(gal_plan* p, const SampleParams<T>& sp, dim3 grid, bool
     if (tma) {
         auto k = sample_kernel_tma<T, WRITE_VIS, DO_CHI2>;
         int rc = set_smem(p, k, G::SMEM); if (rc) return rc;
-        k<<<grid, 256, G::SMEM, st>>>(sp);
+        k<<<grid, G::NT_TMA, G::SMEM, st>>>(sp);
     } else {
-        sample_kernel_plain<T, WRITE_VIS, DO_CHI2><<<grid, 256, 0, st>>>(sp);
+        sample_kernel_plain<T, WRITE_VIS, DO_CHI2><<<grid, G::NT, 0, st>>>(sp);
     }
     return GAL_OK;
 }
@@ -285,7 +285,7 @@ int run_call(gal_plan* p, const T* image, const SweepParams* sw, int C, double d
     if ((rc = reset_call_state(p, st))) return rc;
     if (timed) GAL_CUDA(p, cudaEventRecord(e[0], st));
     const int* ext = p->ext_full;
-    p->last_pruned = want_prune<T>(p, C, M);
+    p->last_pruned = want_prune<T>(p, C, M) && !cs.ix.du_exact_div;   // the extent kernel only has the division shortcut
     if (p->last_pruned) {
         if ((rc = launch_extent<T>(p, C, cs, u, v, M, st))) return rc;
         ext = p->ext;

@@ -9,10 +9,11 @@
 // The spectrum is the u-major array of column pairs written by fft.cuh: pair[ku][kvs] = {F[ku][kvs], F[ku+1][kvs]}.
 //
 // Data movement (sm_100a):
-//   * the per-point arrays u, v, re_obs, im_obs, w are streamed by the TMA engine: one elected
-//     thread issues `cp.async.bulk` copies of whole tiles (256*U points of each array) into a ring
-//     of shared-memory stages, completion signalled on an mbarrier.  The loads cost no registers,
-//     no LSU wavefronts and are always STAGES-1 tiles ahead of the arithmetic;
+//   * the per-point arrays u, v, re_obs, im_obs, w are streamed by the TMA engine: a producer warp
+//     issues `cp.async.bulk` copies of whole tiles (256*U points of each array) into a ring of
+//     shared-memory stages, full/empty mbarriers hand the stages back and forth.  The loads cost the
+//     consumer warps no registers, no instructions and no L1 tag look-ups, and run up to STAGES
+//     tiles ahead of the arithmetic;
 //   * the four spectrum nodes of a point are gathered by lane pairs through the L1 (see below);
 //     that gather is bounded by the L2 -> SM path and by the L1's one line per clock, so it is
 //     shaped to move the fewest sectors and lines, and everything else overlaps with it.
@@ -81,6 +82,54 @@ __device__ __forceinline__ bool cell_inside(const IndexScalars& s, const PointIn
     return q.uidx <= s.fHm1 && q.vidx >= 0.0 && q.vidx < s.fN1;
 }
 
+// floor() and sincos() without the XU pipe.  On sm_100 the 64-bit conversions (FRND.F64, F2I.F64, I2F.F64)
+// issue on the XU pipe at a small fraction of the FP64 rate; with two floors, two conversions and the
+// range reduction of sincospi per point that pipe, not memory, bounded the sampler (ncu: XU 95 % busy).
+// Both are therefore done with plain FP64 adds and integer bit moves.
+//
+// floor of 0 <= x < 2^31 as a double (*fl) and as an int (return): x + 2^52 rounds x to an integer in the
+// low mantissa bits; one compare fixes round-to-nearest into round-down.  fl is exactly floor(x), so the
+// fractional weight x - fl is bit-identical to the listing's.  (Only used for cells inside the grid.)
+__device__ __forceinline__ int floor_small(double x, double* fl) {
+    const double MAGIC = 4503599627370496.0;             // 2^52
+    const double t = __dadd_rn(x, MAGIC);
+    double r = __dsub_rn(t, MAGIC);                      // rint(x)
+    int i = __double2loint(t);
+    if (r > x) { r = __dsub_rn(r, 1.0); i -= 1; }
+    *fl = r;
+    return i;
+}
+
+// sin and cos of 2 pi t for t in turns, |t| < 2^49.  k = rint(4 t) from the same mantissa trick (exact), the
+// remainder r = 4 t - k in [-1/2, 1/2] is exact, a = r pi / 2 lies in [-pi/4, pi/4] where the classic
+// minimax polynomials (fdlibm's kernel coefficients) are good to < 1 ulp; the quadrant k mod 4 then swaps and
+// signs the pair.
+__device__ __forceinline__ void sincos_turns(double t, double* sn, double* cs) {
+    const double MAGIC = 6755399441055744.0;             // 1.5 * 2^52: keeps negative k in range
+    const double t4 = 4.0 * t;
+    const double z = __dadd_rn(t4, MAGIC);
+    const int q = __double2loint(z);
+    const double a = (t4 - (z - MAGIC)) * 1.57079632679489661923;
+    const double a2 = a * a;
+    double ps = 1.58969099521155010221e-10;
+    ps = fma(ps, a2, -2.50507602534068634195e-08);
+    ps = fma(ps, a2, 2.75573137070700676789e-06);
+    ps = fma(ps, a2, -1.98412698298579493134e-04);
+    ps = fma(ps, a2, 8.33333333332248946124e-03);
+    ps = fma(ps, a2, -1.66666666666666324348e-01);
+    const double s = fma(a * a2, ps, a);
+    double pc = -1.13596475577881948265e-11;
+    pc = fma(pc, a2, 2.08757232129817482790e-09);
+    pc = fma(pc, a2, -2.75573143513906633035e-07);
+    pc = fma(pc, a2, 2.48015872894767294178e-05);
+    pc = fma(pc, a2, -1.38888888888741095749e-03);
+    pc = fma(pc, a2, 4.16666666666666019037e-02);
+    const double c = fma(a2 * a2, pc, fma(a2, -0.5, 1.0));
+    const double ss = (q & 1) ? c : s, cc = (q & 1) ? s : c;
+    *sn = (q & 2) ? -ss : ss;
+    *cs = ((q + 1) & 2) ? -cc : cc;
+}
+
 // Node (row = shifted v index, col = u index) of the spectrum extended to all integers by the
 // periodicity and Hermitian symmetry of the DFT of a real image (reading A6).  Rare path (points
 // beyond the half-plane grid), kept out of line.
@@ -115,26 +164,37 @@ struct ExtentParams {
 };
 
 template <typename T>
-__global__ void __launch_bounds__(256) uv_extent_kernel(const ExtentParams p, const T* __restrict__ u,
-                                                        const T* __restrict__ v) {
-    constexpr int EU = 8;
+__global__ void __launch_bounds__(256, 4) uv_extent_kernel(const ExtentParams p, const T* __restrict__ u,
+                                                           const T* __restrict__ v) {
+    // Persistent grid (a whole number of CTAs per SM), EU points per thread and trip; the loads of the next
+    // trip are issued before the arithmetic of this one (register double buffer).
+    constexpr int EU = 4;
     const int N = p.N, H = N >> 1;
     int cmax = 0, rmin = N - 1, rmax = 0;
     const long long stride = (long long)gridDim.x * blockDim.x * EU;
-    for (long long k0 = (long long)blockIdx.x * blockDim.x * EU + threadIdx.x; k0 < p.total; k0 += stride) {
+    long long k0 = (long long)blockIdx.x * blockDim.x * EU + threadIdx.x;
+    double nu[EU], nv[EU];
+    auto fetch = [&](long long kk) {
+#pragma unroll
+        for (int j = 0; j < EU; ++j) {
+            const long long k = kk + j * 256;
+            const bool ok = k < p.total;
+            nu[j] = ok ? (double)__ldcs(u + k) : 0.0;
+            nv[j] = ok ? (double)__ldcs(v + k) : 0.0;      // (0, 0) is the dead-slot cell, already in the extent
+        }
+    };
+    fetch(k0);
+    for (; k0 < p.total; k0 += stride) {
         double pu[EU], pv[EU];
 #pragma unroll
-        for (int j = 0; j < EU; ++j) {
-            const long long k = k0 + j * 256;
-            const bool ok = k < p.total;
-            pu[j] = ok ? (double)__ldcs(u + k) : 0.0;
-            pv[j] = ok ? (double)__ldcs(v + k) : 0.0;      // (0, 0) is the dead-slot cell, already in the extent
-        }
+        for (int j = 0; j < EU; ++j) { pu[j] = nu[j]; pv[j] = nv[j]; }
+        fetch(k0 + stride);
 #pragma unroll
         for (int j = 0; j < EU; ++j) {
-            const PointIndex q = point_index<true>(p.ix, pu[j], pv[j]);
+            const PointIndex q = point_index<false>(p.ix, pu[j], pv[j]);
             if (cell_inside(p.ix, q)) {
-                const int ix = (int)q.uidx, iy = (int)q.vidx;      // both >= 0: truncation == floor
+                double f_;
+                const int ix = floor_small(q.uidx, &f_), iy = floor_small(q.vidx, &f_);
                 cmax = max(cmax, ix + 1);
                 rmin = min(rmin, iy);
                 rmax = max(rmax, iy + 1);
@@ -199,18 +259,21 @@ __device__ __forceinline__ void tma_load_1d(uint32_t dst, const void* src, uint3
 #define GAL_SAMPLE_STAGES 3
 #endif
 #ifndef GAL_SAMPLE_MINB
-#define GAL_SAMPLE_MINB 3
+#define GAL_SAMPLE_MINB 2
 #endif
 
+// The unit of work is a tile of 256*U consecutive points; CTA b takes tiles b, b + gridDim.x, ...; thread t
+// of the 256 consumer threads takes points t, t + 256, ... of the tile.
 template <typename T, bool DO_CHI2> struct SampleGeom {
     static constexpr int U = GAL_SAMPLE_U;
-    static constexpr int NT = 256;
+    static constexpr int NT = 256, NW = NT / 32;                    // consumer threads / warps
+    static constexpr int NT_TMA = NT + 32;                          // + one producer warp (TMA kernel)
     static constexpr int TILE = NT * U;
     static constexpr int NARR = DO_CHI2 ? 5 : 2;
     static constexpr int S = GAL_SAMPLE_STAGES;
-    static constexpr uint32_t ARR_BYTES = TILE * sizeof(T);
+    static constexpr uint32_t ARR_BYTES = TILE * sizeof(T);         // multiple of 16
     static constexpr uint32_t STAGE_BYTES = NARR * ARR_BYTES;
-    static constexpr size_t SMEM = (size_t)S * STAGE_BYTES + 8 * S;
+    static constexpr size_t SMEM = (size_t)S * STAGE_BYTES + 16 * S;
 };
 
 // One column-pair entry through the read-only path: a single 256-bit load in fp64 (sm_100), 128-bit in fp32.
@@ -254,35 +317,32 @@ __device__ __forceinline__ void sample_points(const SampleParams<T>& p, SampleCt
                                               int c) {
     const int N = cx_.N, odd = cx_.odd;
     const NodePair<T>* __restrict__ spec = cx_.spec;
-    double tx[U], ty[U], turns[U];
+    double tx[U], ty[U], turns[U], tx_partner[U];
     bool uneg[U], inside[U];
     cx<T> ga0[U], ga1[U], gb0[U], gb1[U];   // even lane's cell (a) / odd lane's cell (b); column ku+0 / ku+1
 #pragma unroll
     for (int j = 0; j < U; ++j) {
         const PointIndex q = point_index<EXACT>(p.ix, ld(0, j), ld(1, j));
         // bilinear interpolation
-        const double fx0 = floor(q.uidx), fy0 = floor(q.vidx);
-        tx[j] = __dsub_rn(q.uidx, fx0);
-        ty[j] = __dsub_rn(q.vidx, fy0);
-        uneg[j] = q.uneg;
         inside[j] = cell_inside(p.ix, q);
-        // theta / 2 pi in turns (exact range reduction in sincospi)
+        uneg[j] = q.uneg;
+        double fx0, fy0;
+        const int ix0 = floor_small(inside[j] ? q.uidx : 0.0, &fx0), iy0 = floor_small(inside[j] ? q.vidx : 0.0, &fy0);
+        tx[j] = __dsub_rn(q.uidx, fx0);                  // (outside the grid the rare path below redoes this)
+        ty[j] = __dsub_rn(q.vidx, fy0);
+        // theta / 2 pi in turns (exact range reduction in sincos_turns)
         turns[j] = fma(q.urot, p.dRA_turns, q.vrot * p.dDec_turns);
-#ifdef GAL_DBG_NOGATHER
-        const int off = inside[j] ? ((int)fx0 * N + (int)fy0) & 7 : 0;
-#else
-        const int off = inside[j] ? (int)fx0 * N + (int)fy0 : 0;
-#endif
+        const int off = ix0 * N + iy0;                   // 0 outside
         const int off_partner = __shfl_xor_sync(0xffffffffu, off, 1);
         const NodePair<T> ea = load_pair(spec + ((odd ? off_partner : off) + odd));
         const NodePair<T> eb = load_pair(spec + ((odd ? off : off_partner) + odd));
         ga0[j] = ea.a; ga1[j] = ea.b;
         gb0[j] = eb.a; gb1[j] = eb.b;
+        tx_partner[j] = __shfl_xor_sync(0xffffffffu, tx[j], 1);     // in flight with the gather
     }
 #pragma unroll
     for (int j = 0; j < U; ++j) {
-        const double tx_partner = __shfl_xor_sync(0xffffffffu, tx[j], 1);
-        const double txa = odd ? tx_partner : tx[j], txb = odd ? tx[j] : tx_partner;
+        const double txa = odd ? tx_partner[j] : tx[j], txb = odd ? tx[j] : tx_partner[j];
         // this lane's row (kvs + odd) of both cells, interpolated along u: g0 + t (g1 - g0)
         const double ra_re = fma(txa, (double)ga1[j].x - (double)ga0[j].x, (double)ga0[j].x);
         const double ra_im = fma(txa, (double)ga1[j].y - (double)ga0[j].y, (double)ga0[j].y);
@@ -302,19 +362,16 @@ __device__ __forceinline__ void sample_points(const SampleParams<T>& p, SampleCt
             if (q.uidx > p.ix.fH || q.vidx < 0.0 || q.vidx > p.ix.fN1) ++cx_.oob;
             const cx<T> g00 = node_any<T>(spec, N, iy, ix), g01 = node_any<T>(spec, N, iy, ix + 1);
             const cx<T> g10 = node_any<T>(spec, N, iy + 1, ix), g11 = node_any<T>(spec, N, iy + 1, ix + 1);
-            const double ax = 1.0 - tx[j], ay = 1.0 - ty[j];
-            ReInt = ay * (ax * (double)g00.x + tx[j] * (double)g01.x) + ty[j] * (ax * (double)g10.x + tx[j] * (double)g11.x);
-            ImInt = ay * (ax * (double)g00.y + tx[j] * (double)g01.y) + ty[j] * (ax * (double)g10.y + tx[j] * (double)g11.y);
+            const double txr = __dsub_rn(q.uidx, floor(q.uidx)), tyr = __dsub_rn(q.vidx, floor(q.vidx));
+            const double ax = 1.0 - txr, ay = 1.0 - tyr;
+            ReInt = ay * (ax * (double)g00.x + txr * (double)g01.x) + tyr * (ax * (double)g10.x + txr * (double)g11.x);
+            ImInt = ay * (ax * (double)g00.y + txr * (double)g01.y) + tyr * (ax * (double)g10.y + txr * (double)g11.y);
         }
         if (uneg[j]) ImInt = -ImInt;
         double vr = ReInt, vi = ImInt;
-#ifdef GAL_DBG_NOPHASE
-        if (false) {
-#else
         if (p.has_phase) {
-#endif
             double sn, co;
-            sincospi(2.0 * turns[j], &sn, &co);
+            sincos_turns(turns[j], &sn, &co);
             vr = ReInt * co - ImInt * sn;
             vi = ReInt * sn + ImInt * co;
         }
@@ -334,8 +391,8 @@ __device__ __forceinline__ void sample_points(const SampleParams<T>& p, SampleCt
 // no floating-point atomics.  Also adds this CTA's out-of-grid count.
 template <typename T, bool DO_CHI2>
 __device__ __forceinline__ void sample_finish(const SampleParams<T>& p, int c, double acc, unsigned int oob) {
-    __shared__ double wsum[8];
-    __shared__ unsigned int woob[8];
+    __shared__ double wsum[32];
+    __shared__ unsigned int woob[32];
     __shared__ bool is_last;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
 #pragma unroll
@@ -415,85 +472,94 @@ __device__ __forceinline__ void sample_tile_plain(const SampleParams<T>& p, Samp
     sample_points<T, WRITE_VIS, DO_CHI2, EXACT, U>(p, cx_, ld, kpt, M, c);
 }
 
-// General kernel: any alignment, any du (takes the true division when the shortcut is not valid).
-template <typename T, bool WRITE_VIS, bool DO_CHI2>
-__global__ void __launch_bounds__(256, GAL_SAMPLE_MINB) sample_kernel_plain(const SampleParams<T> p) {
-    constexpr int TILE = SampleGeom<T, DO_CHI2>::TILE;
-    const int c = blockIdx.y;
-    const long long M = p.M;
+template <typename T>
+__device__ __forceinline__ SampleCtx<T> sample_ctx(const SampleParams<T>& p, int c) {
     SampleCtx<T> cx_;
     cx_.N = p.N;
     cx_.spec = p.spec + (long long)c * (p.N / 2 + 1) * p.N;
     cx_.odd = threadIdx.x & 1;
     cx_.acc = 0.0;
     cx_.oob = 0;
-    const long long ntiles = (M + TILE - 1) / TILE;
+    return cx_;
+}
+
+// General kernel (256 threads): any alignment, any du (takes the true division when the shortcut is not valid).
+template <typename T, bool WRITE_VIS, bool DO_CHI2>
+__global__ void __launch_bounds__(256, GAL_SAMPLE_MINB) sample_kernel_plain(const SampleParams<T> p) {
+    using G = SampleGeom<T, DO_CHI2>;
+    const int c = blockIdx.y;
+    const long long M = p.M;
+    SampleCtx<T> cx_ = sample_ctx(p, c);
+    const long long ntiles = (M + G::TILE - 1) / G::TILE;
     for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x)
         sample_tile_plain<T, WRITE_VIS, DO_CHI2, true>(p, cx_, tile, M, c);
     sample_finish<T, DO_CHI2>(p, c, cx_.acc, cx_.oob);
 }
 
-// Fast kernel: every per-point array 16-byte aligned in every channel, du fit for the division shortcut.
-// Thread 0 is the TMA producer: it keeps S-1 whole tiles in flight in a ring of shared-memory stages; the
-// ragged last tile (if any) is read with plain loads by the CTA whose turn it would have been.
+__device__ __forceinline__ void mbar_arrive(uint32_t mb) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(mb) : "memory");
+}
+
+// Fast kernel (256 consumer threads + one producer warp): every per-point array 16-byte aligned in every
+// channel, du fit for the division shortcut.  Warp specialisation: lane 0 of the ninth warp is the TMA
+// producer — it waits for a stage to be released (`empty` mbarrier, one arrival per consumer warp), arms the
+// `full` mbarrier with the byte count and issues the bulk copies of the next tile; the consumer warps wait on
+// `full`, work, and release the stage.  No block-wide barrier in the loop: a consumer warp only ever waits
+// for data, the producer runs up to S tiles ahead.  The ragged last tile (if any) is read with plain loads
+// by the CTA whose turn it would have been.
 template <typename T, bool WRITE_VIS, bool DO_CHI2>
-__global__ void __launch_bounds__(256, GAL_SAMPLE_MINB) sample_kernel_tma(const SampleParams<T> p) {
+__global__ void __launch_bounds__(SampleGeom<T, DO_CHI2>::NT_TMA, GAL_SAMPLE_MINB) sample_kernel_tma(const SampleParams<T> p) {
     using G = SampleGeom<T, DO_CHI2>;
     constexpr int U = G::U, TILE = G::TILE, S = G::S;
     extern __shared__ __align__(128) unsigned char sample_smem[];
-    const int tid = threadIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int c = blockIdx.y;
     const long long M = p.M;
-    SampleCtx<T> cx_;
-    cx_.N = p.N;
-    cx_.spec = p.spec + (long long)c * (p.N / 2 + 1) * p.N;
-    cx_.odd = tid & 1;
-    cx_.acc = 0.0;
-    cx_.oob = 0;
-    const long long nfull = M / TILE;
+    SampleCtx<T> cx_ = sample_ctx(p, c);
+    const int nfull = (int)(M / TILE);
     const uint32_t stage0 = smem_u32(sample_smem);
-    const uint32_t bar0 = stage0 + S * G::STAGE_BYTES;
+    const uint32_t full0 = stage0 + S * G::STAGE_BYTES, empty0 = full0 + 8 * S;
+    if (tid == 0) {
+        for (int s = 0; s < S; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, G::NW); }
+        mbar_fence_init();
+    }
+    __syncthreads();
 
-    // producer state (thread 0 only)
-    uint64_t pol = 0;
-    long long ptile = blockIdx.x;            // next tile to request
-    uint32_t pstage = 0;
-    auto produce = [&]() {
-        if (ptile < nfull) {
-            const uint32_t mb = bar0 + 8 * pstage, dst = stage0 + pstage * G::STAGE_BYTES;
-            const long long k = ptile * TILE + c * M;
-            mbar_expect_tx(mb, G::STAGE_BYTES);
-            tma_load_1d(dst, p.u + k, G::ARR_BYTES, mb, pol);
-            tma_load_1d(dst + G::ARR_BYTES, p.v + k, G::ARR_BYTES, mb, pol);
-            if (DO_CHI2) {
-                tma_load_1d(dst + 2 * G::ARR_BYTES, p.re_obs + k, G::ARR_BYTES, mb, pol);
-                tma_load_1d(dst + 3 * G::ARR_BYTES, p.im_obs + k, G::ARR_BYTES, mb, pol);
-                tma_load_1d(dst + 4 * G::ARR_BYTES, p.w + k, G::ARR_BYTES, mb, pol);
+    if (wid == G::NW) {
+        if (lane == 0) {                                     // ---- producer ----
+            const uint64_t pol = l2_policy_evict_first();
+            uint32_t stage = 0, parity = 1;                  // a fresh mbarrier lets a wait on parity 1 through
+            for (int tile = blockIdx.x; tile < nfull; tile += gridDim.x) {
+                mbar_wait(empty0 + 8 * stage, parity);
+                const uint32_t mb = full0 + 8 * stage, dst = stage0 + stage * G::STAGE_BYTES;
+                const long long k = (long long)tile * TILE + c * M;
+                mbar_expect_tx(mb, G::STAGE_BYTES);
+                tma_load_1d(dst, p.u + k, G::ARR_BYTES, mb, pol);
+                tma_load_1d(dst + G::ARR_BYTES, p.v + k, G::ARR_BYTES, mb, pol);
+                if (DO_CHI2) {
+                    tma_load_1d(dst + 2 * G::ARR_BYTES, p.re_obs + k, G::ARR_BYTES, mb, pol);
+                    tma_load_1d(dst + 3 * G::ARR_BYTES, p.im_obs + k, G::ARR_BYTES, mb, pol);
+                    tma_load_1d(dst + 4 * G::ARR_BYTES, p.w + k, G::ARR_BYTES, mb, pol);
+                }
+                if (++stage == S) { stage = 0; parity ^= 1u; }
             }
         }
-        ptile += gridDim.x;
-        pstage = (pstage + 1 == S) ? 0 : pstage + 1;
-    };
-    if (tid == 0) {
-        for (int s = 0; s < S; ++s) mbar_init(bar0 + 8 * s, 1);
-        mbar_fence_init();
-        pol = l2_policy_evict_first();
-        for (int s = 0; s < S - 1; ++s) produce();
+    } else {                                                 // ---- consumers ----
+        uint32_t stage = 0, parity = 0;
+        int tile = blockIdx.x;
+        for (; tile < nfull; tile += gridDim.x) {
+            mbar_wait(full0 + 8 * stage, parity);
+            const T* st = reinterpret_cast<const T*>(sample_smem + stage * G::STAGE_BYTES) + tid;
+            auto ld = [&](int a, int j) -> double { return (double)st[a * TILE + j * 256]; };
+            auto kpt = [&](int j) -> long long { return (long long)tile * TILE + j * 256 + tid; };
+            sample_points<T, WRITE_VIS, DO_CHI2, false, U>(p, cx_, ld, kpt, M, c);
+            __syncwarp();                                    // every lane has read its last value of this stage
+            if (lane == 0) mbar_arrive(empty0 + 8 * stage);
+            if (++stage == S) { stage = 0; parity ^= 1u; }
+        }
+        if (tile == nfull && (long long)nfull * TILE < M)    // the ragged last tile falls to this CTA
+            sample_tile_plain<T, WRITE_VIS, DO_CHI2, false>(p, cx_, nfull, M, c);
     }
-
-    uint32_t cstage = 0, cparity = 0;
-    for (long long tile = blockIdx.x; tile < nfull; tile += gridDim.x) {
-        __syncthreads();                                 // the stage consumed one trip ago is free again
-        if (tid == 0) produce();
-        mbar_wait(bar0 + 8 * cstage, cparity);
-        const T* st = reinterpret_cast<const T*>(sample_smem + cstage * G::STAGE_BYTES) + tid;
-        auto ld = [&](int a, int j) -> double { return (double)st[a * TILE + j * 256]; };
-        auto kpt = [&](int j) -> long long { return tile * TILE + j * 256 + tid; };
-        sample_points<T, WRITE_VIS, DO_CHI2, false, U>(p, cx_, ld, kpt, M, c);
-        if (++cstage == S) { cstage = 0; cparity ^= 1u; }
-    }
-    if (nfull * TILE < M && (long long)blockIdx.x == nfull % gridDim.x)
-        sample_tile_plain<T, WRITE_VIS, DO_CHI2, false>(p, cx_, nfull, M, c);
     sample_finish<T, DO_CHI2>(p, c, cx_.acc, cx_.oob);
 }
 
