@@ -336,49 +336,52 @@ col_pass_kernel(const ColParams<T> p) {
     cx<T>* smem = reinterpret_cast<cx<T>*>(smem_raw);
     const int tid = threadIdx.x;
     const int f = tid / G::TPF, t = tid % G::TPF;
-    const long long g = (long long)blockIdx.x * F + f;
     const int NU = L / 2 + 1;
-    const int ku = (int)(g % NU);
     // uv extent: columns beyond kumax are skipped, rows outside [rmin, rmax] are not written
     const int kumax = __ldg(p.ext), rmin = __ldg(p.ext + 1), rmax = __ldg(p.ext + 2);
-    {
-        bool any = false;
-#pragma unroll
-        for (int ff = 0; ff < F; ++ff) {
-            const long long gg = (long long)blockIdx.x * F + ff;
-            any = any || (gg < p.cols_total && (int)(gg % NU) <= kumax);
-        }
-        if (!any) return;
-    }
-    const bool valid = g < p.cols_total && ku <= kumax;
-    const cx<T>* col = p.work + (valid ? g : 0) * (long long)L;
-    NodePair<T>* own = p.pair + (valid ? g : 0) * (long long)L;          // .a of this column's entries
-    NodePair<T>* prev = own - (ku > 0 ? L : 0);                          // .b of the entries one column down
     cx<T>* S = smem + f * G::REGION;
+    {
+        const long long grp = blockIdx.x;                   // one group of F columns per CTA
+        const long long g = grp * F + f;
+        const int ku = (int)(g % NU);
+        {
+            bool any = false;
+#pragma unroll
+            for (int ff = 0; ff < F; ++ff) {
+                const long long gg = grp * F + ff;
+                any = any || (gg < p.cols_total && (int)(gg % NU) <= kumax);
+            }
+            if (!any) return;
+        }
+        const bool valid = g < p.cols_total && ku <= kumax;
+        const cx<T>* col = p.work + (valid ? g : 0) * (long long)L;
+        NodePair<T>* own = p.pair + (valid ? g : 0) * (long long)L;          // .a of this column's entries
+        NodePair<T>* prev = own - (ku > 0 ? L : 0);                          // .b of the entries one column down
 
-    fft_steps12<T, R1, R2, R3, G::TPF>(S, t, p.tw, 1, [&](int n) -> cx<T> {
-        return valid ? col[n] : mk<T>(0, 0);
-    });
-    // step 3 straight to global memory: kv = k1 + R1*(c + R2*d); sign (-1)^(ku+kv) folds the image
-    // centre shift, row (kv + N/2) mod N folds the shift along v.  Each value goes to its own entry (.a)
-    // and to the entry of the column before (.b).
-    for (int it = t; it < R1 * R2; it += G::TPF) {
-        const int k1 = it % R1, c = it / R1;
-        const cx<T>* base = S + k1 * G::P1 + c * R3;
-        cx<T> a[R3];
+        fft_steps12<T, R1, R2, R3, G::TPF>(S, t, p.tw, 1, [&](int n) -> cx<T> {
+            return valid ? col[n] : mk<T>(0, 0);
+        });
+        // step 3 straight to global memory: kv = k1 + R1*(c + R2*d); sign (-1)^(ku+kv) folds the image
+        // centre shift, row (kv + N/2) mod N folds the shift along v.  Each value goes to its own entry (.a)
+        // and to the entry of the column before (.b).
+        for (int it = t; it < R1 * R2; it += G::TPF) {
+            const int k1 = it % R1, c = it / R1;
+            const cx<T>* base = S + k1 * G::P1 + c * R3;
+            cx<T> a[R3];
 #pragma unroll
-        for (int b = 0; b < R3; ++b) a[b] = base[b];
-        Dft<T, R3>::run(a);
-        if (valid) {
+            for (int b = 0; b < R3; ++b) a[b] = base[b];
+            Dft<T, R3>::run(a);
+            if (valid) {
 #pragma unroll
-            for (int d = 0; d < R3; ++d) {
-                const int kv = k1 + R1 * (c + R2 * d);
-                const T sgn = ((ku + kv) & 1) ? (T)-1 : (T)1;
-                const int kvs = (kv + L / 2) & (L - 1);
-                if (kvs >= rmin && kvs <= rmax) {
-                    const cx<T> val = mk<T>(sgn * a[d].x, sgn * a[d].y);
-                    own[kvs].a = val;
-                    if (ku > 0) prev[kvs].b = val;
+                for (int d = 0; d < R3; ++d) {
+                    const int kv = k1 + R1 * (c + R2 * d);
+                    const T sgn = ((ku + kv) & 1) ? (T)-1 : (T)1;
+                    const int kvs = (kv + L / 2) & (L - 1);
+                    if (kvs >= rmin && kvs <= rmax) {
+                        const cx<T> val = mk<T>(sgn * a[d].x, sgn * a[d].y);
+                        own[kvs].a = val;
+                        if (ku > 0) prev[kvs].b = val;
+                    }
                 }
             }
         }

@@ -163,6 +163,11 @@ struct ExtentParams {
     int* ext;              // [3], initialised by the host to the cell of the sampler's dead slots
 };
 
+// Every step of the index arithmetic after the rotation is monotone in its argument (a correctly rounded
+// division by du > 0, a rounded addition to N/2, floor), so the extremes of the indices are the indices of
+// the extremes: the loop only tracks max |u'| and min / max of the signed v term (v' where u' >= 0, -v'
+// where u' < 0 — the listing's N/2 - v'/du equals N/2 + (-v')/du bit for bit) and the divisions, the floor and
+// the inside-the-grid test are applied once per warp to those three numbers.
 template <typename T>
 __global__ void __launch_bounds__(256, 4) uv_extent_kernel(const ExtentParams p, const T* __restrict__ u,
                                                            const T* __restrict__ v) {
@@ -170,7 +175,7 @@ __global__ void __launch_bounds__(256, 4) uv_extent_kernel(const ExtentParams p,
     // trip are issued before the arithmetic of this one (register double buffer).
     constexpr int EU = 4;
     const int N = p.N, H = N >> 1;
-    int cmax = 0, rmin = N - 1, rmax = 0;
+    double umax = 0.0, smin = 0.0, smax = 0.0;               // (0, 0): the dead-slot cell, always in the extent
     const long long stride = (long long)gridDim.x * blockDim.x * EU;
     long long k0 = (long long)blockIdx.x * blockDim.x * EU + threadIdx.x;
     double nu[EU], nv[EU];
@@ -180,7 +185,7 @@ __global__ void __launch_bounds__(256, 4) uv_extent_kernel(const ExtentParams p,
             const long long k = kk + j * 256;
             const bool ok = k < p.total;
             nu[j] = ok ? (double)__ldcs(u + k) : 0.0;
-            nv[j] = ok ? (double)__ldcs(v + k) : 0.0;      // (0, 0) is the dead-slot cell, already in the extent
+            nv[j] = ok ? (double)__ldcs(v + k) : 0.0;
         }
     };
     fetch(k0);
@@ -191,25 +196,39 @@ __global__ void __launch_bounds__(256, 4) uv_extent_kernel(const ExtentParams p,
         fetch(k0 + stride);
 #pragma unroll
         for (int j = 0; j < EU; ++j) {
-            const PointIndex q = point_index<false>(p.ix, pu[j], pv[j]);
-            if (cell_inside(p.ix, q)) {
-                double f_;
-                const int ix = floor_small(q.uidx, &f_), iy = floor_small(q.vidx, &f_);
-                cmax = max(cmax, ix + 1);
-                rmin = min(rmin, iy);
-                rmax = max(rmax, iy + 1);
-            } else {
-                cmax = H; rmin = 0; rmax = N - 1;
-            }
+            const double urot = __dsub_rn(__dmul_rn(pu[j], p.ix.cos_PA), __dmul_rn(pv[j], p.ix.sin_PA));
+            const double vrot = __dadd_rn(__dmul_rn(pu[j], p.ix.sin_PA), __dmul_rn(pv[j], p.ix.cos_PA));
+            const double sv = urot < 0.0 ? -vrot : vrot;
+            umax = fmax(umax, fabs(urot));
+            smin = fmin(smin, sv);
+            smax = fmax(smax, sv);
         }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
-        cmax = max(cmax, __shfl_xor_sync(0xffffffffu, cmax, o));
-        rmin = min(rmin, __shfl_xor_sync(0xffffffffu, rmin, o));
-        rmax = max(rmax, __shfl_xor_sync(0xffffffffu, rmax, o));
+        umax = fmax(umax, __shfl_xor_sync(0xffffffffu, umax, o));
+        smin = fmin(smin, __shfl_xor_sync(0xffffffffu, smin, o));
+        smax = fmax(smax, __shfl_xor_sync(0xffffffffu, smax, o));
     }
-    if ((threadIdx.x & 31) == 0) {
+    // one set of atomics per CTA: same-address atomics serialise in L2 and would otherwise be the kernel's tail
+    __shared__ double red[3][8];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (lane == 0) { red[0][wid] = umax; red[1][wid] = smin; red[2][wid] = smax; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int i = 1; i < 8; ++i) {
+            umax = fmax(umax, red[0][i]); smin = fmin(smin, red[1][i]); smax = fmax(smax, red[2][i]);
+        }
+        PointIndex lo, hi;                                    // the two extreme cells of this CTA's points
+        lo.uidx = hi.uidx = div_by<false>(umax, p.ix);
+        lo.vidx = __dadd_rn(p.ix.fH, div_by<false>(smin, p.ix));
+        hi.vidx = __dadd_rn(p.ix.fH, div_by<false>(smax, p.ix));
+        int cmax = H, rmin = 0, rmax = N - 1;                 // a cell leaves the grid: everything (reading A6)
+        if (cell_inside(p.ix, lo) && cell_inside(p.ix, hi)) {
+            cmax = (int)floor(hi.uidx) + 1;
+            rmin = (int)floor(lo.vidx);
+            rmax = (int)floor(hi.vidx) + 1;
+        }
         atomicMax(p.ext + 0, cmax);
         atomicMin(p.ext + 1, rmin);
         atomicMax(p.ext + 2, rmax);
