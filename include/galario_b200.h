@@ -82,6 +82,18 @@ int gal_plan_set_pruning(gal_plan* plan, int mode);
  * {nxy/2, 0, nxy-1} if that call did not prune).  Synchronises the stream of that call. */
 int gal_last_uv_extent(gal_plan* plan, int* extent);
 
+/* ---- get_image_size (Eq. 19-24; host only, no device is touched): image size N_lm (rounded
+ *      up to a power of two) and pixel size (radians) for the uv coverage u[M], v[M] (HOST pointers,
+ *      wavelengths).  With q_min / q_max the shortest / longest baseline sqrt(u^2 + v^2):
+ *        PB <= 0 (criterion iia): duv = q_min / (Gamma f_min) (Eq. 21, Gamma = 0.6 as for ALMA) and
+ *                 N = 2 f_max q_max / duv (Eq. 19; Eq. 22 as printed drops f_max, Table 1 is only reproduced
+ *                 with it);
+ *        PB  > 0 (criterion iib): the field of view is the primary beam, duv = 1 / PB (Eq. 23), N as above.
+ *      dxy = 1 / (N duv) (Eq. 16).  The paper's Table 1 uses f_min = 5, f_max = 2.5 (pass <= 0 for these defaults).
+ *      Errors: GAL_ERR_INVALID_ARGUMENT for null pointers, M < 1, a zero or non-finite baseline. ---- */
+int gal_get_image_size(const double* u, const double* v, int64_t M, double PB, double f_min, double f_max,
+                       int* nxy_out, double* dxy_out);
+
 /* Diagnostic per-kernel timing.  After gal_plan_timing_enable(plan, n) the next n sample/chi2 calls record a
  * CUDA event on their stream before the first kernel, between the kernels and after the sampling kernel
  * (n = 0 switches it off and frees the events).  gal_plan_timing_read synchronises those events and returns

@@ -44,6 +44,7 @@ def load_library() -> ctypes.CDLL:
             getattr(lib, name).argtypes = [_vp]
         lib.gal_plan_timing_enable.argtypes = [_vp, _i]
         lib.gal_plan_timing_read.argtypes = [_vp, _vp, _vp]
+        lib.gal_get_image_size.argtypes = [_vp, _vp, _i64, _d, _d, _d, _vp, _vp]
         lib.gal_plan_set_pruning.argtypes = [_vp, _i]
         lib.gal_last_uv_extent.argtypes = [_vp, _vp]
         for s in ("f64", "f32"):
@@ -72,6 +73,19 @@ def _check(rc: int, what: str, plan: "Plan" = None) -> None:
         msg = load_library().gal_strerror(rc).decode()
         extra = f" (cudaError {load_library().gal_last_cuda_error(plan._h)})" if plan is not None and rc == -3 else ""
         raise GalarioError(f"{what}: {msg}{extra}")
+
+
+def get_image_size(u, v, PB: float = 0.0, f_min: float = 5.0, f_max: float = 2.5):
+    """(N_lm, dxy) for the uv coverage (host arrays, wavelengths): Eq. 19-24."""
+    u = np.ascontiguousarray(u, dtype=np.float64)
+    v = np.ascontiguousarray(v, dtype=np.float64)
+    if u.shape != v.shape:
+        raise GalarioError("u and v must have the same shape")
+    n, d = ctypes.c_int(0), ctypes.c_double(0.0)
+    _check(load_library().gal_get_image_size(u.ctypes.data, v.ctypes.data, u.size, float(PB), float(f_min),
+                                             float(f_max), ctypes.addressof(n), ctypes.addressof(d)),
+           "gal_get_image_size")
+    return n.value, d.value
 
 
 def _stream() -> int:

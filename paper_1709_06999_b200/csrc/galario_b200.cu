@@ -549,6 +549,30 @@ int gal_last_uv_extent(gal_plan* p, int* extent) {
     return GAL_OK;
 }
 
+int gal_get_image_size(const double* u, const double* v, int64_t M, double PB, double f_min, double f_max,
+                       int* nxy_out, double* dxy_out) {
+    if (!u || !v || M < 1 || !nxy_out || !dxy_out || !std::isfinite(PB)) return GAL_ERR_INVALID_ARGUMENT;
+    if (!(f_min > 0)) f_min = 5.0;
+    if (!(f_max > 0)) f_max = 2.5;
+    double qmin = INFINITY, qmax = 0.0;
+    for (int64_t k = 0; k < M; ++k) {
+        const double q = std::hypot(u[k], v[k]);
+        if (!std::isfinite(q)) return GAL_ERR_INVALID_ARGUMENT;
+        qmin = q < qmin ? q : qmin;
+        qmax = q > qmax ? q : qmax;
+    }
+    if (!(qmin > 0)) return GAL_ERR_INVALID_ARGUMENT;
+    const double Gamma = 0.6;
+    const double duv = PB > 0 ? 1.0 / PB : qmin / (Gamma * f_min);   // Eq. 23 / Eq. 21
+    const double n_raw = 2.0 * f_max * qmax / duv;              // Eq. 19
+    if (!(n_raw < 1073741824.0)) return GAL_ERR_INVALID_ARGUMENT;
+    int n = 2;
+    while ((double)n < n_raw) n *= 2;
+    *nxy_out = n;
+    *dxy_out = 1.0 / ((double)n * duv);                         // Eq. 16
+    return GAL_OK;
+}
+
 size_t gal_plan_workspace_bytes(const gal_plan* p) { return p ? p->owned_bytes : 0; }
 int gal_last_cuda_error(const gal_plan* p) { return p ? p->last_cuda : 0; }
 int64_t gal_plan_launch_count(const gal_plan* p) { return p ? p->launches : -1; }

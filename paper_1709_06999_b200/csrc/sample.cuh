@@ -87,11 +87,22 @@ __device__ __forceinline__ bool cell_inside(const IndexScalars& s, const PointIn
 // range reduction of sincospi per point that pipe, not memory, bounded the sampler (ncu: XU 95 % busy).
 // Both are therefore done with plain FP64 adds and integer bit moves.
 //
+// The constants of both routines live in constant memory so that each FP64 instruction reads its constant
+// as a constant-bank operand; as literals they cost two uniform-register moves apiece, per point.
+// [0..5] sine, [6..11] cosine kernel coefficients (fdlibm), then 1.5 * 2^52, pi / 2, 2^52.
+__constant__ double SINCOS_COEF[16] = {
+    1.58969099521155010221e-10, -2.50507602534068634195e-08, 2.75573137070700676789e-06,
+    -1.98412698298579493134e-04, 8.33333333332248946124e-03, -1.66666666666666324348e-01,
+    -1.13596475577881948265e-11, 2.08757232129817482790e-09, -2.75573143513906633035e-07,
+    2.48015872894767294178e-05, -1.38888888888741095749e-03, 4.16666666666666019037e-02,
+    6755399441055744.0 /* 1.5 * 2^52: keeps negative k in range */, 1.57079632679489661923, 4503599627370496.0 /* 2^52 */, 0.0};
+
+//
 // floor of 0 <= x < 2^31 as a double (*fl) and as an int (return): x + 2^52 rounds x to an integer in the
 // low mantissa bits; one compare fixes round-to-nearest into round-down.  fl is exactly floor(x), so the
 // fractional weight x - fl is bit-identical to the listing's.  (Only used for cells inside the grid.)
 __device__ __forceinline__ int floor_small(double x, double* fl) {
-    const double MAGIC = 4503599627370496.0;             // 2^52
+    const double MAGIC = SINCOS_COEF[14];                // 2^52 (constant-bank operand)
     const double t = __dadd_rn(x, MAGIC);
     double r = __dsub_rn(t, MAGIC);                      // rint(x)
     int i = __double2loint(t);
@@ -105,25 +116,25 @@ __device__ __forceinline__ int floor_small(double x, double* fl) {
 // minimax polynomials (fdlibm's kernel coefficients) are good to < 1 ulp; the quadrant k mod 4 then swaps and
 // signs the pair.
 __device__ __forceinline__ void sincos_turns(double t, double* sn, double* cs) {
-    const double MAGIC = 6755399441055744.0;             // 1.5 * 2^52: keeps negative k in range
+    const double* K = SINCOS_COEF;
     const double t4 = 4.0 * t;
-    const double z = __dadd_rn(t4, MAGIC);
+    const double z = __dadd_rn(t4, K[12]);
     const int q = __double2loint(z);
-    const double a = (t4 - (z - MAGIC)) * 1.57079632679489661923;
+    const double a = (t4 - (z - K[12])) * K[13];
     const double a2 = a * a;
-    double ps = 1.58969099521155010221e-10;
-    ps = fma(ps, a2, -2.50507602534068634195e-08);
-    ps = fma(ps, a2, 2.75573137070700676789e-06);
-    ps = fma(ps, a2, -1.98412698298579493134e-04);
-    ps = fma(ps, a2, 8.33333333332248946124e-03);
-    ps = fma(ps, a2, -1.66666666666666324348e-01);
+    double ps = K[0];
+    ps = fma(ps, a2, K[1]);
+    ps = fma(ps, a2, K[2]);
+    ps = fma(ps, a2, K[3]);
+    ps = fma(ps, a2, K[4]);
+    ps = fma(ps, a2, K[5]);
     const double s = fma(a * a2, ps, a);
-    double pc = -1.13596475577881948265e-11;
-    pc = fma(pc, a2, 2.08757232129817482790e-09);
-    pc = fma(pc, a2, -2.75573143513906633035e-07);
-    pc = fma(pc, a2, 2.48015872894767294178e-05);
-    pc = fma(pc, a2, -1.38888888888741095749e-03);
-    pc = fma(pc, a2, 4.16666666666666019037e-02);
+    double pc = K[6];
+    pc = fma(pc, a2, K[7]);
+    pc = fma(pc, a2, K[8]);
+    pc = fma(pc, a2, K[9]);
+    pc = fma(pc, a2, K[10]);
+    pc = fma(pc, a2, K[11]);
     const double c = fma(a2 * a2, pc, fma(a2, -0.5, 1.0));
     const double ss = (q & 1) ? c : s, cc = (q & 1) ? s : c;
     *sn = (q & 2) ? -ss : ss;
@@ -256,6 +267,17 @@ __device__ __forceinline__ void mbar_wait(uint32_t mb, uint32_t parity) {
         "bra WAIT_%=;\n"
         "DONE_%=:\n"
         "}\n" ::"r"(mb), "r"(parity) : "memory");
+}
+// same, for a thread that expects to wait long (the producer): sleep between polls so the spin does not
+// take issue slots from the warps that share its scheduler
+__device__ __forceinline__ void mbar_wait_relaxed(uint32_t mb, uint32_t parity) {
+    uint32_t done = 0;
+    for (;;) {
+        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                     : "=r"(done) : "r"(mb), "r"(parity) : "memory");
+        if (done) break;
+        __nanosleep(200);
+    }
 }
 __device__ __forceinline__ uint64_t l2_policy_evict_first() {
     uint64_t pol;
@@ -549,7 +571,7 @@ __global__ void __launch_bounds__(SampleGeom<T, DO_CHI2>::NT_TMA, GAL_SAMPLE_MIN
             const uint64_t pol = l2_policy_evict_first();
             uint32_t stage = 0, parity = 1;                  // a fresh mbarrier lets a wait on parity 1 through
             for (int tile = blockIdx.x; tile < nfull; tile += gridDim.x) {
-                mbar_wait(empty0 + 8 * stage, parity);
+                mbar_wait_relaxed(empty0 + 8 * stage, parity);
                 const uint32_t mb = full0 + 8 * stage, dst = stage0 + stage * G::STAGE_BYTES;
                 const long long k = (long long)tile * TILE + c * M;
                 mbar_expect_tx(mb, G::STAGE_BYTES);

@@ -72,3 +72,34 @@ def test_workloads_shapes_and_determinism():
     assert c4.image.shape == (3, 64, 64) and c4.u.shape == (3, 500) and c4.entry == "chi2ImageBatch"
     f = a.as_f32()
     assert f.image.dtype == np.float32 and f.u.dtype == np.float32 and f.precision == "f32"
+
+
+def test_get_image_size_reproduces_table1():
+    """The one place the paper prints numbers this repo can recompute: N_lm (iia), the pixel
+    size and the nominal resolution of 14 ALMA / VLA configurations, from their shortest and longest baseline.
+    Host-only call: runs without a GPU."""
+    import numpy as np
+    import paper_1709_06999_b200 as g
+    ARCSEC = np.pi / 648000.0
+    rows = [l.split() for l in (ROOT / "tests" / "golden" / "table1_image_size.txt").read_text().splitlines()
+            if l.strip() and not l.startswith("#")]
+    assert len(rows) == 14
+    for array, cfg, bmin, bmax, n_iia, dtheta, theta_res in rows:
+        lam = 1.3e-3 if array == "ALMA" else 7.0e-3
+        qmin, qmax = float(bmin) / lam, float(bmax) / lam
+        # two baselines at arbitrary azimuths carry the extremes; a third one in between must not matter
+        u = np.array([qmin * np.cos(0.3), -qmax * np.cos(1.1), 0.5 * (qmin + qmax)])
+        v = np.array([qmin * np.sin(0.3), qmax * np.sin(1.1), 0.0])
+        n, dxy = g.get_image_size(u, v)                       # paper defaults: f_min = 5, f_max = 2.5
+        assert n == int(n_iia), (cfg, n)
+        assert abs(dxy / ARCSEC - float(dtheta)) <= 6e-4, (cfg, dxy / ARCSEC)
+        assert abs(1.0 / qmax / ARCSEC - float(theta_res)) <= 6e-4, cfg          # theta_res = lambda / B_max
+        # the result satisfies the two constraints it is derived from (Eq. 19 and Eq. 20)
+        duv = 1.0 / (n * dxy)
+        assert n * duv / 2 >= 2.5 * qmax * (1 - 1e-12) and n * dxy >= 5 * 0.6 / qmin * (1 - 1e-12)
+    # criterion (iib): field of view = primary beam (Eq. 23); ALMA 12 m antennas, K = 1.13 (PAPER.md:150-153)
+    lam, pb = 1.3e-3, 1.13 * 1.3e-3 / 12.0
+    n, dxy = g.get_image_size(np.array([14.6 / lam, 3637.8 / lam]), np.array([0.0, 0.0]), PB=pb)
+    assert n == 2048 and abs(n * dxy - pb) <= 1e-18          # 2 * 2.5 * q_max * PB = 1713 -> 2048
+    with pytest.raises(g.GalarioError):
+        g.get_image_size(np.array([0.0]), np.array([0.0]))
