@@ -40,6 +40,14 @@ template <typename T> using cx = typename Vec2<T>::type;
 // one entry of the sampled spectrum: the node of this column (.a) and of the next one (.b)
 template <typename T> struct __align__(2 * sizeof(cx<T>)) NodePair { cx<T> a, b; };
 
+// Programmatic dependent launch (sm_90+): let the next kernel of the chain start placing its CTAs, and wait
+// until the kernel before this one has completed and its writes are visible.  Every kernel of a call does both
+// before its first global-memory access (harmless when launched without the attribute).
+__device__ __forceinline__ void pdl_wait() {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
 template <typename T> __device__ __forceinline__ cx<T> mk(T x, T y) { cx<T> r; r.x = x; r.y = y; return r; }
 template <typename V> __device__ __forceinline__ V cadd(V a, V b) { a.x += b.x; a.y += b.y; return a; }
 template <typename V> __device__ __forceinline__ V csub(V a, V b) { a.x -= b.x; a.y -= b.y; return a; }
@@ -260,6 +268,7 @@ row_pass_kernel(const RowParams<T> p) {
     const long long row = row0 + f;
     const bool valid = row < p.rows_total;
     cx<T>* S = smem + f * G::REGION;
+    pdl_wait();
 
     if (SWEEP) {
         const int i = (int)(row % N);
@@ -337,6 +346,7 @@ col_pass_kernel(const ColParams<T> p) {
     const int tid = threadIdx.x;
     const int f = tid / G::TPF, t = tid % G::TPF;
     const int NU = L / 2 + 1;
+    pdl_wait();
     // uv extent: columns beyond kumax are skipped, rows outside [rmin, rmax] are not written
     const int kumax = __ldg(p.ext), rmin = __ldg(p.ext + 1), rmax = __ldg(p.ext + 2);
     cx<T>* S = smem + f * G::REGION;

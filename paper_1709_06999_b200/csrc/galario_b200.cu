@@ -75,6 +75,20 @@ template <typename K> int set_smem(gal_plan* p, K kernel, size_t bytes) {
     return GAL_OK;
 }
 
+// Programmatic dependent launch: the kernels of one call form a chain on the stream; each is launched with
+// programmatic stream serialisation so that its CTAs are placed and run their prologue while the kernel before
+// drains, and each waits (`griddepcontrol.wait`, fft.cuh: pdl_wait) before it touches memory.
+template <typename... KArgs, typename... Args>
+cudaError_t launch_chain(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 // ---------------------------------------------------------------------------------------------
 // FFT launchers
 // ---------------------------------------------------------------------------------------------
@@ -93,11 +107,11 @@ int launch_row(gal_plan* p, const T* image, const SweepParams* sw, int batch, co
     if (sw) {
         auto k = row_pass_kernel<T, R1, R2, R3, F, true>;
         int rc = set_smem(p, k, G::SMEM); if (rc) return rc;
-        k<<<grid, G::NT, G::SMEM, st>>>(rp);
+        GAL_CUDA(p, launch_chain(k, dim3(grid), dim3(G::NT), G::SMEM, st, rp));
     } else {
         auto k = row_pass_kernel<T, R1, R2, R3, F, false>;
         int rc = set_smem(p, k, G::SMEM); if (rc) return rc;
-        k<<<grid, G::NT, G::SMEM, st>>>(rp);
+        GAL_CUDA(p, launch_chain(k, dim3(grid), dim3(G::NT), G::SMEM, st, rp));
     }
     p->launches++;
     GAL_CUDA(p, cudaGetLastError());
@@ -118,7 +132,7 @@ int launch_col(gal_plan* p, int batch, const int* ext, cudaStream_t st) {
     const unsigned grid = (unsigned)((cp.cols_total + F - 1) / F);
     auto k = col_pass_kernel<T, R1, R2, R3, F>;
     int rc = set_smem(p, k, G::SMEM); if (rc) return rc;
-    k<<<grid, G::NT, G::SMEM, st>>>(cp);
+    GAL_CUDA(p, launch_chain(k, dim3(grid), dim3(G::NT), G::SMEM, st, cp));
     p->launches++;
     GAL_CUDA(p, cudaGetLastError());
     return GAL_OK;
@@ -210,7 +224,7 @@ int launch_extent(gal_plan* p, int C, const CallScalars& cs, const T* u, const T
     const long long cap = (long long)p->sm_count * 4;
     if (blocks > cap) blocks = cap;
     if (blocks < 1) blocks = 1;
-    uv_extent_kernel<T><<<(unsigned)blocks, 256, 0, st>>>(ep, u, v);
+    GAL_CUDA(p, launch_chain(uv_extent_kernel<T>, dim3((unsigned)blocks), dim3(256), 0, st, ep, u, v));
     p->launches++;
     GAL_CUDA(p, cudaGetLastError());
     return GAL_OK;
@@ -224,9 +238,9 @@ int launch_sample_kernel(gal_plan* p, const SampleParams<T>& sp, dim3 grid, bool
     if (tma) {
         auto k = sample_kernel_tma<T, WRITE_VIS, DO_CHI2>;
         int rc = set_smem(p, k, G::SMEM); if (rc) return rc;
-        k<<<grid, G::NT_TMA, G::SMEM, st>>>(sp);
+        GAL_CUDA(p, launch_chain(k, grid, dim3(G::NT_TMA), G::SMEM, st, sp));
     } else {
-        sample_kernel_plain<T, WRITE_VIS, DO_CHI2><<<grid, G::NT, 0, st>>>(sp);
+        GAL_CUDA(p, launch_chain(sample_kernel_plain<T, WRITE_VIS, DO_CHI2>, grid, dim3(G::NT), 0, st, sp));
     }
     return GAL_OK;
 }

@@ -187,6 +187,7 @@ __global__ void __launch_bounds__(256, 4) uv_extent_kernel(const ExtentParams p,
     constexpr int EU = 4;
     const int N = p.N, H = N >> 1;
     double umax = 0.0, smin = 0.0, smax = 0.0;               // (0, 0): the dead-slot cell, always in the extent
+    pdl_wait();
     const long long stride = (long long)gridDim.x * blockDim.x * EU;
     long long k0 = (long long)blockIdx.x * blockDim.x * EU + threadIdx.x;
     double nu[EU], nv[EU];
@@ -531,6 +532,7 @@ __global__ void __launch_bounds__(256, GAL_SAMPLE_MINB) sample_kernel_plain(cons
     const int c = blockIdx.y;
     const long long M = p.M;
     SampleCtx<T> cx_ = sample_ctx(p, c);
+    pdl_wait();
     const long long ntiles = (M + G::TILE - 1) / G::TILE;
     for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x)
         sample_tile_plain<T, WRITE_VIS, DO_CHI2, true>(p, cx_, tile, M, c);
@@ -564,6 +566,7 @@ __global__ void __launch_bounds__(SampleGeom<T, DO_CHI2>::NT_TMA, GAL_SAMPLE_MIN
         for (int s = 0; s < S; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, G::NW); }
         mbar_fence_init();
     }
+    pdl_wait();
     __syncthreads();
 
     if (wid == G::NW) {
