@@ -27,8 +27,13 @@ struct gal_plan {
     unsigned long long* oob = nullptr;   // call_state[0]; the uv extent follows it
     int* ext = nullptr;                  // {kumax, rmin, rmax} of the current call (device)
     int* ext_full = nullptr;             // constant {nxy/2, 0, nxy-1}: no pruning
-    void* call_state = nullptr;          // [oob (8 B) | ext (12 B) | pad] re-initialised per call from call_init
+    // Per-call device state [oob (8 B) | ext (12 B) | done ticket (4 B) | pad], two copies used alternately:
+    // the sampling kernel of call k re-arms the copy call k+1 will use, so no reset operation sits between
+    // two calls on the stream (an explicit copy from call_init is only needed when that did not happen).
+    void* call_state = nullptr;          // 2 x 32 B
     void* call_init = nullptr;
+    int cur = 0;                         // copy used by the most recent call
+    bool next_armed = false;             // the other copy has been / will be re-armed by that call's sampler
     int prune_mode = 1;                  // 0 never, 1 auto, 2 always
     bool last_pruned = false;            // did the most recent call compute a uv extent?
     std::set<const void*> smem_set;      // kernels whose dynamic shared-memory limit has been raised
@@ -198,7 +203,12 @@ CallScalars call_scalars(const gal_plan* p, double dxy, double dRA, double dDec,
 // Re-arm the per-call device state: out-of-grid counter = 0, uv extent = the cell of the dead slots
 // (column 0..1, rows N/2..N/2+1), which the sampler reads with weight 0 for the points past the end.
 int reset_call_state(gal_plan* p, cudaStream_t st) {
-    GAL_CUDA(p, cudaMemcpyAsync(p->call_state, p->call_init, 32, cudaMemcpyDeviceToDevice, st));
+    p->cur ^= 1;
+    p->oob = (unsigned long long*)((char*)p->call_state + 32 * p->cur);
+    p->ext = (int*)((char*)p->oob + 8);
+    if (!p->next_armed)
+        GAL_CUDA(p, cudaMemcpyAsync(p->oob, p->call_init, 32, cudaMemcpyDeviceToDevice, st));
+    p->next_armed = false;
     return GAL_OK;
 }
 
@@ -266,6 +276,8 @@ int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T
     sp.chi2_per_channel = chi2_pc;
     sp.chi2_total = chi2_tot;
     sp.oob = p->oob;
+    sp.done = (unsigned int*)((char*)p->oob + 20);
+    sp.next_state = (unsigned long long*)((char*)p->call_state + 32 * (p->cur ^ 1));
     // one CTA works through tiles blockIdx.x, blockIdx.x + gridDim.x, ...: a whole number of CTAs per SM
     const int tile = SampleGeom<T, true>::TILE;
     const long long ntiles = (M + tile - 1) / tile;
@@ -283,6 +295,7 @@ int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T
     if (rc) return rc;
     p->launches++;
     GAL_CUDA(p, cudaGetLastError());
+    p->next_armed = true;                 // the last CTA of this launch re-arms the other copy of the call state
     return GAL_OK;
 }
 
@@ -470,7 +483,7 @@ int gal_plan_create(gal_plan** out, int nxy, int batch, int precision_bits, int 
     if ((e = cudaMalloc((void**)&p->partials, sizeof(double) * (size_t)batch * p->max_gx)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     if ((e = cudaMalloc((void**)&p->tickets, sizeof(unsigned int) * (batch + 1))) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     if ((e = cudaMalloc((void**)&p->chi2_scratch, sizeof(double) * batch)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
-    if ((e = cudaMalloc(&p->call_state, 32)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
+    if ((e = cudaMalloc(&p->call_state, 64)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     if ((e = cudaMalloc(&p->call_init, 32)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     if ((e = cudaMalloc((void**)&p->ext_full, 16)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     p->oob = (unsigned long long*)p->call_state;
@@ -480,6 +493,7 @@ int gal_plan_create(gal_plan** out, int nxy, int batch, int precision_bits, int 
         int full[4] = {nxy / 2, 0, nxy - 1, 0};
         if ((e = cudaMemcpy(p->call_init, init, 32, cudaMemcpyHostToDevice)) != cudaSuccess) return fail(GAL_ERR_CUDA, e);
         if ((e = cudaMemcpy(p->call_state, init, 32, cudaMemcpyHostToDevice)) != cudaSuccess) return fail(GAL_ERR_CUDA, e);
+        if ((e = cudaMemcpy((char*)p->call_state + 32, init, 32, cudaMemcpyHostToDevice)) != cudaSuccess) return fail(GAL_ERR_CUDA, e);
         if ((e = cudaMemcpy(p->ext_full, full, 16, cudaMemcpyHostToDevice)) != cudaSuccess) return fail(GAL_ERR_CUDA, e);
     }
     if ((e = cudaMalloc((void**)&p->st_chi2, sizeof(double))) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);

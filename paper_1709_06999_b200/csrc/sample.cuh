@@ -45,7 +45,9 @@ template <typename T> struct SampleParams {
     unsigned int* tickets; // [C + 1]
     double* chi2_per_channel; // [C] or null
     double* chi2_total;       // [1] or null
-    unsigned long long* oob;  // [1]
+    unsigned long long* oob;  // [1]: this call's out-of-grid counter
+    unsigned int* done;       // [1]: CTAs of this launch that have finished
+    unsigned long long* next_state;  // the copy of the per-call state the NEXT call will use (32 B)
 };
 
 // Correctly rounded a / b from r = RN(1/b) (Markstein): q0 = RN(a r); rem = a - q0 b (exact in an
@@ -449,6 +451,14 @@ __device__ __forceinline__ void sample_finish(const SampleParams<T>& p, int c, d
         unsigned int ob = 0;
         for (int i = 0; i < (int)(blockDim.x >> 5); ++i) { s += wsum[i]; ob += woob[i]; }
         if (ob) atomicAdd(p.oob, (unsigned long long)ob);
+        // the last CTA of the launch re-arms the state of the next call: counter 0, extent = the dead-slot cell
+        if (atomicAdd(p.done, 1u) == gridDim.x * gridDim.y - 1) {
+            int* nx = reinterpret_cast<int*>(p.next_state);
+            nx[0] = 0; nx[1] = 0;
+            nx[2] = 1; nx[3] = p.N / 2; nx[4] = p.N / 2 + 1;
+            nx[5] = 0;                                          // its own done ticket
+            *p.done = 0;
+        }
         if (DO_CHI2) {
             p.partials[(long long)c * gridDim.x + blockIdx.x] = s;
             __threadfence();

@@ -380,6 +380,29 @@ def test_unaligned_arrays_take_the_plain_load_path(g, dtype):
     assert float(ca.cpu()[0]) == float(cu.cpu()[0])
 
 
+def test_per_call_state_across_calls(g, orc):
+    """The out-of-grid counter and the uv extent belong to ONE call: the two device copies of that state are used
+    alternately and re-armed by the sampler of the call before (or by an explicit copy after an M = 0 call)."""
+    w = W.config(0)
+    plan = g.Plan(w.nxy)
+    t = dev
+    _, ref_oob = orc.sampleImage(w.image, w.dxy, w.u, w.v, w.PA, w.dRA, w.dDec, return_oob=True)
+    assert ref_oob > 0
+    inside = (np.hypot(w.u, w.v) < 0.3 / w.dxy)
+    ui, vi = w.u[inside], w.v[inside]
+    e = torch.empty(0, dtype=torch.float64, device="cuda")
+    for rep in range(3):
+        plan.sampleImage(t(w.image), w.dxy, t(w.u), t(w.v), w.PA, w.dRA, w.dDec)
+        assert plan.last_oob_count() == ref_oob and plan.last_uv_extent() == (w.nxy // 2, 0, w.nxy - 1)
+        plan.chi2Image(t(w.image), w.dxy, t(ui), t(vi), t(w.re_obs[inside]), t(w.im_obs[inside]), t(w.w[inside]),
+                       w.dRA, w.dDec, w.PA)
+        ext = plan.last_uv_extent()
+        assert plan.last_oob_count() == 0 and ext[0] < w.nxy // 2 and ext[1] > 0 and ext[2] < w.nxy - 1
+        if rep == 1:
+            plan.chi2Image(t(w.image), w.dxy, e, e, e, e, e)
+            assert plan.last_oob_count() == 0
+
+
 # ---------------------------------------------------------------------------------------------
 # edge cases
 # ---------------------------------------------------------------------------------------------
