@@ -256,6 +256,24 @@ def main():
     ms_step = ms_total / args.steps
     value = world * args.steps / (ms_total * 1e-3)
 
+    # the same step on a BOUND uv set (gal_plan_bind_uv: the caller promises u, v stay unchanged, as in a fit of one
+    # observation; the per-call uv-extent kernel is skipped).  Reported beside the headline, not instead of it.
+    plan.bind_uv(u, v)
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    b0, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    b0.record()
+    for _ in range(args.steps):
+        step()
+    b1.record()
+    barrier()
+    ms_bound = max_over_ranks(b0.elapsed_time(b1), world, dev) / args.steps
+    bound_uv = {"ms_per_step": ms_bound, "value": world / (ms_bound * 1e-3), "unit": UNIT,
+                "chi2_identical": bool(float(out.cpu()[0]) == chi2_val),
+                "extent_violations": plan.last_extent_violations(), "uv_extent": list(plan.last_uv_extent())}
+    plan.unbind_uv()
+
     # per-kernel durations, live, CUDA events on the launching stream between the kernels
     ksteps = min(args.steps, 200)
     plan.timing_enable(ksteps)
@@ -317,7 +335,7 @@ def main():
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic", "config": base_config(w, "f64"), "clocks": clk.summary(), "e2e": e2e,
         "gpu_launches": int(launches), "roofline": roofline, "step_roofline": step_roofline, "kernels": kernels,
-        "visibilities_per_s": value * w.M, "chi2": chi2_val, "multi_gpu": "replicas only",
+        "visibilities_per_s": value * w.M, "chi2": chi2_val, "multi_gpu": "replicas only", "bound_uv": bound_uv,
         "paper_context": "GTX 1060, M=1e6, PCIe copies included: chi2Image 4096^2 = 59 ms (PAPER.md:619); not like for like",
     }
 

@@ -82,6 +82,20 @@ int gal_plan_set_pruning(gal_plan* plan, int mode);
  * {nxy/2, 0, nxy-1} if that call did not prune).  Synchronises the stream of that call. */
 int gal_last_uv_extent(gal_plan* plan, int* extent);
 
+/* Bound uv set (not in the paper; the use it serves is the paper's own: one observation, many model evaluations,
+ * PAPER.md:39-49).  gal_plan_bind_uv declares that the C x M device arrays u and v will keep their contents
+ * until the binding is replaced or removed.  It reduces them once to their largest baseline length r_max
+ * (one kernel, synchronises `stream`).  Later sample/chi2 calls that pass the same u, v, M (and C) skip the
+ * per-call uv-extent kernel: rotation by any PA leaves abs(u'), abs(v') <= r_max, so the extent is the square
+ * of half-width r_max / du + 2 cells about the centre, a few per cent larger than the exact one; results are
+ * bit-identical.  The sampler verifies every point against that extent: gal_last_extent_violations() returns
+ * the number of points of the most recent call that fell outside (0 unless the promise was broken, in which
+ * case that call's results are invalid).  Pruning mode 0 ignores the binding. */
+int gal_plan_bind_uv_f64(gal_plan* plan, const double* u, const double* v, int64_t M, int C, void* stream);
+int gal_plan_bind_uv_f32(gal_plan* plan, const float* u, const float* v, int64_t M, int C, void* stream);
+int gal_plan_unbind_uv(gal_plan* plan);
+int64_t gal_last_extent_violations(gal_plan* plan);
+
 /* ---- get_image_size (Eq. 19-24; host only, no device is touched): image size N_lm (rounded
  *      up to a power of two) and pixel size (radians) for the uv coverage u[M], v[M] (HOST pointers,
  *      wavelengths).  With q_min / q_max the shortest / longest baseline sqrt(u^2 + v^2):

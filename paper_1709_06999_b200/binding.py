@@ -46,6 +46,11 @@ def load_library() -> ctypes.CDLL:
         lib.gal_plan_timing_read.argtypes = [_vp, _vp, _vp]
         lib.gal_get_image_size.argtypes = [_vp, _vp, _i64, _d, _d, _d, _vp, _vp]
         lib.gal_plan_set_pruning.argtypes = [_vp, _i]
+        lib.gal_plan_unbind_uv.argtypes = [_vp]
+        lib.gal_last_extent_violations.argtypes = [_vp]
+        lib.gal_last_extent_violations.restype = _i64
+        for s in ("f64", "f32"):
+            getattr(lib, f"gal_plan_bind_uv_{s}").argtypes = [_vp, _vp, _vp, _i64, _i, _vp]
         lib.gal_last_uv_extent.argtypes = [_vp, _vp]
         for s in ("f64", "f32"):
             getattr(lib, f"gal_sweep_{s}").argtypes = [_vp, _vp, _i, _d, _d, _d, _d, _vp, _vp]
@@ -148,6 +153,20 @@ class Plan:
     def set_pruning(self, mode: int) -> None:
         """0 = never, 1 = automatic (default), 2 = always: see gal_plan_set_pruning."""
         _check(self._lib.gal_plan_set_pruning(self._h, int(mode)), "gal_plan_set_pruning", self)
+
+    def bind_uv(self, u, v) -> None:
+        """Promise that u and v ([M] or [C][M] CUDA tensors) keep their contents: later calls that pass these
+        very tensors skip the per-call uv-extent kernel (gal_plan_bind_uv)."""
+        C = 1 if u.dim() == 1 else u.shape[0]
+        M = u.shape[-1]
+        _check(self._fn("plan_bind_uv")(self._h, self._dev(u, "u"), self._dev(v, "v"), M, C, _stream()),
+               "gal_plan_bind_uv", self)
+
+    def unbind_uv(self) -> None:
+        _check(self._lib.gal_plan_unbind_uv(self._h), "gal_plan_unbind_uv", self)
+
+    def last_extent_violations(self) -> int:
+        return int(self._lib.gal_last_extent_violations(self._h))
 
     def last_uv_extent(self):
         """(kumax, kvs_min, kvs_max) the most recent call's transform was pruned to."""

@@ -36,6 +36,15 @@ struct gal_plan {
     bool next_armed = false;             // the other copy has been / will be re-armed by that call's sampler
     int prune_mode = 1;                  // 0 never, 1 auto, 2 always
     bool last_pruned = false;            // did the most recent call compute a uv extent?
+    // bound uv set (gal_plan_bind_uv): addresses, size, the rotation-invariant radius, and the extent derived
+    // from it for the pixel size seen last (device copy used by the FFT passes and checked by the sampler)
+    const void* b_u = nullptr; const void* b_v = nullptr;
+    int64_t b_M = 0; int b_C = 0;
+    double b_rmax = 0.0, b_dxy = 0.0;
+    int b_ext[3] = {0, 0, 0};
+    int* b_ext_dev = nullptr;            // [4]
+    unsigned long long* b_r2 = nullptr;  // [1] scratch of the radius kernel
+    bool last_bound = false;             // the most recent call used the bound extent
     std::set<const void*> smem_set;      // kernels whose dynamic shared-memory limit has been raised
     int max_gx = 0;
     size_t owned_bytes = 0;
@@ -278,6 +287,8 @@ int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T
     sp.oob = p->oob;
     sp.done = (unsigned int*)((char*)p->oob + 20);
     sp.next_state = (unsigned long long*)((char*)p->call_state + 32 * (p->cur ^ 1));
+    sp.viol = (unsigned long long*)((char*)p->oob + 24);
+    sp.ext_check = (p->last_bound && p->b_ext[0] < p->nxy / 2) ? p->b_ext_dev : nullptr;
     // one CTA works through tiles blockIdx.x, blockIdx.x + gridDim.x, ...: a whole number of CTAs per SM
     const int tile = SampleGeom<T, true>::TILE;
     const long long ntiles = (M + tile - 1) / tile;
@@ -313,6 +324,27 @@ int run_call(gal_plan* p, const T* image, const SweepParams* sw, int C, double d
     if (timed) GAL_CUDA(p, cudaEventRecord(e[0], st));
     const int* ext = p->ext_full;
     p->last_pruned = want_prune<T>(p, C, M) && !cs.ix.du_exact_div;   // the extent kernel only has the division shortcut
+    p->last_bound = false;
+    if (p->prune_mode != 0 && M > 0 && p->b_u == (const void*)u && p->b_v == (const void*)v && p->b_M == M && p->b_C == C) {
+        // bound uv set: the extent follows from the radius computed once at bind time, for any PA.  The index of
+        // a rotated coordinate is at most r_max / du (+ rounding: two cells of margin); rows are symmetric about N/2.
+        if (p->b_dxy != dxy) {
+            const int H = p->nxy / 2;
+            const double imax = p->b_rmax / cs.ix.du;
+            int e3[4] = {H, 0, p->nxy - 1, 0};
+            if (imax + 3.0 < (double)(H - 1)) {
+                const int k = (int)imax + 2;
+                e3[0] = k + 1; e3[1] = H - k - 1; e3[2] = H + k + 1;
+            }
+            GAL_CUDA(p, cudaMemcpyAsync(p->b_ext_dev, e3, sizeof(e3), cudaMemcpyHostToDevice, st));
+            GAL_CUDA(p, cudaStreamSynchronize(st));           // e3 is on the stack; once per (binding, dxy)
+            p->b_ext[0] = e3[0]; p->b_ext[1] = e3[1]; p->b_ext[2] = e3[2];
+            p->b_dxy = dxy;
+        }
+        p->last_bound = true;
+        p->last_pruned = false;
+        ext = p->b_ext_dev;
+    }
     if (p->last_pruned) {
         if ((rc = launch_extent<T>(p, C, cs, u, v, M, st))) return rc;
         ext = p->ext;
@@ -442,6 +474,35 @@ int do_host_call(gal_plan* p, const T* image, const T* I, int nr, double Rmin, d
 
 }  // namespace
 
+extern "C" int gal_plan_unbind_uv(gal_plan* p);
+
+namespace {
+
+template <typename T>
+int do_bind_uv(gal_plan* p, const T* u, const T* v, int64_t M, int C, void* stream) {
+    if (!prec_ok<T>(p) || !u || !v || M < 1 || C < 1 || C > p->batch) return GAL_ERR_INVALID_ARGUMENT;
+    DeviceGuard g(p->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    gal_plan_unbind_uv(p);
+    GAL_CUDA(p, cudaMemsetAsync(p->b_r2, 0, 8, st));
+    const long long total = (long long)C * M;
+    long long blocks = (total + 1023) / 1024;
+    if (blocks > (long long)p->sm_count * 8) blocks = (long long)p->sm_count * 8;
+    uv_radius_kernel<T><<<(unsigned)blocks, 256, 0, st>>>(u, v, total, p->b_r2);
+    p->launches++;
+    GAL_CUDA(p, cudaGetLastError());
+    unsigned long long bits = 0;
+    GAL_CUDA(p, cudaMemcpyAsync(&bits, p->b_r2, 8, cudaMemcpyDeviceToHost, st));
+    GAL_CUDA(p, cudaStreamSynchronize(st));
+    double r2; memcpy(&r2, &bits, 8);
+    if (!std::isfinite(r2)) return GAL_ERR_INVALID_ARGUMENT;
+    p->b_rmax = std::sqrt(r2) * (1.0 + 1e-12);
+    p->b_u = u; p->b_v = v; p->b_M = M; p->b_C = C;
+    return GAL_OK;
+}
+
+}  // namespace
+
 // =============================================================================================
 // C ABI
 // =============================================================================================
@@ -486,6 +547,8 @@ int gal_plan_create(gal_plan** out, int nxy, int batch, int precision_bits, int 
     if ((e = cudaMalloc(&p->call_state, 64)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     if ((e = cudaMalloc(&p->call_init, 32)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     if ((e = cudaMalloc((void**)&p->ext_full, 16)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
+    if ((e = cudaMalloc((void**)&p->b_ext_dev, 16)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
+    if ((e = cudaMalloc((void**)&p->b_r2, 8)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     p->oob = (unsigned long long*)p->call_state;
     p->ext = (int*)((char*)p->call_state + 8);
     {
@@ -527,7 +590,7 @@ int gal_plan_destroy(gal_plan* p) {
     DeviceGuard g(p->device);
     cudaFree(p->spec); cudaFree(p->work); cudaFree(p->tw); cudaFree(p->partials); cudaFree(p->tickets); cudaFree(p->chi2_scratch);
     for (cudaEvent_t e : p->tev) cudaEventDestroy(e);
-    cudaFree(p->call_state); cudaFree(p->call_init); cudaFree(p->ext_full); cudaFree(p->st_image); cudaFree(p->st_pts); cudaFree(p->st_out); cudaFree(p->st_chi2);
+    cudaFree(p->call_state); cudaFree(p->call_init); cudaFree(p->ext_full); cudaFree(p->b_ext_dev); cudaFree(p->b_r2); cudaFree(p->st_image); cudaFree(p->st_pts); cudaFree(p->st_out); cudaFree(p->st_chi2);
     delete p;
     return GAL_OK;
 }
@@ -573,6 +636,7 @@ int gal_last_uv_extent(gal_plan* p, int* extent) {
     if (!p || !extent) return GAL_ERR_INVALID_ARGUMENT;
     DeviceGuard g(p->device);
     GAL_CUDA(p, cudaStreamSynchronize(p->last_stream));
+    if (p->last_bound) { extent[0] = p->b_ext[0]; extent[1] = p->b_ext[1]; extent[2] = p->b_ext[2]; return GAL_OK; }
     GAL_CUDA(p, cudaMemcpy(extent, p->last_pruned ? p->ext : p->ext_full, 3 * sizeof(int), cudaMemcpyDeviceToHost));
     return GAL_OK;
 }
@@ -601,6 +665,22 @@ int gal_get_image_size(const double* u, const double* v, int64_t M, double PB, d
     return GAL_OK;
 }
 
+int gal_plan_unbind_uv(gal_plan* p) {
+    if (!p) return GAL_ERR_INVALID_ARGUMENT;
+    p->b_u = p->b_v = nullptr; p->b_M = 0; p->b_C = 0; p->b_dxy = 0.0; p->last_bound = false;
+    return GAL_OK;
+}
+
+int64_t gal_last_extent_violations(gal_plan* p) {
+    if (!p) return -1;
+    if (!p->last_bound) return 0;
+    DeviceGuard g(p->device);
+    unsigned long long h = 0;
+    if (cudaStreamSynchronize(p->last_stream) != cudaSuccess) return -1;
+    if (cudaMemcpy(&h, (char*)p->oob + 24, sizeof(h), cudaMemcpyDeviceToHost) != cudaSuccess) return -1;
+    return (int64_t)h;
+}
+
 size_t gal_plan_workspace_bytes(const gal_plan* p) { return p ? p->owned_bytes : 0; }
 int gal_last_cuda_error(const gal_plan* p) { return p ? p->last_cuda : 0; }
 int64_t gal_plan_launch_count(const gal_plan* p) { return p ? p->launches : -1; }
@@ -615,6 +695,9 @@ int64_t gal_last_oob_count(gal_plan* p) {
 }
 
 #define GAL_DEFINE_PRECISION(SFX, T)                                                                                  \
+    int gal_plan_bind_uv_##SFX(gal_plan* p, const T* u, const T* v, int64_t M, int C, void* stream) {                 \
+        return do_bind_uv<T>(p, u, v, M, C, stream);                                                                  \
+    }                                                                                                                 \
     int gal_sweep_##SFX(gal_plan* p, const T* I, int nr, double Rmin, double dR, double dxy, double inc, T* out,      \
                         void* stream) {                                                                               \
         return do_sweep<T>(p, I, nr, Rmin, dR, dxy, inc, out, stream);                                                \

@@ -48,6 +48,8 @@ template <typename T> struct SampleParams {
     unsigned long long* oob;  // [1]: this call's out-of-grid counter
     unsigned int* done;       // [1]: CTAs of this launch that have finished
     unsigned long long* next_state;  // the copy of the per-call state the NEXT call will use (32 B)
+    const int* ext_check;     // extent of a bound uv set to verify every point against, or null
+    unsigned long long* viol; // [1]: points whose cell lies outside ext_check
 };
 
 // Correctly rounded a / b from r = RN(1/b) (Markstein): q0 = RN(a r); rem = a - q0 b (exact in an
@@ -340,6 +342,8 @@ template <typename T> struct SampleCtx {
     int odd;               // lane parity
     double acc;            // chi2 partial of this thread
     unsigned int oob;      // points of this thread beyond the half-plane grid
+    unsigned int viol;     // points of this thread outside the extent of the bound uv set
+    int ck_kumax, ck_rmin, ck_rmax;   // that extent ({N, 0, N}: nothing to check)
 };
 
 // U points of one thread: rotate, index, gather, interpolate, phase, chi2 / store.
@@ -377,6 +381,7 @@ __device__ __forceinline__ void sample_points(const SampleParams<T>& p, SampleCt
         // theta / 2 pi in turns (exact range reduction in sincos_turns)
         turns[j] = fma(q.urot, p.dRA_turns, q.vrot * p.dDec_turns);
         const int off = ix0 * N + iy0;                   // 0 outside
+        if (ix0 + 1 > cx_.ck_kumax || iy0 < cx_.ck_rmin || iy0 + 1 > cx_.ck_rmax || (!inside[j] && cx_.ck_kumax < N)) ++cx_.viol;
         const int off_partner = __shfl_xor_sync(0xffffffffu, off, 1);
         const NodePair<T> ea = load_pair(spec + ((odd ? off_partner : off) + odd));
         const NodePair<T> eb = load_pair(spec + ((odd ? off : off_partner) + odd));
@@ -434,7 +439,12 @@ __device__ __forceinline__ void sample_points(const SampleParams<T>& p, SampleCt
 // Deterministic reduction: warp shuffle -> block -> per-block partial -> last block (ticket), fixed order,
 // no floating-point atomics.  Also adds this CTA's out-of-grid count.
 template <typename T, bool DO_CHI2>
-__device__ __forceinline__ void sample_finish(const SampleParams<T>& p, int c, double acc, unsigned int oob) {
+__device__ __forceinline__ void sample_finish(const SampleParams<T>& p, int c, double acc, unsigned int oob,
+                                              unsigned int viol) {
+    if (p.ext_check) {                                       // rare: a bound uv set is being verified
+        viol = __reduce_add_sync(0xffffffffu, viol);
+        if ((threadIdx.x & 31) == 0 && viol) atomicAdd(p.viol, (unsigned long long)viol);
+    }
     __shared__ double wsum[32];
     __shared__ unsigned int woob[32];
     __shared__ bool is_last;
@@ -457,6 +467,7 @@ __device__ __forceinline__ void sample_finish(const SampleParams<T>& p, int c, d
             nx[0] = 0; nx[1] = 0;
             nx[2] = 1; nx[3] = p.N / 2; nx[4] = p.N / 2 + 1;
             nx[5] = 0;                                          // its own done ticket
+            nx[6] = 0; nx[7] = 0;                               // and its extent-violation counter
             *p.done = 0;
         }
         if (DO_CHI2) {
@@ -532,6 +543,9 @@ __device__ __forceinline__ SampleCtx<T> sample_ctx(const SampleParams<T>& p, int
     cx_.odd = threadIdx.x & 1;
     cx_.acc = 0.0;
     cx_.oob = 0;
+    cx_.viol = 0;
+    cx_.ck_kumax = p.N; cx_.ck_rmin = 0; cx_.ck_rmax = p.N;
+    if (p.ext_check) { cx_.ck_kumax = __ldg(p.ext_check); cx_.ck_rmin = __ldg(p.ext_check + 1); cx_.ck_rmax = __ldg(p.ext_check + 2); }
     return cx_;
 }
 
@@ -546,7 +560,7 @@ __global__ void __launch_bounds__(256, GAL_SAMPLE_MINB) sample_kernel_plain(cons
     const long long ntiles = (M + G::TILE - 1) / G::TILE;
     for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x)
         sample_tile_plain<T, WRITE_VIS, DO_CHI2, true>(p, cx_, tile, M, c);
-    sample_finish<T, DO_CHI2>(p, c, cx_.acc, cx_.oob);
+    sample_finish<T, DO_CHI2>(p, c, cx_.acc, cx_.oob, cx_.viol);
 }
 
 __device__ __forceinline__ void mbar_arrive(uint32_t mb) {
@@ -614,7 +628,22 @@ __global__ void __launch_bounds__(SampleGeom<T, DO_CHI2>::NT_TMA, GAL_SAMPLE_MIN
         if (tile == nfull && (long long)nfull * TILE < M)    // the ragged last tile falls to this CTA
             sample_tile_plain<T, WRITE_VIS, DO_CHI2, false>(p, cx_, nfull, M, c);
     }
-    sample_finish<T, DO_CHI2>(p, c, cx_.acc, cx_.oob);
+    sample_finish<T, DO_CHI2>(p, c, cx_.acc, cx_.oob, cx_.viol);
+}
+
+// max over the points of u^2 + v^2 (bit pattern of a non-negative double orders like an integer): the
+// rotation-invariant bound a bound uv set's extent is derived from (gal_plan_bind_uv).
+template <typename T>
+__global__ void __launch_bounds__(256) uv_radius_kernel(const T* __restrict__ u, const T* __restrict__ v, long long total,
+                                                        unsigned long long* r2max_bits) {
+    double m = 0.0;
+    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < total; k += (long long)gridDim.x * blockDim.x) {
+        const double a = (double)__ldcs(u + k), b = (double)__ldcs(v + k);
+        m = fmax(m, fma(a, a, b * b));
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0) atomicMax(r2max_bits, (unsigned long long)__double_as_longlong(m));
 }
 
 }  // namespace galb

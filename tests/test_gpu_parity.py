@@ -380,6 +380,39 @@ def test_unaligned_arrays_take_the_plain_load_path(g, dtype):
     assert float(ca.cpu()[0]) == float(cu.cpu()[0])
 
 
+def test_bound_uv_set(g):
+    """gal_plan_bind_uv: calls on a bound uv set skip the uv-extent kernel (3 launches instead of 4), use an extent
+    that contains the exact one for any PA, give bit-identical results, and a broken promise is detected."""
+    w = W.config(3, nxy=2048, M=300_007, n_src=120)
+    img, u, v, re, im, wt = (dev(a) for a in (w.image, w.u, w.v, w.re_obs, w.im_obs, w.w))
+    free, bound = g.Plan(w.nxy), g.Plan(w.nxy)
+    bound.bind_uv(u, v)
+    for PA in (w.PA, 0.3, 2.5, -1.2):
+        a = free.sampleImage(img, w.dxy, u, v, PA, w.dRA, w.dDec)
+        exact = free.last_uv_extent()
+        n0 = bound.launch_count()
+        b = bound.sampleImage(img, w.dxy, u, v, PA, w.dRA, w.dDec)
+        assert bound.launch_count() - n0 == 3
+        ext = bound.last_uv_extent()
+        assert ext[0] >= exact[0] and ext[1] <= exact[1] and ext[2] >= exact[2] and ext[0] < w.nxy // 2
+        assert torch.equal(a, b) and bound.last_extent_violations() == 0
+        ca = free.chi2Image(img, w.dxy, u, v, re, im, wt, w.dRA, w.dDec, PA)
+        cb = bound.chi2Image(img, w.dxy, u, v, re, im, wt, w.dRA, w.dDec, PA)
+        assert float(ca.cpu()[0]) == float(cb.cpu()[0]) and bound.last_extent_violations() == 0
+    # other arrays of the same size are not the bound set: the call computes its own extent
+    u2 = u.clone()
+    n0 = bound.launch_count()
+    bound.sampleImage(img, w.dxy, u2, v, w.PA, w.dRA, w.dDec)
+    assert bound.launch_count() - n0 == 4 and bound.last_extent_violations() == 0
+    # a broken promise (contents changed in place) is reported
+    u.mul_(1.7)
+    bound.sampleImage(img, w.dxy, u, v, w.PA, w.dRA, w.dDec)
+    assert bound.last_extent_violations() > 0
+    bound.unbind_uv()
+    c = bound.sampleImage(img, w.dxy, u, v, w.PA, w.dRA, w.dDec)
+    assert bound.last_extent_violations() == 0 and torch.equal(c, free.sampleImage(img, w.dxy, u, v, w.PA, w.dRA, w.dDec))
+
+
 def test_per_call_state_across_calls(g, orc):
     """The out-of-grid counter and the uv extent belong to ONE call: the two device copies of that state are used
     alternately and re-armed by the sampler of the call before (or by an explicit copy after an M = 0 call)."""
