@@ -119,12 +119,17 @@ __device__ __forceinline__ int floor_small(double x, double* fl) {
 // remainder r = 4 t - k in [-1/2, 1/2] is exact, a = r pi / 2 lies in [-pi/4, pi/4] where the classic
 // minimax polynomials (fdlibm's kernel coefficients) are good to < 1 ulp; the quadrant k mod 4 then swaps and
 // signs the pair.
-__device__ __forceinline__ void sincos_turns(double t, double* sn, double* cs) {
+// In _f32 (every array stored as float, tolerance 1e-4 of the peak) only the reduction stays in double — it
+// is what keeps the phase of a 1e7-wavelength baseline exact — and the polynomials run in float.
+__device__ __forceinline__ double quarter_reduce(double t, int* q) {
     const double* K = SINCOS_COEF;
     const double t4 = 4.0 * t;
     const double z = __dadd_rn(t4, K[12]);
-    const int q = __double2loint(z);
-    const double a = (t4 - (z - K[12])) * K[13];
+    *q = __double2loint(z);
+    return (t4 - (z - K[12])) * K[13];
+}
+__device__ __forceinline__ void sincos_quarter(double a, int q, double* sn, double* cs) {
+    const double* K = SINCOS_COEF;
     const double a2 = a * a;
     double ps = K[0];
     ps = fma(ps, a2, K[1]);
@@ -141,6 +146,21 @@ __device__ __forceinline__ void sincos_turns(double t, double* sn, double* cs) {
     pc = fma(pc, a2, K[11]);
     const double c = fma(a2 * a2, pc, fma(a2, -0.5, 1.0));
     const double ss = (q & 1) ? c : s, cc = (q & 1) ? s : c;
+    *sn = (q & 2) ? -ss : ss;
+    *cs = ((q + 1) & 2) ? -cc : cc;
+}
+__device__ __forceinline__ void sincos_quarter(float a, int q, float* sn, float* cs) {
+    const float a2 = a * a;                       // single-precision kernels on [-pi/4, pi/4]: error < 1e-7
+    float ps = 2.7557314297e-06f;
+    ps = fmaf(ps, a2, -1.9841270114e-04f);
+    ps = fmaf(ps, a2, 8.3333337680e-03f);
+    ps = fmaf(ps, a2, -1.6666667163e-01f);
+    const float s = fmaf(a * a2, ps, a);
+    float pc = 2.4801587642e-05f;
+    pc = fmaf(pc, a2, -1.3888889225e-03f);
+    pc = fmaf(pc, a2, 4.1666667908e-02f);
+    const float c = fmaf(a2 * a2, pc, fmaf(a2, -0.5f, 1.0f));
+    const float ss = (q & 1) ? c : s, cc = (q & 1) ? s : c;
     *sn = (q & 2) ? -ss : ss;
     *cs = ((q + 1) & 2) ? -cc : cc;
 }
@@ -347,7 +367,7 @@ template <typename T> struct SampleCtx {
 };
 
 // U points of one thread: rotate, index, gather, interpolate, phase, chi2 / store.
-//   ld(a, j): value a (0 = u, 1 = v, 2 = re_obs, 3 = im_obs, 4 = w) of this thread's j-th point, as double;
+//   ld(a, j): value a (0 = u, 1 = v, 2 = re_obs, 3 = im_obs, 4 = w) of this thread's j-th point;
 //             points past the end read as u = v = 0 with weight 0 (cell (0, N/2), always inside).
 //   kpt(j):   global index of that point (only used to store the visibility).
 //
@@ -365,20 +385,22 @@ __device__ __forceinline__ void sample_points(const SampleParams<T>& p, SampleCt
                                               int c) {
     const int N = cx_.N, odd = cx_.odd;
     const NodePair<T>* __restrict__ spec = cx_.spec;
-    double tx[U], ty[U], turns[U], tx_partner[U];
+    using R = T;                            // type of the value arithmetic (interpolation, phase product, chi2 terms)
+    R tx[U], ty[U], tx_partner[U];
+    double turns[U];
     bool uneg[U], inside[U];
     cx<T> ga0[U], ga1[U], gb0[U], gb1[U];   // even lane's cell (a) / odd lane's cell (b); column ku+0 / ku+1
 #pragma unroll
     for (int j = 0; j < U; ++j) {
-        const PointIndex q = point_index<EXACT>(p.ix, ld(0, j), ld(1, j));
+        const PointIndex q = point_index<EXACT>(p.ix, (double)ld(0, j), (double)ld(1, j));
         // bilinear interpolation
         inside[j] = cell_inside(p.ix, q);
         uneg[j] = q.uneg;
         double fx0, fy0;
         const int ix0 = floor_small(inside[j] ? q.uidx : 0.0, &fx0), iy0 = floor_small(inside[j] ? q.vidx : 0.0, &fy0);
-        tx[j] = __dsub_rn(q.uidx, fx0);                  // (outside the grid the rare path below redoes this)
-        ty[j] = __dsub_rn(q.vidx, fy0);
-        // theta / 2 pi in turns (exact range reduction in sincos_turns)
+        tx[j] = (R)__dsub_rn(q.uidx, fx0);               // (outside the grid the rare path below redoes this)
+        ty[j] = (R)__dsub_rn(q.vidx, fy0);
+        // theta / 2 pi in turns (exact range reduction in quarter_reduce)
         turns[j] = fma(q.urot, p.dRA_turns, q.vrot * p.dDec_turns);
         const int off = ix0 * N + iy0;                   // 0 outside
         if (ix0 + 1 > cx_.ck_kumax || iy0 < cx_.ck_rmin || iy0 + 1 > cx_.ck_rmax || (!inside[j] && cx_.ck_kumax < N)) ++cx_.viol;
@@ -391,47 +413,49 @@ __device__ __forceinline__ void sample_points(const SampleParams<T>& p, SampleCt
     }
 #pragma unroll
     for (int j = 0; j < U; ++j) {
-        const double txa = odd ? tx_partner[j] : tx[j], txb = odd ? tx[j] : tx_partner[j];
+        const R txa = odd ? tx_partner[j] : tx[j], txb = odd ? tx[j] : tx_partner[j];
         // this lane's row (kvs + odd) of both cells, interpolated along u: g0 + t (g1 - g0)
-        const double ra_re = fma(txa, (double)ga1[j].x - (double)ga0[j].x, (double)ga0[j].x);
-        const double ra_im = fma(txa, (double)ga1[j].y - (double)ga0[j].y, (double)ga0[j].y);
-        const double rb_re = fma(txb, (double)gb1[j].x - (double)gb0[j].x, (double)gb0[j].x);
-        const double rb_im = fma(txb, (double)gb1[j].y - (double)gb0[j].y, (double)gb0[j].y);
+        const R ra_re = fma(txa, ga1[j].x - ga0[j].x, ga0[j].x);
+        const R ra_im = fma(txa, ga1[j].y - ga0[j].y, ga0[j].y);
+        const R rb_re = fma(txb, gb1[j].x - gb0[j].x, gb0[j].x);
+        const R rb_im = fma(txb, gb1[j].y - gb0[j].y, gb0[j].y);
         // the even lane keeps row kvs of cell a and needs row kvs+1 of it; the odd lane keeps row kvs+1 of
         // cell b and needs row kvs: mine + w (other - mine), w = ty (even) or 1 - ty (odd)
-        const double o_re = __shfl_xor_sync(0xffffffffu, odd ? ra_re : rb_re, 1);
-        const double o_im = __shfl_xor_sync(0xffffffffu, odd ? ra_im : rb_im, 1);
-        const double m_re = odd ? rb_re : ra_re, m_im = odd ? rb_im : ra_im;
-        const double wy = odd ? 1.0 - ty[j] : ty[j];
-        double ReInt = fma(wy, o_re - m_re, m_re);
-        double ImInt = fma(wy, o_im - m_im, m_im);
+        const R o_re = __shfl_xor_sync(0xffffffffu, odd ? ra_re : rb_re, 1);
+        const R o_im = __shfl_xor_sync(0xffffffffu, odd ? ra_im : rb_im, 1);
+        const R m_re = odd ? rb_re : ra_re, m_im = odd ? rb_im : ra_im;
+        const R wy = odd ? (R)1 - ty[j] : ty[j];
+        R ReInt = fma(wy, o_re - m_re, m_re);
+        R ImInt = fma(wy, o_im - m_im, m_im);
         if (!inside[j]) {           // rare: the cell leaves the half-plane grid (reading A6); dead slots never get here
-            const PointIndex q = point_index<EXACT>(p.ix, ld(0, j), ld(1, j));
+            const PointIndex q = point_index<EXACT>(p.ix, (double)ld(0, j), (double)ld(1, j));
             const long long ix = (long long)floor(q.uidx), iy = (long long)floor(q.vidx);
             if (q.uidx > p.ix.fH || q.vidx < 0.0 || q.vidx > p.ix.fN1) ++cx_.oob;
             const cx<T> g00 = node_any<T>(spec, N, iy, ix), g01 = node_any<T>(spec, N, iy, ix + 1);
             const cx<T> g10 = node_any<T>(spec, N, iy + 1, ix), g11 = node_any<T>(spec, N, iy + 1, ix + 1);
             const double txr = __dsub_rn(q.uidx, floor(q.uidx)), tyr = __dsub_rn(q.vidx, floor(q.vidx));
             const double ax = 1.0 - txr, ay = 1.0 - tyr;
-            ReInt = ay * (ax * (double)g00.x + txr * (double)g01.x) + tyr * (ax * (double)g10.x + txr * (double)g11.x);
-            ImInt = ay * (ax * (double)g00.y + txr * (double)g01.y) + tyr * (ax * (double)g10.y + txr * (double)g11.y);
+            ReInt = (R)(ay * (ax * (double)g00.x + txr * (double)g01.x) + tyr * (ax * (double)g10.x + txr * (double)g11.x));
+            ImInt = (R)(ay * (ax * (double)g00.y + txr * (double)g01.y) + tyr * (ax * (double)g10.y + txr * (double)g11.y));
         }
         if (uneg[j]) ImInt = -ImInt;
-        double vr = ReInt, vi = ImInt;
+        R vr = ReInt, vi = ImInt;
         if (p.has_phase) {
-            double sn, co;
-            sincos_turns(turns[j], &sn, &co);
+            int qd;
+            const double a = quarter_reduce(turns[j], &qd);
+            R sn, co;
+            sincos_quarter((R)a, qd, &sn, &co);
             vr = ReInt * co - ImInt * sn;
             vi = ReInt * sn + ImInt * co;
         }
         if (WRITE_VIS) {
             const long long k = kpt(j);
-            if (k < M) __stcs(reinterpret_cast<cx<T>*>(p.vis) + c * M + k, mk<T>((T)vr, (T)vi));
+            if (k < M) __stcs(reinterpret_cast<cx<T>*>(p.vis) + c * M + k, mk<T>(vr, vi));
         }
         if (DO_CHI2) {                                      // PAPER.md:718 (Eq. 10); w = 0 for dead slots
-            const double dr = vr - ld(2, j);
-            const double di = vi - ld(3, j);
-            cx_.acc = fma(fma(dr, dr, di * di), ld(4, j), cx_.acc);
+            const R dr = vr - ld(2, j);
+            const R di = vi - ld(3, j);
+            cx_.acc += (double)(fma(dr, dr, di * di) * ld(4, j));
         }
     }
 }
@@ -525,11 +549,11 @@ __device__ __forceinline__ void sample_tile_plain(const SampleParams<T>& p, Samp
     const T* __restrict__ g2 = DO_CHI2 ? p.re_obs + c * M : nullptr;
     const T* __restrict__ g3 = DO_CHI2 ? p.im_obs + c * M : nullptr;
     const T* __restrict__ g4 = DO_CHI2 ? p.w + c * M : nullptr;
-    auto ld = [&](int a, int j) -> double {
+    auto ld = [&](int a, int j) -> T {
         const long long k = k0 + j * 256;
-        if (k >= M) return 0.0;
+        if (k >= M) return (T)0;
         const T* g = a == 0 ? g0 : a == 1 ? g1 : a == 2 ? g2 : a == 3 ? g3 : g4;
-        return (double)__ldcs(g + k);
+        return __ldcs(g + k);
     };
     auto kpt = [&](int j) -> long long { return k0 + j * 256; };
     sample_points<T, WRITE_VIS, DO_CHI2, EXACT, U>(p, cx_, ld, kpt, M, c);
@@ -618,7 +642,7 @@ __global__ void __launch_bounds__(SampleGeom<T, DO_CHI2>::NT_TMA, GAL_SAMPLE_MIN
         for (; tile < nfull; tile += gridDim.x) {
             mbar_wait(full0 + 8 * stage, parity);
             const T* st = reinterpret_cast<const T*>(sample_smem + stage * G::STAGE_BYTES) + tid;
-            auto ld = [&](int a, int j) -> double { return (double)st[a * TILE + j * 256]; };
+            auto ld = [&](int a, int j) -> T { return st[a * TILE + j * 256]; };
             auto kpt = [&](int j) -> long long { return (long long)tile * TILE + j * 256 + tid; };
             sample_points<T, WRITE_VIS, DO_CHI2, false, U>(p, cx_, ld, kpt, M, c);
             __syncwarp();                                    // every lane has read its last value of this stage
