@@ -399,6 +399,67 @@ col_pass_kernel(const ColParams<T> p) {
 }
 
 // ------------------------------------------------------------------------------------------
+// Column pass for N = 2 L beyond the longest three-step transform (N = 8192): one column per CTA as two
+// interleaved L-point transforms (even and odd samples, the two regions of an F = 2 geometry) and one
+// radix-2 combination  X[k] = E[k] + W_N^k O[k],  X[k + L] = E[k] - W_N^k O[k]  that writes straight to the
+// column pairs with the same sign / row folds and pruning as col_pass_kernel.
+// ------------------------------------------------------------------------------------------
+template <typename T, int R1, int R2, int R3>
+__global__ void __launch_bounds__(Geom<T, R1, R2, R3, 2>::NT)
+col_pass_x2_kernel(const ColParams<T> p) {
+    using G = Geom<T, R1, R2, R3, 2>;
+    constexpr int L = G::L;                    // = N / 2
+    constexpr int N = 2 * L, NU = N / 2 + 1;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cx<T>* smem = reinterpret_cast<cx<T>*>(smem_raw);
+    const int tid = threadIdx.x;
+    const int f = tid / G::TPF, t = tid % G::TPF;
+    pdl_wait();
+    const int kumax = __ldg(p.ext), rmin = __ldg(p.ext + 1), rmax = __ldg(p.ext + 2);
+    const long long g = blockIdx.x;
+    const int ku = (int)(g % NU);
+    if (ku > kumax) return;
+    const cx<T>* col = p.work + g * (long long)N;
+    NodePair<T>* own = p.pair + g * (long long)N;
+    NodePair<T>* prev = own - (ku > 0 ? N : 0);
+    cx<T>* S = smem + f * G::REGION;
+
+    fft_steps12<T, R1, R2, R3, G::TPF>(S, t, p.tw, 2, [&](int n) -> cx<T> { return col[2 * n + f]; });
+    if (R3 > 1) {                              // step 3, in place (as in the row pass)
+        for (int it = t; it < R1 * R2; it += G::TPF) {
+            const int k1 = it % R1, c = it / R1;
+            cx<T>* base = S + k1 * G::P1 + c * R3;
+            cx<T> a[R3];
+#pragma unroll
+            for (int b = 0; b < R3; ++b) a[b] = base[b];
+            Dft<T, R3>::run(a);
+#pragma unroll
+            for (int d = 0; d < R3; ++d) base[d] = a[d];
+        }
+    }
+    __syncthreads();
+    const cx<T>* SE = smem;
+    const cx<T>* SO = smem + G::REGION;
+    for (int k = tid; k < L; k += G::NT) {
+        const cx<T> E = SE[G::zaddr(k)];
+        const cx<T> WO = cmul(__ldg(p.tw + k), SO[G::zaddr(k)]);
+        const T sgn = ((ku + k) & 1) ? (T)-1 : (T)1;          // L is even: kv = k and k + L have one parity
+        const cx<T> x0 = cadd(E, WO), x1 = csub(E, WO);
+        const int kvs0 = k + L, kvs1 = k;                     // (kv + N/2) mod N for kv = k, k + L
+        if (kvs0 >= rmin && kvs0 <= rmax) {
+            const cx<T> val = mk<T>(sgn * x0.x, sgn * x0.y);
+            own[kvs0].a = val;
+            if (ku > 0) prev[kvs0].b = val;
+        }
+        if (kvs1 >= rmin && kvs1 <= rmax) {
+            const cx<T> val = mk<T>(sgn * x1.x, sgn * x1.y);
+            own[kvs1].a = val;
+            if (ku > 0) prev[kvs1].b = val;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
 // Standalone sweep (image written to memory) and the u-major -> paper-layout transpose.
 // ------------------------------------------------------------------------------------------
 template <typename T>

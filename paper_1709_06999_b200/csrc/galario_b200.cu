@@ -152,6 +152,24 @@ int launch_col(gal_plan* p, int batch, const int* ext, cudaStream_t st) {
     return GAL_OK;
 }
 
+template <typename T, int R1, int R2, int R3>
+int launch_col_x2(gal_plan* p, int batch, const int* ext, cudaStream_t st) {
+    using G = Geom<T, R1, R2, R3, 2>;
+    ColParams<T> cp;
+    cp.work = (const cx<T>*)p->work;
+    cp.pair = (NodePair<T>*)p->spec;
+    cp.tw = (const cx<T>*)p->tw;
+    cp.N = p->nxy;
+    cp.cols_total = (long long)batch * (p->nxy / 2 + 1);
+    cp.ext = ext;
+    auto k = col_pass_x2_kernel<T, R1, R2, R3>;
+    int rc = set_smem(p, k, G::SMEM); if (rc) return rc;
+    GAL_CUDA(p, launch_chain(k, dim3((unsigned)cp.cols_total), dim3(G::NT), G::SMEM, st, cp));
+    p->launches++;
+    GAL_CUDA(p, cudaGetLastError());
+    return GAL_OK;
+}
+
 // Radix plans.  Row FFT length is nxy/2, column FFT length is nxy.
 template <typename T>
 int fft2(gal_plan* p, const T* image, const SweepParams* sw, int batch, const int* ext, cudaStream_t st) {
@@ -172,6 +190,9 @@ int fft2(gal_plan* p, const T* image, const SweepParams* sw, int batch, const in
         GAL_FFT_CASE(1024, RR(8, 8, 8, 4), RR(16, 8, 8, 4))
         GAL_FFT_CASE(2048, RR(16, 8, 8, 4), RR(16, 16, 8, 2))
         GAL_FFT_CASE(4096, RR(16, 16, 8, 2), RR(16, 16, 16, 1))
+        case 8192:      // column length 8192 = 2 x 4096: two interleaved transforms + one radix-2 combination
+            rc = launch_row<T, 16, 16, 16, 1>(p, image, sw, batch, ext, st); if (rc) return rc;
+            return launch_col_x2<T, 16, 16, 16>(p, batch, ext, st);
 #undef RR
 #undef GAL_FFT_CASE
         default:
@@ -526,7 +547,7 @@ int gal_plan_create(gal_plan** out, int nxy, int batch, int precision_bits, int 
     *out = nullptr;
     if (!is_pow2(nxy) || nxy < 8 || batch < 1 || (precision_bits != 64 && precision_bits != 32) || device < 0)
         return GAL_ERR_INVALID_ARGUMENT;
-    if (nxy > 4096) return GAL_ERR_UNSUPPORTED;
+    if (nxy > 8192) return GAL_ERR_UNSUPPORTED;
     gal_plan* p = new (std::nothrow) gal_plan();
     if (!p) return GAL_ERR_ALLOC;
     p->nxy = nxy; p->batch = batch; p->bits = precision_bits; p->device = device;

@@ -47,7 +47,7 @@ def threads(orc):
 # ---------------------------------------------------------------------------------------------
 # S2+S3+S4: the transform alone, every supported size (several tiles, both FFT code paths)
 # ---------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("n", [8, 16, 32, 64, 128, 256, 512, 1024, 2048, 4096])
+@pytest.mark.parametrize("n", [8, 16, 32, 64, 128, 256, 512, 1024, 2048, 4096, 8192])
 def test_fft2_shifted_matches_oracle_f64(g, orc, n):
     rng = np.random.default_rng(n)
     img = rng.standard_normal((n, n))
@@ -58,7 +58,7 @@ def test_fft2_shifted_matches_oracle_f64(g, orc, n):
     assert np.abs(out - ref).max() <= 1e-12 * np.abs(ref).max()
 
 
-@pytest.mark.parametrize("n", [8, 64, 512, 4096])
+@pytest.mark.parametrize("n", [8, 64, 512, 4096, 8192])
 def test_fft2_shifted_matches_oracle_f32(g, orc, n):
     rng = np.random.default_rng(n + 1)
     img = rng.random((n, n)).astype(np.float32)
@@ -476,7 +476,7 @@ def test_empty_single_and_ragged_M(g, orc):
 
 
 def test_smallest_and_largest_nxy_end_to_end(g, orc):
-    for n, M in ((8, 100), (4096, 1000)):
+    for n, M in ((8, 100), (4096, 1000), (8192, 50_001)):
         rng = np.random.default_rng(n)
         dxy = 0.01 * ARCSEC
         du = 1.0 / (n * dxy)
@@ -494,7 +494,7 @@ def test_error_codes(g):
     assert lib.gal_plan_create(ctypes.byref(h), 100, 1, 64, 0) == -1        # not a power of two
     assert lib.gal_plan_create(ctypes.byref(h), 256, 0, 64, 0) == -1        # batch < 1
     assert lib.gal_plan_create(ctypes.byref(h), 256, 1, 16, 0) == -1        # precision
-    assert lib.gal_plan_create(ctypes.byref(h), 8192, 1, 64, 0) == -4       # unsupported size
+    assert lib.gal_plan_create(ctypes.byref(h), 16384, 1, 64, 0) == -4      # unsupported size
     assert lib.gal_plan_create(None, 256, 1, 64, 0) == -1
     plan = g.Plan(64)
     img = torch.zeros(64, 64, dtype=torch.float64, device="cuda")
