@@ -90,7 +90,9 @@ int gal_last_uv_extent(gal_plan* plan, int* extent);
  * of half-width r_max / du + 2 cells about the centre, a few per cent larger than the exact one; results are
  * bit-identical.  The sampler verifies every point against that extent: gal_last_extent_violations() returns
  * the number of points of the most recent call that fell outside (0 unless the promise was broken, in which
- * case that call's results are invalid).  Pruning mode 0 ignores the binding. */
+ * case that call's results are invalid).  Pruning mode 0 ignores the binding.  The first call on a binding, and
+ * the first with a new dxy, synchronise the stream once (the extent is uploaded); all later calls are
+ * asynchronous as usual. */
 int gal_plan_bind_uv_f64(gal_plan* plan, const double* u, const double* v, int64_t M, int C, void* stream);
 int gal_plan_bind_uv_f32(gal_plan* plan, const float* u, const float* v, int64_t M, int C, void* stream);
 int gal_plan_unbind_uv(gal_plan* plan);
@@ -173,6 +175,27 @@ int gal_chi2_image_batch_f32(gal_plan* plan, const float* images, int C, double 
                              const float* v, const float* re_obs, const float* im_obs, const float* w,
                              int64_t M, double dRA, double dDec, double PA, double* chi2_per_channel,
                              double* chi2_total, void* stream);
+
+/* ---- multi-source composition ("summing up the visibilities of each single source ... applying a
+ *      different complex phase"): one model image placed S times,
+ *        V(u, v) = sum_s scale[s] * sampleImage(image; dRA[s], dDec[s], PA[s])(u, v),
+ *      with ONE transform of the image.  dRA, dDec, PA, scale are HOST arrays of S doubles (scale may be NULL:
+ *      all 1); every other array is a device array as in the single-source calls.  chi2 compares the summed
+ *      visibilities with the observations.  gal_last_oob_count() is summed over the sources. ---- */
+int gal_sample_image_multi_f64(gal_plan* plan, const double* image, double dxy, const double* u, const double* v,
+                               int64_t M, int S, const double* dRA, const double* dDec, const double* PA,
+                               const double* scale, double* vis_out, void* stream);
+int gal_sample_image_multi_f32(gal_plan* plan, const float* image, double dxy, const float* u, const float* v,
+                               int64_t M, int S, const double* dRA, const double* dDec, const double* PA,
+                               const double* scale, float* vis_out, void* stream);
+int gal_chi2_image_multi_f64(gal_plan* plan, const double* image, double dxy, const double* u, const double* v,
+                             const double* re_obs, const double* im_obs, const double* w, int64_t M, int S,
+                             const double* dRA, const double* dDec, const double* PA, const double* scale,
+                             double* chi2_out, void* stream);
+int gal_chi2_image_multi_f32(gal_plan* plan, const float* image, double dxy, const float* u, const float* v,
+                             const float* re_obs, const float* im_obs, const float* w, int64_t M, int S,
+                             const double* dRA, const double* dDec, const double* PA, const double* scale,
+                             double* chi2_out, void* stream);
 
 /* ---- HOST-pointer entry points (the paper's calling convention): every array is in
  *      host memory; the call stages it through plan-owned device buffers on `stream`, runs the same

@@ -66,6 +66,11 @@ def load_library() -> ctypes.CDLL:
                                                               _d, _d, _d, _d, _vp, _vp]
             getattr(lib, f"gal_chi2_image_batch_{s}").argtypes = [_vp, _vp, _i, _d, _vp, _vp, _vp, _vp, _vp, _i64, _d,
                                                                   _d, _d, _vp, _vp, _vp]
+        for s in ("f64", "f32"):
+            getattr(lib, f"gal_sample_image_multi_{s}").argtypes = [_vp, _vp, _d, _vp, _vp, _i64, _i, _vp, _vp, _vp, _vp,
+                                                                    _vp, _vp]
+            getattr(lib, f"gal_chi2_image_multi_{s}").argtypes = [_vp, _vp, _d, _vp, _vp, _vp, _vp, _vp, _i64, _i, _vp,
+                                                                  _vp, _vp, _vp, _vp, _vp]
         lib.gal_sample_image_host_f64.argtypes = [_vp, _vp, _d, _vp, _vp, _i64, _d, _d, _d, _vp, _vp]
         lib.gal_chi2_profile_host_f64.argtypes = [_vp, _vp, _i, _d, _d, _d, _vp, _vp, _vp, _vp, _vp, _i64, _d, _d, _d,
                                                   _d, _vp, _vp]
@@ -153,6 +158,33 @@ class Plan:
     def set_pruning(self, mode: int) -> None:
         """0 = never, 1 = automatic (default), 2 = always: see gal_plan_set_pruning."""
         _check(self._lib.gal_plan_set_pruning(self._h, int(mode)), "gal_plan_set_pruning", self)
+
+    @staticmethod
+    def _placements(placements):
+        """[(dRA, dDec, PA[, scale]), ...] -> four host double arrays."""
+        a = np.array([tuple(pl) + (1.0,) * (4 - len(pl)) for pl in placements], dtype=np.float64).reshape(-1, 4)
+        return [np.ascontiguousarray(a[:, i]) for i in range(4)]
+
+    def sampleImageMulti(self, image, dxy, u, v, placements, out=None):
+        """sum_s scale_s * sampleImage(image; dRA_s, dDec_s, PA_s): one transform, S placements."""
+        M = u.numel()
+        out = torch.empty(M, dtype=self._cdtype, device=u.device) if out is None else out
+        dRA, dDec, PA, sc = self._placements(placements)
+        _check(self._fn("sample_image_multi")(self._h, self._dev(image, "image"), dxy, self._dev(u, "u"),
+                                              self._dev(v, "v"), M, len(dRA), dRA.ctypes.data, dDec.ctypes.data,
+                                              PA.ctypes.data, sc.ctypes.data, out.data_ptr(), _stream()),
+               "gal_sample_image_multi", self)
+        return out
+
+    def chi2ImageMulti(self, image, dxy, u, v, re_obs, im_obs, w, placements, out=None):
+        out = torch.empty(1, dtype=torch.float64, device=u.device) if out is None else out
+        dRA, dDec, PA, sc = self._placements(placements)
+        _check(self._fn("chi2_image_multi")(self._h, self._dev(image, "image"), dxy, self._dev(u, "u"),
+                                            self._dev(v, "v"), self._dev(re_obs, "re_obs"), self._dev(im_obs, "im_obs"),
+                                            self._dev(w, "w"), u.numel(), len(dRA), dRA.ctypes.data, dDec.ctypes.data,
+                                            PA.ctypes.data, sc.ctypes.data, out.data_ptr(), _stream()),
+               "gal_chi2_image_multi", self)
+        return out
 
     def bind_uv(self, u, v) -> None:
         """Promise that u and v ([M] or [C][M] CUDA tensors) keep their contents: later calls that pass these

@@ -45,6 +45,8 @@ struct gal_plan {
     int* b_ext_dev = nullptr;            // [4]
     unsigned long long* b_r2 = nullptr;  // [1] scratch of the radius kernel
     bool last_bound = false;             // the most recent call used the bound extent
+    double cur_amp = 1.0; int cur_accumulate = 0;   // multi-source composition: set around launch_sample
+    void* st_vis = nullptr; size_t st_vis_bytes = 0; // summed visibilities of a chi2 multi-source call
     std::set<const void*> smem_set;      // kernels whose dynamic shared-memory limit has been raised
     int max_gx = 0;
     size_t owned_bytes = 0;
@@ -300,6 +302,7 @@ int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T
     sp.M = M;
     sp.u = u; sp.v = v; sp.re_obs = re; sp.im_obs = im; sp.w = w; sp.vis = vis;
     sp.ix = cs.ix;
+    sp.amp = p->cur_amp; sp.accumulate = p->cur_accumulate;
     sp.dRA_turns = cs.dRA_turns; sp.dDec_turns = cs.dDec_turns; sp.has_phase = cs.has_phase;
     sp.partials = p->partials;
     sp.tickets = p->tickets;
@@ -453,6 +456,67 @@ int grow(gal_plan* p, void** buf, size_t* have, size_t want) {
     GAL_CUDA(p, cudaMalloc(buf, want));
     *have = want;
     p->owned_bytes += want;
+    return GAL_OK;
+}
+
+// Multi-source composition: one model image, S placements
+// (dRA_s, dDec_s, PA_s, scale_s); V = sum_s scale_s V_s by the linearity of the transform.  One FFT (pruned to
+// the union of the sources' uv extents), then one sampling launch per source that adds into vis; for chi2 the sum
+// goes to a plan-owned buffer and a last kernel compares it with the observations.
+template <typename T>
+int do_multi(gal_plan* p, const T* image, double dxy, const T* u, const T* v, const T* re, const T* im, const T* w,
+             int64_t M, int S, const double* dRA, const double* dDec, const double* PA, const double* scale, T* vis,
+             double* chi2, void* stream) {
+    if (!prec_ok<T>(p) || !image || !(dxy > 0) || M < 0 || S < 1 || S > 4096 || !dRA || !dDec || !PA) return GAL_ERR_INVALID_ARGUMENT;
+    if (!vis && !chi2) return GAL_ERR_INVALID_ARGUMENT;
+    if (M > 0 && (!u || !v || (chi2 && (!re || !im || !w)))) return GAL_ERR_INVALID_ARGUMENT;
+    for (int s = 0; s < S; ++s)
+        if (!std::isfinite(dRA[s]) || !std::isfinite(dDec[s]) || !std::isfinite(PA[s]) || (scale && !std::isfinite(scale[s])))
+            return GAL_ERR_INVALID_ARGUMENT;
+    DeviceGuard g(p->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    p->last_stream = st;
+    int rc;
+    if (M == 0) {
+        if (chi2) GAL_CUDA(p, cudaMemsetAsync(chi2, 0, sizeof(double), st));
+        return GAL_OK;
+    }
+    T* target = vis;
+    if (!vis) {
+        if ((rc = grow(p, &p->st_vis, &p->st_vis_bytes, (size_t)2 * M * sizeof(T)))) return rc;
+        target = (T*)p->st_vis;
+    }
+    if ((rc = reset_call_state(p, st))) return rc;
+    std::vector<CallScalars> cs(S);
+    bool prune = want_prune<T>(p, 1, M * S);
+    for (int s = 0; s < S; ++s) { cs[s] = call_scalars(p, dxy, dRA[s], dDec[s], PA[s]); prune = prune && !cs[s].ix.du_exact_div; }
+    p->last_pruned = prune; p->last_bound = false;
+    const int* ext = p->ext_full;
+    if (prune) {                                      // the atomics of the S launches form the union of the extents
+        for (int s = 0; s < S; ++s) if ((rc = launch_extent<T>(p, 1, cs[s], u, v, M, st))) return rc;
+        ext = p->ext;
+    }
+    if ((rc = fft2<T>(p, image, nullptr, 1, ext, st))) return rc;
+    for (int s = 0; s < S; ++s) {
+        p->cur_amp = scale ? scale[s] : 1.0;
+        p->cur_accumulate = s > 0;
+        rc = launch_sample<T>(p, 1, cs[s], u, v, nullptr, nullptr, nullptr, M, target, nullptr, nullptr, st);
+        p->cur_amp = 1.0; p->cur_accumulate = 0;
+        if (rc) return rc;
+    }
+    if (!vis) {
+        SampleParams<T> sp = {};
+        sp.N = p->nxy; sp.M = M; sp.vis = target; sp.re_obs = re; sp.im_obs = im; sp.w = w;
+        sp.partials = p->partials; sp.tickets = p->tickets; sp.chi2_per_channel = chi2; sp.chi2_total = nullptr;
+        sp.oob = p->oob; sp.done = (unsigned int*)((char*)p->oob + 20);
+        sp.next_state = (unsigned long long*)((char*)p->call_state + 32 * (p->cur ^ 1));
+        sp.viol = (unsigned long long*)((char*)p->oob + 24); sp.ext_check = nullptr;
+        long long blocks = (M + 1023) / 1024;
+        if (blocks > p->max_gx) blocks = p->max_gx;
+        GAL_CUDA(p, launch_chain(chi2_from_vis_kernel<T>, dim3((unsigned)blocks), dim3(256), 0, st, sp));
+        p->launches++;
+        GAL_CUDA(p, cudaGetLastError());
+    }
     return GAL_OK;
 }
 
@@ -613,7 +677,7 @@ int gal_plan_destroy(gal_plan* p) {
     DeviceGuard g(p->device);
     cudaFree(p->spec); cudaFree(p->work); cudaFree(p->tw); cudaFree(p->partials); cudaFree(p->tickets); cudaFree(p->chi2_scratch);
     for (cudaEvent_t e : p->tev) cudaEventDestroy(e);
-    cudaFree(p->call_state); cudaFree(p->call_init); cudaFree(p->ext_full); cudaFree(p->b_ext_dev); cudaFree(p->b_r2); cudaFree(p->st_image); cudaFree(p->st_pts); cudaFree(p->st_out); cudaFree(p->st_chi2);
+    cudaFree(p->call_state); cudaFree(p->call_init); cudaFree(p->ext_full); cudaFree(p->b_ext_dev); cudaFree(p->b_r2); cudaFree(p->st_vis); cudaFree(p->st_image); cudaFree(p->st_pts); cudaFree(p->st_out); cudaFree(p->st_chi2);
     delete p;
     return GAL_OK;
 }
@@ -765,6 +829,20 @@ int64_t gal_last_oob_count(gal_plan* p) {
         if (!p || !images || !chi2_pc || C < 1) return GAL_ERR_INVALID_ARGUMENT;                                      \
         return do_sample_image<T>(p, images, nullptr, C, dxy, u, v, re, im, w, M, dRA, dDec, PA, nullptr, chi2_pc,    \
                                   chi2_tot, stream);                                                                  \
+    }                                                                                                                 \
+    int gal_sample_image_multi_##SFX(gal_plan* p, const T* image, double dxy, const T* u, const T* v, int64_t M,      \
+                                     int S, const double* dRA, const double* dDec, const double* PA,                  \
+                                     const double* scale, T* vis, void* stream) {                                     \
+        if (M > 0 && !vis) return GAL_ERR_INVALID_ARGUMENT;                                                           \
+        if (M == 0) return GAL_OK;                                                                                    \
+        return do_multi<T>(p, image, dxy, u, v, nullptr, nullptr, nullptr, M, S, dRA, dDec, PA, scale, vis, nullptr,  \
+                           stream);                                                                                   \
+    }                                                                                                                 \
+    int gal_chi2_image_multi_##SFX(gal_plan* p, const T* image, double dxy, const T* u, const T* v, const T* re,      \
+                                   const T* im, const T* w, int64_t M, int S, const double* dRA, const double* dDec,  \
+                                   const double* PA, const double* scale, double* chi2, void* stream) {               \
+        if (!chi2) return GAL_ERR_INVALID_ARGUMENT;                                                                   \
+        return do_multi<T>(p, image, dxy, u, v, re, im, w, M, S, dRA, dDec, PA, scale, nullptr, chi2, stream);        \
     }                                                                                                                 \
     int gal_chi2_image_host_##SFX(gal_plan* p, const T* image, double dxy, const T* u, const T* v, const T* re,       \
                                   const T* im, const T* w, int64_t M, double dRA, double dDec, double PA,             \

@@ -41,6 +41,8 @@ template <typename T> struct SampleParams {
     IndexScalars ix;
     double dRA_turns, dDec_turns;  // rotated offsets in turns: theta / 2 pi = u' dRA_turns + v' dDec_turns
     int has_phase;         // 0 when both rotated offsets are 0 (theta == 0 exactly)
+    double amp;            // factor on the visibilities (1 except for multi-source composition)
+    int accumulate;        // sample*: add to what vis already holds (sources after the first) instead of storing
     double* partials;      // [C][gridDim.x]
     unsigned int* tickets; // [C + 1]
     double* chi2_per_channel; // [C] or null
@@ -448,9 +450,14 @@ __device__ __forceinline__ void sample_points(const SampleParams<T>& p, SampleCt
             vr = ReInt * co - ImInt * sn;
             vi = ReInt * sn + ImInt * co;
         }
+        if (p.amp != 1.0) { vr *= (R)p.amp; vi *= (R)p.amp; }   // multi-source composition only
         if (WRITE_VIS) {
             const long long k = kpt(j);
-            if (k < M) __stcs(reinterpret_cast<cx<T>*>(p.vis) + c * M + k, mk<T>(vr, vi));
+            if (k < M) {
+                cx<T>* dst = reinterpret_cast<cx<T>*>(p.vis) + c * M + k;
+                if (p.accumulate) { const cx<T> old = *dst; vr += old.x; vi += old.y; }
+                __stcs(dst, mk<T>(vr, vi));
+            }
         }
         if (DO_CHI2) {                                      // PAPER.md:718 (Eq. 10); w = 0 for dead slots
             const R dr = vr - ld(2, j);
@@ -653,6 +660,23 @@ __global__ void __launch_bounds__(SampleGeom<T, DO_CHI2>::NT_TMA, GAL_SAMPLE_MIN
             sample_tile_plain<T, WRITE_VIS, DO_CHI2, false>(p, cx_, nfull, M, c);
     }
     sample_finish<T, DO_CHI2>(p, c, cx_.acc, cx_.oob, cx_.viol);
+}
+
+// chi2 of visibilities that are already in memory (multi-source composition: the sum over the sources has to be
+// complete before it is compared with the observations).  Same deterministic reduction as the sampler.
+template <typename T>
+__global__ void __launch_bounds__(256) chi2_from_vis_kernel(const SampleParams<T> p) {
+    pdl_wait();
+    const cx<T>* vis = reinterpret_cast<const cx<T>*>(p.vis);
+    double acc = 0.0;
+    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < p.M; k += (long long)gridDim.x * blockDim.x) {
+        const cx<T> vv = __ldcs(vis + k);
+        const double dr = (double)vv.x - (double)__ldcs(p.re_obs + k), di = (double)vv.y - (double)__ldcs(p.im_obs + k);
+        acc = fma(fma(dr, dr, di * di), (double)__ldcs(p.w + k), acc);
+    }
+    SampleParams<T> q = p;
+    q.ext_check = nullptr;
+    sample_finish<T, true>(q, 0, acc, 0u, 0u);
 }
 
 // max over the points of u^2 + v^2 (bit pattern of a non-negative double orders like an integer): the

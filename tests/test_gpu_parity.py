@@ -413,6 +413,37 @@ def test_bound_uv_set(g):
     assert bound.last_extent_violations() == 0 and torch.equal(c, free.sampleImage(img, w.dxy, u, v, w.PA, w.dRA, w.dDec))
 
 
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+def test_multi_source_composition(g, orc, dtype):
+    """one model image placed S times, V = sum_s scale_s V_s with one transform; against the oracle's
+    single-source visibilities summed in numpy, and chi2 against the oracle's chi2 of that sum."""
+    w = W.config(3, nxy=1024, M=120_011, n_src=40)
+    if dtype == torch.float32:
+        w = w.as_f32()
+    f = lambda a: np.asarray(a, dtype=np.float64)
+    places = [(w.dRA, w.dDec, w.PA), (-2e-7, 3e-7, 0.4, 0.5), (5e-7, 1e-7, 2.0, 2.0), (0.0, 0.0, -1.0, 0.25)]
+    ref = sum(sc * orc.sampleImage(f(w.image), w.dxy, f(w.u), f(w.v), PA, dRA, dDec, nthreads=threads(orc))
+              for dRA, dDec, PA, sc in [p + (1.0,) * (4 - len(p)) for p in places])
+    ref_chi2 = orc.chi2(ref, f(w.re_obs), f(w.im_obs), f(w.w))
+    plan = g.Plan(w.nxy, 1, dtype)
+    img, u, v, re, im, wt = (dev(a) for a in (w.image, w.u, w.v, w.re_obs, w.im_obs, w.w))
+    res = {}
+    for mode in (1, 0):
+        plan.set_pruning(mode)
+        vis = plan.sampleImageMulti(img, w.dxy, u, v, places)
+        chi2 = float(plan.chi2ImageMulti(img, w.dxy, u, v, re, im, wt, places).cpu()[0])
+        res[mode] = (vis.cpu().numpy(), chi2)
+    vis, chi2 = res[1]
+    assert np.array_equal(vis, res[0][0]) and chi2 == res[0][1]          # pruning (union of the extents) changes nothing
+    if dtype == torch.float64:
+        assert rel_err(vis, ref) <= TOL_VIS_F64 and abs(chi2 - ref_chi2) <= TOL_CHI2_F64 * abs(ref_chi2)
+        one = plan.sampleImageMulti(img, w.dxy, u, v, places[:1])
+        assert torch.equal(one, plan.sampleImage(img, w.dxy, u, v, w.PA, w.dRA, w.dDec))   # S = 1 is the plain call
+    else:
+        assert np.abs(vis - ref).max() <= TOL_VIS_F32 * np.abs(ref).max()
+        assert abs(chi2 - ref_chi2) <= TOL_CHI2_F32 * abs(ref_chi2)
+
+
 def test_per_call_state_across_calls(g, orc):
     """The out-of-grid counter and the uv extent belong to ONE call: the two device copies of that state are used
     alternately and re-armed by the sampler of the call before (or by an explicit copy after an M = 0 call)."""
