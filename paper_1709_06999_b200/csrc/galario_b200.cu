@@ -23,7 +23,6 @@ struct gal_plan {
     void* tw = nullptr;              // cx<T>[nxy]
     double* partials = nullptr;      // [batch][max_gx]
     unsigned int* tickets = nullptr; // [batch + 1]
-    double* chi2_scratch = nullptr;  // [batch]
     unsigned long long* oob = nullptr;   // call_state[0]; the uv extent follows it
     int* ext = nullptr;                  // {kumax, rmin, rmax} of the current call (device)
     int* ext_full = nullptr;             // constant {nxy/2, 0, nxy-1}: no pruning
@@ -630,7 +629,6 @@ int gal_plan_create(gal_plan** out, int nxy, int batch, int precision_bits, int 
     if ((e = cudaMalloc(&p->tw, (size_t)nxy * esz)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     if ((e = cudaMalloc((void**)&p->partials, sizeof(double) * (size_t)batch * p->max_gx)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     if ((e = cudaMalloc((void**)&p->tickets, sizeof(unsigned int) * (batch + 1))) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
-    if ((e = cudaMalloc((void**)&p->chi2_scratch, sizeof(double) * batch)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     if ((e = cudaMalloc(&p->call_state, 64)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     if ((e = cudaMalloc(&p->call_init, 32)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     if ((e = cudaMalloc((void**)&p->ext_full, 16)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
@@ -648,7 +646,7 @@ int gal_plan_create(gal_plan** out, int nxy, int batch, int precision_bits, int 
     }
     if ((e = cudaMalloc((void**)&p->st_chi2, sizeof(double))) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     p->owned_bytes = spec_bytes + work_bytes + (size_t)nxy * esz + sizeof(double) * (size_t)batch * p->max_gx +
-                     sizeof(unsigned int) * (batch + 1) + sizeof(double) * batch + 16;
+                     sizeof(unsigned int) * (batch + 1) + 176;
     if ((e = cudaMemset(p->tickets, 0, sizeof(unsigned int) * (batch + 1))) != cudaSuccess) return fail(GAL_ERR_CUDA, e);
     // the workspace starts as zeros (pruned calls leave parts of it unwritten; they are never sampled)
     if ((e = cudaMemset(p->spec, 0, spec_bytes)) != cudaSuccess) return fail(GAL_ERR_CUDA, e);
@@ -675,7 +673,7 @@ int gal_plan_create(gal_plan** out, int nxy, int batch, int precision_bits, int 
 int gal_plan_destroy(gal_plan* p) {
     if (!p) return GAL_ERR_INVALID_ARGUMENT;
     DeviceGuard g(p->device);
-    cudaFree(p->spec); cudaFree(p->work); cudaFree(p->tw); cudaFree(p->partials); cudaFree(p->tickets); cudaFree(p->chi2_scratch);
+    cudaFree(p->spec); cudaFree(p->work); cudaFree(p->tw); cudaFree(p->partials); cudaFree(p->tickets);
     for (cudaEvent_t e : p->tev) cudaEventDestroy(e);
     cudaFree(p->call_state); cudaFree(p->call_init); cudaFree(p->ext_full); cudaFree(p->b_ext_dev); cudaFree(p->b_r2); cudaFree(p->st_vis); cudaFree(p->st_image); cudaFree(p->st_pts); cudaFree(p->st_out); cudaFree(p->st_chi2);
     delete p;

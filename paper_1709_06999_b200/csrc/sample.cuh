@@ -167,22 +167,36 @@ __device__ __forceinline__ void sincos_quarter(float a, int q, float* sn, float*
     *cs = ((q + 1) & 2) ? -cc : cc;
 }
 
-// Node (row = shifted v index, col = u index) of the spectrum extended to all integers by the
-// periodicity and Hermitian symmetry of the DFT of a real image (reading A6).  Rare path (points
-// beyond the half-plane grid), kept out of line.
+// Node (kv mod N, ku mod N) of the spectrum extended to all integers by the periodicity and Hermitian symmetry
+// of the DFT of a real image (reading A6): columns 0..N/2 are stored; column cu > N/2 is the conjugate of column
+// N - cu at row -kv.  Used for the points whose cell leaves the half-plane grid; 32-bit index arithmetic.
 template <typename T>
-__device__ __noinline__ cx<T> node_any(const NodePair<T>* __restrict__ spec, int N, long long row, long long col) {
-    const int H = N >> 1;
-    long long kv = row - H;
-    long long cu = col & (long long)(N - 1);          // N is a power of two: floor-mod
-    if (cu <= H) {
-        const long long r = ((kv & (N - 1)) + H) & (N - 1);
-        return __ldg(&spec[cu * N + r].a);
-    }
-    const long long r = (((-kv) & (N - 1)) + H) & (N - 1);
-    cx<T> g = __ldg(&spec[(N - cu) * N + r].a);
+__device__ __forceinline__ cx<T> node_wrapped(const NodePair<T>* __restrict__ spec, int N, int cu, int kvm) {
+    const int H = N >> 1, m = N - 1;
+    if (cu <= H) return __ldg(&spec[cu * N + ((kvm + H) & m)].a);
+    cx<T> g = __ldg(&spec[(N - cu) * N + (((N - kvm) + H) & m)].a);
     g.y = -g.y;
     return g;
+}
+
+// Bilinear interpolation of the extended spectrum at (uidx, vidx) anywhere in the plane: the listing's
+// interpolation on wrapped nodes.  Out of line: one call per out-of-grid point keeps the hot
+// loop of the sampler free of this code.
+template <typename T>
+__device__ __noinline__ cx<double> wrapped_cell(const NodePair<T>* __restrict__ spec, int N, double uidx, double vidx) {
+    const double fx = floor(uidx), fy = floor(vidx);
+    const long long ix = (long long)fx, iy = (long long)fy;
+    const int m = N - 1, H = N >> 1;                        // N is a power of two: & m is the floor-mod
+    const int c0 = (int)(ix & m), c1 = (int)((ix + 1) & m);
+    const int kv0 = (int)((iy - H) & m), kv1 = (int)((iy + 1 - H) & m);
+    const cx<T> g00 = node_wrapped<T>(spec, N, c0, kv0), g01 = node_wrapped<T>(spec, N, c1, kv0);
+    const cx<T> g10 = node_wrapped<T>(spec, N, c0, kv1), g11 = node_wrapped<T>(spec, N, c1, kv1);
+    const double txr = __dsub_rn(uidx, fx), tyr = __dsub_rn(vidx, fy);
+    const double ax = 1.0 - txr, ay = 1.0 - tyr;
+    cx<double> r;
+    r.x = ay * (ax * (double)g00.x + txr * (double)g01.x) + tyr * (ax * (double)g10.x + txr * (double)g11.x);
+    r.y = ay * (ax * (double)g00.y + txr * (double)g01.y) + tyr * (ax * (double)g10.y + txr * (double)g11.y);
+    return r;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -431,14 +445,10 @@ __device__ __forceinline__ void sample_points(const SampleParams<T>& p, SampleCt
         R ImInt = fma(wy, o_im - m_im, m_im);
         if (!inside[j]) {           // rare: the cell leaves the half-plane grid (reading A6); dead slots never get here
             const PointIndex q = point_index<EXACT>(p.ix, (double)ld(0, j), (double)ld(1, j));
-            const long long ix = (long long)floor(q.uidx), iy = (long long)floor(q.vidx);
             if (q.uidx > p.ix.fH || q.vidx < 0.0 || q.vidx > p.ix.fN1) ++cx_.oob;
-            const cx<T> g00 = node_any<T>(spec, N, iy, ix), g01 = node_any<T>(spec, N, iy, ix + 1);
-            const cx<T> g10 = node_any<T>(spec, N, iy + 1, ix), g11 = node_any<T>(spec, N, iy + 1, ix + 1);
-            const double txr = __dsub_rn(q.uidx, floor(q.uidx)), tyr = __dsub_rn(q.vidx, floor(q.vidx));
-            const double ax = 1.0 - txr, ay = 1.0 - tyr;
-            ReInt = (R)(ay * (ax * (double)g00.x + txr * (double)g01.x) + tyr * (ax * (double)g10.x + txr * (double)g11.x));
-            ImInt = (R)(ay * (ax * (double)g00.y + txr * (double)g01.y) + tyr * (ax * (double)g10.y + txr * (double)g11.y));
+            const cx<double> g = wrapped_cell<T>(spec, N, q.uidx, q.vidx);
+            ReInt = (R)g.x;
+            ImInt = (R)g.y;
         }
         if (uneg[j]) ImInt = -ImInt;
         R vr = ReInt, vi = ImInt;
