@@ -39,6 +39,13 @@ template <typename T> using cx = typename Vec2<T>::type;
 
 // one entry of the sampled spectrum: the node of this column (.a) and of the next one (.b)
 template <typename T> struct __align__(2 * sizeof(cx<T>)) NodePair { cx<T> a, b; };
+// whole-entry stores: one 256-bit store in fp64 (sm_100), 128-bit in fp32
+__device__ __forceinline__ void store_pair(NodePair<double>* p, const NodePair<double>& e) {
+    asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(e.a.x), "d"(e.a.y), "d"(e.b.x), "d"(e.b.y) : "memory");
+}
+__device__ __forceinline__ void store_pair(NodePair<float>* p, const NodePair<float>& e) {
+    *reinterpret_cast<float4*>(p) = make_float4(e.a.x, e.a.y, e.b.x, e.b.y);
+}
 
 // Programmatic dependent launch (sm_90+): let the next kernel of the chain start placing its CTAs, and wait
 // until the kernel before this one has completed and its writes are visible.  Every kernel of a call does both
@@ -371,28 +378,67 @@ col_pass_kernel(const ColParams<T> p) {
         fft_steps12<T, R1, R2, R3, G::TPF>(S, t, p.tw, 1, [&](int n) -> cx<T> {
             return valid ? col[n] : mk<T>(0, 0);
         });
-        // step 3 straight to global memory: kv = k1 + R1*(c + R2*d); sign (-1)^(ku+kv) folds the image
-        // centre shift, row (kv + N/2) mod N folds the shift along v.  Each value goes to its own entry (.a)
-        // and to the entry of the column before (.b).
-        for (int it = t; it < R1 * R2; it += G::TPF) {
-            const int k1 = it % R1, c = it / R1;
-            const cx<T>* base = S + k1 * G::P1 + c * R3;
-            cx<T> a[R3];
+        // step 3; kv = k1 + R1*(c + R2*d); sign (-1)^(ku+kv) folds the image centre shift, row (kv + N/2) mod N
+        // folds the shift along v.  Each value goes to its own entry (.a) and to the entry of the column
+        // before (.b).
+        if constexpr (F == 1) {
+            // one column per CTA: straight from registers to global memory, two 16-byte stores per value
+            for (int it = t; it < R1 * R2; it += G::TPF) {
+                const int k1 = it % R1, c = it / R1;
+                const cx<T>* base = S + k1 * G::P1 + c * R3;
+                cx<T> a[R3];
 #pragma unroll
-            for (int b = 0; b < R3; ++b) a[b] = base[b];
-            Dft<T, R3>::run(a);
-            if (valid) {
+                for (int b = 0; b < R3; ++b) a[b] = base[b];
+                Dft<T, R3>::run(a);
+                if (valid) {
 #pragma unroll
-                for (int d = 0; d < R3; ++d) {
-                    const int kv = k1 + R1 * (c + R2 * d);
-                    const T sgn = ((ku + kv) & 1) ? (T)-1 : (T)1;
-                    const int kvs = (kv + L / 2) & (L - 1);
-                    if (kvs >= rmin && kvs <= rmax) {
-                        const cx<T> val = mk<T>(sgn * a[d].x, sgn * a[d].y);
-                        own[kvs].a = val;
-                        if (ku > 0) prev[kvs].b = val;
+                    for (int d = 0; d < R3; ++d) {
+                        const int kv = k1 + R1 * (c + R2 * d);
+                        const T sgn = ((ku + kv) & 1) ? (T)-1 : (T)1;
+                        const int kvs = (kv + L / 2) & (L - 1);
+                        if (kvs >= rmin && kvs <= rmax) {
+                            const cx<T> val = mk<T>(sgn * a[d].x, sgn * a[d].y);
+                            own[kvs].a = val;
+                            if (ku > 0) prev[kvs].b = val;
+                        }
                     }
                 }
+            }
+        } else {
+            // several adjacent columns per CTA: the signed results go back to shared memory and are written
+            // out as whole entries {F[ku], F[ku+1]} (one 32-byte store in fp64, a full sector) wherever both
+            // columns are in this CTA; only the first column's .b of the entry before and the last column's .a
+            // remain half-sector stores.
+            for (int it = t; it < R1 * R2; it += G::TPF) {
+                const int k1 = it % R1, c = it / R1;
+                cx<T>* base = S + k1 * G::P1 + c * R3;
+                cx<T> a[R3];
+#pragma unroll
+                for (int b = 0; b < R3; ++b) a[b] = base[b];
+                Dft<T, R3>::run(a);
+                const T sgn = ((ku + k1) & 1) ? (T)-1 : (T)1;     // R1 is even: kv and k1 have one parity
+#pragma unroll
+                for (int d = 0; d < R3; ++d) base[d] = mk<T>(sgn * a[d].x, sgn * a[d].y);
+            }
+            __syncthreads();
+            const long long g0 = grp * F;
+            for (int idx = tid; idx < F * L; idx += G::NT) {
+                const int ff = idx / L, kvs = idx % L;
+                const long long gg = g0 + ff;
+                const int kuf = (int)(gg % NU);
+                if (gg >= p.cols_total || kuf > kumax || kvs < rmin || kvs > rmax) continue;
+                const int za = G::zaddr((kvs + L / 2) & (L - 1));
+                const cx<T> x = smem[ff * G::REGION + za];
+                NodePair<T>* e = p.pair + gg * (long long)L + kvs;
+                if (ff + 1 < F && kuf < L / 2 && kuf + 1 <= kumax) {
+                    NodePair<T> pr;
+                    pr.a = x;
+                    pr.b = smem[(ff + 1) * G::REGION + za];
+                    store_pair(e, pr);
+                } else {
+                    e->a = x;
+                }
+                if (ff == 0 && kuf > 0) (e - L)->b = x;
             }
         }
     }
