@@ -316,9 +316,10 @@ int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T
     const int tile = SampleGeom<T, true>::TILE;
     const long long ntiles = (M + tile - 1) / tile;
     long long cap = (long long)p->sm_count * GAL_SAMPLE_MINB;
-    // batched: CTAs are placed channel by channel (blockIdx.x fastest); a quarter of the resident CTAs per
-    // channel keeps about four channels' spectra (not dozens) competing for the L2 at any time
-    if (C > 1) cap = (cap + 3) / 4;
+    // batched: CTAs are placed channel by channel (blockIdx.x fastest); an eighth of the resident CTAs per
+    // channel keeps about eight channels' spectra (not dozens) competing for the L2 at any time and gives every
+    // CTA enough tiles to amortise its prologue and reduction (measured at cfg 4: 2: 573, 4: 481, 8: 420 us)
+    if (C > 1) cap = (cap + 7) / 8;
     if (cap > p->max_gx) cap = p->max_gx;
     long long gx = ntiles < cap ? ntiles : cap;
     if (gx < 1) gx = 1;
