@@ -227,21 +227,40 @@ struct SweepParams {
     const void* I;      // profile, T[nr]
     int nr;
     double Rmin, dR, Rmax, dxy, inc_cos;
+    double r_dR, r_inc;      // RN(1 / dR), RN(1 / inc_cos) for the exact-division shortcut
+    int true_div;            // 1: a reciprocal is not usable (host check), take true divisions
 };
+
+// a / b, correctly rounded, from r = RN(1 / b) (Markstein; see sample.cuh div_by): bit-identical to the IEEE
+// division the listing performs, at 3 FP64 operations instead of a division sequence.
+__device__ __forceinline__ double div_exact(double a, double b, double r, int true_div) {
+    if (true_div) return __ddiv_rn(a, b);
+    const double q0 = __dmul_rn(a, r);
+    return __fma_rn(__fma_rn(-q0, b, a), r, q0);
+}
+// (double)n for 0 <= n < 2^31 without the conversion pipe: 2^52 + n is exact, minus 2^52
+__device__ __forceinline__ double int_to_double(int n) {
+    return __dsub_rn(__hiloint2double(0x43300000, n), 4503599627370496.0);
+}
 
 template <typename T>
 __device__ __forceinline__ double sweep_pixel(const SweepParams& sp, int N, int i, int j) {
-    const double fN = (double)N;
-    const double y = __dmul_rn(__dmul_rn(__dsub_rn(0.5, __ddiv_rn((double)i, fN)), sp.dxy), fN);
-    const double x = __dmul_rn(__dmul_rn(__dsub_rn(0.5, __ddiv_rn((double)j, fN)), sp.dxy), fN);
-    const double xs = __ddiv_rn(x, sp.inc_cos);
+    // N is a power of two: i / N is the exact product i * (1 / N).  The other divisions use the reciprocal
+    // shortcut; floor() and the int <-> double conversions go through the 2^52 mantissa trick (all exact).
+    const double fN = int_to_double(N), rN = 1.0 / fN;
+    const double y = __dmul_rn(__dmul_rn(__dsub_rn(0.5, __dmul_rn(int_to_double(i), rN)), sp.dxy), fN);
+    const double x = __dmul_rn(__dmul_rn(__dsub_rn(0.5, __dmul_rn(int_to_double(j), rN)), sp.dxy), fN);
+    const double xs = div_exact(x, sp.inc_cos, sp.r_inc, sp.true_div);
     const double r = __dsqrt_rn(__dadd_rn(__dmul_rn(xs, xs), __dmul_rn(y, y)));
     if (!(r >= sp.Rmin && r <= sp.Rmax)) return 0.0;
-    const double pos = __ddiv_rn(__dsub_rn(r, sp.Rmin), sp.dR);
-    long long k = (long long)floor(pos);
+    const double pos = div_exact(__dsub_rn(r, sp.Rmin), sp.dR, sp.r_dR, sp.true_div);
+    // k = floor(pos) clamped to [0, nr - 2]; pos >= 0 here and far below 2^31 (pos <= nr - 1 + rounding)
+    const double tk = __dadd_rn(pos, 4503599627370496.0);
+    int k = __double2loint(tk);
+    if (__dsub_rn(tk, 4503599627370496.0) > pos) k -= 1;
     if (k >= sp.nr - 1) k = sp.nr - 2;
     if (k < 0) k = 0;
-    const double t = __dsub_rn(pos, (double)k);
+    const double t = __dsub_rn(pos, int_to_double(k));
     const T* I = (const T*)sp.I;
     const double i0 = (double)__ldg(I + k), i1 = (double)__ldg(I + k + 1);
     const double val = __dadd_rn(i0, __dmul_rn(t, __dsub_rn(i1, i0)));

@@ -399,6 +399,13 @@ bool sweep_args(const gal_plan* p, const void* I, int nr, double Rmin, double dR
     if (!(std::fabs(inc) < 1.5707963267948966) || !(c > 0)) return false;
     sw->I = I; sw->nr = nr; sw->Rmin = Rmin; sw->dR = dR; sw->dxy = dxy; sw->inc_cos = c;
     sw->Rmax = Rmin + dR * (double)(nr - 1);
+    sw->r_dR = 1.0 / dR;
+    sw->r_inc = 1.0 / c;
+    auto bad = [](double b, double r) {     // Markstein's shortcut needs a normal divisor whose significand is not all ones
+        uint64_t bits; memcpy(&bits, &b, 8);
+        return ((bits & 0xFFFFFFFFFFFFFull) == 0xFFFFFFFFFFFFFull) || !std::isnormal(b) || !std::isnormal(r);
+    };
+    sw->true_div = (bad(dR, sw->r_dR) || bad(c, sw->r_inc)) ? 1 : 0;
     (void)p;
     return true;
 }
