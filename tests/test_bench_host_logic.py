@@ -22,6 +22,15 @@ def test_algorithmic_bytes_match_survey_table():
     assert S["sample"] == 160_000_000
     F = bench.algorithmic_bytes(4096, 5_000_000, 4)
     assert F["step"] * 2 == B["step"]
+    # a pruned call: only columns 0..kumax are written and transformed, only rows kvs_min..kvs_max written back,
+    # u and v are read a second time by the uv-extent kernel
+    P = bench.algorithmic_bytes(4096, 5_000_000, 8, extent=(505, 1590, 2282))
+    assert P["uv_extent"] == 80_000_000
+    assert P["row_pass"] == 4096 * 4096 * 8 + 506 * 4096 * 16
+    assert P["col_pass"] == 506 * 4096 * 16 + 506 * 693 * 16
+    assert P["step"] < B["step"] and P["sample"] == B["sample"]
+    whole = bench.algorithmic_bytes(4096, 5_000_000, 8, extent=(2048, 0, 4095))
+    assert whole["row_pass"] == B["row_pass"] and whole["col_pass"] == B["col_pass"]
 
 
 def _worker(rank, world, port, q):
