@@ -53,7 +53,7 @@ def algorithmic_bytes(nxy: int, M: int, esz: int, entry: str = "chi2Image", exte
         kumax, rmin, rmax = extent
         cols = kumax + 1
         row = img + cols * nxy * 2 * esz
-        col = cols * nxy * 2 * esz + cols * (rmax - rmin + 1) * 2 * esz
+        col = cols * nxy * 2 * esz + cols * (rmax - rmin + 1) * 4 * esz   # column pairs: every value written twice
         ext = 2 * esz * M
     return {"uv_extent": ext, "row_pass": row, "col_pass": col, "sample": samp, "step": ext + row + col + samp}
 

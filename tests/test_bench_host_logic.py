@@ -27,10 +27,10 @@ def test_algorithmic_bytes_match_survey_table():
     P = bench.algorithmic_bytes(4096, 5_000_000, 8, extent=(505, 1590, 2282))
     assert P["uv_extent"] == 80_000_000
     assert P["row_pass"] == 4096 * 4096 * 8 + 506 * 4096 * 16
-    assert P["col_pass"] == 506 * 4096 * 16 + 506 * 693 * 16
+    assert P["col_pass"] == 506 * 4096 * 16 + 506 * 693 * 32             # column pairs: written twice
     assert P["step"] < B["step"] and P["sample"] == B["sample"]
     whole = bench.algorithmic_bytes(4096, 5_000_000, 8, extent=(2048, 0, 4095))
-    assert whole["row_pass"] == B["row_pass"] and whole["col_pass"] == B["col_pass"]
+    assert whole["row_pass"] == B["row_pass"] and whole["col_pass"] == B["col_pass"] + 4096 * 2049 * 16
 
 
 def _worker(rank, world, port, q):
