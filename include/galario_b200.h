@@ -56,7 +56,8 @@ typedef struct gal_plan gal_plan;
 
 /* Create a plan for images of nxy x nxy pixels, up to `batch` images per call (1 for everything but
  * the batched cube), precision_bits = 64 or 32, on CUDA device `device`.  Allocates the twiddle table
- * and the workspace (batch * nxy * (nxy/2+1) complex numbers + reduction scratch). */
+ * and the workspace (3 * batch * nxy * (nxy/2+1) complex numbers: the row-transformed image and the spectrum
+ * as column pairs, plus reduction scratch). */
 int gal_plan_create(gal_plan** out, int nxy, int batch, int precision_bits, int device);
 int gal_plan_destroy(gal_plan* plan);
 /* Bytes of device memory the plan owns (workspace + tables + staging). */
