@@ -44,7 +44,6 @@ struct gal_plan {
     int* b_ext_dev = nullptr;            // [4]
     unsigned long long* b_r2 = nullptr;  // [1] scratch of the radius kernel
     bool last_bound = false;             // the most recent call used the bound extent
-    double cur_amp = 1.0; int cur_accumulate = 0;   // multi-source composition: set around launch_sample
     void* st_vis = nullptr; size_t st_vis_bytes = 0; // summed visibilities of a chi2 multi-source call
     std::set<const void*> smem_set;      // kernels whose dynamic shared-memory limit has been raised
     int max_gx = 0;
@@ -208,6 +207,8 @@ struct CallScalars {
     IndexScalars ix;
     double dRA_turns, dDec_turns;
     int has_phase;
+    double amp = 1.0;      // factor on the visibilities and accumulate-into-vis flag: multi-source composition only
+    int accumulate = 0;
 };
 
 // host-side scalars, plain double arithmetic in the listing's order.  The
@@ -301,7 +302,7 @@ int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T
     sp.M = M;
     sp.u = u; sp.v = v; sp.re_obs = re; sp.im_obs = im; sp.w = w; sp.vis = vis;
     sp.ix = cs.ix;
-    sp.amp = p->cur_amp; sp.accumulate = p->cur_accumulate;
+    sp.amp = cs.amp; sp.accumulate = cs.accumulate;
     sp.dRA_turns = cs.dRA_turns; sp.dDec_turns = cs.dDec_turns; sp.has_phase = cs.has_phase;
     sp.partials = p->partials;
     sp.tickets = p->tickets;
@@ -505,11 +506,9 @@ int do_multi(gal_plan* p, const T* image, double dxy, const T* u, const T* v, co
     }
     if ((rc = fft2<T>(p, image, nullptr, 1, ext, st))) return rc;
     for (int s = 0; s < S; ++s) {
-        p->cur_amp = scale ? scale[s] : 1.0;
-        p->cur_accumulate = s > 0;
-        rc = launch_sample<T>(p, 1, cs[s], u, v, nullptr, nullptr, nullptr, M, target, nullptr, nullptr, st);
-        p->cur_amp = 1.0; p->cur_accumulate = 0;
-        if (rc) return rc;
+        cs[s].amp = scale ? scale[s] : 1.0;
+        cs[s].accumulate = s > 0;
+        if ((rc = launch_sample<T>(p, 1, cs[s], u, v, nullptr, nullptr, nullptr, M, target, nullptr, nullptr, st))) return rc;
     }
     if (!vis) {
         SampleParams<T> sp = {};
