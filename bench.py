@@ -171,7 +171,7 @@ def run_reference(args, rank: int):
     if rank != 0:
         return
     import oracle
-    from paper_1709_06999_b200 import workloads
+    import workloads
     oracle.build()
     w = workloads.config(3)
     T = oracle.host_threads()
@@ -215,7 +215,7 @@ def main():
 
     import torch
     import paper_1709_06999_b200 as g
-    from paper_1709_06999_b200 import workloads
+    import workloads
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the galario-b200 path has no CPU fallback")
     g.load_library()

@@ -31,7 +31,7 @@ def build(force: bool = False) -> Path:
     """Compile the oracle with g++ (-O2, C++17).  Building the checker is not using it."""
     if force or not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
         tmp = _LIB.with_suffix(f".so.tmp{os.getpid()}")
-        cmd = ["g++", "-O2", "-std=c++17", "-shared", "-fPIC", "-pthread", str(_SRC), "-o", str(tmp)]
+        cmd = ["g++", "-O2", "-ffp-contract=off", "-std=c++17", "-shared", "-fPIC", "-pthread", str(_SRC), "-o", str(tmp)]
         subprocess.run(cmd, check=True)
         os.replace(tmp, _LIB)
     return _LIB
@@ -158,16 +158,18 @@ def chi2Profile(I, Rmin, dR, nxy, dxy, u, v, re_obs, im_obs, w, dRA=0.0, dDec=0.
     return out.value
 
 
-def chi2ImageBatch(images, dxy, u, v, re_obs, im_obs, w, dRA=0.0, dDec=0.0, PA=0.0, nthreads: int = 1):
-    """images [C][n][n]; u, v, re_obs, im_obs, w [C][M].  Returns (chi2[C], total)."""
+def chi2ImageBatch(images, dxy, u, v, re_obs, im_obs, w, dRA=0.0, dDec=0.0, PA=0.0, nthreads: int = 1,
+                   return_oob: bool = False):
+    """images [C][n][n]; u, v, re_obs, im_obs, w [C][M].  Returns (chi2[C], total[, out-of-grid points])."""
     images = _f64(images)
     C, n, _ = images.shape
     u, v, re_obs, im_obs, w = _f64(u), _f64(v), _f64(re_obs), _f64(im_obs), _f64(w)
     M = u.shape[1]
     per = np.empty(C, dtype=np.float64)
     tot = ctypes.c_double(0.0)
+    oob = ctypes.c_int64(0)
     _check(lib().orc_chi2_image_batch(_p(images), ctypes.c_int(C), ctypes.c_int(n), ctypes.c_double(dxy), _p(u),
                                       _p(v), _p(re_obs), _p(im_obs), _p(w), ctypes.c_int64(M),
                                       ctypes.c_double(dRA), ctypes.c_double(dDec), ctypes.c_double(PA), _p(per),
-                                      ctypes.byref(tot), None, ctypes.c_int(nthreads)), "chi2ImageBatch")
-    return per, tot.value
+                                      ctypes.byref(tot), ctypes.byref(oob), ctypes.c_int(nthreads)), "chi2ImageBatch")
+    return (per, tot.value, oob.value) if return_oob else (per, tot.value)

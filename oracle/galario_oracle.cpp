@@ -17,7 +17,7 @@
 // Gaussian closed forms, Hermitian symmetry, Parseval, PA = 90 deg identity, chi2
 // invariants, scipy.interp1d for the sweep.  No function here is "parity unpinned".
 //
-// Build: g++ -O2 -std=c++17 -shared -fPIC -pthread galario_oracle.cpp -o liboracle.so
+// Build: g++ -O2 -ffp-contract=off -std=c++17 -shared -fPIC -pthread galario_oracle.cpp -o liboracle.so
 //
 // All pointers are HOST pointers, all arrays are double, caller-owned.  Complex arrays
 // are interleaved (re, im).  Functions return 0 on success, negative on bad arguments.

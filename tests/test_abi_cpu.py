@@ -60,7 +60,7 @@ def test_product_never_imports_oracle_and_oracle_never_imports_product():
 
 def test_workloads_shapes_and_determinism():
     import numpy as np
-    from paper_1709_06999_b200 import workloads as W
+    import workloads as W
     a, b = W.config(0), W.config(0)
     assert a.nxy == 256 and a.M == 10_000 and a.image.shape == (256, 256)
     assert np.array_equal(a.u, b.u) and np.array_equal(a.image, b.image) and np.array_equal(a.re_obs, b.re_obs)

@@ -12,7 +12,7 @@ import numpy as np
 import pytest
 import torch
 
-from paper_1709_06999_b200 import workloads as W
+import workloads as W
 
 pytestmark = pytest.mark.gpu
 
@@ -223,6 +223,8 @@ def test_config3_full_f32(g, orc, cfg3_full):
 
 
 def test_config4_full(g, orc):
+    """All 128 channels at the launch geometry bench.py times (grid.y = 128), each against the oracle, the total
+    against the oracle's, and the out-of-grid count against the oracle's summed count."""
     w = W.config(4)
     C = w.image.shape[0]
     plan = g.Plan(w.nxy, C)
@@ -230,14 +232,29 @@ def test_config4_full(g, orc):
                                    w.dRA, w.dDec, w.PA)
     oob = plan.last_oob_count()
     per, tot = per.cpu().numpy(), float(tot.cpu()[0])
-    # the oracle computes sampled channels one by one; the total is checked by its definition
-    for c in (0, 1, 37, 63, 64, 100, 127):
-        r = orc.chi2Image(w.image[c], w.dxy, w.u[c], w.v[c], w.re_obs[c], w.im_obs[c], w.w[c], w.dRA, w.dDec, w.PA,
-                          nthreads=threads(orc))
-        assert abs(per[c] - r) <= TOL_CHI2_F64 * abs(r), c
-    import math
-    assert abs(tot - math.fsum(per)) <= 1e-13 * tot
-    assert oob > 0          # 16 km at 230 GHz reaches index 609 > 512: some points wrap (reading A6)
+    rper, rtot, roob = orc.chi2ImageBatch(w.image, w.dxy, w.u, w.v, w.re_obs, w.im_obs, w.w, w.dRA, w.dDec, w.PA,
+                                          nthreads=threads(orc), return_oob=True)
+    assert per.shape == rper.shape == (C,)
+    assert (np.abs(per - rper) <= TOL_CHI2_F64 * np.abs(rper)).all(), np.argmax(np.abs(per - rper) / np.abs(rper))
+    assert abs(tot - rtot) <= TOL_CHI2_F64 * abs(rtot)
+    assert oob == roob and oob > 0      # 16 km at 230 GHz reaches index 609 > 512: some points wrap (reading A6)
+
+
+def test_config4_reduced_batch_f32(g, orc):
+    """gal_chi2_image_batch_f32 against the fp64 oracle on the fp32-rounded inputs (reading A14), per channel and
+    total, at the fp32 chi2 tolerance; the out-of-grid count is an integer decision taken in double on both sides."""
+    w = W.config(4, nxy=256, M=20_011, C=5).as_f32()
+    plan = g.Plan(w.nxy, 5, torch.float32)
+    per, tot = plan.chi2ImageBatch(dev(w.image), w.dxy, dev(w.u), dev(w.v), dev(w.re_obs), dev(w.im_obs), dev(w.w),
+                                   w.dRA, w.dDec, w.PA)
+    oob = plan.last_oob_count()
+    f = lambda a: np.asarray(a, dtype=np.float64)
+    rper, rtot, roob = orc.chi2ImageBatch(f(w.image), w.dxy, f(w.u), f(w.v), f(w.re_obs), f(w.im_obs), f(w.w),
+                                          w.dRA, w.dDec, w.PA, nthreads=threads(orc), return_oob=True)
+    per, tot = per.cpu().numpy(), float(tot.cpu()[0])
+    assert (np.abs(per - rper) <= TOL_CHI2_F32 * np.abs(rper)).all()
+    assert abs(tot - rtot) <= TOL_CHI2_F32 * abs(rtot)
+    assert oob == roob
 
 
 # ---------------------------------------------------------------------------------------------
@@ -444,6 +461,28 @@ def test_multi_source_composition(g, orc, dtype):
         assert abs(chi2 - ref_chi2) <= TOL_CHI2_F32 * abs(ref_chi2)
 
 
+def test_multi_source_with_out_of_grid_points(g, orc):
+    """Multi-source on config 0 (7.5 % of the points leave the half-plane grid after the rotation, reading A6): the
+    union of the extents is the whole plane; S = 2 exercises one accumulate step, S = 3 two; the out-of-grid count
+    is summed over the sources."""
+    w = W.config(0)
+    plan = g.Plan(w.nxy)
+    img, u, v, re, im, wt = (dev(a) for a in (w.image, w.u, w.v, w.re_obs, w.im_obs, w.w))
+    for places in ([(w.dRA, w.dDec, w.PA), (1e-7, -2e-7, 1.1, 0.5)],
+                   [(w.dRA, w.dDec, w.PA, 0.7), (0.0, 0.0, 0.0, 1.0), (-3e-7, 2e-7, 2.5, 0.3)]):
+        ref, roob = 0.0, 0
+        for dRA, dDec, PA, sc in [p + (1.0,) * (4 - len(p)) for p in places]:
+            vs, o = orc.sampleImage(w.image, w.dxy, w.u, w.v, PA, dRA, dDec, nthreads=threads(orc), return_oob=True)
+            ref, roob = ref + sc * vs, roob + o
+        vis = plan.sampleImageMulti(img, w.dxy, u, v, places).cpu().numpy()
+        assert plan.last_oob_count() == roob and roob > 0
+        assert plan.last_uv_extent() == (w.nxy // 2, 0, w.nxy - 1)
+        assert rel_err(vis, ref) <= TOL_VIS_F64
+        chi2 = float(plan.chi2ImageMulti(img, w.dxy, u, v, re, im, wt, places).cpu()[0])
+        ref_chi2 = orc.chi2(ref, w.re_obs, w.im_obs, w.w)
+        assert abs(chi2 - ref_chi2) <= TOL_CHI2_F64 * abs(ref_chi2)
+
+
 def test_per_call_state_across_calls(g, orc):
     """The out-of-grid counter and the uv extent belong to ONE call: the two device copies of that state are used
     alternately and re-armed by the sampler of the call before (or by an explicit copy after an M = 0 call)."""
@@ -513,9 +552,17 @@ def test_smallest_and_largest_nxy_end_to_end(g, orc):
         du = 1.0 / (n * dxy)
         img = rng.random((n, n))
         u, v = rng.uniform(-0.45 * n, 0.45 * n, M) * du, rng.uniform(-0.45 * n, 0.45 * n, M) * du
-        vis = g.Plan(n).sampleImage(dev(img), dxy, dev(u), dev(v), 0.3, 1e-7, 1e-7).cpu().numpy()
+        plan = g.Plan(n)
+        vis = plan.sampleImage(dev(img), dxy, dev(u), dev(v), 0.3, 1e-7, 1e-7).cpu().numpy()
         ref = orc.sampleImage(img, dxy, u, v, 0.3, 1e-7, 1e-7, nthreads=threads(orc))
         assert rel_err(vis, ref) <= TOL_VIS_F64
+        # chi2 at the same size: observations = the oracle's visibilities + noise, seeded weights
+        re_o = ref.real + 1e-3 * rng.standard_normal(M)
+        im_o = ref.imag + 1e-3 * rng.standard_normal(M)
+        wt = rng.lognormal(np.log(1e6), 0.5, M)
+        chi2 = float(plan.chi2Image(dev(img), dxy, dev(u), dev(v), dev(re_o), dev(im_o), dev(wt), 1e-7, 1e-7, 0.3).cpu()[0])
+        ref_chi2 = orc.chi2(ref, re_o, im_o, wt)
+        assert abs(chi2 - ref_chi2) <= TOL_CHI2_F64 * abs(ref_chi2), n
 
 
 def test_error_codes(g):
