@@ -27,41 +27,9 @@
 // Shared-memory address of element (k1, a|c, b|d): k1*P1 + (a|c)*R3 + (b|d), P1 = R2*R3 + 1 (odd),
 // which makes every access pattern of the three steps bank-conflict free for 8/16-byte elements.
 #pragma once
-#include <cuda_runtime.h>
-#include <stdint.h>
+#include "common.cuh"
 
 namespace galb {
-
-template <typename T> struct Vec2;
-template <> struct Vec2<double> { using type = double2; };
-template <> struct Vec2<float> { using type = float2; };
-template <typename T> using cx = typename Vec2<T>::type;
-
-// one entry of the sampled spectrum: the node of this column (.a) and of the next one (.b)
-template <typename T> struct __align__(2 * sizeof(cx<T>)) NodePair { cx<T> a, b; };
-// whole-entry stores: one 256-bit store in fp64 (sm_100), 128-bit in fp32
-__device__ __forceinline__ void store_pair(NodePair<double>* p, const NodePair<double>& e) {
-    asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(e.a.x), "d"(e.a.y), "d"(e.b.x), "d"(e.b.y) : "memory");
-}
-__device__ __forceinline__ void store_pair(NodePair<float>* p, const NodePair<float>& e) {
-    *reinterpret_cast<float4*>(p) = make_float4(e.a.x, e.a.y, e.b.x, e.b.y);
-}
-
-// Programmatic dependent launch (sm_90+): let the next kernel of the chain start placing its CTAs, and wait
-// until the kernel before this one has completed and its writes are visible.  Every kernel of a call does both
-// before its first global-memory access (harmless when launched without the attribute).
-__device__ __forceinline__ void pdl_wait() {
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    asm volatile("griddepcontrol.wait;" ::: "memory");
-}
-
-template <typename T> __device__ __forceinline__ cx<T> mk(T x, T y) { cx<T> r; r.x = x; r.y = y; return r; }
-template <typename V> __device__ __forceinline__ V cadd(V a, V b) { a.x += b.x; a.y += b.y; return a; }
-template <typename V> __device__ __forceinline__ V csub(V a, V b) { a.x -= b.x; a.y -= b.y; return a; }
-template <typename V> __device__ __forceinline__ V cmul(V a, V b) {
-    V r; r.x = a.x * b.x - a.y * b.y; r.y = a.x * b.y + a.y * b.x; return r;
-}
-template <typename V> __device__ __forceinline__ V mul_mi(V a) { V r; r.x = a.y; r.y = -a.x; return r; }  // * (-i)
 
 // ------------------------------------------------------------------------------------------
 // Radix-R DFTs on register arrays, forward kernel exp(-2 pi i nk/R), natural-order output.
@@ -223,14 +191,6 @@ __device__ __forceinline__ void fft_steps12(cx<T>* S, int t, const cx<T>* __rest
 // listing and individually rounded (no FMA contraction) so that the hard-edge decisions
 // r < Rmin, r > Rmax agree with a plain IEEE evaluation.
 // ------------------------------------------------------------------------------------------
-struct SweepParams {
-    const void* I;      // profile, T[nr]
-    int nr;
-    double Rmin, dR, Rmax, dxy, inc_cos;
-    double r_dR, r_inc;      // RN(1 / dR), RN(1 / inc_cos) for the exact-division shortcut
-    int true_div;            // 1: a reciprocal is not usable (host check), take true divisions
-};
-
 // a / b, correctly rounded, from r = RN(1 / b) (Markstein; see sample.cuh div_by): bit-identical to the IEEE
 // division the listing performs, at 3 FP64 operations instead of a division sequence.
 __device__ __forceinline__ double div_exact(double a, double b, double r, int true_div) {

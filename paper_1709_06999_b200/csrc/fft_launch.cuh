@@ -1,0 +1,134 @@
+// fft_launch.cuh — launch geometry and radix plans of the FFT passes; included by fft_f64.cu / fft_f32.cu, which
+// instantiate it for one precision each.
+#pragma once
+#include <cstring>
+
+#include "fft.cuh"
+#include "plan.h"
+
+namespace galb {
+
+// ---------------------------------------------------------------------------------------------
+// FFT launchers
+// ---------------------------------------------------------------------------------------------
+template <typename T, int R1, int R2, int R3, int F>
+int launch_row(gal_plan* p, const T* image, const SweepParams* sw, int batch, const int* ext, cudaStream_t st) {
+    using G = Geom<T, R1, R2, R3, F>;
+    RowParams<T> rp;
+    rp.image = image;
+    rp.spec = (cx<T>*)p->work;
+    rp.tw = (const cx<T>*)p->tw;
+    rp.N = p->nxy;
+    rp.rows_total = batch * p->nxy;
+    rp.ext = ext;
+    if (sw) rp.sweep = *sw; else memset(&rp.sweep, 0, sizeof(rp.sweep));
+    const unsigned grid = (unsigned)((rp.rows_total + F - 1) / F);
+    if (sw) {
+        auto k = row_pass_kernel<T, R1, R2, R3, F, true>;
+        int rc = set_smem(p, k, G::SMEM); if (rc) return rc;
+        GAL_CUDA(p, launch_chain(k, dim3(grid), dim3(G::NT), G::SMEM, st, rp));
+    } else {
+        auto k = row_pass_kernel<T, R1, R2, R3, F, false>;
+        int rc = set_smem(p, k, G::SMEM); if (rc) return rc;
+        GAL_CUDA(p, launch_chain(k, dim3(grid), dim3(G::NT), G::SMEM, st, rp));
+    }
+    p->launches++;
+    GAL_CUDA(p, cudaGetLastError());
+    if (p->t_split) GAL_CUDA(p, cudaEventRecord(p->t_split[2], st));
+    return GAL_OK;
+}
+
+template <typename T, int R1, int R2, int R3, int F>
+int launch_col(gal_plan* p, int batch, const int* ext, cudaStream_t st) {
+    using G = Geom<T, R1, R2, R3, F>;
+    ColParams<T> cp;
+    cp.work = (const cx<T>*)p->work;
+    cp.pair = (NodePair<T>*)p->spec;
+    cp.tw = (const cx<T>*)p->tw;
+    cp.N = p->nxy;
+    cp.cols_total = (long long)batch * (p->nxy / 2 + 1);
+    cp.ext = ext;
+    const unsigned grid = (unsigned)((cp.cols_total + F - 1) / F);
+    auto k = col_pass_kernel<T, R1, R2, R3, F>;
+    int rc = set_smem(p, k, G::SMEM); if (rc) return rc;
+    GAL_CUDA(p, launch_chain(k, dim3(grid), dim3(G::NT), G::SMEM, st, cp));
+    p->launches++;
+    GAL_CUDA(p, cudaGetLastError());
+    return GAL_OK;
+}
+
+template <typename T, int R1, int R2, int R3>
+int launch_col_x2(gal_plan* p, int batch, const int* ext, cudaStream_t st) {
+    using G = Geom<T, R1, R2, R3, 2>;
+    ColParams<T> cp;
+    cp.work = (const cx<T>*)p->work;
+    cp.pair = (NodePair<T>*)p->spec;
+    cp.tw = (const cx<T>*)p->tw;
+    cp.N = p->nxy;
+    cp.cols_total = (long long)batch * (p->nxy / 2 + 1);
+    cp.ext = ext;
+    auto k = col_pass_x2_kernel<T, R1, R2, R3>;
+    int rc = set_smem(p, k, G::SMEM); if (rc) return rc;
+    GAL_CUDA(p, launch_chain(k, dim3((unsigned)cp.cols_total), dim3(G::NT), G::SMEM, st, cp));
+    p->launches++;
+    GAL_CUDA(p, cudaGetLastError());
+    return GAL_OK;
+}
+
+// Radix plans.  Row FFT length is nxy/2, column FFT length is nxy.
+template <typename T>
+int fft2(gal_plan* p, const T* image, const SweepParams* sw, int batch, const int* ext, cudaStream_t st) {
+    int rc;
+    switch (p->nxy) {
+#define GAL_FFT_CASE(NXY, ROW, COL)                                         \
+    case NXY:                                                               \
+        rc = launch_row<T, ROW>(p, image, sw, batch, ext, st); if (rc) return rc; \
+        return launch_col<T, COL>(p, batch, ext, st);
+#define RR(...) __VA_ARGS__
+        GAL_FFT_CASE(8, RR(4, 1, 1, 8), RR(8, 1, 1, 8))
+        GAL_FFT_CASE(16, RR(8, 1, 1, 16), RR(16, 1, 1, 16))
+        GAL_FFT_CASE(32, RR(16, 1, 1, 16), RR(8, 4, 1, 16))
+        GAL_FFT_CASE(64, RR(8, 4, 1, 16), RR(8, 8, 1, 16))
+        GAL_FFT_CASE(128, RR(8, 8, 1, 16), RR(16, 8, 1, 16))
+        GAL_FFT_CASE(256, RR(16, 8, 1, 16), RR(16, 16, 1, 8))
+        GAL_FFT_CASE(512, RR(16, 16, 1, 8), RR(8, 8, 8, 4))
+        GAL_FFT_CASE(1024, RR(8, 8, 8, 4), RR(16, 8, 8, 4))
+        GAL_FFT_CASE(2048, RR(16, 8, 8, 4), RR(16, 16, 8, 2))
+        GAL_FFT_CASE(4096, RR(16, 16, 8, 2), RR(16, 16, 16, 1))
+        case 8192:      // column length 8192 = 2 x 4096: two interleaved transforms + one radix-2 combination
+            rc = launch_row<T, 16, 16, 16, 1>(p, image, sw, batch, ext, st); if (rc) return rc;
+            return launch_col_x2<T, 16, 16, 16>(p, batch, ext, st);
+#undef RR
+#undef GAL_FFT_CASE
+        default:
+            return GAL_ERR_UNSUPPORTED;
+    }
+}
+
+
+template <typename T>
+int launch_sweep(gal_plan* p, const SweepParams& sw, T* out, cudaStream_t st) {
+    const long long total = (long long)p->nxy * p->nxy;
+    long long blocks = (total + 255) / 256;
+    if (blocks > p->sm_count * 16) blocks = p->sm_count * 16;
+    sweep_kernel<T><<<(unsigned)blocks, 256, 0, st>>>(sw, p->nxy, out);
+    p->launches++;
+    GAL_CUDA(p, cudaGetLastError());
+    return GAL_OK;
+}
+
+template <typename T>
+int launch_transpose(gal_plan* p, T* out, cudaStream_t st) {
+    dim3 grid((p->nxy + 31) / 32, (p->nxy / 2 + 1 + 31) / 32), block(32, 8);
+    transpose_to_paper_layout_kernel<T><<<grid, block, 0, st>>>((const NodePair<T>*)p->spec, (cx<T>*)out, p->nxy);
+    p->launches++;
+    GAL_CUDA(p, cudaGetLastError());
+    return GAL_OK;
+}
+
+#define GAL_INSTANTIATE_FFT(T)                                                                             \
+    template int fft2<T>(gal_plan*, const T*, const SweepParams*, int, const int*, cudaStream_t);          \
+    template int launch_sweep<T>(gal_plan*, const SweepParams&, T*, cudaStream_t);                         \
+    template int launch_transpose<T>(gal_plan*, T*, cudaStream_t);
+
+}  // namespace galb

@@ -10,207 +10,17 @@
 #include <set>
 #include <vector>
 
-#include "fft.cuh"
-#include "sample.cuh"
+#include "plan.h"
 
 using namespace galb;
-
-struct gal_plan {
-    int nxy = 0, batch = 0, bits = 0, device = 0;
-    int sm_count = 148;
-    void* spec = nullptr;            // NodePair<T>[batch][nxy/2+1][nxy]: the sampled spectrum (column pairs)
-    void* work = nullptr;            // cx<T>[batch][nxy/2+1][nxy]: row-pass output
-    void* tw = nullptr;              // cx<T>[nxy]
-    double* partials = nullptr;      // [batch][max_gx]
-    unsigned int* tickets = nullptr; // [batch + 1]
-    unsigned long long* oob = nullptr;   // call_state[0]; the uv extent follows it
-    int* ext = nullptr;                  // {kumax, rmin, rmax} of the current call (device)
-    int* ext_full = nullptr;             // constant {nxy/2, 0, nxy-1}: no pruning
-    // Per-call device state [oob (8 B) | ext (12 B) | done ticket (4 B) | pad], two copies used alternately:
-    // the sampling kernel of call k re-arms the copy call k+1 will use, so no reset operation sits between
-    // two calls on the stream (an explicit copy from call_init is only needed when that did not happen).
-    void* call_state = nullptr;          // 2 x 32 B
-    void* call_init = nullptr;
-    int cur = 0;                         // copy used by the most recent call
-    bool next_armed = false;             // the other copy has been / will be re-armed by that call's sampler
-    int prune_mode = 1;                  // 0 never, 1 auto, 2 always
-    bool last_pruned = false;            // did the most recent call compute a uv extent?
-    // bound uv set (gal_plan_bind_uv): addresses, size, the rotation-invariant radius, and the extent derived
-    // from it for the pixel size seen last (device copy used by the FFT passes and checked by the sampler)
-    const void* b_u = nullptr; const void* b_v = nullptr;
-    int64_t b_M = 0; int b_C = 0;
-    double b_rmax = 0.0, b_dxy = 0.0;
-    int b_ext[3] = {0, 0, 0};
-    int* b_ext_dev = nullptr;            // [4]
-    unsigned long long* b_r2 = nullptr;  // [1] scratch of the radius kernel
-    bool last_bound = false;             // the most recent call used the bound extent
-    void* st_vis = nullptr; size_t st_vis_bytes = 0; // summed visibilities of a chi2 multi-source call
-    std::set<const void*> smem_set;      // kernels whose dynamic shared-memory limit has been raised
-    int max_gx = 0;
-    size_t owned_bytes = 0;
-    int last_cuda = 0;
-    int64_t launches = 0;
-    cudaStream_t last_stream = nullptr;
-    // staging for the _host_ entry points (grown on demand)
-    void* st_image = nullptr; size_t st_image_bytes = 0;
-    void* st_pts = nullptr;   size_t st_pts_bytes = 0;
-    void* st_out = nullptr;   size_t st_out_bytes = 0;
-    double* st_chi2 = nullptr;
-    // optional per-kernel timing (gal_plan_timing_enable): 5 events per call
-    std::vector<cudaEvent_t> tev;
-    int t_max_calls = 0, t_calls = 0;
-    cudaEvent_t* t_split = nullptr;  // when set, the row launcher records t_split[2] after its kernel
-};
 
 namespace {
 
 inline bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
 
-#define GAL_CUDA(plan, call)                                   \
-    do {                                                       \
-        cudaError_t e__ = (call);                              \
-        if (e__ != cudaSuccess) {                              \
-            (plan)->last_cuda = (int)e__;                      \
-            return e__ == cudaErrorMemoryAllocation ? GAL_ERR_ALLOC : GAL_ERR_CUDA; \
-        }                                                      \
-    } while (0)
-
-struct DeviceGuard {
-    int prev = -1;
-    explicit DeviceGuard(int dev) { cudaGetDevice(&prev); if (prev != dev) cudaSetDevice(dev); else prev = -1; }
-    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
-};
-
-template <typename K> int set_smem(gal_plan* p, K kernel, size_t bytes) {
-    if (bytes > 48 * 1024 && !p->smem_set.count((const void*)kernel)) {
-        GAL_CUDA(p, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
-        p->smem_set.insert((const void*)kernel);
-    }
-    return GAL_OK;
-}
-
-// Programmatic dependent launch: the kernels of one call form a chain on the stream; each is launched with
-// programmatic stream serialisation so that its CTAs are placed and run their prologue while the kernel before
-// drains, and each waits (`griddepcontrol.wait`, fft.cuh: pdl_wait) before it touches memory.
-template <typename... KArgs, typename... Args>
-cudaError_t launch_chain(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr; cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
-}
-
-// ---------------------------------------------------------------------------------------------
-// FFT launchers
-// ---------------------------------------------------------------------------------------------
-template <typename T, int R1, int R2, int R3, int F>
-int launch_row(gal_plan* p, const T* image, const SweepParams* sw, int batch, const int* ext, cudaStream_t st) {
-    using G = Geom<T, R1, R2, R3, F>;
-    RowParams<T> rp;
-    rp.image = image;
-    rp.spec = (cx<T>*)p->work;
-    rp.tw = (const cx<T>*)p->tw;
-    rp.N = p->nxy;
-    rp.rows_total = batch * p->nxy;
-    rp.ext = ext;
-    if (sw) rp.sweep = *sw; else memset(&rp.sweep, 0, sizeof(rp.sweep));
-    const unsigned grid = (unsigned)((rp.rows_total + F - 1) / F);
-    if (sw) {
-        auto k = row_pass_kernel<T, R1, R2, R3, F, true>;
-        int rc = set_smem(p, k, G::SMEM); if (rc) return rc;
-        GAL_CUDA(p, launch_chain(k, dim3(grid), dim3(G::NT), G::SMEM, st, rp));
-    } else {
-        auto k = row_pass_kernel<T, R1, R2, R3, F, false>;
-        int rc = set_smem(p, k, G::SMEM); if (rc) return rc;
-        GAL_CUDA(p, launch_chain(k, dim3(grid), dim3(G::NT), G::SMEM, st, rp));
-    }
-    p->launches++;
-    GAL_CUDA(p, cudaGetLastError());
-    if (p->t_split) GAL_CUDA(p, cudaEventRecord(p->t_split[2], st));
-    return GAL_OK;
-}
-
-template <typename T, int R1, int R2, int R3, int F>
-int launch_col(gal_plan* p, int batch, const int* ext, cudaStream_t st) {
-    using G = Geom<T, R1, R2, R3, F>;
-    ColParams<T> cp;
-    cp.work = (const cx<T>*)p->work;
-    cp.pair = (NodePair<T>*)p->spec;
-    cp.tw = (const cx<T>*)p->tw;
-    cp.N = p->nxy;
-    cp.cols_total = (long long)batch * (p->nxy / 2 + 1);
-    cp.ext = ext;
-    const unsigned grid = (unsigned)((cp.cols_total + F - 1) / F);
-    auto k = col_pass_kernel<T, R1, R2, R3, F>;
-    int rc = set_smem(p, k, G::SMEM); if (rc) return rc;
-    GAL_CUDA(p, launch_chain(k, dim3(grid), dim3(G::NT), G::SMEM, st, cp));
-    p->launches++;
-    GAL_CUDA(p, cudaGetLastError());
-    return GAL_OK;
-}
-
-template <typename T, int R1, int R2, int R3>
-int launch_col_x2(gal_plan* p, int batch, const int* ext, cudaStream_t st) {
-    using G = Geom<T, R1, R2, R3, 2>;
-    ColParams<T> cp;
-    cp.work = (const cx<T>*)p->work;
-    cp.pair = (NodePair<T>*)p->spec;
-    cp.tw = (const cx<T>*)p->tw;
-    cp.N = p->nxy;
-    cp.cols_total = (long long)batch * (p->nxy / 2 + 1);
-    cp.ext = ext;
-    auto k = col_pass_x2_kernel<T, R1, R2, R3>;
-    int rc = set_smem(p, k, G::SMEM); if (rc) return rc;
-    GAL_CUDA(p, launch_chain(k, dim3((unsigned)cp.cols_total), dim3(G::NT), G::SMEM, st, cp));
-    p->launches++;
-    GAL_CUDA(p, cudaGetLastError());
-    return GAL_OK;
-}
-
-// Radix plans.  Row FFT length is nxy/2, column FFT length is nxy.
-template <typename T>
-int fft2(gal_plan* p, const T* image, const SweepParams* sw, int batch, const int* ext, cudaStream_t st) {
-    int rc;
-    switch (p->nxy) {
-#define GAL_FFT_CASE(NXY, ROW, COL)                                         \
-    case NXY:                                                               \
-        rc = launch_row<T, ROW>(p, image, sw, batch, ext, st); if (rc) return rc; \
-        return launch_col<T, COL>(p, batch, ext, st);
-#define RR(...) __VA_ARGS__
-        GAL_FFT_CASE(8, RR(4, 1, 1, 8), RR(8, 1, 1, 8))
-        GAL_FFT_CASE(16, RR(8, 1, 1, 16), RR(16, 1, 1, 16))
-        GAL_FFT_CASE(32, RR(16, 1, 1, 16), RR(8, 4, 1, 16))
-        GAL_FFT_CASE(64, RR(8, 4, 1, 16), RR(8, 8, 1, 16))
-        GAL_FFT_CASE(128, RR(8, 8, 1, 16), RR(16, 8, 1, 16))
-        GAL_FFT_CASE(256, RR(16, 8, 1, 16), RR(16, 16, 1, 8))
-        GAL_FFT_CASE(512, RR(16, 16, 1, 8), RR(8, 8, 8, 4))
-        GAL_FFT_CASE(1024, RR(8, 8, 8, 4), RR(16, 8, 8, 4))
-        GAL_FFT_CASE(2048, RR(16, 8, 8, 4), RR(16, 16, 8, 2))
-        GAL_FFT_CASE(4096, RR(16, 16, 8, 2), RR(16, 16, 16, 1))
-        case 8192:      // column length 8192 = 2 x 4096: two interleaved transforms + one radix-2 combination
-            rc = launch_row<T, 16, 16, 16, 1>(p, image, sw, batch, ext, st); if (rc) return rc;
-            return launch_col_x2<T, 16, 16, 16>(p, batch, ext, st);
-#undef RR
-#undef GAL_FFT_CASE
-        default:
-            return GAL_ERR_UNSUPPORTED;
-    }
-}
-
 // ---------------------------------------------------------------------------------------------
 // per-call scalars, uv extent, sampling launcher
 // ---------------------------------------------------------------------------------------------
-struct CallScalars {
-    IndexScalars ix;
-    double dRA_turns, dDec_turns;
-    int has_phase;
-    double amp = 1.0;      // factor on the visibilities and accumulate-into-vis flag: multi-source composition only
-    int accumulate = 0;
-};
-
 // host-side scalars, plain double arithmetic in the listing's order.  The
 // phase offsets are kept in turns (the listing's 2 pi factor is applied inside sincospi, exactly).
 CallScalars call_scalars(const gal_plan* p, double dxy, double dRA, double dDec, double PA) {
@@ -253,88 +63,6 @@ bool want_prune(const gal_plan* p, int C, int64_t M) {
     const double ext_bytes = 2.0 * sizeof(T) * (double)M * C;
     const double spec_bytes = 2.0 * sizeof(T) * (double)(p->nxy / 2 + 1) * p->nxy * C;
     return ext_bytes <= 0.25 * 3.0 * spec_bytes;
-}
-
-template <typename T>
-int launch_extent(gal_plan* p, int C, const CallScalars& cs, const T* u, const T* v, int64_t M, cudaStream_t st) {
-    ExtentParams ep;
-    ep.N = p->nxy;
-    ep.total = (long long)C * M;
-    ep.ix = cs.ix;
-    ep.ext = p->ext;
-    long long blocks = (ep.total + 1023) / 1024;
-    const long long cap = (long long)p->sm_count * 4;
-    if (blocks > cap) blocks = cap;
-    if (blocks < 1) blocks = 1;
-    GAL_CUDA(p, launch_chain(uv_extent_kernel<T>, dim3((unsigned)blocks), dim3(256), 0, st, ep, u, v));
-    p->launches++;
-    GAL_CUDA(p, cudaGetLastError());
-    return GAL_OK;
-}
-
-inline bool aligned16(const void* q) { return ((uintptr_t)q & 15u) == 0; }
-
-template <typename T, bool WRITE_VIS, bool DO_CHI2>
-int launch_sample_kernel(gal_plan* p, const SampleParams<T>& sp, dim3 grid, bool tma, cudaStream_t st) {
-    using G = SampleGeom<T, DO_CHI2>;
-    if (tma) {
-        auto k = sample_kernel_tma<T, WRITE_VIS, DO_CHI2>;
-        int rc = set_smem(p, k, G::SMEM); if (rc) return rc;
-        GAL_CUDA(p, launch_chain(k, grid, dim3(G::NT_TMA), G::SMEM, st, sp));
-    } else {
-        GAL_CUDA(p, launch_chain(sample_kernel_plain<T, WRITE_VIS, DO_CHI2>, grid, dim3(G::NT), 0, st, sp));
-    }
-    return GAL_OK;
-}
-
-template <typename T>
-int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T* v, const T* re, const T* im,
-                  const T* w, int64_t M, T* vis, double* chi2_pc, double* chi2_tot, cudaStream_t st) {
-    const bool do_chi2 = (vis == nullptr);
-    if (M == 0) {
-        if (chi2_pc) GAL_CUDA(p, cudaMemsetAsync(chi2_pc, 0, sizeof(double) * C, st));
-        if (chi2_tot) GAL_CUDA(p, cudaMemsetAsync(chi2_tot, 0, sizeof(double), st));
-        return GAL_OK;
-    }
-    SampleParams<T> sp;
-    sp.spec = (const NodePair<T>*)p->spec;
-    sp.N = p->nxy;
-    sp.M = M;
-    sp.u = u; sp.v = v; sp.re_obs = re; sp.im_obs = im; sp.w = w; sp.vis = vis;
-    sp.ix = cs.ix;
-    sp.amp = cs.amp; sp.accumulate = cs.accumulate;
-    sp.dRA_turns = cs.dRA_turns; sp.dDec_turns = cs.dDec_turns; sp.has_phase = cs.has_phase;
-    sp.partials = p->partials;
-    sp.tickets = p->tickets;
-    sp.chi2_per_channel = chi2_pc;
-    sp.chi2_total = chi2_tot;
-    sp.oob = p->oob;
-    sp.done = (unsigned int*)((char*)p->oob + 20);
-    sp.next_state = (unsigned long long*)((char*)p->call_state + 32 * (p->cur ^ 1));
-    sp.viol = (unsigned long long*)((char*)p->oob + 24);
-    sp.ext_check = (p->last_bound && p->b_ext[0] < p->nxy / 2) ? p->b_ext_dev : nullptr;
-    // one CTA works through tiles blockIdx.x, blockIdx.x + gridDim.x, ...: a whole number of CTAs per SM
-    const int tile = SampleGeom<T, true>::TILE;
-    const long long ntiles = (M + tile - 1) / tile;
-    long long cap = (long long)p->sm_count * GAL_SAMPLE_MINB;
-    // batched: CTAs are placed channel by channel (blockIdx.x fastest); an eighth of the resident CTAs per
-    // channel keeps about eight channels' spectra (not dozens) competing for the L2 at any time and gives every
-    // CTA enough tiles to amortise its prologue and reduction (measured at cfg 4: 2: 573, 4: 481, 8: 420 us)
-    if (C > 1) cap = (cap + 7) / 8;
-    if (cap > p->max_gx) cap = p->max_gx;
-    long long gx = ntiles < cap ? ntiles : cap;
-    if (gx < 1) gx = 1;
-    dim3 grid((unsigned)gx, (unsigned)C);
-    // the TMA path needs 16-byte aligned tiles in every channel (and a du fit for the division shortcut)
-    bool tma = !cs.ix.du_exact_div && aligned16(u) && aligned16(v) && (C == 1 || ((size_t)M * sizeof(T)) % 16 == 0);
-    if (do_chi2) tma = tma && aligned16(re) && aligned16(im) && aligned16(w);
-    int rc = do_chi2 ? launch_sample_kernel<T, false, true>(p, sp, grid, tma, st)
-                     : launch_sample_kernel<T, true, false>(p, sp, grid, tma, st);
-    if (rc) return rc;
-    p->launches++;
-    GAL_CUDA(p, cudaGetLastError());
-    p->next_armed = true;                 // the last CTA of this launch re-arms the other copy of the call state
-    return GAL_OK;
 }
 
 // One whole call: [uv extent] -> row pass -> column pass -> sampling, with (diagnostic mode,
@@ -434,13 +162,7 @@ int do_sweep(gal_plan* p, const T* I, int nr, double Rmin, double dR, double dxy
     DeviceGuard g(p->device);
     cudaStream_t st = (cudaStream_t)stream;
     p->last_stream = st;
-    const long long total = (long long)p->nxy * p->nxy;
-    long long blocks = (total + 255) / 256;
-    if (blocks > p->sm_count * 16) blocks = p->sm_count * 16;
-    sweep_kernel<T><<<(unsigned)blocks, 256, 0, st>>>(sw, p->nxy, out);
-    p->launches++;
-    GAL_CUDA(p, cudaGetLastError());
-    return GAL_OK;
+    return launch_sweep<T>(p, sw, out, st);
 }
 
 template <typename T>
@@ -451,11 +173,7 @@ int do_fft2_shifted(gal_plan* p, const T* image, T* out, void* stream) {
     p->last_stream = st;
     int rc = fft2<T>(p, image, nullptr, 1, p->ext_full, st);
     if (rc) return rc;
-    dim3 grid((p->nxy + 31) / 32, (p->nxy / 2 + 1 + 31) / 32), block(32, 8);
-    transpose_to_paper_layout_kernel<T><<<grid, block, 0, st>>>((const NodePair<T>*)p->spec, (cx<T>*)out, p->nxy);
-    p->launches++;
-    GAL_CUDA(p, cudaGetLastError());
-    return GAL_OK;
+    return launch_transpose<T>(p, out, st);
 }
 
 int grow(gal_plan* p, void** buf, size_t* have, size_t want) {
@@ -510,19 +228,7 @@ int do_multi(gal_plan* p, const T* image, double dxy, const T* u, const T* v, co
         cs[s].accumulate = s > 0;
         if ((rc = launch_sample<T>(p, 1, cs[s], u, v, nullptr, nullptr, nullptr, M, target, nullptr, nullptr, st))) return rc;
     }
-    if (!vis) {
-        SampleParams<T> sp = {};
-        sp.N = p->nxy; sp.M = M; sp.vis = target; sp.re_obs = re; sp.im_obs = im; sp.w = w;
-        sp.partials = p->partials; sp.tickets = p->tickets; sp.chi2_per_channel = chi2; sp.chi2_total = nullptr;
-        sp.oob = p->oob; sp.done = (unsigned int*)((char*)p->oob + 20);
-        sp.next_state = (unsigned long long*)((char*)p->call_state + 32 * (p->cur ^ 1));
-        sp.viol = (unsigned long long*)((char*)p->oob + 24); sp.ext_check = nullptr;
-        long long blocks = (M + 1023) / 1024;
-        if (blocks > p->max_gx) blocks = p->max_gx;
-        GAL_CUDA(p, launch_chain(chi2_from_vis_kernel<T>, dim3((unsigned)blocks), dim3(256), 0, st, sp));
-        p->launches++;
-        GAL_CUDA(p, cudaGetLastError());
-    }
+    if (!vis) return launch_chi2_from_vis<T>(p, target, re, im, w, M, chi2, st);
     return GAL_OK;
 }
 
@@ -578,12 +284,7 @@ int do_bind_uv(gal_plan* p, const T* u, const T* v, int64_t M, int C, void* stre
     cudaStream_t st = (cudaStream_t)stream;
     gal_plan_unbind_uv(p);
     GAL_CUDA(p, cudaMemsetAsync(p->b_r2, 0, 8, st));
-    const long long total = (long long)C * M;
-    long long blocks = (total + 1023) / 1024;
-    if (blocks > (long long)p->sm_count * 8) blocks = (long long)p->sm_count * 8;
-    uv_radius_kernel<T><<<(unsigned)blocks, 256, 0, st>>>(u, v, total, p->b_r2);
-    p->launches++;
-    GAL_CUDA(p, cudaGetLastError());
+    { int rc = launch_uv_radius<T>(p, u, v, (long long)C * M, st); if (rc) return rc; }
     unsigned long long bits = 0;
     GAL_CUDA(p, cudaMemcpyAsync(&bits, p->b_r2, 8, cudaMemcpyDeviceToHost, st));
     GAL_CUDA(p, cudaStreamSynchronize(st));

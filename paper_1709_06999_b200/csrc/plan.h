@@ -1,0 +1,111 @@
+// plan.h — the plan object and the launcher interface between the C ABI (galario_b200.cu) and the per-precision
+// kernel translation units (fft_f64.cu, fft_f32.cu, sample_f64.cu, sample_f32.cu).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <set>
+#include <vector>
+
+#include "../../include/galario_b200.h"
+#include "types.h"
+
+struct gal_plan {
+    int nxy = 0, batch = 0, bits = 0, device = 0;
+    int sm_count = 148;
+    void* spec = nullptr;            // NodePair<T>[batch][nxy/2+1][nxy]: the sampled spectrum (column pairs)
+    void* work = nullptr;            // cx<T>[batch][nxy/2+1][nxy]: row-pass output
+    void* tw = nullptr;              // cx<T>[nxy]
+    double* partials = nullptr;      // [batch][max_gx]
+    unsigned int* tickets = nullptr; // [batch + 1]
+    unsigned long long* oob = nullptr;   // call_state[0]; the uv extent follows it
+    int* ext = nullptr;                  // {kumax, rmin, rmax} of the current call (device)
+    int* ext_full = nullptr;             // constant {nxy/2, 0, nxy-1}: no pruning
+    // Per-call device state [oob (8 B) | ext (12 B) | done ticket (4 B) | pad], two copies used alternately:
+    // the sampling kernel of call k re-arms the copy call k+1 will use, so no reset operation sits between
+    // two calls on the stream (an explicit copy from call_init is only needed when that did not happen).
+    void* call_state = nullptr;          // 2 x 32 B
+    void* call_init = nullptr;
+    int cur = 0;                         // copy used by the most recent call
+    bool next_armed = false;             // the other copy has been / will be re-armed by that call's sampler
+    int prune_mode = 1;                  // 0 never, 1 auto, 2 always
+    bool last_pruned = false;            // did the most recent call compute a uv extent?
+    // bound uv set (gal_plan_bind_uv): addresses, size, the rotation-invariant radius, and the extent derived
+    // from it for the pixel size seen last (device copy used by the FFT passes and checked by the sampler)
+    const void* b_u = nullptr; const void* b_v = nullptr;
+    int64_t b_M = 0; int b_C = 0;
+    double b_rmax = 0.0, b_dxy = 0.0;
+    int b_ext[3] = {0, 0, 0};
+    int* b_ext_dev = nullptr;            // [4]
+    unsigned long long* b_r2 = nullptr;  // [1] scratch of the radius kernel
+    bool last_bound = false;             // the most recent call used the bound extent
+    void* st_vis = nullptr; size_t st_vis_bytes = 0; // summed visibilities of a chi2 multi-source call
+    std::set<const void*> smem_set;      // kernels whose dynamic shared-memory limit has been raised
+    int max_gx = 0;
+    size_t owned_bytes = 0;
+    int last_cuda = 0;
+    int64_t launches = 0;
+    cudaStream_t last_stream = nullptr;
+    // staging for the _host_ entry points (grown on demand)
+    void* st_image = nullptr; size_t st_image_bytes = 0;
+    void* st_pts = nullptr;   size_t st_pts_bytes = 0;
+    void* st_out = nullptr;   size_t st_out_bytes = 0;
+    double* st_chi2 = nullptr;
+    // optional per-kernel timing (gal_plan_timing_enable): 5 events per call
+    std::vector<cudaEvent_t> tev;
+    int t_max_calls = 0, t_calls = 0;
+    cudaEvent_t* t_split = nullptr;  // when set, the row launcher records t_split[2] after its kernel
+};
+
+namespace galb {
+
+#define GAL_CUDA(plan, call)                                   \
+    do {                                                       \
+        cudaError_t e__ = (call);                              \
+        if (e__ != cudaSuccess) {                              \
+            (plan)->last_cuda = (int)e__;                      \
+            return e__ == cudaErrorMemoryAllocation ? GAL_ERR_ALLOC : GAL_ERR_CUDA; \
+        }                                                      \
+    } while (0)
+
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(int dev) { cudaGetDevice(&prev); if (prev != dev) cudaSetDevice(dev); else prev = -1; }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+template <typename K> inline int set_smem(gal_plan* p, K kernel, size_t bytes) {
+    if (bytes > 48 * 1024 && !p->smem_set.count((const void*)kernel)) {
+        GAL_CUDA(p, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+        p->smem_set.insert((const void*)kernel);
+    }
+    return GAL_OK;
+}
+
+// Programmatic dependent launch: the kernels of one call form a chain on the stream; each is launched with
+// programmatic stream serialisation so that its CTAs are placed and run their prologue while the kernel before
+// drains, and each waits (`griddepcontrol.wait`, fft.cuh: pdl_wait) before it touches memory.
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_chain(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
+// ---- launchers, one explicit instantiation per precision (T = double in *_f64.cu, float in *_f32.cu) ----
+// row pass + column pass of `batch` images (or of the swept profile) pruned to the device-resident extent `ext`
+template <typename T> int fft2(gal_plan* p, const T* image, const SweepParams* sw, int batch, const int* ext, cudaStream_t st);
+template <typename T> int launch_sweep(gal_plan* p, const SweepParams& sw, T* out, cudaStream_t st);
+template <typename T> int launch_transpose(gal_plan* p, T* out, cudaStream_t st);
+template <typename T> int launch_extent(gal_plan* p, int C, const CallScalars& cs, const T* u, const T* v, int64_t M, cudaStream_t st);
+template <typename T> int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T* v, const T* re, const T* im,
+                                        const T* w, int64_t M, T* vis, double* chi2_pc, double* chi2_tot, cudaStream_t st);
+template <typename T> int launch_chi2_from_vis(gal_plan* p, const T* vis, const T* re, const T* im, const T* w, int64_t M,
+                                               double* chi2, cudaStream_t st);
+template <typename T> int launch_uv_radius(gal_plan* p, const T* u, const T* v, long long total, cudaStream_t st);
+
+}  // namespace galb

@@ -18,18 +18,9 @@
 //     that gather is bounded by the L2 -> SM path and by the L1's one line per clock, so it is
 //     shaped to move the fewest sectors and lines, and everything else overlaps with it.
 #pragma once
-#include "fft.cuh"
+#include "common.cuh"
 
 namespace galb {
-
-// Scalars of one call that the index arithmetic needs (host-computed).  They sit
-// in the kernel parameter block so the compiler reads them as constant-bank operands, not registers.
-struct IndexScalars {
-    double du, rdu;        // du = 1/(N dxy); rdu = RN(1/du) for the exact-division shortcut
-    double cos_PA, sin_PA;
-    double fH, fHm1, fN1;  // N/2, N/2 - 1, N - 1 as doubles
-    int du_exact_div;      // 1: rdu is not usable, take a true division
-};
 
 template <typename T> struct SampleParams {
     const NodePair<T>* spec;   // [C][N/2+1][N] column pairs (fft.cuh)
@@ -96,7 +87,7 @@ __device__ __forceinline__ bool cell_inside(const IndexScalars& s, const PointIn
 // The constants of both routines live in constant memory so that each FP64 instruction reads its constant
 // as a constant-bank operand; as literals they cost two uniform-register moves apiece, per point.
 // [0..5] sine, [6..11] cosine kernel coefficients (fdlibm), then 1.5 * 2^52, pi / 2, 2^52.
-__constant__ double SINCOS_COEF[16] = {
+static __constant__ double SINCOS_COEF[16] = {
     1.58969099521155010221e-10, -2.50507602534068634195e-08, 2.75573137070700676789e-06,
     -1.98412698298579493134e-04, 8.33333333332248946124e-03, -1.66666666666666324348e-01,
     -1.13596475577881948265e-11, 2.08757232129817482790e-09, -2.75573143513906633035e-07,
@@ -285,51 +276,6 @@ __global__ void __launch_bounds__(256, 4) uv_extent_kernel(const ExtentParams p,
         atomicMin(p.ext + 1, rmin);
         atomicMax(p.ext + 2, rmax);
     }
-}
-
-// ------------------------------------------------------------------------------------------
-// mbarrier + TMA bulk-copy wrappers (PTX, sm_90+/sm_100a).
-// ------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint32_t mb, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(mb), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
-__device__ __forceinline__ void mbar_expect_tx(uint32_t mb, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mb), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t mb, uint32_t parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(mb), "r"(parity) : "memory");
-}
-// same, for a thread that expects to wait long (the producer): sleep between polls so the spin does not
-// take issue slots from the warps that share its scheduler
-__device__ __forceinline__ void mbar_wait_relaxed(uint32_t mb, uint32_t parity) {
-    uint32_t done = 0;
-    for (;;) {
-        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
-                     : "=r"(done) : "r"(mb), "r"(parity) : "memory");
-        if (done) break;
-        __nanosleep(200);
-    }
-}
-__device__ __forceinline__ uint64_t l2_policy_evict_first() {
-    uint64_t pol;
-    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
-    return pol;
-}
-// global -> shared bulk copy (TMA, 1-D): 16-byte aligned addresses, size a multiple of 16 bytes.
-__device__ __forceinline__ void tma_load_1d(uint32_t dst, const void* src, uint32_t bytes, uint32_t mb, uint64_t pol) {
-    asm volatile(
-        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
-        ::"r"(dst), "l"(src), "r"(bytes), "r"(mb), "l"(pol) : "memory");
 }
 
 // Points per thread and tile (U), stages of the shared-memory ring, resident CTAs per SM the register
@@ -602,10 +548,6 @@ __global__ void __launch_bounds__(256, GAL_SAMPLE_MINB) sample_kernel_plain(cons
     for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x)
         sample_tile_plain<T, WRITE_VIS, DO_CHI2, true>(p, cx_, tile, M, c);
     sample_finish<T, DO_CHI2>(p, c, cx_.acc, cx_.oob, cx_.viol);
-}
-
-__device__ __forceinline__ void mbar_arrive(uint32_t mb) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(mb) : "memory");
 }
 
 // Fast kernel (256 consumer threads + one producer warp): every per-point array 16-byte aligned in every

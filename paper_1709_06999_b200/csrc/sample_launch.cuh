@@ -1,0 +1,125 @@
+// sample_launch.cuh — launch geometry of the per-point kernels; included by sample_f64.cu / sample_f32.cu.
+#pragma once
+#include "plan.h"
+#include "sample.cuh"
+
+namespace galb {
+
+template <typename T>
+int launch_extent(gal_plan* p, int C, const CallScalars& cs, const T* u, const T* v, int64_t M, cudaStream_t st) {
+    ExtentParams ep;
+    ep.N = p->nxy;
+    ep.total = (long long)C * M;
+    ep.ix = cs.ix;
+    ep.ext = p->ext;
+    long long blocks = (ep.total + 1023) / 1024;
+    const long long cap = (long long)p->sm_count * 4;
+    if (blocks > cap) blocks = cap;
+    if (blocks < 1) blocks = 1;
+    GAL_CUDA(p, launch_chain(uv_extent_kernel<T>, dim3((unsigned)blocks), dim3(256), 0, st, ep, u, v));
+    p->launches++;
+    GAL_CUDA(p, cudaGetLastError());
+    return GAL_OK;
+}
+
+inline bool aligned16(const void* q) { return ((uintptr_t)q & 15u) == 0; }
+
+template <typename T, bool WRITE_VIS, bool DO_CHI2>
+int launch_sample_kernel(gal_plan* p, const SampleParams<T>& sp, dim3 grid, bool tma, cudaStream_t st) {
+    using G = SampleGeom<T, DO_CHI2>;
+    if (tma) {
+        auto k = sample_kernel_tma<T, WRITE_VIS, DO_CHI2>;
+        int rc = set_smem(p, k, G::SMEM); if (rc) return rc;
+        GAL_CUDA(p, launch_chain(k, grid, dim3(G::NT_TMA), G::SMEM, st, sp));
+    } else {
+        GAL_CUDA(p, launch_chain(sample_kernel_plain<T, WRITE_VIS, DO_CHI2>, grid, dim3(G::NT), 0, st, sp));
+    }
+    return GAL_OK;
+}
+
+template <typename T>
+int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T* v, const T* re, const T* im,
+                  const T* w, int64_t M, T* vis, double* chi2_pc, double* chi2_tot, cudaStream_t st) {
+    const bool do_chi2 = (vis == nullptr);
+    if (M == 0) {
+        if (chi2_pc) GAL_CUDA(p, cudaMemsetAsync(chi2_pc, 0, sizeof(double) * C, st));
+        if (chi2_tot) GAL_CUDA(p, cudaMemsetAsync(chi2_tot, 0, sizeof(double), st));
+        return GAL_OK;
+    }
+    SampleParams<T> sp;
+    sp.spec = (const NodePair<T>*)p->spec;
+    sp.N = p->nxy;
+    sp.M = M;
+    sp.u = u; sp.v = v; sp.re_obs = re; sp.im_obs = im; sp.w = w; sp.vis = vis;
+    sp.ix = cs.ix;
+    sp.amp = cs.amp; sp.accumulate = cs.accumulate;
+    sp.dRA_turns = cs.dRA_turns; sp.dDec_turns = cs.dDec_turns; sp.has_phase = cs.has_phase;
+    sp.partials = p->partials;
+    sp.tickets = p->tickets;
+    sp.chi2_per_channel = chi2_pc;
+    sp.chi2_total = chi2_tot;
+    sp.oob = p->oob;
+    sp.done = (unsigned int*)((char*)p->oob + 20);
+    sp.next_state = (unsigned long long*)((char*)p->call_state + 32 * (p->cur ^ 1));
+    sp.viol = (unsigned long long*)((char*)p->oob + 24);
+    sp.ext_check = (p->last_bound && p->b_ext[0] < p->nxy / 2) ? p->b_ext_dev : nullptr;
+    // one CTA works through tiles blockIdx.x, blockIdx.x + gridDim.x, ...: a whole number of CTAs per SM
+    const int tile = SampleGeom<T, true>::TILE;
+    const long long ntiles = (M + tile - 1) / tile;
+    long long cap = (long long)p->sm_count * GAL_SAMPLE_MINB;
+    // batched: CTAs are placed channel by channel (blockIdx.x fastest); an eighth of the resident CTAs per
+    // channel keeps about eight channels' spectra (not dozens) competing for the L2 at any time and gives every
+    // CTA enough tiles to amortise its prologue and reduction (measured at cfg 4: 2: 573, 4: 481, 8: 420 us)
+    if (C > 1) cap = (cap + 7) / 8;
+    if (cap > p->max_gx) cap = p->max_gx;
+    long long gx = ntiles < cap ? ntiles : cap;
+    if (gx < 1) gx = 1;
+    dim3 grid((unsigned)gx, (unsigned)C);
+    // the TMA path needs 16-byte aligned tiles in every channel (and a du fit for the division shortcut)
+    bool tma = !cs.ix.du_exact_div && aligned16(u) && aligned16(v) && (C == 1 || ((size_t)M * sizeof(T)) % 16 == 0);
+    if (do_chi2) tma = tma && aligned16(re) && aligned16(im) && aligned16(w);
+    int rc = do_chi2 ? launch_sample_kernel<T, false, true>(p, sp, grid, tma, st)
+                     : launch_sample_kernel<T, true, false>(p, sp, grid, tma, st);
+    if (rc) return rc;
+    p->launches++;
+    GAL_CUDA(p, cudaGetLastError());
+    p->next_armed = true;                 // the last CTA of this launch re-arms the other copy of the call state
+    return GAL_OK;
+}
+
+template <typename T>
+int launch_chi2_from_vis(gal_plan* p, const T* vis, const T* re, const T* im, const T* w, int64_t M, double* chi2,
+                         cudaStream_t st) {
+    SampleParams<T> sp = {};
+    sp.N = p->nxy; sp.M = M; sp.vis = const_cast<T*>(vis); sp.re_obs = re; sp.im_obs = im; sp.w = w;
+    sp.partials = p->partials; sp.tickets = p->tickets; sp.chi2_per_channel = chi2; sp.chi2_total = nullptr;
+    sp.oob = p->oob; sp.done = (unsigned int*)((char*)p->oob + 20);
+    sp.next_state = (unsigned long long*)((char*)p->call_state + 32 * (p->cur ^ 1));
+    sp.viol = (unsigned long long*)((char*)p->oob + 24); sp.ext_check = nullptr;
+    long long blocks = (M + 1023) / 1024;
+    if (blocks > p->max_gx) blocks = p->max_gx;
+    GAL_CUDA(p, launch_chain(chi2_from_vis_kernel<T>, dim3((unsigned)blocks), dim3(256), 0, st, sp));
+    p->launches++;
+    GAL_CUDA(p, cudaGetLastError());
+    return GAL_OK;
+}
+
+template <typename T>
+int launch_uv_radius(gal_plan* p, const T* u, const T* v, long long total, cudaStream_t st) {
+    long long blocks = (total + 1023) / 1024;
+    if (blocks > (long long)p->sm_count * 8) blocks = (long long)p->sm_count * 8;
+    uv_radius_kernel<T><<<(unsigned)blocks, 256, 0, st>>>(u, v, total, p->b_r2);
+    p->launches++;
+    GAL_CUDA(p, cudaGetLastError());
+    return GAL_OK;
+}
+
+#define GAL_INSTANTIATE_SAMPLE(T)                                                                                      \
+    template int launch_extent<T>(gal_plan*, int, const CallScalars&, const T*, const T*, int64_t, cudaStream_t);      \
+    template int launch_sample<T>(gal_plan*, int, const CallScalars&, const T*, const T*, const T*, const T*, const T*, \
+                                  int64_t, T*, double*, double*, cudaStream_t);                                        \
+    template int launch_chi2_from_vis<T>(gal_plan*, const T*, const T*, const T*, const T*, int64_t, double*,          \
+                                         cudaStream_t);                                                                \
+    template int launch_uv_radius<T>(gal_plan*, const T*, const T*, long long, cudaStream_t);
+
+}  // namespace galb
