@@ -33,29 +33,32 @@ METRIC = "chi2Image evals/s at nxy=4096,M=5e6 fp64"
 UNIT = "evals/s"
 
 
-def algorithmic_bytes(nxy: int, M: int, esz: int, entry: str = "chi2Image", extent=None):
-    """what the method must move, per kernel and per step (bytes).
+def algorithmic_bytes(nxy: int, M: int, esz: int, entry: str = "chi2Image", extent=None, C: int = 1):
+    """what the METHOD must move, per kernel and per step (bytes).
 
-    extent = None: the two-pass transform of the whole half plane (the table of §8(d); `step` is the
-    figure the 60 % target is read against).  extent = (kumax, kvs_min, kvs_max): what the kernels of a
-    pruned call have to move — only columns 0..kumax are written by the row pass and transformed by the
-    column pass, only rows kvs_min..kvs_max are written back — plus the extra read of u, v by the
-    uv-extent kernel."""
-    img = nxy * nxy * esz
+    extent = None: the two-pass transform of the whole half plane (the table of §8(d)).
+    extent = (kumax, kvs_min, kvs_max): the method's bytes of a transform pruned to that part of the half plane —
+    the image is read once, only columns 0..kumax of the row-transformed image are written and read back, only
+    rows kvs_min..kvs_max of those columns are written as the spectrum (once).  What this implementation moves on
+    top of that (the uv-extent kernel re-reads u and v; the column-pair layout stores every value twice) is NOT
+    counted: it lowers the achieved fraction instead.  *Profile entries read no image (the sweep is evaluated in
+    the row-pass loader); sample* entries stream u, v in and V out (4 reals per point), chi2* five reals in."""
+    img = 0 if "Profile" in entry else nxy * nxy * esz
     per_point = 5 * esz if entry.startswith("chi2") else 4 * esz
-    samp = per_point * M               # u, v, re, im, w in (or u, v in + V out)
+    samp = per_point * M
     if extent is None:
         spec = nxy * (nxy // 2 + 1) * 2 * esz
         row = img + spec               # read image, write half-spectrum
         col = 2 * spec                 # read + write half-spectrum
-        ext = 0
     else:
         kumax, rmin, rmax = extent
         cols = kumax + 1
         row = img + cols * nxy * 2 * esz
-        col = cols * nxy * 2 * esz + cols * (rmax - rmin + 1) * 4 * esz   # column pairs: every value written twice
-        ext = 2 * esz * M
-    return {"uv_extent": ext, "row_pass": row, "col_pass": col, "sample": samp, "step": ext + row + col + samp}
+        col = cols * nxy * 2 * esz + cols * (rmax - rmin + 1) * 2 * esz
+    out = {"uv_extent": 0, "row_pass": row, "col_pass": col, "sample": samp}
+    out = {k: C * v for k, v in out.items()}
+    out["step"] = sum(out.values())
+    return out
 
 
 def measured_peaks():
@@ -193,6 +196,116 @@ def run_reference(args, rank: int):
         "gpu_launches": 0}))
 
 
+def event_time_ms(fn, steps: int, torch) -> float:
+    """`steps` back-to-back calls between two CUDA events on the current stream (synchronised on both sides)."""
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / steps
+
+
+def kernel_times_ms(plan, fn, steps: int, torch):
+    """Per-kernel durations of `fn`'s calls, live: CUDA events recorded by the plan between its kernels."""
+    plan.timing_enable(steps)
+    for _ in range(steps):
+        fn()
+    torch.cuda.synchronize()
+    ms, n = plan.timing_read()
+    plan.timing_enable(0)
+    return dict(zip(("uv_extent", "row_pass", "col_pass", "sample"), ms)), n
+
+
+def measure_case(g, torch, dev, peak, name, w, dtype, entry, prune, steps, warmup, bind=False):
+    """One row of the `other` block: us per call, fraction of the HBM roofline on the method's bytes (whole plane,
+    and of the extent the call pruned to), per-kernel us.  Same event timing as the headline."""
+    up = lambda a: torch.as_tensor(np.ascontiguousarray(a), device=dev)
+    esz = 8 if dtype == torch.float64 else 4
+    C = w.image.shape[0] if entry == "chi2ImageBatch" else 1
+    plan = g.Plan(w.nxy, C, dtype, dev.index)
+    plan.set_pruning(prune)
+    u, v = up(w.u), up(w.v)
+    if entry == "sampleImage":
+        image = up(w.image)
+        out = torch.empty(w.M, dtype=torch.complex128 if esz == 8 else torch.complex64, device=dev)
+        fn = lambda: plan.sampleImage(image, w.dxy, u, v, w.PA, w.dRA, w.dDec, out=out)
+    else:
+        re, im, wt = up(w.re_obs), up(w.im_obs), up(w.w)
+        if entry == "chi2Profile":
+            prof = up(w.profile)
+            out = torch.empty(1, dtype=torch.float64, device=dev)
+            fn = lambda: plan.chi2Profile(prof, w.Rmin, w.dR, w.dxy, u, v, re, im, wt, w.dRA, w.dDec, w.PA, w.inc, out=out)
+        elif entry == "chi2ImageBatch":
+            image = up(w.image)
+            out = torch.empty(C + 1, dtype=torch.float64, device=dev)
+            fn = lambda: plan.chi2ImageBatch(image, w.dxy, u, v, re, im, wt, w.dRA, w.dDec, w.PA, out=out)
+        else:
+            image = up(w.image)
+            out = torch.empty(1, dtype=torch.float64, device=dev)
+            fn = lambda: plan.chi2Image(image, w.dxy, u, v, re, im, wt, w.dRA, w.dDec, w.PA, out=out)
+        if bind:
+            plan.bind_obs(u, v, re, im, wt)
+    for _ in range(warmup):
+        fn()
+    ms = event_time_ms(fn, steps, torch)
+    kms, _ = kernel_times_ms(plan, fn, min(steps, 100), torch)
+    extent = tuple(plan.last_uv_extent())
+    whole = (w.nxy // 2, 0, w.nxy - 1)
+    B = algorithmic_bytes(w.nxy, w.M, esz, entry, None, C)
+    Bp = algorithmic_bytes(w.nxy, w.M, esz, entry, extent, C) if extent != whole else B
+    row = {"case": name, "entry": entry, "dtype": "f64" if esz == 8 else "f32", "nxy": w.nxy, "M": w.M, "C": C,
+           "prune_mode": prune, "bound_obs": bool(bind), "us_per_call": 1e3 * ms, "uv_extent": list(extent),
+           "pruned": extent != whole,
+           "method_bytes_whole_plane": B["step"], "frac_whole_plane_bytes": B["step"] / (ms * 1e-3) / 1e9 / peak,
+           "method_bytes_this_extent": Bp["step"], "frac": Bp["step"] / (ms * 1e-3) / 1e9 / peak,
+           "kernels_us": {k: round(1e3 * t, 2) for k, t in kms.items() if t > 0},
+           "kernels_frac": {k: round(Bp[k] / (t * 1e-3) / 1e9 / peak, 3) for k, t in kms.items() if t > 0 and Bp[k] > 0}}
+    del plan
+    torch.cuda.empty_cache()
+    return row
+
+
+def measure_other(g, torch, dev, peak, w3, args):
+    """Every other BASELINE.json config, the whole-plane path, fp32, sampleImage and nxy = 8192, measured in this
+    run with the headline's method.  Workloads are the seeded generators' full sizes."""
+    import workloads
+    rows = []
+    S, Wm = args.other_steps, 5
+
+    def add(*a, **k):
+        try:
+            rows.append(measure_case(g, torch, dev, peak, *a, steps=S, warmup=Wm, **k))
+        except Exception as exc:                       # a failing case is reported, not hidden
+            rows.append({"case": a[0], "error": repr(exc)})
+
+    f64, f32 = torch.float64, torch.float32
+    add("cfg3 f64 chi2Image, whole plane (prune 0)", w3, f64, "chi2Image", 0)
+    add("cfg3 f64 chi2Image, bound observations", w3, f64, "chi2Image", 1, bind=True)
+    add("cfg3 f64 sampleImage", w3, f64, "sampleImage", 1)
+    w3f = w3.as_f32()
+    add("cfg3 f32 chi2Image", w3f, f32, "chi2Image", 1)
+    add("cfg3 f32 sampleImage", w3f, f32, "sampleImage", 1)
+    add("cfg3 f32 chi2Image, whole plane (prune 0)", w3f, f32, "chi2Image", 0)
+    del w3f
+    w2 = workloads.config(2)
+    add("cfg2 f64 chi2Image", w2, f64, "chi2Image", 1)
+    # nxy = 8192 (SURVEY 8(f) row 4): a seeded random image, the cfg-2 uv set scaled to the same pixel indices
+    rng = np.random.default_rng(8192)
+    w8 = workloads.Workload("n8192", "chi2Image", 8192, w2.dxy * 2048 / 8192, w2.u, w2.v, w2.re_obs, w2.im_obs, w2.w,
+                            w2.dRA, w2.dDec, w2.PA, image=rng.random((8192, 8192)))
+    add("nxy=8192 f64 chi2Image (cfg-2 uv set, random image)", w8, f64, "chi2Image", 1)
+    del w8, w2
+    add("cfg1 f64 chi2Profile", workloads.config(1), f64, "chi2Profile", 1)
+    add("cfg0 f64 chi2Image", workloads.config(0), f64, "chi2Image", 1)
+    w4 = workloads.config(4)
+    add("cfg4 f64 chi2ImageBatch (128 channels)", w4, f64, "chi2ImageBatch", 1)
+    add("cfg4 f64 chi2ImageBatch (128 channels), bound observations", w4, f64, "chi2ImageBatch", 1, bind=True)
+    return rows
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -201,6 +314,8 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other", action="store_true", help="skip the `other` block (every other config and path)")
+    ap.add_argument("--other-steps", type=int, default=50)
     ap.add_argument("--prune", type=int, default=1, choices=[0, 1, 2],
                     help="gal_plan_set_pruning mode: 0 never, 1 automatic (library default), 2 always")
     args = ap.parse_args()
@@ -256,59 +371,38 @@ def main():
     ms_step = ms_total / args.steps
     value = world * args.steps / (ms_total * 1e-3)
 
-    # the same step on a BOUND uv set (gal_plan_bind_uv: the caller promises u, v stay unchanged, as in a fit of one
-    # observation; the per-call uv-extent kernel is skipped).  Reported beside the headline, not instead of it.
-    plan.bind_uv(u, v)
-    for _ in range(args.warmup):
-        step()
-    barrier()
-    b0, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    b0.record()
-    for _ in range(args.steps):
-        step()
-    b1.record()
-    barrier()
-    ms_bound = max_over_ranks(b0.elapsed_time(b1), world, dev) / args.steps
-    bound_uv = {"ms_per_step": ms_bound, "value": world / (ms_bound * 1e-3), "unit": UNIT,
-                "chi2_identical": bool(float(out.cpu()[0]) == chi2_val),
-                "extent_violations": plan.last_extent_violations(), "uv_extent": list(plan.last_uv_extent())}
-    plan.unbind_uv()
-
     # per-kernel durations, live, CUDA events on the launching stream between the kernels
-    ksteps = min(args.steps, 200)
-    plan.timing_enable(ksteps)
-    for _ in range(ksteps):
-        step()
-    torch.cuda.synchronize()
-    (ms_ext, ms_row, ms_col, ms_samp), ncalls = plan.timing_read()
-    plan.timing_enable(0)
+    kms, ncalls = kernel_times_ms(plan, step, min(args.steps, 200), torch)
     extent = plan.last_uv_extent()
     pruned = tuple(extent) != (w.nxy // 2, 0, w.nxy - 1)
 
     peak, peak_src = measured_peaks()
     B = algorithmic_bytes(w.nxy, w.M, esz)                                   # whole half plane
-    Bk = algorithmic_bytes(w.nxy, w.M, esz, extent=extent) if pruned else B  # what this call's kernels must move
+    Bk = algorithmic_bytes(w.nxy, w.M, esz, extent=extent) if pruned else B  # the method's bytes of this extent
     kernels = []
-    ms_sum = max(ms_ext + ms_row + ms_col + ms_samp, 1e-12)
-    for name, ms in (("uv_extent", ms_ext), ("row_pass", ms_row), ("col_pass", ms_col), ("sample", ms_samp)):
-        if name == "uv_extent" and not pruned:
+    ms_sum = max(sum(kms.values()), 1e-12)
+    for name, ms in kms.items():
+        if ms <= 0:
             continue
         gbs = Bk[name] / (ms * 1e-3) / 1e9
         kernels.append({"kernel": name, "ms": ms, "algorithmic_bytes": Bk[name], "achieved_gbs": gbs,
                         "frac": gbs / peak, "share_of_step": ms / ms_sum})
     dom = max(kernels, key=lambda k: k["ms"])
     roofline = {"bound": "hbm", "kernel": dom["kernel"], "achieved": dom["achieved_gbs"], "peak": peak, "unit": "GB/s",
-                "frac": dom["frac"], "traffic": ncu_traffic(dom["kernel"]), "peak_source": peak_src,
-                "ms_per_launch": dom["ms"], "launches_timed": ncalls}
-    step_gbs = B["step"] / (ms_step * 1e-3) / 1e9
+                "frac": dom["frac"], "traffic": ncu_traffic(dom["kernel"]),
+                "traffic_source": "committed ncu --set full summary (profiles/*_ncu_traffic.csv), not measured in this run",
+                "peak_source": peak_src, "ms_per_launch": dom["ms"], "launches_timed": ncalls}
+    whole_gbs = B["step"] / (ms_step * 1e-3) / 1e9
     moved_gbs = Bk["step"] / (ms_step * 1e-3) / 1e9
-    step_roofline = {"bound": "hbm", "algorithmic_bytes": B["step"], "achieved": step_gbs, "peak": peak,
-                     "unit": "GB/s", "frac": step_gbs / peak, "target_frac": 0.60,
+    step_roofline = {"bound": "hbm", "algorithmic_bytes": Bk["step"], "achieved": moved_gbs, "peak": peak,
+                     "unit": "GB/s", "frac": moved_gbs / peak, "target_frac": 0.60,
                      "pruned_transform": pruned, "uv_extent": list(extent),
-                     "bytes_this_call_must_move": Bk["step"], "achieved_moved": moved_gbs, "frac_moved": moved_gbs / peak,
-                     "note": "frac: the two-pass whole-half-plane byte count of SURVEY.md 8(d) over the step time (the "
-                             "60 % target); frac_moved: the bytes the pruned call really has to move (image, reachable "
-                             "columns/rows of the spectrum, per-point arrays, u and v twice) over the same time"}
+                     "whole_plane_bytes": B["step"], "frac_whole_plane_credit": whole_gbs / peak,
+                     "note": "frac: the method's bytes of the extent this call pruned to (image once, reachable columns "
+                             "of the row-transformed image out and in, reachable rows of the spectrum out once, "
+                             "per-point arrays once) over the step time; frac_whole_plane_credit: SURVEY.md 8(d)'s "
+                             "two-pass whole-half-plane byte count over the same time (credits traffic a pruned call "
+                             "never moves; the whole-plane path itself is measured in `other`)"}
 
     # end to end through the host-pointer C-ABI call: pinned host inputs, H2D + kernels + D2H each step
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
@@ -329,13 +423,14 @@ def main():
            "d2h_bytes_per_step": 8, "steps": args.e2e_steps, "ms_per_step": e2e_ms / args.e2e_steps,
            "api": "gal_chi2_image_host_f64 (pinned host buffers in, chi2 to a host double out)",
            "matches_device_path": bool(e2e_chi2 == chi2_val)}
+    del himg, hu, hv, hre, him, hw
 
     result = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic", "config": base_config(w, "f64"), "clocks": clk.summary(), "e2e": e2e,
         "gpu_launches": int(launches), "roofline": roofline, "step_roofline": step_roofline, "kernels": kernels,
-        "visibilities_per_s": value * w.M, "chi2": chi2_val, "multi_gpu": "replicas only", "bound_uv": bound_uv,
+        "visibilities_per_s": value * w.M, "chi2": chi2_val, "multi_gpu": "replicas only",
         "paper_context": "GTX 1060, M=1e6, PCIe copies included: chi2Image 4096^2 = 59 ms (PAPER.md:619); not like for like",
     }
 
@@ -349,6 +444,10 @@ def main():
                                   "sample": f"the full configs[3] workload (one evaluation), best of 3 with {T} threads",
                                   "value_1thread": 1.0 / t1, "seconds_T_threads": tT, "seconds_1_thread": t1,
                                   "chi2_rel_diff_vs_gpu": abs(chi2_o - chi2_val) / abs(chi2_o)}
+    if rank == 0 and world == 1 and not args.no_other:
+        del plan, image, u, v, re, im, wt
+        torch.cuda.empty_cache()
+        result["other"] = measure_other(g, torch, dev, peak, w, args)
     if rank == 0:
         print(json.dumps(result))
     if world > 1:

@@ -112,6 +112,31 @@ __device__ __forceinline__ void twiddle_powers(cx<T> w1, cx<T>* w) {
     for (int k = 2; k < R; ++k) w[k] = (k & 1) ? cmul(w[k / 2], w[k / 2 + 1]) : cmul(w[k / 2], w[k / 2]);
 }
 
+// w * exp(-2 pi i d / M) for M = 8 or 16 and a compile-time d (after unrolling): the roots of unity are literals.
+template <typename T, int M>
+__device__ __forceinline__ cx<T> mul_root(cx<T> w, int d) {
+    const T h = (T)0.70710678118654752440, c1 = (T)0.92387953251128675613, s1 = (T)0.38268343236508977173;
+    const int e = (M == 16) ? d : 2 * d;                          // exponent in 16ths of a turn
+    switch (e & 15) {
+        case 0: return w;
+        case 1: return cmul(w, mk<T>(c1, -s1));
+        case 2: return mk<T>((w.x + w.y) * h, (w.y - w.x) * h);
+        case 3: return cmul(w, mk<T>(s1, -c1));
+        case 4: return mul_mi(w);
+        case 5: return cmul(w, mk<T>(-s1, -c1));
+        case 6: return mk<T>((w.y - w.x) * h, -(w.x + w.y) * h);
+        case 7: return cmul(w, mk<T>(-c1, -s1));
+        case 8: return mk<T>(-w.x, -w.y);
+        case 9: return cmul(w, mk<T>(-c1, s1));
+        case 10: return mk<T>(-(w.x + w.y) * h, (w.x - w.y) * h);
+        case 11: return cmul(w, mk<T>(-s1, c1));
+        case 12: return mk<T>(-w.y, w.x);
+        case 13: return cmul(w, mk<T>(s1, c1));
+        case 14: return mk<T>((w.x - w.y) * h, (w.x + w.y) * h);
+        default: return cmul(w, mk<T>(c1, s1));
+    }
+}
+
 // ------------------------------------------------------------------------------------------
 // Geometry of one L-point FFT in shared memory.
 // ------------------------------------------------------------------------------------------
@@ -299,8 +324,8 @@ row_pass_kernel(const RowParams<T> p) {
         const cx<T>* Sf = smem + ff * G::REGION;
         const cx<T> zk = Sf[G::zaddr(k)];
         const cx<T> zm = Sf[G::zaddr((L - k) % L)];
-        const cx<T> E = mk<T>((T)0.5 * (zk.x + zm.x), (T)0.5 * (zk.y - zm.y));
-        const cx<T> O = mk<T>((T)0.5 * (zk.y + zm.y), (T)-0.5 * (zk.x - zm.x));
+        const cx<T> E = mk<T>(zk.x + zm.x, zk.y - zm.y);          // 2 E and 2 O: the factor 1/2 is folded into
+        const cx<T> O = mk<T>(zk.y + zm.y, zm.x - zk.x);          // the column pass's sign (exact)
         const cx<T> WO = cmul(__ldg(p.tw + k), O);
         const cx<T> xk = cadd(E, WO);
         cx<T> xm = csub(E, WO);
@@ -311,8 +336,220 @@ row_pass_kernel(const RowParams<T> p) {
 }
 
 // ------------------------------------------------------------------------------------------
+// Row pass, pipelined (nxy = 1024 .. 4096; same result as row_pass_kernel).
+//
+// Persistent CTAs (one per SM).  A CTA is NG groups of GT = TPF * F consumer threads plus one producer warp.
+// A group transforms F adjacent image rows at a time, LANE-INTERLEAVED: thread gtid works on row gtid % F as
+// FFT thread gtid / F, so the F results for one ku sit in adjacent lanes and every store instruction writes
+// F * sizeof(complex) contiguous bytes per ku (whole 32-byte sectors in fp64 with F = 2).
+//   * Staging: lane 0 of the producer warp streams whole rows with `cp.async.bulk` (TMA) into a ring of NS
+//     slots (one slot = F row regions), full/empty mbarriers; the rows land linearly at the start of the
+//     regions they are transformed in, so the loads of the next NS - NG row blocks are in flight while the
+//     groups compute.  The image is an input of the call, not a product of the kernel before in the chain, so
+//     the producer does not wait for the programmatic dependency: its first loads overlap the kernel before.
+//   * Step 1 reads the linear row (conflict free), a group barrier separates those reads from the writes of
+//     the padded cube; step 2 is in place; step 3 is FUSED with the real-FFT untangle in registers: a thread
+//     takes a work item (k1, c) together with the item that holds the mirrored indices L - k —
+//     (R1 - k1, R2 - 1 - c) for k1 != 0, (0, R2 - c) for k1 = 0 — so Z[k] and Z[L - k] of all its outputs are
+//     its own registers: no third exchange through shared memory, no barrier, and the slot is released to
+//     the producer as soon as the step-3 operands are read.
+//   * Groups synchronise with named barriers (bar.sync id, GT), never the whole CTA, so the NG groups drift
+//     into different phases and the FP64 pipe, the shared-memory pipe and the store path overlap.
+// ------------------------------------------------------------------------------------------
+template <typename T, int R1, int R2, int R3, int F> struct RowGeom {
+    static constexpr int L = R1 * R2 * R3;
+    static constexpr int RMAX = cmax(R1, cmax(R2, R3));
+    static_assert(R1 == RMAX, "step 1 must be exactly one work item per thread (in-place landing buffer)");
+    static_assert(R2 >= 2 && R3 >= 2 && R1 % 2 == 0 && R2 % 2 == 0 && R3 % 2 == 0, "three-step plans only");
+    static constexpr int TPF = L / RMAX;                                // threads per row
+    static constexpr int GT = TPF * F;                                  // threads per group
+    static_assert(GT % 32 == 0, "a group is a whole number of warps");
+    static constexpr int P1 = R2 * R3 + 1;
+    static constexpr int BG = 128 / (int)sizeof(cx<T>);
+    static_assert(F <= BG, "rows per group");
+    static constexpr int SKEW = BG / F;                                 // region stride mod BG: rows interleave the banks
+    static constexpr int BASE = R1 * P1;                                // >= L: the linear row fits
+    static constexpr int REGION = BASE + ((SKEW - BASE % BG) % BG + BG) % BG;
+    static constexpr uint32_t SLOT_BYTES = (uint32_t)REGION * F * sizeof(cx<T>);
+    static_assert((REGION * sizeof(cx<T>)) % 16 == 0, "bulk-copy destination alignment");
+};
+
+__device__ __forceinline__ void group_barrier(int id, int nthreads) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+template <typename T, int R1, int R2, int R3, int F, int NG, int NS, bool SWEEP>
+__global__ void __launch_bounds__(RowGeom<T, R1, R2, R3, F>::GT * NG + 32, 1)
+row_pipe_kernel(const RowParams<T> p) {
+    using G = RowGeom<T, R1, R2, R3, F>;
+    constexpr int L = G::L, TPF = G::TPF, GT = G::GT, P1 = G::P1, REGION = G::REGION;
+    constexpr int N2 = R2 * R3, H1 = R1 / 2, NPAIR = R1 * R2 / 2;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    cx<T>* smem = reinterpret_cast<cx<T>*>(smem_raw);
+    const uint32_t full0 = smem_u32(smem_raw) + NS * G::SLOT_BYTES, empty0 = full0 + 8 * NS;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int N = p.N;
+    const long long nblk = p.rows_total / F;                 // F divides nxy: a block never straddles two images
+    if (tid == 0) {
+        for (int s = 0; s < NS; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, GT / 32); }
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    if (tid >= NG * GT) {                                    // ---- producer warp ----
+        if (!SWEEP && lane == 0) {
+            const uint64_t pol = l2_policy_evict_first();
+            const uint32_t row_bytes = (uint32_t)N * sizeof(T);
+            uint32_t slot = 0, parity = 1;                   // a fresh mbarrier lets a wait on parity 1 through
+            for (long long blk = blockIdx.x; blk < nblk; blk += gridDim.x) {
+                mbar_wait_relaxed(empty0 + 8 * slot, parity);
+                const uint32_t mb = full0 + 8 * slot;
+                const uint32_t dst = smem_u32(smem_raw) + slot * G::SLOT_BYTES;
+                mbar_expect_tx(mb, F * row_bytes);
+#pragma unroll
+                for (int f = 0; f < F; ++f)
+                    tma_load_1d(dst + f * (uint32_t)(REGION * sizeof(cx<T>)), p.image + (blk * F + f) * (long long)N, row_bytes, mb, pol);
+                if (++slot == NS) { slot = 0; parity ^= 1u; }
+            }
+        }
+        return;
+    }
+
+    // ---- consumer groups ----
+    const int g = tid / GT, gtid = tid % GT;
+    const int t = gtid / F, f = gtid % F;
+    const int bar_id = 1 + g;
+    pdl_wait();
+    const int kumax = __ldg(p.ext);
+    const int NU = N / 2 + 1;
+    const cx<T>* __restrict__ tw = p.tw;
+    // the only table reads of steps 1 and 2: one base twiddle each, W_L^t and W_(R2 R3)^(t mod R3)
+    const cx<T> wb1 = __ldg(tw + 2 * t);
+    static_assert(TPF % R3 == 0, "the step-2 twiddle index is the same for every work item of a thread");
+    const cx<T> wb2 = __ldg(tw + (t % R3) * (2 * R1));
+    long long q = g;
+    for (long long blk = blockIdx.x + (long long)gridDim.x * g; blk < nblk; blk += (long long)gridDim.x * NG, q += NG) {
+        const int slot = SWEEP ? g : (int)(q % NS);           // (no ring without the producer: one slot per group)
+        const uint32_t par = (uint32_t)((q / NS) & 1);
+        cx<T>* S = smem + (size_t)slot * F * REGION + (size_t)f * REGION;
+        const long long row = blk * F + f;
+        // step 1: DFT_R1 over n1, twiddle W_L^(n2 k1), n2 = t
+        {
+            cx<T> a[R1];
+            if (SWEEP) {
+                const int i = (int)(row % N);
+#pragma unroll
+                for (int n1 = 0; n1 < R1; ++n1) {
+                    const int n = N2 * n1 + t;
+                    a[n1] = mk<T>((T)sweep_pixel<T>(p.sweep, N, i, 2 * n), (T)sweep_pixel<T>(p.sweep, N, i, 2 * n + 1));
+                }
+            } else {
+                mbar_wait(full0 + 8 * slot, par);
+#pragma unroll
+                for (int n1 = 0; n1 < R1; ++n1) a[n1] = S[N2 * n1 + t];
+                group_barrier(bar_id, GT);                   // every linear read before the first padded write
+            }
+            Dft<T, R1>::run(a);
+            S[t] = a[0];
+            cx<T> w[R1];
+            twiddle_powers<T, R1>(wb1, w);
+#pragma unroll
+            for (int k1 = 1; k1 < R1; ++k1) S[k1 * P1 + t] = cmul(a[k1], w[k1]);
+        }
+        group_barrier(bar_id, GT);
+        // step 2: DFT_R2 over a, twiddle W_(R2 R3)^(b c), in place per work item
+        for (int it = t; it < R1 * R3; it += TPF) {
+            const int b = it % R3, k1 = it / R3;
+            cx<T>* base = S + k1 * P1 + b;
+            cx<T> a[R2];
+#pragma unroll
+            for (int i = 0; i < R2; ++i) a[i] = base[i * R3];
+            Dft<T, R2>::run(a);
+            base[0] = a[0];
+            cx<T> w[R2];
+            twiddle_powers<T, R2>(wb2, w);
+#pragma unroll
+            for (int c = 1; c < R2; ++c) base[c * R3] = cmul(a[c], w[c]);
+        }
+        group_barrier(bar_id, GT);
+        // step 3 fused with the untangle of the packed real transform:
+        //   E = (Z[k] + conj Z[L-k]) / 2,  O = -i (Z[k] - conj Z[L-k]) / 2,  W = exp(-2 pi i k / N)
+        //   X[k] = E + W O,   X[L-k] = conj(E - W O)     (k = 0 gives X[0] and X[L])
+        cx<T>* out = p.spec + (row / N) * (long long)NU * N + (row % N);
+        auto butterfly = [&](const cx<T> zk, const cx<T> zm, const cx<T> W, const int k) {
+            const int km = L - k;
+            const bool sk = k <= kumax, sm = km <= kumax;
+            if (!sk && !sm) return;
+            const cx<T> E = mk<T>(zk.x + zm.x, zk.y - zm.y);      // 2 E and 2 O: the factor 1/2 is folded into the
+            const cx<T> O = mk<T>(zk.y + zm.y, zm.x - zk.x);      // column pass's sign (exact)
+            const cx<T> WO = cmul(W, O);
+            if (sk) out[(long long)k * N] = cadd(E, WO);
+            if (sm) { cx<T> xm = csub(E, WO); xm.y = -xm.y; out[(long long)km * N] = xm; }
+        };
+        bool released = SWEEP;
+        for (int j = t; j < NPAIR; j += TPF) {
+            const int k1h = j % H1, cc = j / H1;
+            int pk1, pc, qk1, qc;
+            bool special = false;
+            if (k1h != 0) { pk1 = k1h; pc = cc; qk1 = R1 - k1h; qc = R2 - 1 - cc; }
+            else if (cc < R2 / 2) { pk1 = H1; pc = cc; qk1 = H1; qc = R2 - 1 - cc; }
+            else if (cc > R2 / 2) { pk1 = 0; pc = cc - R2 / 2; qk1 = 0; qc = R2 - pc; }
+            else { special = true; pk1 = 0; pc = 0; qk1 = 0; qc = R2 / 2; }      // the two self-mirrored items
+            // untangle twiddles W_N^k, k = k0 + R1 R2 d: one table value times the (2 R3)-th roots of unity, formed
+            // in registers (with the ring resident the L1 is too small to keep the table)
+            const cx<T> w0 = __ldg(tw + (pk1 + R1 * pc));
+            const cx<T> w0b = special ? __ldg(tw + R1 * (R2 / 2)) : w0;
+            cx<T> a[R3], m[R3];
+            {
+                const cx<T>* pa = S + pk1 * P1 + pc * R3;
+                const cx<T>* pm = S + qk1 * P1 + qc * R3;
+#pragma unroll
+                for (int b = 0; b < R3; ++b) { a[b] = pa[b]; m[b] = pm[b]; }
+            }
+            if (!SWEEP && j + TPF >= NPAIR) {                // this thread's last read of the slot: hand it back
+                fence_proxy_async_smem();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(empty0 + 8 * slot);
+                released = true;
+            }
+            Dft<T, R3>::run(a);
+            Dft<T, R3>::run(m);
+            if (!special) {
+#pragma unroll
+                for (int d = 0; d < R3; ++d)
+                    butterfly(a[d], m[R3 - 1 - d], mul_root<T, 2 * R3>(w0, d), pk1 + R1 * (pc + R2 * d));
+            } else {
+                butterfly(a[0], a[0], mk<T>(1, 0), 0);
+#pragma unroll
+                for (int d = 1; d <= R3 / 2; ++d) butterfly(a[d], a[R3 - d], mul_root<T, 2 * R3>(mk<T>(1, 0), d), R1 * R2 * d);
+#pragma unroll
+                for (int d = 0; d < R3 / 2; ++d)
+                    butterfly(m[d], m[R3 - 1 - d], mul_root<T, 2 * R3>(w0b, d), R1 * (R2 / 2 + R2 * d));
+            }
+        }
+        if (!released) {                                     // warps without a step-3 work item (NPAIR < TPF)
+            fence_proxy_async_smem();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty0 + 8 * slot);
+        }
+        if (SWEEP) group_barrier(bar_id, GT);                // the region is rewritten by the next block's step 1
+    }
+}
+
+// ------------------------------------------------------------------------------------------
 // Column pass (in place).
 // ------------------------------------------------------------------------------------------
+// Layout of the sampled spectrum.  A call pruned to a part of the half plane writes COLUMN PAIRS
+// (pair[ku][kvs] = {F[ku][kvs], F[ku+1][kvs]}, every value twice: two sectors per sampled point; the doubled
+// write is a few MB).  A call that needs the WHOLE half plane (extent == {N/2, 0, N-1}: pruning off, or points
+// that wrap, reading A6) writes every value ONCE, single[ku][kvs]: the column pass then moves 2 instead of 3
+// spectrum volumes and the gather pays three sectors per point instead of two.  Both layouts live in the same
+// plan buffer; the column pass and the sampler take the decision from the same device-resident extent.
+__device__ __forceinline__ bool extent_is_whole_plane(const int* ext, int N) {
+    return __ldg(ext) >= N / 2 && __ldg(ext + 1) <= 0 && __ldg(ext + 2) >= N - 1;
+}
+
 template <typename T> struct ColParams {
     const cx<T>* work;     // [batch][N/2+1][N], written by the row pass
     NodePair<T>* pair;     // [batch][N/2+1][N], the sampled spectrum
@@ -335,6 +572,7 @@ col_pass_kernel(const ColParams<T> p) {
     pdl_wait();
     // uv extent: columns beyond kumax are skipped, rows outside [rmin, rmax] are not written
     const int kumax = __ldg(p.ext), rmin = __ldg(p.ext + 1), rmax = __ldg(p.ext + 2);
+    const bool single = extent_is_whole_plane(p.ext, L);
     cx<T>* S = smem + f * G::REGION;
     {
         const long long grp = blockIdx.x;                   // one group of F columns per CTA
@@ -353,6 +591,7 @@ col_pass_kernel(const ColParams<T> p) {
         const cx<T>* col = p.work + (valid ? g : 0) * (long long)L;
         NodePair<T>* own = p.pair + (valid ? g : 0) * (long long)L;          // .a of this column's entries
         NodePair<T>* prev = own - (ku > 0 ? L : 0);                          // .b of the entries one column down
+        cx<T>* sown = reinterpret_cast<cx<T>*>(p.pair) + (valid ? g : 0) * (long long)L;   // single-copy layout
 
         fft_steps12<T, R1, R2, R3, G::TPF>(S, t, p.tw, 1, [&](int n) -> cx<T> {
             return valid ? col[n] : mk<T>(0, 0);
@@ -373,12 +612,16 @@ col_pass_kernel(const ColParams<T> p) {
 #pragma unroll
                     for (int d = 0; d < R3; ++d) {
                         const int kv = k1 + R1 * (c + R2 * d);
-                        const T sgn = ((ku + kv) & 1) ? (T)-1 : (T)1;
+                        const T sgn = ((ku + kv) & 1) ? (T)-0.5 : (T)0.5;
                         const int kvs = (kv + L / 2) & (L - 1);
                         if (kvs >= rmin && kvs <= rmax) {
                             const cx<T> val = mk<T>(sgn * a[d].x, sgn * a[d].y);
-                            own[kvs].a = val;
-                            if (ku > 0) prev[kvs].b = val;
+                            if (single) {
+                                sown[kvs] = val;
+                            } else {
+                                own[kvs].a = val;
+                                if (ku > 0) prev[kvs].b = val;
+                            }
                         }
                     }
                 }
@@ -395,7 +638,7 @@ col_pass_kernel(const ColParams<T> p) {
 #pragma unroll
                 for (int b = 0; b < R3; ++b) a[b] = base[b];
                 Dft<T, R3>::run(a);
-                const T sgn = ((ku + k1) & 1) ? (T)-1 : (T)1;     // R1 is even: kv and k1 have one parity
+                const T sgn = ((ku + k1) & 1) ? (T)-0.5 : (T)0.5;     // R1 is even: kv and k1 have one parity
 #pragma unroll
                 for (int d = 0; d < R3; ++d) base[d] = mk<T>(sgn * a[d].x, sgn * a[d].y);
             }
@@ -408,6 +651,7 @@ col_pass_kernel(const ColParams<T> p) {
                 if (gg >= p.cols_total || kuf > kumax || kvs < rmin || kvs > rmax) continue;
                 const int za = G::zaddr((kvs + L / 2) & (L - 1));
                 const cx<T> x = smem[ff * G::REGION + za];
+                if (single) { reinterpret_cast<cx<T>*>(p.pair)[gg * (long long)L + kvs] = x; continue; }
                 NodePair<T>* e = p.pair + gg * (long long)L + kvs;
                 if (ff + 1 < F && kuf < L / 2 && kuf + 1 <= kumax) {
                     NodePair<T> pr;
@@ -447,6 +691,8 @@ col_pass_x2_kernel(const ColParams<T> p) {
     const cx<T>* col = p.work + g * (long long)N;
     NodePair<T>* own = p.pair + g * (long long)N;
     NodePair<T>* prev = own - (ku > 0 ? N : 0);
+    cx<T>* sown = reinterpret_cast<cx<T>*>(p.pair) + g * (long long)N;
+    const bool single = extent_is_whole_plane(p.ext, N);
     cx<T>* S = smem + f * G::REGION;
 
     fft_steps12<T, R1, R2, R3, G::TPF>(S, t, p.tw, 2, [&](int n) -> cx<T> { return col[2 * n + f]; });
@@ -468,18 +714,16 @@ col_pass_x2_kernel(const ColParams<T> p) {
     for (int k = tid; k < L; k += G::NT) {
         const cx<T> E = SE[G::zaddr(k)];
         const cx<T> WO = cmul(__ldg(p.tw + k), SO[G::zaddr(k)]);
-        const T sgn = ((ku + k) & 1) ? (T)-1 : (T)1;          // L is even: kv = k and k + L have one parity
+        const T sgn = ((ku + k) & 1) ? (T)-0.5 : (T)0.5;          // L is even: kv = k and k + L have one parity
         const cx<T> x0 = cadd(E, WO), x1 = csub(E, WO);
         const int kvs0 = k + L, kvs1 = k;                     // (kv + N/2) mod N for kv = k, k + L
         if (kvs0 >= rmin && kvs0 <= rmax) {
             const cx<T> val = mk<T>(sgn * x0.x, sgn * x0.y);
-            own[kvs0].a = val;
-            if (ku > 0) prev[kvs0].b = val;
+            if (single) { sown[kvs0] = val; } else { own[kvs0].a = val; if (ku > 0) prev[kvs0].b = val; }
         }
         if (kvs1 >= rmin && kvs1 <= rmax) {
             const cx<T> val = mk<T>(sgn * x1.x, sgn * x1.y);
-            own[kvs1].a = val;
-            if (ku > 0) prev[kvs1].b = val;
+            if (single) { sown[kvs1] = val; } else { own[kvs1].a = val; if (ku > 0) prev[kvs1].b = val; }
         }
     }
 }
@@ -497,15 +741,16 @@ __global__ void sweep_kernel(SweepParams sp, int N, T* __restrict__ image) {
     }
 }
 
-// out[kvs][ku] = pair[ku][kvs].a   (paper layout [N][N/2+1])
+// out[kvs][ku] = single[ku][kvs]   (paper layout [N][N/2+1]; the whole-plane transform of
+// gal_fft2_shifted_* leaves the spectrum in the single-copy layout)
 template <typename T>
-__global__ void transpose_to_paper_layout_kernel(const NodePair<T>* __restrict__ spec, cx<T>* __restrict__ out, int N) {
+__global__ void transpose_to_paper_layout_kernel(const cx<T>* __restrict__ spec, cx<T>* __restrict__ out, int N) {
     __shared__ cx<T> tile[32][33];
     const int NU = N / 2 + 1;
     const int kv0 = blockIdx.x * 32, ku0 = blockIdx.y * 32;
     for (int r = threadIdx.y; r < 32; r += blockDim.y) {
         const int ku = ku0 + r, kv = kv0 + threadIdx.x;
-        if (ku < NU && kv < N) tile[r][threadIdx.x] = spec[(long long)ku * N + kv].a;
+        if (ku < NU && kv < N) tile[r][threadIdx.x] = spec[(long long)ku * N + kv];
     }
     __syncthreads();
     for (int r = threadIdx.y; r < 32; r += blockDim.y) {

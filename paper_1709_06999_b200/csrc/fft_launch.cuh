@@ -38,6 +38,38 @@ int launch_row(gal_plan* p, const T* image, const SweepParams* sw, int batch, co
     return GAL_OK;
 }
 
+// Pipelined row pass (fft.cuh: row_pipe_kernel): persistent grid, one CTA per SM.
+template <typename T, int R1, int R2, int R3, int F, int NG, int NS>
+int launch_row_pipe(gal_plan* p, const T* image, const SweepParams* sw, int batch, const int* ext, cudaStream_t st) {
+    using G = RowGeom<T, R1, R2, R3, F>;
+    static_assert(NS >= NG, "one slot per group at least");
+    RowParams<T> rp;
+    rp.image = image;
+    rp.spec = (cx<T>*)p->work;
+    rp.tw = (const cx<T>*)p->tw;
+    rp.N = p->nxy;
+    rp.rows_total = batch * p->nxy;
+    rp.ext = ext;
+    if (sw) rp.sweep = *sw; else memset(&rp.sweep, 0, sizeof(rp.sweep));
+    const long long nblk = rp.rows_total / F;
+    const unsigned grid = (unsigned)(nblk < p->sm_count ? nblk : p->sm_count);
+    const size_t smem = (size_t)NS * G::SLOT_BYTES + 16 * NS;
+    const dim3 block(G::GT * NG + 32);
+    if (sw) {
+        auto k = row_pipe_kernel<T, R1, R2, R3, F, NG, NS, true>;
+        int rc = set_smem(p, k, smem); if (rc) return rc;
+        GAL_CUDA(p, launch_chain(k, dim3(grid), block, smem, st, rp));
+    } else {
+        auto k = row_pipe_kernel<T, R1, R2, R3, F, NG, NS, false>;
+        int rc = set_smem(p, k, smem); if (rc) return rc;
+        GAL_CUDA(p, launch_chain(k, dim3(grid), block, smem, st, rp));
+    }
+    p->launches++;
+    GAL_CUDA(p, cudaGetLastError());
+    if (p->t_split) GAL_CUDA(p, cudaEventRecord(p->t_split[2], st));
+    return GAL_OK;
+}
+
 template <typename T, int R1, int R2, int R3, int F>
 int launch_col(gal_plan* p, int batch, const int* ext, cudaStream_t st) {
     using G = Geom<T, R1, R2, R3, F>;
@@ -75,6 +107,24 @@ int launch_col_x2(gal_plan* p, int batch, const int* ext, cudaStream_t st) {
     return GAL_OK;
 }
 
+// Groups per CTA and ring slots of the pipelined row pass: fp64 slots are 66 KB (two groups, three slots);
+// fp32 slots are half that (three groups, five slots).
+#ifndef GAL_ROW_NG64
+#define GAL_ROW_NG64 2
+#endif
+#ifndef GAL_ROW_NS64
+#define GAL_ROW_NS64 3
+#endif
+#ifndef GAL_ROW_NG32
+#define GAL_ROW_NG32 3
+#endif
+#ifndef GAL_ROW_NS32
+#define GAL_ROW_NS32 5
+#endif
+template <typename T> struct RowPipeCfg;
+template <> struct RowPipeCfg<double> { static constexpr int NG = GAL_ROW_NG64, NS = GAL_ROW_NS64; };
+template <> struct RowPipeCfg<float> { static constexpr int NG = GAL_ROW_NG32, NS = GAL_ROW_NS32; };
+
 // Radix plans.  Row FFT length is nxy/2, column FFT length is nxy.
 template <typename T>
 int fft2(gal_plan* p, const T* image, const SweepParams* sw, int batch, const int* ext, cudaStream_t st) {
@@ -92,9 +142,17 @@ int fft2(gal_plan* p, const T* image, const SweepParams* sw, int batch, const in
         GAL_FFT_CASE(128, RR(8, 8, 1, 16), RR(16, 8, 1, 16))
         GAL_FFT_CASE(256, RR(16, 8, 1, 16), RR(16, 16, 1, 8))
         GAL_FFT_CASE(512, RR(16, 16, 1, 8), RR(8, 8, 8, 4))
-        GAL_FFT_CASE(1024, RR(8, 8, 8, 4), RR(16, 8, 8, 4))
-        GAL_FFT_CASE(2048, RR(16, 8, 8, 4), RR(16, 16, 8, 2))
-        GAL_FFT_CASE(4096, RR(16, 16, 8, 2), RR(16, 16, 16, 1))
+        // nxy >= 1024: the pipelined row pass (row_mode 0 keeps the plain one, for comparison)
+#define GAL_FFT_CASE_PIPE(NXY, ROW, PIPE, COL)                                   \
+    case NXY:                                                                    \
+        rc = p->row_mode ? launch_row_pipe<T, PIPE, RowPipeCfg<T>::NG, RowPipeCfg<T>::NS>(p, image, sw, batch, ext, st) \
+                         : launch_row<T, ROW>(p, image, sw, batch, ext, st);     \
+        if (rc) return rc;                                                       \
+        return launch_col<T, COL>(p, batch, ext, st);
+        GAL_FFT_CASE_PIPE(1024, RR(8, 8, 8, 4), RR(16, 8, 4, 8), RR(16, 8, 8, 4))
+        GAL_FFT_CASE_PIPE(2048, RR(16, 8, 8, 4), RR(16, 8, 8, 4), RR(16, 16, 8, 2))
+        GAL_FFT_CASE_PIPE(4096, RR(16, 16, 8, 2), RR(16, 16, 8, 2), RR(16, 16, 16, 1))
+#undef GAL_FFT_CASE_PIPE
         case 8192:      // column length 8192 = 2 x 4096: two interleaved transforms + one radix-2 combination
             rc = launch_row<T, 16, 16, 16, 1>(p, image, sw, batch, ext, st); if (rc) return rc;
             return launch_col_x2<T, 16, 16, 16>(p, batch, ext, st);
@@ -120,7 +178,7 @@ int launch_sweep(gal_plan* p, const SweepParams& sw, T* out, cudaStream_t st) {
 template <typename T>
 int launch_transpose(gal_plan* p, T* out, cudaStream_t st) {
     dim3 grid((p->nxy + 31) / 32, (p->nxy / 2 + 1 + 31) / 32), block(32, 8);
-    transpose_to_paper_layout_kernel<T><<<grid, block, 0, st>>>((const NodePair<T>*)p->spec, (cx<T>*)out, p->nxy);
+    transpose_to_paper_layout_kernel<T><<<grid, block, 0, st>>>((const cx<T>*)p->spec, (cx<T>*)out, p->nxy);
     p->launches++;
     GAL_CUDA(p, cudaGetLastError());
     return GAL_OK;

@@ -5,6 +5,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <set>
@@ -105,6 +106,7 @@ int run_call(gal_plan* p, const T* image, const SweepParams* sw, int C, double d
         ext = p->ext;
     }
     if (timed) GAL_CUDA(p, cudaEventRecord(e[1], st));
+    p->cur_ext = ext;
     if (M > 0) {                                      // no points: nothing to transform for
         p->t_split = e;
         rc = fft2<T>(p, image, sw, C, ext, st);
@@ -222,6 +224,7 @@ int do_multi(gal_plan* p, const T* image, double dxy, const T* u, const T* v, co
         for (int s = 0; s < S; ++s) if ((rc = launch_extent<T>(p, 1, cs[s], u, v, M, st))) return rc;
         ext = p->ext;
     }
+    p->cur_ext = ext;
     if ((rc = fft2<T>(p, image, nullptr, 1, ext, st))) return rc;
     for (int s = 0; s < S; ++s) {
         cs[s].amp = scale ? scale[s] : 1.0;
@@ -322,6 +325,7 @@ int gal_plan_create(gal_plan** out, int nxy, int batch, int precision_bits, int 
     gal_plan* p = new (std::nothrow) gal_plan();
     if (!p) return GAL_ERR_ALLOC;
     p->nxy = nxy; p->batch = batch; p->bits = precision_bits; p->device = device;
+    if (const char* e = getenv("GAL_ROW_PIPE")) p->row_mode = atoi(e) != 0;    // diagnostic switch
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || device >= ndev) { delete p; return GAL_ERR_CUDA; }
     DeviceGuard g(device);

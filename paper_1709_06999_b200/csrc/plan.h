@@ -21,6 +21,7 @@ struct gal_plan {
     unsigned long long* oob = nullptr;   // call_state[0]; the uv extent follows it
     int* ext = nullptr;                  // {kumax, rmin, rmax} of the current call (device)
     int* ext_full = nullptr;             // constant {nxy/2, 0, nxy-1}: no pruning
+    const int* cur_ext = nullptr;        // extent the current call's transform is pruned to (device); also selects the layout
     // Per-call device state [oob (8 B) | ext (12 B) | done ticket (4 B) | pad], two copies used alternately:
     // the sampling kernel of call k re-arms the copy call k+1 will use, so no reset operation sits between
     // two calls on the stream (an explicit copy from call_init is only needed when that did not happen).
@@ -29,6 +30,7 @@ struct gal_plan {
     int cur = 0;                         // copy used by the most recent call
     bool next_armed = false;             // the other copy has been / will be re-armed by that call's sampler
     int prune_mode = 1;                  // 0 never, 1 auto, 2 always
+    int row_mode = 0;                    // 1: pipelined row pass where built (nxy 1024..4096); 0: the plain one (GAL_ROW_PIPE=0)
     bool last_pruned = false;            // did the most recent call compute a uv extent?
     // bound uv set (gal_plan_bind_uv): addresses, size, the rotation-invariant radius, and the extent derived
     // from it for the pixel size seen last (device copy used by the FFT passes and checked by the sampler)

@@ -18,6 +18,8 @@
 //     that gather is bounded by the L2 -> SM path and by the L1's one line per clock, so it is
 //     shaped to move the fewest sectors and lines, and everything else overlaps with it.
 #pragma once
+#include <type_traits>
+
 #include "common.cuh"
 
 namespace galb {
@@ -41,9 +43,15 @@ template <typename T> struct SampleParams {
     unsigned long long* oob;  // [1]: this call's out-of-grid counter
     unsigned int* done;       // [1]: CTAs of this launch that have finished
     unsigned long long* next_state;  // the copy of the per-call state the NEXT call will use (32 B)
+    const int* ext;           // the extent the transform was pruned to: whole plane = single-copy layout (fft.cuh)
     const int* ext_check;     // extent of a bound uv set to verify every point against, or null
     unsigned long long* viol; // [1]: points whose cell lies outside ext_check
 };
+
+// Which layout did the column pass write?  Same rule as fft.cuh: extent_is_whole_plane.
+__device__ __forceinline__ bool extent_is_whole(const int* ext, int N) {
+    return __ldg(ext) >= N / 2 && __ldg(ext + 1) <= 0 && __ldg(ext + 2) >= N - 1;
+}
 
 // Correctly rounded a / b from r = RN(1/b) (Markstein): q0 = RN(a r); rem = a - q0 b (exact in an
 // FMA); q = RN(q0 + rem r).  Bit-identical to __ddiv_rn for the operand ranges met here (finite,
@@ -161,11 +169,14 @@ __device__ __forceinline__ void sincos_quarter(float a, int q, float* sn, float*
 // Node (kv mod N, ku mod N) of the spectrum extended to all integers by the periodicity and Hermitian symmetry
 // of the DFT of a real image (reading A6): columns 0..N/2 are stored; column cu > N/2 is the conjugate of column
 // N - cu at row -kv.  Used for the points whose cell leaves the half-plane grid; 32-bit index arithmetic.
-template <typename T>
+template <typename T, bool PAIR>
 __device__ __forceinline__ cx<T> node_wrapped(const NodePair<T>* __restrict__ spec, int N, int cu, int kvm) {
     const int H = N >> 1, m = N - 1;
-    if (cu <= H) return __ldg(&spec[cu * N + ((kvm + H) & m)].a);
-    cx<T> g = __ldg(&spec[(N - cu) * N + (((N - kvm) + H) & m)].a);
+    auto at = [&](int e) -> cx<T> {
+        return PAIR ? __ldg(&spec[e].a) : __ldg(reinterpret_cast<const cx<T>*>(spec) + e);
+    };
+    if (cu <= H) return at(cu * N + ((kvm + H) & m));
+    cx<T> g = at((N - cu) * N + (((N - kvm) + H) & m));
     g.y = -g.y;
     return g;
 }
@@ -173,15 +184,15 @@ __device__ __forceinline__ cx<T> node_wrapped(const NodePair<T>* __restrict__ sp
 // Bilinear interpolation of the extended spectrum at (uidx, vidx) anywhere in the plane: the listing's
 // interpolation on wrapped nodes.  Out of line: one call per out-of-grid point keeps the hot
 // loop of the sampler free of this code.
-template <typename T>
+template <typename T, bool PAIR>
 __device__ __noinline__ cx<double> wrapped_cell(const NodePair<T>* __restrict__ spec, int N, double uidx, double vidx) {
     const double fx = floor(uidx), fy = floor(vidx);
     const long long ix = (long long)fx, iy = (long long)fy;
     const int m = N - 1, H = N >> 1;                        // N is a power of two: & m is the floor-mod
     const int c0 = (int)(ix & m), c1 = (int)((ix + 1) & m);
     const int kv0 = (int)((iy - H) & m), kv1 = (int)((iy + 1 - H) & m);
-    const cx<T> g00 = node_wrapped<T>(spec, N, c0, kv0), g01 = node_wrapped<T>(spec, N, c1, kv0);
-    const cx<T> g10 = node_wrapped<T>(spec, N, c0, kv1), g11 = node_wrapped<T>(spec, N, c1, kv1);
+    const cx<T> g00 = node_wrapped<T, PAIR>(spec, N, c0, kv0), g01 = node_wrapped<T, PAIR>(spec, N, c1, kv0);
+    const cx<T> g10 = node_wrapped<T, PAIR>(spec, N, c0, kv1), g11 = node_wrapped<T, PAIR>(spec, N, c1, kv1);
     const double txr = __dsub_rn(uidx, fx), tyr = __dsub_rn(vidx, fy);
     const double ax = 1.0 - txr, ay = 1.0 - tyr;
     cx<double> r;
@@ -342,7 +353,7 @@ template <typename T> struct SampleCtx {
 // single-copy layout and 126 for one 16-byte load per node and lane).  Each lane then interpolates its row
 // along u for both cells, one shuffle hands the row the partner needs across, and the owner finishes its
 // own point.
-template <typename T, bool WRITE_VIS, bool DO_CHI2, bool EXACT, int U, typename LD, typename KP>
+template <typename T, bool WRITE_VIS, bool DO_CHI2, bool EXACT, int U, bool PAIR, typename LD, typename KP>
 __device__ __forceinline__ void sample_points(const SampleParams<T>& p, SampleCtx<T>& cx_, LD ld, KP kpt, long long M,
                                               int c) {
     const int N = cx_.N, odd = cx_.odd;
@@ -367,10 +378,17 @@ __device__ __forceinline__ void sample_points(const SampleParams<T>& p, SampleCt
         const int off = ix0 * N + iy0;                   // 0 outside
         if (ix0 + 1 > cx_.ck_kumax || iy0 < cx_.ck_rmin || iy0 + 1 > cx_.ck_rmax || (!inside[j] && cx_.ck_kumax < N)) ++cx_.viol;
         const int off_partner = __shfl_xor_sync(0xffffffffu, off, 1);
-        const NodePair<T> ea = load_pair(spec + ((odd ? off_partner : off) + odd));
-        const NodePair<T> eb = load_pair(spec + ((odd ? off : off_partner) + odd));
-        ga0[j] = ea.a; ga1[j] = ea.b;
-        gb0[j] = eb.a; gb1[j] = eb.b;
+        const int ia = (odd ? off_partner : off) + odd, ib = (odd ? off : off_partner) + odd;
+        if (PAIR) {
+            const NodePair<T> ea = load_pair(spec + ia);
+            const NodePair<T> eb = load_pair(spec + ib);
+            ga0[j] = ea.a; ga1[j] = ea.b;
+            gb0[j] = eb.a; gb1[j] = eb.b;
+        } else {                    // single-copy layout: the same four values from columns ku and ku + 1
+            const cx<T>* __restrict__ sg = reinterpret_cast<const cx<T>*>(spec);
+            ga0[j] = __ldg(sg + ia); ga1[j] = __ldg(sg + ia + N);
+            gb0[j] = __ldg(sg + ib); gb1[j] = __ldg(sg + ib + N);
+        }
         tx_partner[j] = __shfl_xor_sync(0xffffffffu, tx[j], 1);     // in flight with the gather
     }
 #pragma unroll
@@ -392,7 +410,7 @@ __device__ __forceinline__ void sample_points(const SampleParams<T>& p, SampleCt
         if (!inside[j]) {           // rare: the cell leaves the half-plane grid (reading A6); dead slots never get here
             const PointIndex q = point_index<EXACT>(p.ix, (double)ld(0, j), (double)ld(1, j));
             if (q.uidx > p.ix.fH || q.vidx < 0.0 || q.vidx > p.ix.fN1) ++cx_.oob;
-            const cx<double> g = wrapped_cell<T>(spec, N, q.uidx, q.vidx);
+            const cx<double> g = wrapped_cell<T, PAIR>(spec, N, q.uidx, q.vidx);
             ReInt = (R)g.x;
             ImInt = (R)g.y;
         }
@@ -502,7 +520,7 @@ __device__ __forceinline__ void sample_finish(const SampleParams<T>& p, int c, d
 }
 
 // One tile by plain (guarded) loads straight from global memory.
-template <typename T, bool WRITE_VIS, bool DO_CHI2, bool EXACT>
+template <typename T, bool WRITE_VIS, bool DO_CHI2, bool EXACT, bool PAIR>
 __device__ __forceinline__ void sample_tile_plain(const SampleParams<T>& p, SampleCtx<T>& cx_, long long tile, long long M,
                                                   int c) {
     constexpr int U = SampleGeom<T, DO_CHI2>::U, TILE = SampleGeom<T, DO_CHI2>::TILE;
@@ -519,14 +537,17 @@ __device__ __forceinline__ void sample_tile_plain(const SampleParams<T>& p, Samp
         return __ldcs(g + k);
     };
     auto kpt = [&](int j) -> long long { return k0 + j * 256; };
-    sample_points<T, WRITE_VIS, DO_CHI2, EXACT, U>(p, cx_, ld, kpt, M, c);
+    sample_points<T, WRITE_VIS, DO_CHI2, EXACT, U, PAIR>(p, cx_, ld, kpt, M, c);
 }
 
 template <typename T>
 __device__ __forceinline__ SampleCtx<T> sample_ctx(const SampleParams<T>& p, int c) {
     SampleCtx<T> cx_;
     cx_.N = p.N;
-    cx_.spec = p.spec + (long long)c * (p.N / 2 + 1) * p.N;
+    // channel c of the batch: [N/2+1][N] entries, column pairs or (whole-plane extent) single values
+    const long long plane = (long long)c * (p.N / 2 + 1) * p.N;
+    cx_.spec = extent_is_whole(p.ext, p.N) ? reinterpret_cast<const NodePair<T>*>(reinterpret_cast<const cx<T>*>(p.spec) + plane)
+                                           : p.spec + plane;
     cx_.odd = threadIdx.x & 1;
     cx_.acc = 0.0;
     cx_.oob = 0;
@@ -545,8 +566,13 @@ __global__ void __launch_bounds__(256, GAL_SAMPLE_MINB) sample_kernel_plain(cons
     SampleCtx<T> cx_ = sample_ctx(p, c);
     pdl_wait();
     const long long ntiles = (M + G::TILE - 1) / G::TILE;
-    for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x)
-        sample_tile_plain<T, WRITE_VIS, DO_CHI2, true>(p, cx_, tile, M, c);
+    if (extent_is_whole(p.ext, p.N)) {
+        for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x)
+            sample_tile_plain<T, WRITE_VIS, DO_CHI2, true, false>(p, cx_, tile, M, c);
+    } else {
+        for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x)
+            sample_tile_plain<T, WRITE_VIS, DO_CHI2, true, true>(p, cx_, tile, M, c);
+    }
     sample_finish<T, DO_CHI2>(p, c, cx_.acc, cx_.oob, cx_.viol);
 }
 
@@ -596,20 +622,24 @@ __global__ void __launch_bounds__(SampleGeom<T, DO_CHI2>::NT_TMA, GAL_SAMPLE_MIN
             }
         }
     } else {                                                 // ---- consumers ----
-        uint32_t stage = 0, parity = 0;
-        int tile = blockIdx.x;
-        for (; tile < nfull; tile += gridDim.x) {
-            mbar_wait(full0 + 8 * stage, parity);
-            const T* st = reinterpret_cast<const T*>(sample_smem + stage * G::STAGE_BYTES) + tid;
-            auto ld = [&](int a, int j) -> T { return st[a * TILE + j * 256]; };
-            auto kpt = [&](int j) -> long long { return (long long)tile * TILE + j * 256 + tid; };
-            sample_points<T, WRITE_VIS, DO_CHI2, false, U>(p, cx_, ld, kpt, M, c);
-            __syncwarp();                                    // every lane has read its last value of this stage
-            if (lane == 0) mbar_arrive(empty0 + 8 * stage);
-            if (++stage == S) { stage = 0; parity ^= 1u; }
-        }
-        if (tile == nfull && (long long)nfull * TILE < M)    // the ragged last tile falls to this CTA
-            sample_tile_plain<T, WRITE_VIS, DO_CHI2, false>(p, cx_, nfull, M, c);
+        auto consume = [&](auto pair_tag) {                  // the loop, once per spectrum layout
+            constexpr bool PAIR = decltype(pair_tag)::value;
+            uint32_t stage = 0, parity = 0;
+            int tile = blockIdx.x;
+            for (; tile < nfull; tile += gridDim.x) {
+                mbar_wait(full0 + 8 * stage, parity);
+                const T* st = reinterpret_cast<const T*>(sample_smem + stage * G::STAGE_BYTES) + tid;
+                auto ld = [&](int a, int j) -> T { return st[a * TILE + j * 256]; };
+                auto kpt = [&](int j) -> long long { return (long long)tile * TILE + j * 256 + tid; };
+                sample_points<T, WRITE_VIS, DO_CHI2, false, U, PAIR>(p, cx_, ld, kpt, M, c);
+                __syncwarp();                                // every lane has read its last value of this stage
+                if (lane == 0) mbar_arrive(empty0 + 8 * stage);
+                if (++stage == S) { stage = 0; parity ^= 1u; }
+            }
+            if (tile == nfull && (long long)nfull * TILE < M)    // the ragged last tile falls to this CTA
+                sample_tile_plain<T, WRITE_VIS, DO_CHI2, false, PAIR>(p, cx_, nfull, M, c);
+        };
+        if (extent_is_whole(p.ext, p.N)) consume(std::false_type{}); else consume(std::true_type{});
     }
     sample_finish<T, DO_CHI2>(p, c, cx_.acc, cx_.oob, cx_.viol);
 }

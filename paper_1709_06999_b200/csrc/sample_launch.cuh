@@ -62,6 +62,7 @@ int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T
     sp.done = (unsigned int*)((char*)p->oob + 20);
     sp.next_state = (unsigned long long*)((char*)p->call_state + 32 * (p->cur ^ 1));
     sp.viol = (unsigned long long*)((char*)p->oob + 24);
+    sp.ext = p->cur_ext;
     sp.ext_check = (p->last_bound && p->b_ext[0] < p->nxy / 2) ? p->b_ext_dev : nullptr;
     // one CTA works through tiles blockIdx.x, blockIdx.x + gridDim.x, ...: a whole number of CTAs per SM
     const int tile = SampleGeom<T, true>::TILE;
