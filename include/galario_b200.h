@@ -51,6 +51,7 @@ extern "C" {
 #define GAL_ERR_ALLOC (-2)            /* device or host allocation failed */
 #define GAL_ERR_CUDA (-3)             /* a CUDA call failed; see gal_last_cuda_error() */
 #define GAL_ERR_UNSUPPORTED (-4)      /* valid in the paper but not built here (nxy = 16384) */
+#define GAL_ERR_BINDING_VIOLATED (-5) /* an earlier call found a bound (u, v) set changed: that call's results are invalid; the binding is dropped */
 
 typedef struct gal_plan gal_plan;
 
@@ -98,6 +99,28 @@ int gal_plan_bind_uv_f64(gal_plan* plan, const double* u, const double* v, int64
 int gal_plan_bind_uv_f32(gal_plan* plan, const float* u, const float* v, int64_t M, int C, void* stream);
 int gal_plan_unbind_uv(gal_plan* plan);
 int64_t gal_last_extent_violations(gal_plan* plan);
+
+/* Bound observation set (same use case: the observations of a fit never change).  gal_plan_bind_obs declares that
+ * the C x M device arrays u, v, re_obs, im_obs, w keep their contents.  The plan makes a PRIVATE copy of the five
+ * arrays reordered along a space-filling (Morton) curve of the uv plane folded to u >= 0, so that the 32 points of
+ * a warp fall into a few neighbouring cells of the spectrum for any PA and the bilinear gather
+ * is served from L1 instead of L2 (hand-written stable radix sort, a few kernels, synchronises `stream`; the copy
+ * costs 5 C M reals of device memory).  It also binds (u, v) as gal_plan_bind_uv does.  Later chi2* calls
+ * (gal_chi2_image_*, gal_chi2_profile_*, gal_chi2_image_batch_*) that pass these very five pointers with the same M
+ * and C sample the private copy and skip the uv-extent kernel: chi2 is a sum over the points (Eq. 10)
+ * and does not depend on their order beyond rounding (the reduction stays deterministic: the permutation is the
+ * unique order by (Morton key, original index)).  Changing the contents of the arrays afterwards has NO effect on
+ * those calls until the set is bound again.  sample* calls and chi2 calls with other observation pointers use the
+ * (u, v) binding only.  gal_plan_unbind_obs (= gal_plan_unbind_uv) drops both.
+ * Sticky error: a sample/chi2 call on a bound (u, v) set whose points left the bound extent (the promise was broken)
+ * sets a flag; the next sample/chi2 call on the plan after that call has finished returns
+ * GAL_ERR_BINDING_VIOLATED without launching anything and drops the binding.  Results of the offending call are
+ * undefined.  Errors: as gal_plan_bind_uv; GAL_ERR_UNSUPPORTED for M >= 2^32. */
+int gal_plan_bind_obs_f64(gal_plan* plan, const double* u, const double* v, const double* re_obs, const double* im_obs,
+                          const double* w, int64_t M, int C, void* stream);
+int gal_plan_bind_obs_f32(gal_plan* plan, const float* u, const float* v, const float* re_obs, const float* im_obs,
+                          const float* w, int64_t M, int C, void* stream);
+int gal_plan_unbind_obs(gal_plan* plan);
 
 /* ---- get_image_size (Eq. 19-24; host only, no device is touched): image size N_lm (rounded
  *      up to a power of two) and pixel size (radians) for the uv coverage u[M], v[M] (HOST pointers,

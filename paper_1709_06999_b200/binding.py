@@ -51,6 +51,9 @@ def load_library() -> ctypes.CDLL:
         lib.gal_last_extent_violations.restype = _i64
         for s in ("f64", "f32"):
             getattr(lib, f"gal_plan_bind_uv_{s}").argtypes = [_vp, _vp, _vp, _i64, _i, _vp]
+        lib.gal_plan_unbind_obs.argtypes = [_vp]
+        for s in ("f64", "f32"):
+            getattr(lib, f"gal_plan_bind_obs_{s}").argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _i64, _i, _vp]
         lib.gal_last_uv_extent.argtypes = [_vp, _vp]
         for s in ("f64", "f32"):
             getattr(lib, f"gal_sweep_{s}").argtypes = [_vp, _vp, _i, _d, _d, _d, _d, _vp, _vp]
@@ -193,6 +196,18 @@ class Plan:
         M = u.shape[-1]
         _check(self._fn("plan_bind_uv")(self._h, self._dev(u, "u"), self._dev(v, "v"), M, C, _stream()),
                "gal_plan_bind_uv", self)
+
+    def bind_obs(self, u, v, re_obs, im_obs, w) -> None:
+        """Promise that the five observation arrays ([M] or [C][M]) keep their contents: later chi2 calls that pass
+        these very tensors sample the plan's private, uv-sorted copy (gal_plan_bind_obs)."""
+        C = 1 if u.dim() == 1 else u.shape[0]
+        M = u.shape[-1]
+        _check(self._fn("plan_bind_obs")(self._h, self._dev(u, "u"), self._dev(v, "v"), self._dev(re_obs, "re_obs"),
+                                         self._dev(im_obs, "im_obs"), self._dev(w, "w"), M, C, _stream()),
+               "gal_plan_bind_obs", self)
+
+    def unbind_obs(self) -> None:
+        _check(self._lib.gal_plan_unbind_obs(self._h), "gal_plan_unbind_obs", self)
 
     def unbind_uv(self) -> None:
         _check(self._lib.gal_plan_unbind_uv(self._h), "gal_plan_unbind_uv", self)

@@ -15,6 +15,9 @@
 
 using namespace galb;
 
+extern "C" int gal_plan_unbind_uv(gal_plan* p);
+extern "C" int gal_plan_unbind_obs(gal_plan* p);
+
 namespace {
 
 inline bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
@@ -81,7 +84,18 @@ int run_call(gal_plan* p, const T* image, const SweepParams* sw, int C, double d
     const int* ext = p->ext_full;
     p->last_pruned = want_prune<T>(p, C, M) && !cs.ix.du_exact_div;   // the extent kernel only has the division shortcut
     p->last_bound = false;
-    if (p->prune_mode != 0 && M > 0 && p->b_u == (const void*)u && p->b_v == (const void*)v && p->b_M == M && p->b_C == C) {
+    p->last_obs = false;
+    const bool uv_bound = M > 0 && p->b_u == (const void*)u && p->b_v == (const void*)v && p->b_M == M && p->b_C == C;
+    if (uv_bound && !vis && p->o_buf && p->o_src[2] == (const void*)re && p->o_src[3] == (const void*)im &&
+        p->o_src[4] == (const void*)w) {
+        // bound observation set: chi2 does not depend on the order of the points, so sample the plan's private copy,
+        // sorted along a space-filling curve of the uv plane (sort.cuh)
+        const size_t plane = (size_t)C * M;
+        const T* o = (const T*)p->o_buf;
+        u = o; v = o + plane; re = o + 2 * plane; im = o + 3 * plane; w = o + 4 * plane;
+        p->last_obs = true;
+    }
+    if (p->prune_mode != 0 && uv_bound) {
         // bound uv set: the extent follows from the radius computed once at bind time, for any PA.  The index of
         // a rotated coordinate is at most r_max / du (+ rounding: two cells of margin); rows are symmetric about N/2.
         if (p->b_dxy != dxy) {
@@ -151,6 +165,11 @@ int do_sample_image(gal_plan* p, const T* image, const SweepParams* sw, int C, d
     if (chi2 && (!chi2_pc && !chi2_tot)) return GAL_ERR_INVALID_ARGUMENT;
     if (chi2 && M > 0 && (!re || !im || !w)) return GAL_ERR_INVALID_ARGUMENT;
     if (!std::isfinite(dRA) || !std::isfinite(dDec) || !std::isfinite(PA)) return GAL_ERR_INVALID_ARGUMENT;
+    if (p->viol_host && *(volatile unsigned int*)p->viol_host) {      // an earlier call found the bound uv set changed
+        *(volatile unsigned int*)p->viol_host = 0;
+        gal_plan_unbind_obs(p);
+        return GAL_ERR_BINDING_VIOLATED;
+    }
     DeviceGuard g(p->device);
     cudaStream_t st = (cudaStream_t)stream;
     p->last_stream = st;
@@ -277,6 +296,7 @@ int do_host_call(gal_plan* p, const T* image, const T* I, int nr, double Rmin, d
 }  // namespace
 
 extern "C" int gal_plan_unbind_uv(gal_plan* p);
+extern "C" int gal_plan_unbind_obs(gal_plan* p);
 
 namespace {
 
@@ -285,7 +305,7 @@ int do_bind_uv(gal_plan* p, const T* u, const T* v, int64_t M, int C, void* stre
     if (!prec_ok<T>(p) || !u || !v || M < 1 || C < 1 || C > p->batch) return GAL_ERR_INVALID_ARGUMENT;
     DeviceGuard g(p->device);
     cudaStream_t st = (cudaStream_t)stream;
-    gal_plan_unbind_uv(p);
+    gal_plan_unbind_obs(p);
     GAL_CUDA(p, cudaMemsetAsync(p->b_r2, 0, 8, st));
     { int rc = launch_uv_radius<T>(p, u, v, (long long)C * M, st); if (rc) return rc; }
     unsigned long long bits = 0;
@@ -295,6 +315,24 @@ int do_bind_uv(gal_plan* p, const T* u, const T* v, int64_t M, int C, void* stre
     if (!std::isfinite(r2)) return GAL_ERR_INVALID_ARGUMENT;
     p->b_rmax = std::sqrt(r2) * (1.0 + 1e-12);
     p->b_u = u; p->b_v = v; p->b_M = M; p->b_C = C;
+    return GAL_OK;
+}
+
+template <typename T>
+int do_bind_obs(gal_plan* p, const T* u, const T* v, const T* re, const T* im, const T* w, int64_t M, int C, void* stream) {
+    if (!re || !im || !w) return GAL_ERR_INVALID_ARGUMENT;
+    if (M >= (int64_t)1 << 32) return GAL_ERR_UNSUPPORTED;                  // 32-bit permutation indices
+    int rc = do_bind_uv<T>(p, u, v, M, C, stream);                        // validates, leaves r_max and the uv binding
+    if (rc) return rc;
+    DeviceGuard g(p->device);
+    const size_t bytes = (size_t)5 * C * M * sizeof(T);
+    if ((rc = grow(p, &p->o_buf, &p->o_bytes, bytes))) { gal_plan_unbind_uv(p); return rc; }
+    if ((rc = launch_bind_sort<T>(p, u, v, re, im, w, M, C, p->b_rmax, (T*)p->o_buf, (cudaStream_t)stream))) {
+        gal_plan_unbind_obs(p);
+        return rc;
+    }
+    p->o_src[0] = u; p->o_src[1] = v; p->o_src[2] = re; p->o_src[3] = im; p->o_src[4] = w;
+    p->o_M = M; p->o_C = C;
     return GAL_OK;
 }
 
@@ -312,6 +350,7 @@ const char* gal_strerror(int code) {
         case GAL_ERR_ALLOC: return "allocation failed";
         case GAL_ERR_CUDA: return "CUDA error (see gal_last_cuda_error)";
         case GAL_ERR_UNSUPPORTED: return "unsupported size";
+        case GAL_ERR_BINDING_VIOLATED: return "a bound (u, v) set changed after gal_plan_bind_uv / gal_plan_bind_obs";
         default: return "unknown error";
     }
 }
@@ -346,6 +385,9 @@ int gal_plan_create(gal_plan** out, int nxy, int batch, int precision_bits, int 
     if ((e = cudaMalloc((void**)&p->ext_full, 16)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     if ((e = cudaMalloc((void**)&p->b_ext_dev, 16)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     if ((e = cudaMalloc((void**)&p->b_r2, 8)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
+    if ((e = cudaHostAlloc((void**)&p->viol_host, sizeof(unsigned int), cudaHostAllocMapped)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
+    *p->viol_host = 0;
+    if ((e = cudaHostGetDevicePointer((void**)&p->viol_dev, p->viol_host, 0)) != cudaSuccess) return fail(GAL_ERR_CUDA, e);
     p->oob = (unsigned long long*)p->call_state;
     p->ext = (int*)((char*)p->call_state + 8);
     {
@@ -387,6 +429,7 @@ int gal_plan_destroy(gal_plan* p) {
     DeviceGuard g(p->device);
     cudaFree(p->spec); cudaFree(p->work); cudaFree(p->tw); cudaFree(p->partials); cudaFree(p->tickets);
     for (cudaEvent_t e : p->tev) cudaEventDestroy(e);
+    cudaFree(p->o_buf); if (p->viol_host) cudaFreeHost(p->viol_host);
     cudaFree(p->call_state); cudaFree(p->call_init); cudaFree(p->ext_full); cudaFree(p->b_ext_dev); cudaFree(p->b_r2); cudaFree(p->st_vis); cudaFree(p->st_image); cudaFree(p->st_pts); cudaFree(p->st_out); cudaFree(p->st_chi2);
     delete p;
     return GAL_OK;
@@ -462,9 +505,14 @@ int gal_get_image_size(const double* u, const double* v, int64_t M, double PB, d
     return GAL_OK;
 }
 
-int gal_plan_unbind_uv(gal_plan* p) {
+int gal_plan_unbind_uv(gal_plan* p) { return gal_plan_unbind_obs(p); }
+
+int gal_plan_unbind_obs(gal_plan* p) {
     if (!p) return GAL_ERR_INVALID_ARGUMENT;
     p->b_u = p->b_v = nullptr; p->b_M = 0; p->b_C = 0; p->b_dxy = 0.0; p->last_bound = false;
+    for (auto& q : p->o_src) q = nullptr;
+    p->o_M = 0; p->o_C = 0; p->last_obs = false;         // (the private copy's memory is kept for the next binding)
+    if (p->viol_host) *(volatile unsigned int*)p->viol_host = 0;
     return GAL_OK;
 }
 
@@ -494,6 +542,10 @@ int64_t gal_last_oob_count(gal_plan* p) {
 #define GAL_DEFINE_PRECISION(SFX, T)                                                                                  \
     int gal_plan_bind_uv_##SFX(gal_plan* p, const T* u, const T* v, int64_t M, int C, void* stream) {                 \
         return do_bind_uv<T>(p, u, v, M, C, stream);                                                                  \
+    }                                                                                                                 \
+    int gal_plan_bind_obs_##SFX(gal_plan* p, const T* u, const T* v, const T* re, const T* im, const T* w, int64_t M, \
+                                int C, void* stream) {                                                                \
+        return do_bind_obs<T>(p, u, v, re, im, w, M, C, stream);                                                      \
     }                                                                                                                 \
     int gal_sweep_##SFX(gal_plan* p, const T* I, int nr, double Rmin, double dR, double dxy, double inc, T* out,      \
                         void* stream) {                                                                               \

@@ -41,6 +41,15 @@ struct gal_plan {
     int* b_ext_dev = nullptr;            // [4]
     unsigned long long* b_r2 = nullptr;  // [1] scratch of the radius kernel
     bool last_bound = false;             // the most recent call used the bound extent
+    // bound observation set (gal_plan_bind_obs): the caller's five arrays (identity of the binding) and the plan's
+    // private copy of them, sorted along a space-filling curve of the uv plane (sort.cuh); o_buf = [5][C][M]
+    const void* o_src[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    int64_t o_M = 0; int o_C = 0;
+    void* o_buf = nullptr; size_t o_bytes = 0;
+    bool last_obs = false;               // the most recent call sampled the private copy
+    // set (from the device, plain store to mapped host memory) by a sampler that found a point outside the extent
+    // of a bound uv set: the promise was broken; the next call returns GAL_ERR_BINDING_VIOLATED
+    unsigned int* viol_host = nullptr; unsigned int* viol_dev = nullptr;
     void* st_vis = nullptr; size_t st_vis_bytes = 0; // summed visibilities of a chi2 multi-source call
     std::set<const void*> smem_set;      // kernels whose dynamic shared-memory limit has been raised
     int max_gx = 0;
@@ -108,6 +117,9 @@ template <typename T> int launch_sample(gal_plan* p, int C, const CallScalars& c
                                         const T* w, int64_t M, T* vis, double* chi2_pc, double* chi2_tot, cudaStream_t st);
 template <typename T> int launch_chi2_from_vis(gal_plan* p, const T* vis, const T* re, const T* im, const T* w, int64_t M,
                                                double* chi2, cudaStream_t st);
+// bind_obs: sort channel by channel, write the five sorted arrays to dst = [5][C][M]
+template <typename T> int launch_bind_sort(gal_plan* p, const T* u, const T* v, const T* re, const T* im, const T* w, int64_t M,
+                                           int C, double rmax, T* dst, cudaStream_t st);
 template <typename T> int launch_uv_radius(gal_plan* p, const T* u, const T* v, long long total, cudaStream_t st);
 
 }  // namespace galb

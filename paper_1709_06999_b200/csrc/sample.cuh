@@ -46,6 +46,7 @@ template <typename T> struct SampleParams {
     const int* ext;           // the extent the transform was pruned to: whole plane = single-copy layout (fft.cuh)
     const int* ext_check;     // extent of a bound uv set to verify every point against, or null
     unsigned long long* viol; // [1]: points whose cell lies outside ext_check
+    unsigned int* viol_flag;  // mapped host memory: set when viol becomes non-zero (sticky, read by the next call)
 };
 
 // Which layout did the column pass write?  Same rule as fft.cuh: extent_is_whole_plane.
@@ -448,7 +449,7 @@ __device__ __forceinline__ void sample_finish(const SampleParams<T>& p, int c, d
                                               unsigned int viol) {
     if (p.ext_check) {                                       // rare: a bound uv set is being verified
         viol = __reduce_add_sync(0xffffffffu, viol);
-        if ((threadIdx.x & 31) == 0 && viol) atomicAdd(p.viol, (unsigned long long)viol);
+        if ((threadIdx.x & 31) == 0 && viol) { atomicAdd(p.viol, (unsigned long long)viol); *(volatile unsigned int*)p.viol_flag = 1u; }
     }
     __shared__ double wsum[32];
     __shared__ unsigned int woob[32];

@@ -2,6 +2,7 @@
 #pragma once
 #include "plan.h"
 #include "sample.cuh"
+#include "sort.cuh"
 
 namespace galb {
 
@@ -63,7 +64,8 @@ int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T
     sp.next_state = (unsigned long long*)((char*)p->call_state + 32 * (p->cur ^ 1));
     sp.viol = (unsigned long long*)((char*)p->oob + 24);
     sp.ext = p->cur_ext;
-    sp.ext_check = (p->last_bound && p->b_ext[0] < p->nxy / 2) ? p->b_ext_dev : nullptr;
+    sp.ext_check = (p->last_bound && !p->last_obs && p->b_ext[0] < p->nxy / 2) ? p->b_ext_dev : nullptr;
+    sp.viol_flag = p->viol_dev;
     // one CTA works through tiles blockIdx.x, blockIdx.x + gridDim.x, ...: a whole number of CTAs per SM
     const int tile = SampleGeom<T, true>::TILE;
     const long long ntiles = (M + tile - 1) / tile;
@@ -115,12 +117,55 @@ int launch_uv_radius(gal_plan* p, const T* u, const T* v, long long total, cudaS
     return GAL_OK;
 }
 
+// gal_plan_bind_obs: Morton keys, three stable 8-bit radix passes over (key, index), gather (sort.cuh).  Bind-time
+// only: temporary buffers are allocated and freed here and the stream is synchronised.
+template <typename T>
+int launch_bind_sort(gal_plan* p, const T* u, const T* v, const T* re, const T* im, const T* w, int64_t M, int C,
+                     double rmax, T* dst, cudaStream_t st) {
+    const int ntiles = (int)((M + SORT_TILE - 1) / SORT_TILE);
+    unsigned int *key[2] = {nullptr, nullptr}, *idx[2] = {nullptr, nullptr}, *hist = nullptr;
+    auto release = [&]() { cudaFree(key[0]); cudaFree(key[1]); cudaFree(idx[0]); cudaFree(idx[1]); cudaFree(hist); };
+    const size_t nb = sizeof(unsigned int) * (size_t)M;
+    cudaError_t e = cudaSuccess;
+    for (int i = 0; i < 2 && e == cudaSuccess; ++i) { e = cudaMalloc(&key[i], nb); if (e == cudaSuccess) e = cudaMalloc(&idx[i], nb); }
+    if (e == cudaSuccess) e = cudaMalloc(&hist, sizeof(unsigned int) * 256 * (size_t)ntiles);
+    if (e != cudaSuccess) { release(); p->last_cuda = (int)e; return GAL_ERR_ALLOC; }
+    const size_t sc_smem = sizeof(unsigned short) * 256 * SORT_STRIDE;
+    e = cudaFuncSetAttribute(radix_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sc_smem);
+    long long gb = (M + 255) / 256;
+    if (gb > (long long)p->sm_count * 8) gb = (long long)p->sm_count * 8;
+    const double inv_rmax = rmax > 0 ? 1.0 / rmax : 0.0;
+    for (int c = 0; c < C && e == cudaSuccess; ++c) {
+        const size_t o = (size_t)c * M;
+        uv_key_kernel<T><<<(unsigned)gb, 256, 0, st>>>(u + o, v + o, M, inv_rmax, key[0], idx[0]);
+        int cur = 0;
+        for (int shift = 0; shift < 24; shift += 8, cur ^= 1) {
+            radix_hist_kernel<<<ntiles, SORT_NT, 0, st>>>(key[cur], M, shift, hist, ntiles);
+            scan_exclusive_kernel<<<1, 1024, 0, st>>>(hist, 256LL * ntiles);
+            radix_scatter_kernel<<<ntiles, SORT_NT, sc_smem, st>>>(key[cur], idx[cur], M, shift, hist, ntiles, key[cur ^ 1],
+                                                                    idx[cur ^ 1]);
+        }
+        T* d = dst + o;
+        const size_t plane = (size_t)C * M;
+        gather_obs_kernel<T><<<(unsigned)gb, 256, 0, st>>>(idx[cur], M, u + o, v + o, re + o, im + o, w + o, d, d + plane,
+                                                           d + 2 * plane, d + 3 * plane, d + 4 * plane);
+        p->launches += 11;
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    release();
+    if (e != cudaSuccess) { p->last_cuda = (int)e; return GAL_ERR_CUDA; }
+    return GAL_OK;
+}
+
 #define GAL_INSTANTIATE_SAMPLE(T)                                                                                      \
     template int launch_extent<T>(gal_plan*, int, const CallScalars&, const T*, const T*, int64_t, cudaStream_t);      \
     template int launch_sample<T>(gal_plan*, int, const CallScalars&, const T*, const T*, const T*, const T*, const T*, \
                                   int64_t, T*, double*, double*, cudaStream_t);                                        \
     template int launch_chi2_from_vis<T>(gal_plan*, const T*, const T*, const T*, const T*, int64_t, double*,          \
                                          cudaStream_t);                                                                \
+    template int launch_bind_sort<T>(gal_plan*, const T*, const T*, const T*, const T*, const T*, int64_t, int, double, T*, \
+                                     cudaStream_t);                                                                    \
     template int launch_uv_radius<T>(gal_plan*, const T*, const T*, long long, cudaStream_t);
 
 }  // namespace galb

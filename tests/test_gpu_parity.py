@@ -421,13 +421,96 @@ def test_bound_uv_set(g):
     n0 = bound.launch_count()
     bound.sampleImage(img, w.dxy, u2, v, w.PA, w.dRA, w.dDec)
     assert bound.launch_count() - n0 == 4 and bound.last_extent_violations() == 0
-    # a broken promise (contents changed in place) is reported
+    # a broken promise (contents changed in place) is reported: by the counter, and loudly by the next call
     u.mul_(1.7)
+    bound.sampleImage(img, w.dxy, u, v, w.PA, w.dRA, w.dDec)
+    assert bound.last_extent_violations() > 0
+    with pytest.raises(g.GalarioError, match="bound"):
+        bound.sampleImage(img, w.dxy, u, v, w.PA, w.dRA, w.dDec)
+    # ... which also dropped the binding: the plan works again, unbound
+    c = bound.sampleImage(img, w.dxy, u, v, w.PA, w.dRA, w.dDec)
+    assert bound.last_extent_violations() == 0 and torch.equal(c, free.sampleImage(img, w.dxy, u, v, w.PA, w.dRA, w.dDec))
+    # an explicit unbind after polling the counter clears the pending error as well
+    bound.bind_uv(u, v)
+    u.mul_(1.3)
     bound.sampleImage(img, w.dxy, u, v, w.PA, w.dRA, w.dDec)
     assert bound.last_extent_violations() > 0
     bound.unbind_uv()
     c = bound.sampleImage(img, w.dxy, u, v, w.PA, w.dRA, w.dDec)
-    assert bound.last_extent_violations() == 0 and torch.equal(c, free.sampleImage(img, w.dxy, u, v, w.PA, w.dRA, w.dDec))
+    assert torch.equal(c, free.sampleImage(img, w.dxy, u, v, w.PA, w.dRA, w.dDec))
+
+
+@pytest.mark.parametrize("idx,kw,dtype", [(2, dict(nxy=1024, M=200_003), torch.float64),
+                                          (3, dict(nxy=2048, M=300_007, n_src=120), torch.float64),
+                                          (3, dict(nxy=2048, M=300_007, n_src=120), torch.float32),
+                                          (0, dict(), torch.float64)])
+def test_bound_observation_set(g, orc, idx, kw, dtype):
+    """gal_plan_bind_obs: chi2 calls on a bound observation set sample the plan's private, uv-sorted copy.  The sum
+    runs over the same points in another order: against the oracle at the chi2 tolerance, bit-identical from call to
+    call and from binding to binding (the permutation is unique), three launches per call, no uv-extent kernel."""
+    w = W.config(idx, **kw)
+    f32 = dtype == torch.float32
+    if f32:
+        w = w.as_f32()
+    tol = TOL_CHI2_F32 if f32 else TOL_CHI2_F64
+    f = lambda a: np.asarray(a, dtype=np.float64)
+    ref, roob = orc.sampleImage(f(w.image), w.dxy, f(w.u), f(w.v), w.PA, w.dRA, w.dDec, nthreads=threads(orc), return_oob=True)
+    ref_chi2 = orc.chi2(ref, f(w.re_obs), f(w.im_obs), f(w.w))
+    plan = g.Plan(w.nxy, 1, dtype)
+    img, u, v, re, im, wt = (dev(a) for a in (w.image, w.u, w.v, w.re_obs, w.im_obs, w.w))
+    plan.bind_obs(u, v, re, im, wt)
+    n0 = plan.launch_count()
+    a = float(plan.chi2Image(img, w.dxy, u, v, re, im, wt, w.dRA, w.dDec, w.PA).cpu()[0])
+    assert plan.launch_count() - n0 == 3
+    assert plan.last_oob_count() == roob
+    assert abs(a - ref_chi2) <= tol * abs(ref_chi2)
+    b = float(plan.chi2Image(img, w.dxy, u, v, re, im, wt, w.dRA, w.dDec, w.PA).cpu()[0])
+    plan.bind_obs(u, v, re, im, wt)
+    c = float(plan.chi2Image(img, w.dxy, u, v, re, im, wt, w.dRA, w.dDec, w.PA).cpu()[0])
+    assert a == b == c
+    # another PA and offset on the same binding (the sort is rotation-agnostic)
+    ref2 = orc.sampleImage(f(w.image), w.dxy, f(w.u), f(w.v), w.PA + 1.0, -w.dRA, 2 * w.dDec, nthreads=threads(orc))
+    d = float(plan.chi2Image(img, w.dxy, u, v, re, im, wt, -w.dRA, 2 * w.dDec, w.PA + 1.0).cpu()[0])
+    r2 = orc.chi2(ref2, f(w.re_obs), f(w.im_obs), f(w.w))
+    assert abs(d - r2) <= tol * abs(r2)
+    # sampleImage on the bound (u, v) keeps the caller's order
+    vis = plan.sampleImage(img, w.dxy, u, v, w.PA, w.dRA, w.dDec).cpu().numpy()
+    if f32:
+        assert np.abs(vis - ref).max() <= TOL_VIS_F32 * np.abs(ref).max()
+    else:
+        assert rel_err(vis, ref) <= TOL_VIS_F64
+    # other observation pointers: the (u, v) binding still applies, the private copy does not
+    re2 = re.clone()
+    e = float(plan.chi2Image(img, w.dxy, u, v, re2, im, wt, w.dRA, w.dDec, w.PA).cpu()[0])
+    assert abs(e - ref_chi2) <= tol * abs(ref_chi2)
+    # the copy is private: changing the caller's arrays has no effect until the set is bound again
+    re.add_(1.0)
+    assert float(plan.chi2Image(img, w.dxy, u, v, re, im, wt, w.dRA, w.dDec, w.PA).cpu()[0]) == a
+    plan.unbind_obs()
+    changed = float(plan.chi2Image(img, w.dxy, u, v, re, im, wt, w.dRA, w.dDec, w.PA).cpu()[0])
+    rc = orc.chi2(ref, f(w.re_obs) + 1.0, f(w.im_obs), f(w.w))
+    assert abs(changed - rc) <= tol * abs(rc)
+
+
+def test_bound_observation_set_batch_and_profile(g, orc):
+    w = W.config(4, nxy=256, M=20_000, C=5)
+    plan = g.Plan(w.nxy, 5)
+    img, u, v, re, im, wt = (dev(a) for a in (w.image, w.u, w.v, w.re_obs, w.im_obs, w.w))
+    plan.bind_obs(u, v, re, im, wt)
+    per, tot = plan.chi2ImageBatch(img, w.dxy, u, v, re, im, wt, w.dRA, w.dDec, w.PA)
+    rper, rtot, roob = orc.chi2ImageBatch(w.image, w.dxy, w.u, w.v, w.re_obs, w.im_obs, w.w, w.dRA, w.dDec, w.PA,
+                                          nthreads=threads(orc), return_oob=True)
+    assert (np.abs(per.cpu().numpy() - rper) <= TOL_CHI2_F64 * np.abs(rper)).all()
+    assert abs(float(tot.cpu()[0]) - rtot) <= TOL_CHI2_F64 * abs(rtot)
+    assert plan.last_oob_count() == roob
+    w1 = W.config(1, nxy=512, M=50_001, nr=1000)
+    p1 = g.Plan(w1.nxy)
+    prof, u, v, re, im, wt = (dev(a) for a in (w1.profile, w1.u, w1.v, w1.re_obs, w1.im_obs, w1.w))
+    p1.bind_obs(u, v, re, im, wt)
+    c = float(p1.chi2Profile(prof, w1.Rmin, w1.dR, w1.dxy, u, v, re, im, wt, w1.dRA, w1.dDec, w1.PA, w1.inc).cpu()[0])
+    r = orc.chi2Profile(w1.profile, w1.Rmin, w1.dR, w1.nxy, w1.dxy, w1.u, w1.v, w1.re_obs, w1.im_obs, w1.w, w1.dRA,
+                        w1.dDec, w1.PA, w1.inc, nthreads=threads(orc))
+    assert abs(c - r) <= TOL_CHI2_F64 * abs(r)
 
 
 @pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
