@@ -173,3 +173,28 @@ def chi2ImageBatch(images, dxy, u, v, re_obs, im_obs, w, dRA=0.0, dDec=0.0, PA=0
                                       ctypes.c_double(dRA), ctypes.c_double(dDec), ctypes.c_double(PA), _p(per),
                                       ctypes.byref(tot), ctypes.byref(oob), ctypes.c_int(nthreads)), "chi2ImageBatch")
     return (per, tot.value, oob.value) if return_oob else (per, tot.value)
+
+
+def sampleProfileHankel(I, Rmin, dR, u, v, inc=0.0, PA=0.0, dRA=0.0, dDec=0.0, nthreads: int = 1):
+    """Direct Hankel-transform evaluation of Eq. 25 on the profile grid; no image, no FFT."""
+    I, u, v = _f64(I), _f64(u), _f64(v)
+    M = u.size
+    vis = np.empty(M, dtype=np.complex128)
+    _check(lib().orc_sample_profile_hankel(_p(I), ctypes.c_int(I.size), ctypes.c_double(Rmin), ctypes.c_double(dR),
+                                           _p(u), _p(v), ctypes.c_int64(M), ctypes.c_double(dRA),
+                                           ctypes.c_double(dDec), ctypes.c_double(PA), ctypes.c_double(inc),
+                                           vis.ctypes.data_as(_c_double_p), ctypes.c_int(nthreads)),
+           "sampleProfileHankel")
+    return vis
+
+
+def chi2ProfileHankel(I, Rmin, dR, u, v, re_obs, im_obs, w, dRA=0.0, dDec=0.0, PA=0.0, inc=0.0,
+                      nthreads: int = 1) -> float:
+    I, u, v, re_obs, im_obs, w = _f64(I), _f64(u), _f64(v), _f64(re_obs), _f64(im_obs), _f64(w)
+    out = ctypes.c_double(0.0)
+    _check(lib().orc_chi2_profile_hankel(_p(I), ctypes.c_int(I.size), ctypes.c_double(Rmin), ctypes.c_double(dR),
+                                         _p(u), _p(v), _p(re_obs), _p(im_obs), _p(w), ctypes.c_int64(u.size),
+                                         ctypes.c_double(dRA), ctypes.c_double(dDec), ctypes.c_double(PA),
+                                         ctypes.c_double(inc), ctypes.byref(out), ctypes.c_int(nthreads)),
+           "chi2ProfileHankel")
+    return out.value

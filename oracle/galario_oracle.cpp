@@ -15,7 +15,9 @@
 // Pins (tests/test_oracle_*.py, run with -m "not gpu"): brute-force sky-coordinate DFT
 // at nxy <= 64, the Appendix-D listing re-run with numpy.fft + scipy, delta-source and
 // Gaussian closed forms, Hermitian symmetry, Parseval, PA = 90 deg identity, chi2
-// invariants, scipy.interp1d for the sweep.  No function here is "parity unpinned".
+// invariants, scipy.interp1d for the sweep; the Hankel evaluation (H1) by the Gaussian and uniform-disc
+// closed forms, an elliptical Gaussian (inclination, PA), scipy quadrature and the paper's own 1e-5
+// agreement with sampleProfile.  No function here is "parity unpinned".
 //
 // Build: g++ -O2 -ffp-contract=off -std=c++17 -shared -fPIC -pthread galario_oracle.cpp -o liboracle.so
 //
@@ -287,6 +289,50 @@ int sweep_T(const double* I, int nr, double Rmin_, double dR_, int N, double dxy
     return 0;
 }
 
+// ---------------------------------------------------------------------------------------
+// H1: direct Hankel-transform evaluation of an axisymmetric profile (Eq. 25)
+//       V(rho) = 2 pi int_0^inf I(r) J0(2 pi rho r) r dr,   rho = deprojected uv distance,
+// the analytic result the paper checks sampleProfile against, offered as an
+// alternative to sweep + FFT + interpolation for axisymmetric models.
+// Readings (A20): the profile is the one the sweep uses — samples I[k] at
+// R_k = Rmin + k dR, zero outside [Rmin, Rmax]; the integral is the
+// composite trapezoid rule on that grid; the sweep stretches the East-West axis by 1/cos inc
+// (PAPER.md:740), so by the scaling theorem the transform is cos(inc) V(rho) at
+// rho = sqrt((u' cos inc)^2 + v'^2); (u', v') and the phase follow the listing
+// exactly as in sample_spectrum_T.  J0 is the standard library's
+// std::cyl_bessel_j(0, x).  The result is real before the phase factor.
+// ---------------------------------------------------------------------------------------
+int hankel_sample(const double* I, int nr, double Rmin, double dR, const double* u, const double* v, int64_t M,
+                  double dRA, double dDec, double PA, double inc, double* vis, int nthreads) {
+    if (!I || nr < 2 || !(dR > 0) || M < 0 || (M > 0 && (!u || !v || !vis))) return -1;
+    const double inc_cos = std::cos(inc);
+    if (!(inc_cos > 0)) return -1;
+    const double pi = Pi<double>::v();
+    const double cos_PA = std::cos(PA), sin_PA = std::sin(PA);
+    dRA *= 2 * pi;
+    dDec *= 2 * pi;
+    const double dRArot = dRA * cos_PA - dDec * sin_PA;
+    const double dDecrot = dRA * sin_PA + dDec * cos_PA;
+    parallel_chunks(M, nthreads, [&](int, int64_t b, int64_t e) {
+        for (int64_t k = b; k < e; ++k) {
+            const double urot = u[k] * cos_PA - v[k] * sin_PA;
+            const double vrot = u[k] * sin_PA + v[k] * cos_PA;
+            const double rho = std::sqrt((urot * inc_cos) * (urot * inc_cos) + vrot * vrot);
+            long double acc = 0;
+            for (int j = 0; j < nr; ++j) {
+                const double r = Rmin + dR * (double)j;
+                const double term = I[j] * std::cyl_bessel_j(0.0, 2 * pi * rho * r) * r;
+                acc += (j == 0 || j == nr - 1) ? 0.5L * term : (long double)term;
+            }
+            const double V = 2 * pi * inc_cos * dR * (double)acc;
+            const double theta = urot * dRArot + vrot * dDecrot;
+            vis[2 * k] = V * std::cos(theta);
+            vis[2 * k + 1] = V * std::sin(theta);
+        }
+    });
+    return 0;
+}
+
 }  // namespace
 
 // =========================================================================================
@@ -402,6 +448,24 @@ int orc_chi2_image_batch(const double* images, int C, int nxy, double dxy, const
     }
     if (chi2_total) *chi2_total = (double)tot;
     if (oob) *oob = oob_all;
+    return 0;
+}
+
+// H1.  sampleProfile by the direct Hankel transform of Eq. 25; vis[2M] interleaved.
+int orc_sample_profile_hankel(const double* I, int nr, double Rmin, double dR, const double* u, const double* v,
+                              int64_t M, double dRA, double dDec, double PA, double inc, double* vis, int nthreads) {
+    return hankel_sample(I, nr, Rmin, dR, u, v, M, dRA, dDec, PA, inc, vis, nthreads);
+}
+
+// chi2Profile by the same evaluation = H1 then O8.
+int orc_chi2_profile_hankel(const double* I, int nr, double Rmin, double dR, const double* u, const double* v,
+                            const double* re_obs, const double* im_obs, const double* w, int64_t M, double dRA,
+                            double dDec, double PA, double inc, double* chi2, int nthreads) {
+    if (!chi2 || M < 0) return -1;
+    std::vector<double> vis((size_t)2 * std::max<int64_t>(M, 1));
+    int rc = hankel_sample(I, nr, Rmin, dR, u, v, M, dRA, dDec, PA, inc, vis.data(), nthreads);
+    if (rc) return rc;
+    *chi2 = chi2_of(vis.data(), re_obs, im_obs, w, M, nthreads);
     return 0;
 }
 
