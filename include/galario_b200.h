@@ -187,6 +187,31 @@ int gal_chi2_profile_f32(gal_plan* plan, const float* I, int nr, double Rmin, do
                          const float* w, int64_t M, double dRA, double dDec, double PA, double inc,
                          double* chi2_out, void* stream);
 
+/* ---- sampleProfile / chi2Profile by the DIRECT HANKEL TRANSFORM of the profile (Eq. 25:
+ *      V(rho) = 2 pi int I(r) J0(2 pi rho r) r dr, the analytic result the paper validates sampleProfile against,
+ *      PAPER.md:370-404).  An alternative evaluation for axisymmetric models: no image, no
+ *      FFT, no interpolation error; cost O(M nr).  Composite trapezoid rule on the profile grid R_k = Rmin + k dR
+ *      (profile zero outside, as in the sweep); inclination as in the sweep (East-West axis
+ *      stretched by 1/cos inc): V = cos(inc) V(rho), rho = sqrt((u' cos inc)^2 + v'^2) with (u', v')
+ *      rotated by PA; phase exp(+2 pi i (u dRA + v dDec)).  There is no dxy and no nxy: the plan only lends its
+ *      reduction scratch.  Agrees with gal_sample_profile_* to the FFT route's own accuracy (1e-5 of the peak at
+ *      the nodes of the uv grid; the bilinear interpolation error elsewhere).  Arguments as gal_sample_profile_* /
+ *      gal_chi2_profile_* without dxy. ---- */
+int gal_sample_profile_hankel_f64(gal_plan* plan, const double* I, int nr, double Rmin, double dR, const double* u,
+                                  const double* v, int64_t M, double dRA, double dDec, double PA, double inc,
+                                  double* vis_out, void* stream);
+int gal_sample_profile_hankel_f32(gal_plan* plan, const float* I, int nr, double Rmin, double dR, const float* u,
+                                  const float* v, int64_t M, double dRA, double dDec, double PA, double inc,
+                                  float* vis_out, void* stream);
+int gal_chi2_profile_hankel_f64(gal_plan* plan, const double* I, int nr, double Rmin, double dR, const double* u,
+                                const double* v, const double* re_obs, const double* im_obs, const double* w,
+                                int64_t M, double dRA, double dDec, double PA, double inc, double* chi2_out,
+                                void* stream);
+int gal_chi2_profile_hankel_f32(gal_plan* plan, const float* I, int nr, double Rmin, double dR, const float* u,
+                                const float* v, const float* re_obs, const float* im_obs, const float* w,
+                                int64_t M, double dRA, double dDec, double PA, double inc, double* chi2_out,
+                                void* stream);
+
 /* ---- batched spectral cube (not in the paper; motivated at PAPER.md:45; reading A17):
  *      C <= plan batch independent chi2Image problems sharing (nxy, dxy, dRA, dDec, PA, M).
  *      images [C][nxy][nxy]; u, v, re_obs, im_obs, w each [C][M]; chi2_per_channel[C] and

@@ -70,6 +70,11 @@ def load_library() -> ctypes.CDLL:
             getattr(lib, f"gal_chi2_image_batch_{s}").argtypes = [_vp, _vp, _i, _d, _vp, _vp, _vp, _vp, _vp, _i64, _d,
                                                                   _d, _d, _vp, _vp, _vp]
         for s in ("f64", "f32"):
+            getattr(lib, f"gal_sample_profile_hankel_{s}").argtypes = [_vp, _vp, _i, _d, _d, _vp, _vp, _i64, _d, _d, _d, _d,
+                                                                       _vp, _vp]
+            getattr(lib, f"gal_chi2_profile_hankel_{s}").argtypes = [_vp, _vp, _i, _d, _d, _vp, _vp, _vp, _vp, _vp, _i64,
+                                                                     _d, _d, _d, _d, _vp, _vp]
+        for s in ("f64", "f32"):
             getattr(lib, f"gal_sample_image_multi_{s}").argtypes = [_vp, _vp, _d, _vp, _vp, _i64, _i, _vp, _vp, _vp, _vp,
                                                                     _vp, _vp]
             getattr(lib, f"gal_chi2_image_multi_{s}").argtypes = [_vp, _vp, _d, _vp, _vp, _vp, _vp, _vp, _i64, _i, _vp,
@@ -263,6 +268,23 @@ class Plan:
                                         self._dev(v, "v"), self._dev(re_obs, "re_obs"), self._dev(im_obs, "im_obs"),
                                         self._dev(w, "w"), u.numel(), dRA, dDec, PA, inc, out.data_ptr(), _stream()),
                "gal_chi2_profile", self)
+        return out
+
+    def sampleProfileHankel(self, I, Rmin, dR, u, v, inc=0.0, PA=0.0, dRA=0.0, dDec=0.0, out=None):
+        """sampleProfile by the direct Hankel transform of Eq. 25 (no image, no FFT)."""
+        M = u.numel()
+        out = torch.empty(M, dtype=self._cdtype, device=u.device) if out is None else out
+        _check(self._fn("sample_profile_hankel")(self._h, self._dev(I, "I"), I.numel(), Rmin, dR, self._dev(u, "u"),
+                                                 self._dev(v, "v"), M, dRA, dDec, PA, inc, out.data_ptr(), _stream()),
+               "gal_sample_profile_hankel", self)
+        return out
+
+    def chi2ProfileHankel(self, I, Rmin, dR, u, v, re_obs, im_obs, w, dRA=0.0, dDec=0.0, PA=0.0, inc=0.0, out=None):
+        out = torch.empty(1, dtype=torch.float64, device=u.device) if out is None else out
+        _check(self._fn("chi2_profile_hankel")(self._h, self._dev(I, "I"), I.numel(), Rmin, dR, self._dev(u, "u"),
+                                               self._dev(v, "v"), self._dev(re_obs, "re_obs"),
+                                               self._dev(im_obs, "im_obs"), self._dev(w, "w"), u.numel(), dRA, dDec,
+                                               PA, inc, out.data_ptr(), _stream()), "gal_chi2_profile_hankel", self)
         return out
 
     def chi2ImageBatch(self, images, dxy, u, v, re_obs, im_obs, w, dRA=0.0, dDec=0.0, PA=0.0, out=None):

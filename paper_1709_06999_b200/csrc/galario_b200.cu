@@ -176,6 +176,29 @@ int do_sample_image(gal_plan* p, const T* image, const SweepParams* sw, int C, d
     return run_call<T>(p, image, sw, C, dxy, u, v, re, im, w, M, dRA, dDec, PA, vis, chi2_pc, chi2_tot, st);
 }
 
+// sampleProfile / chi2Profile by the direct Hankel transform (hankel.cuh): one kernel, no transform, nxy unused.
+template <typename T>
+int do_hankel(gal_plan* p, const T* I, int nr, double Rmin, double dR, const T* u, const T* v, const T* re, const T* im,
+              const T* w, int64_t M, double dRA, double dDec, double PA, double inc, T* vis, double* chi2, void* stream) {
+    SweepParams sw;
+    if (!prec_ok<T>(p) || M < 0 || !sweep_args(p, I, nr, Rmin, dR, 1.0, inc, &sw)) return GAL_ERR_INVALID_ARGUMENT;
+    if (!vis && !chi2) return GAL_ERR_INVALID_ARGUMENT;
+    if (M > 0 && (!u || !v || (!vis && (!re || !im || !w)))) return GAL_ERR_INVALID_ARGUMENT;
+    if (!std::isfinite(dRA) || !std::isfinite(dDec) || !std::isfinite(PA)) return GAL_ERR_INVALID_ARGUMENT;
+    DeviceGuard g(p->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    p->last_stream = st;
+    if (M == 0) {
+        if (chi2) GAL_CUDA(p, cudaMemsetAsync(chi2, 0, sizeof(double), st));
+        return GAL_OK;
+    }
+    int rc;
+    if ((rc = reset_call_state(p, st))) return rc;
+    p->last_pruned = false; p->last_bound = false; p->last_obs = false;
+    const CallScalars cs = call_scalars(p, 1.0 / p->nxy, dRA, dDec, PA);      // only the rotation and the phase are used
+    return launch_hankel<T>(p, sw, cs, u, v, re, im, w, M, vis, vis ? nullptr : chi2, st);
+}
+
 template <typename T>
 int do_sweep(gal_plan* p, const T* I, int nr, double Rmin, double dR, double dxy, double inc, T* out, void* stream) {
     SweepParams sw;
@@ -584,6 +607,19 @@ int64_t gal_last_oob_count(gal_plan* p) {
         if (!sweep_args(p, I, nr, Rmin, dR, dxy, inc, &sw) || !chi2) return GAL_ERR_INVALID_ARGUMENT;                 \
         return do_sample_image<T>(p, nullptr, &sw, 1, dxy, u, v, re, im, w, M, dRA, dDec, PA, nullptr, chi2, nullptr, \
                                   stream);                                                                            \
+    }                                                                                                                 \
+    int gal_sample_profile_hankel_##SFX(gal_plan* p, const T* I, int nr, double Rmin, double dR, const T* u, const T* v,  \
+                                        int64_t M, double dRA, double dDec, double PA, double inc, T* vis, void* stream) { \
+        if (M > 0 && !vis) return GAL_ERR_INVALID_ARGUMENT;                                                           \
+        if (M == 0) return GAL_OK;                                                                                    \
+        return do_hankel<T>(p, I, nr, Rmin, dR, u, v, nullptr, nullptr, nullptr, M, dRA, dDec, PA, inc, vis, nullptr,  \
+                            stream);                                                                                  \
+    }                                                                                                                 \
+    int gal_chi2_profile_hankel_##SFX(gal_plan* p, const T* I, int nr, double Rmin, double dR, const T* u, const T* v, \
+                                      const T* re, const T* im, const T* w, int64_t M, double dRA, double dDec,       \
+                                      double PA, double inc, double* chi2, void* stream) {                            \
+        if (!chi2) return GAL_ERR_INVALID_ARGUMENT;                                                                   \
+        return do_hankel<T>(p, I, nr, Rmin, dR, u, v, re, im, w, M, dRA, dDec, PA, inc, nullptr, chi2, stream);       \
     }                                                                                                                 \
     int gal_chi2_image_batch_##SFX(gal_plan* p, const T* images, int C, double dxy, const T* u, const T* v,           \
                                    const T* re, const T* im, const T* w, int64_t M, double dRA, double dDec,          \

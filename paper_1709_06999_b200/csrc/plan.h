@@ -120,6 +120,8 @@ template <typename T> int launch_chi2_from_vis(gal_plan* p, const T* vis, const 
 // bind_obs: sort channel by channel, write the five sorted arrays to dst = [5][C][M]
 template <typename T> int launch_bind_sort(gal_plan* p, const T* u, const T* v, const T* re, const T* im, const T* w, int64_t M,
                                            int C, double rmax, T* dst, cudaStream_t st);
+template <typename T> int launch_hankel(gal_plan* p, const SweepParams& sw, const CallScalars& cs, const T* u, const T* v, const T* re,
+                                        const T* im, const T* w, int64_t M, T* vis, double* chi2, cudaStream_t st);
 template <typename T> int launch_uv_radius(gal_plan* p, const T* u, const T* v, long long total, cudaStream_t st);
 
 }  // namespace galb

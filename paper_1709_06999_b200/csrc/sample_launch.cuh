@@ -3,6 +3,7 @@
 #include "plan.h"
 #include "sample.cuh"
 #include "sort.cuh"
+#include "hankel.cuh"
 
 namespace galb {
 
@@ -158,6 +159,30 @@ int launch_bind_sort(gal_plan* p, const T* u, const T* v, const T* re, const T* 
     return GAL_OK;
 }
 
+// Direct Hankel evaluation (hankel.cuh): one warp per point, eight warps per CTA.
+template <typename T>
+int launch_hankel(gal_plan* p, const SweepParams& sw, const CallScalars& cs, const T* u, const T* v, const T* re, const T* im,
+                  const T* w, int64_t M, T* vis, double* chi2, cudaStream_t st) {
+    HankelParams h;
+    h.I = sw.I; h.nr = sw.nr; h.Rmin = sw.Rmin; h.dR = sw.dR; h.inc_cos = sw.inc_cos;
+    h.cos_PA = cs.ix.cos_PA; h.sin_PA = cs.ix.sin_PA; h.dRA_turns = cs.dRA_turns; h.dDec_turns = cs.dDec_turns;
+    h.has_phase = cs.has_phase;
+    SampleParams<T> sp = {};
+    sp.N = p->nxy; sp.M = M; sp.u = u; sp.v = v; sp.re_obs = re; sp.im_obs = im; sp.w = w; sp.vis = vis;
+    sp.partials = p->partials; sp.tickets = p->tickets; sp.chi2_per_channel = chi2; sp.chi2_total = nullptr;
+    sp.oob = p->oob; sp.done = (unsigned int*)((char*)p->oob + 20);
+    sp.next_state = (unsigned long long*)((char*)p->call_state + 32 * (p->cur ^ 1));
+    sp.viol = (unsigned long long*)((char*)p->oob + 24); sp.ext_check = nullptr; sp.viol_flag = p->viol_dev;
+    long long blocks = (M + 7) / 8;
+    if (blocks > p->max_gx) blocks = p->max_gx;
+    if (vis) GAL_CUDA(p, launch_chain(hankel_kernel<T, true, false>, dim3((unsigned)blocks), dim3(256), 0, st, h, sp));
+    else GAL_CUDA(p, launch_chain(hankel_kernel<T, false, true>, dim3((unsigned)blocks), dim3(256), 0, st, h, sp));
+    p->launches++;
+    GAL_CUDA(p, cudaGetLastError());
+    p->next_armed = true;
+    return GAL_OK;
+}
+
 #define GAL_INSTANTIATE_SAMPLE(T)                                                                                      \
     template int launch_extent<T>(gal_plan*, int, const CallScalars&, const T*, const T*, int64_t, cudaStream_t);      \
     template int launch_sample<T>(gal_plan*, int, const CallScalars&, const T*, const T*, const T*, const T*, const T*, \
@@ -166,6 +191,8 @@ int launch_bind_sort(gal_plan* p, const T* u, const T* v, const T* re, const T* 
                                          cudaStream_t);                                                                \
     template int launch_bind_sort<T>(gal_plan*, const T*, const T*, const T*, const T*, const T*, int64_t, int, double, T*, \
                                      cudaStream_t);                                                                    \
+    template int launch_hankel<T>(gal_plan*, const SweepParams&, const CallScalars&, const T*, const T*, const T*, const T*, \
+                                  const T*, int64_t, T*, double*, cudaStream_t);                                       \
     template int launch_uv_radius<T>(gal_plan*, const T*, const T*, long long, cudaStream_t);
 
 }  // namespace galb
