@@ -297,7 +297,13 @@ def measure_other(g, torch, dev, peak, w3, args):
     w8 = workloads.Workload("n8192", "chi2Image", 8192, w2.dxy * 2048 / 8192, w2.u, w2.v, w2.re_obs, w2.im_obs, w2.w,
                             w2.dRA, w2.dDec, w2.PA, image=rng.random((8192, 8192)))
     add("nxy=8192 f64 chi2Image (cfg-2 uv set, random image)", w8, f64, "chi2Image", 1)
-    del w8, w2
+    del w8
+    # nxy = 16384, the paper's largest size (810 ms per chi2Image on a GTX 1060 with M = 1e6,
+    # copies included; context only)
+    w16 = workloads.Workload("n16384", "chi2Image", 16384, w2.dxy * 2048 / 16384, w2.u, w2.v, w2.re_obs, w2.im_obs,
+                             w2.w, w2.dRA, w2.dDec, w2.PA, image=rng.random((16384, 16384)))
+    add("nxy=16384 f64 chi2Image (cfg-2 uv set, random image)", w16, f64, "chi2Image", 1)
+    del w16, w2
     add("cfg1 f64 chi2Profile", workloads.config(1), f64, "chi2Profile", 1)
     add("cfg0 f64 chi2Image", workloads.config(0), f64, "chi2Image", 1)
     w4 = workloads.config(4)

@@ -27,7 +27,11 @@
  *     profiles in Jy/sr.  dRA > 0 moves the source East, dDec > 0 North, PA is
  *     measured East of North.
  *   - Image layout: row-major [nxy][nxy], row 0 = North, column 0 = East, origin at pixel
- *     [nxy/2][nxy/2].  nxy must be a power of two in [8, 8192].
+ *     [nxy/2][nxy/2].  nxy must be a power of two in [8, 16384] (the paper's range).
+ *   - Alignment: images must be 16-byte aligned, visibility / spectrum outputs aligned to one complex value (16 bytes
+ *     in _f64, 8 in _f32) — the kernels move them as complex pairs and bulk copies; anything else returns
+ *     GAL_ERR_INVALID_ARGUMENT (allocations always qualify; a sub-view at an odd element offset does not).  The
+ *     per-point arrays u, v, re_obs, im_obs, w may have any alignment (16-byte aligned ones take the TMA path).
  *   - Visibilities out: complex interleaved (re, im), 2*M reals.  Observations in:
  *     separate re_obs[M], im_obs[M], w[M].
  *   - (u, v) points whose interpolation cell leaves the half-plane grid are NOT clamped: the spectrum is
@@ -50,7 +54,7 @@ extern "C" {
 #define GAL_ERR_INVALID_ARGUMENT (-1) /* null pointer, bad nxy, M < 0, nr < 2, dR <= 0, dxy <= 0, |inc| >= pi/2, C > plan batch, wrong precision */
 #define GAL_ERR_ALLOC (-2)            /* device or host allocation failed */
 #define GAL_ERR_CUDA (-3)             /* a CUDA call failed; see gal_last_cuda_error() */
-#define GAL_ERR_UNSUPPORTED (-4)      /* valid in the paper but not built here (nxy = 16384) */
+#define GAL_ERR_UNSUPPORTED (-4)      /* a power-of-two nxy above 16384; M >= 2^32 in gal_plan_bind_obs */
 #define GAL_ERR_BINDING_VIOLATED (-5) /* an earlier call found a bound (u, v) set changed: that call's results are invalid; the binding is dropped */
 
 typedef struct gal_plan gal_plan;

@@ -137,10 +137,22 @@ class Plan:
     def _fn(self, name):
         return getattr(self._lib, f"gal_{name}_{self._sfx}")
 
-    def _dev(self, t: torch.Tensor, what: str) -> int:
+    def _dev(self, t: torch.Tensor, what: str, numel: Optional[int] = None) -> int:
         if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == self.dtype and t.is_contiguous()):
             raise GalarioError(f"{what} must be a contiguous CUDA tensor of dtype {self.dtype}")
+        if t.device.index != self.device:
+            raise GalarioError(f"{what} lives on cuda:{t.device.index}, the plan on cuda:{self.device}")
+        if numel is not None and t.numel() != numel:
+            raise GalarioError(f"{what} has {t.numel()} elements, expected {numel}")
         return t.data_ptr()
+
+    def _out(self, out, numel: int, dtype, like: torch.Tensor) -> torch.Tensor:
+        if out is None:
+            return torch.empty(numel, dtype=dtype, device=like.device)
+        if not (isinstance(out, torch.Tensor) and out.is_cuda and out.dtype == dtype and out.is_contiguous()
+                and out.numel() == numel and out.device.index == self.device):
+            raise GalarioError(f"out must be a contiguous cuda:{self.device} tensor of {numel} x {dtype}")
+        return out
 
     def workspace_bytes(self) -> int:
         return int(self._lib.gal_plan_workspace_bytes(self._h))
@@ -229,44 +241,47 @@ class Plan:
     # -- the paper's calls ---------------------------------------------------------------------
     def sweep(self, I, Rmin, dR, dxy, inc=0.0, out=None):
         out = torch.empty((self.nxy, self.nxy), dtype=self.dtype, device=I.device) if out is None else out
-        _check(self._fn("sweep")(self._h, self._dev(I, "I"), I.numel(), Rmin, dR, dxy, inc, self._dev(out, "out"),
+        _check(self._fn("sweep")(self._h, self._dev(I, "I"), I.numel(), Rmin, dR, dxy, inc, self._dev(out, "out", self.nxy ** 2),
                                  _stream()), "gal_sweep", self)
         return out
 
     def fft2_shifted(self, image, out=None):
         if out is None:
             out = torch.empty((self.nxy, self.nxy // 2 + 1), dtype=self._cdtype, device=image.device)
-        _check(self._fn("fft2_shifted")(self._h, self._dev(image, "image"), out.data_ptr(), _stream()),
+        out = self._out(out, self.nxy * (self.nxy // 2 + 1), self._cdtype, image)
+        _check(self._fn("fft2_shifted")(self._h, self._dev(image, "image", self.nxy ** 2), out.data_ptr(), _stream()),
                "gal_fft2_shifted", self)
         return out
 
     def sampleImage(self, image, dxy, u, v, PA=0.0, dRA=0.0, dDec=0.0, out=None):
         M = u.numel()
-        out = torch.empty(M, dtype=self._cdtype, device=u.device) if out is None else out
-        _check(self._fn("sample_image")(self._h, self._dev(image, "image"), dxy, self._dev(u, "u"), self._dev(v, "v"),
+        out = self._out(out, M, self._cdtype, u)
+        _check(self._fn("sample_image")(self._h, self._dev(image, "image", self.nxy ** 2), dxy, self._dev(u, "u"), self._dev(v, "v", M),
                                         M, dRA, dDec, PA, out.data_ptr(), _stream()), "gal_sample_image", self)
         return out
 
     def chi2Image(self, image, dxy, u, v, re_obs, im_obs, w, dRA=0.0, dDec=0.0, PA=0.0, out=None):
-        out = torch.empty(1, dtype=torch.float64, device=u.device) if out is None else out
-        _check(self._fn("chi2_image")(self._h, self._dev(image, "image"), dxy, self._dev(u, "u"), self._dev(v, "v"),
-                                      self._dev(re_obs, "re_obs"), self._dev(im_obs, "im_obs"), self._dev(w, "w"),
-                                      u.numel(), dRA, dDec, PA, out.data_ptr(), _stream()), "gal_chi2_image", self)
+        out = self._out(out, 1, torch.float64, u)
+        M = u.numel()
+        _check(self._fn("chi2_image")(self._h, self._dev(image, "image", self.nxy ** 2), dxy, self._dev(u, "u"), self._dev(v, "v", M),
+                                      self._dev(re_obs, "re_obs", M), self._dev(im_obs, "im_obs", M), self._dev(w, "w", M),
+                                      M, dRA, dDec, PA, out.data_ptr(), _stream()), "gal_chi2_image", self)
         return out
 
     def sampleProfile(self, I, Rmin, dR, dxy, u, v, inc=0.0, PA=0.0, dRA=0.0, dDec=0.0, out=None):
         M = u.numel()
-        out = torch.empty(M, dtype=self._cdtype, device=u.device) if out is None else out
+        out = self._out(out, M, self._cdtype, u)
         _check(self._fn("sample_profile")(self._h, self._dev(I, "I"), I.numel(), Rmin, dR, dxy, self._dev(u, "u"),
-                                          self._dev(v, "v"), M, dRA, dDec, PA, inc, out.data_ptr(), _stream()),
+                                          self._dev(v, "v", M), M, dRA, dDec, PA, inc, out.data_ptr(), _stream()),
                "gal_sample_profile", self)
         return out
 
     def chi2Profile(self, I, Rmin, dR, dxy, u, v, re_obs, im_obs, w, dRA=0.0, dDec=0.0, PA=0.0, inc=0.0, out=None):
-        out = torch.empty(1, dtype=torch.float64, device=u.device) if out is None else out
+        out = self._out(out, 1, torch.float64, u)
+        M = u.numel()
         _check(self._fn("chi2_profile")(self._h, self._dev(I, "I"), I.numel(), Rmin, dR, dxy, self._dev(u, "u"),
-                                        self._dev(v, "v"), self._dev(re_obs, "re_obs"), self._dev(im_obs, "im_obs"),
-                                        self._dev(w, "w"), u.numel(), dRA, dDec, PA, inc, out.data_ptr(), _stream()),
+                                        self._dev(v, "v", M), self._dev(re_obs, "re_obs", M), self._dev(im_obs, "im_obs", M),
+                                        self._dev(w, "w", M), M, dRA, dDec, PA, inc, out.data_ptr(), _stream()),
                "gal_chi2_profile", self)
         return out
 
@@ -290,11 +305,11 @@ class Plan:
     def chi2ImageBatch(self, images, dxy, u, v, re_obs, im_obs, w, dRA=0.0, dDec=0.0, PA=0.0, out=None):
         """images [C][n][n]; u, v, re_obs, im_obs, w [C][M].  Returns (chi2[C], total[1]) on the device."""
         C, M = images.shape[0], u.shape[1]
-        if out is None:
-            out = torch.empty(C + 1, dtype=torch.float64, device=u.device)
-        _check(self._fn("chi2_image_batch")(self._h, self._dev(images, "images"), C, dxy, self._dev(u, "u"),
-                                            self._dev(v, "v"), self._dev(re_obs, "re_obs"), self._dev(im_obs, "im_obs"),
-                                            self._dev(w, "w"), M, dRA, dDec, PA, out.data_ptr(),
+        out = self._out(out, C + 1, torch.float64, u)
+        n = C * M
+        _check(self._fn("chi2_image_batch")(self._h, self._dev(images, "images", C * self.nxy ** 2), C, dxy, self._dev(u, "u", n),
+                                            self._dev(v, "v", n), self._dev(re_obs, "re_obs", n), self._dev(im_obs, "im_obs", n),
+                                            self._dev(w, "w", n), M, dRA, dDec, PA, out.data_ptr(),
                                             out.data_ptr() + 8 * C, _stream()), "gal_chi2_image_batch", self)
         return out[:C], out[C:]
 

@@ -729,6 +729,142 @@ col_pass_x2_kernel(const ColParams<T> p) {
 }
 
 // ------------------------------------------------------------------------------------------
+// nxy = 16384 (the paper's largest size).  A row is 8192 complex numbers (128 KB in fp64), a
+// column 16384 (256 KB): neither fits the three-step transform in one CTA's shared memory.
+//   * Row pass: one row per CTA as two interleaved 4096-point transforms (even / odd samples of the packed
+//     sequence z, the two regions of an F = 2 geometry), one radix-2 combination in place, then the real-FFT
+//     untangle.  It writes image row i to position (i mod 4) N/4 + i / 4 of the u-major work array, i.e. already
+//     DECIMATED BY FOUR for the column transform.
+//   * Column transform N = 4 x 4096 (four-step through global memory):  X[k2 + 4096 k1] =
+//       sum_n1 W_4^(n1 k1) W_N^(n1 k2) Y_n1[k2],   Y_n1 = DFT_4096 of x[n1 + 4 n2] (a contiguous quarter column).
+//     col_sub_kernel transforms one quarter column per CTA in place and applies W_N^(n1 k2); col_comb4_kernel
+//     does the four-point combination and writes the spectrum with the same sign / row folds, layouts and
+//     pruning as col_pass_kernel.  Two extra passes over the reachable columns, nothing else.
+// ------------------------------------------------------------------------------------------
+template <typename T, int R1, int R2, int R3, bool SWEEP>
+__global__ void __launch_bounds__(Geom<T, R1, R2, R3, 2>::NT)
+row_pass_x2_kernel(const RowParams<T> p) {
+    using G = Geom<T, R1, R2, R3, 2>;
+    constexpr int LH = G::L;                   // = N / 4: length of each interleaved transform
+    constexpr int L = 2 * LH;                  // = N / 2: length of the packed complex row
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cx<T>* smem = reinterpret_cast<cx<T>*>(smem_raw);
+    const int tid = threadIdx.x;
+    const int f = tid / G::TPF, t = tid % G::TPF;
+    const int N = p.N;
+    const long long row = blockIdx.x;
+    cx<T>* S = smem + f * G::REGION;
+    pdl_wait();
+    if (SWEEP) {
+        const int i = (int)(row % N);
+        fft_steps12<T, R1, R2, R3, G::TPF>(S, t, p.tw, 4, [&](int m) -> cx<T> {
+            const int n = 2 * m + f;
+            return mk<T>((T)sweep_pixel<T>(p.sweep, N, i, 2 * n), (T)sweep_pixel<T>(p.sweep, N, i, 2 * n + 1));
+        });
+    } else {
+        const cx<T>* z = reinterpret_cast<const cx<T>*>(p.image + row * (long long)N);
+        fft_steps12<T, R1, R2, R3, G::TPF>(S, t, p.tw, 4, [&](int m) -> cx<T> { return __ldcs(z + 2 * m + f); });
+    }
+    if (R3 > 1) {                              // step 3, in place
+        for (int it = t; it < R1 * R2; it += G::TPF) {
+            const int k1 = it % R1, c = it / R1;
+            cx<T>* base = S + k1 * G::P1 + c * R3;
+            cx<T> a[R3];
+#pragma unroll
+            for (int b = 0; b < R3; ++b) a[b] = base[b];
+            Dft<T, R3>::run(a);
+#pragma unroll
+            for (int d = 0; d < R3; ++d) base[d] = a[d];
+        }
+    }
+    __syncthreads();
+    cx<T>* SE = smem;
+    cx<T>* SO = smem + G::REGION;
+    for (int k = tid; k < LH; k += G::NT) {    // Z[k] = E + W_L^k O -> E's slot, Z[k + L/2] = E - W_L^k O -> O's slot
+        const int za = G::zaddr(k);
+        const cx<T> E = SE[za];
+        const cx<T> WO = cmul(__ldg(p.tw + 2 * k), SO[za]);
+        SE[za] = cadd(E, WO);
+        SO[za] = csub(E, WO);
+    }
+    __syncthreads();
+    auto Z = [&](int k) -> cx<T> { return k < LH ? SE[G::zaddr(k)] : SO[G::zaddr(k - LH)]; };
+    const int NU = N / 2 + 1;
+    const int i = (int)(row % N);
+    const int pos = (i & 3) * (N >> 2) + (i >> 2);           // decimated by four for the column transform
+    cx<T>* out = p.spec + (row / N) * (long long)NU * N + pos;
+    const int kumax = __ldg(p.ext);
+    const int kend = kumax < L / 2 ? kumax : L / 2;
+    for (int k = tid; k <= kend; k += G::NT) {               // untangle (factor 1/2 folded into the column pass)
+        const cx<T> zk = Z(k), zm = Z((L - k) % L);
+        const cx<T> E = mk<T>(zk.x + zm.x, zk.y - zm.y);
+        const cx<T> O = mk<T>(zk.y + zm.y, zm.x - zk.x);
+        const cx<T> WO = cmul(__ldg(p.tw + k), O);
+        out[(long long)k * N] = cadd(E, WO);
+        if (L - k <= kumax) { cx<T> xm = csub(E, WO); xm.y = -xm.y; out[(long long)(L - k) * N] = xm; }
+    }
+}
+
+// One quarter column (n1 = blockIdx.x & 3) per CTA: DFT_{N/4} in place, then times W_N^(n1 k2).
+template <typename T, int R1, int R2, int R3>
+__global__ void __launch_bounds__(Geom<T, R1, R2, R3, 1>::NT)
+col_sub_kernel(const ColParams<T> p, cx<T>* __restrict__ work) {
+    using G = Geom<T, R1, R2, R3, 1>;
+    constexpr int LQ = G::L;                   // = N / 4
+    constexpr int N = 4 * LQ, NU = N / 2 + 1;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cx<T>* S = reinterpret_cast<cx<T>*>(smem_raw);
+    const int t = threadIdx.x;
+    pdl_wait();
+    const long long g = blockIdx.x >> 2;
+    const int n1 = blockIdx.x & 3;
+    if ((int)(g % NU) > __ldg(p.ext)) return;
+    cx<T>* q = work + g * (long long)N + (long long)n1 * LQ;
+    fft_steps12<T, R1, R2, R3, G::TPF>(S, t, p.tw, 4, [&](int n) -> cx<T> { return q[n]; });
+    for (int it = t; it < R1 * R2; it += G::TPF) {           // step 3 from shared memory, twiddle, straight to memory
+        const int k1 = it % R1, c = it / R1;
+        const cx<T>* base = S + k1 * G::P1 + c * R3;
+        cx<T> a[R3];
+#pragma unroll
+        for (int b = 0; b < R3; ++b) a[b] = base[b];
+        Dft<T, R3>::run(a);
+#pragma unroll
+        for (int d = 0; d < R3; ++d) {
+            const int k2 = k1 + R1 * (c + R2 * d);
+            q[k2] = n1 ? cmul(a[d], __ldg(p.tw + n1 * k2)) : a[d];
+        }
+    }
+}
+
+// X[k2 + (N/4) k1] = sum_n1 (-i)^(n1 k1) Y_n1[k2]  ->  spectrum (pairs or single copy), sign and row folds, pruned
+template <typename T>
+__global__ void __launch_bounds__(256) col_comb4_kernel(const ColParams<T> p) {
+    const int N = p.N, LQ = N >> 2, NU = N / 2 + 1;
+    pdl_wait();
+    const int kumax = __ldg(p.ext), rmin = __ldg(p.ext + 1), rmax = __ldg(p.ext + 2);
+    const bool single = extent_is_whole_plane(p.ext, N);
+    const long long g = blockIdx.y;
+    const int ku = (int)(g % NU);
+    if (ku > kumax) return;
+    const cx<T>* col = p.work + g * (long long)N;
+    NodePair<T>* own = p.pair + g * (long long)N;
+    NodePair<T>* prev = own - (ku > 0 ? N : 0);
+    cx<T>* sown = reinterpret_cast<cx<T>*>(p.pair) + g * (long long)N;
+    for (int k2 = blockIdx.x * blockDim.x + threadIdx.x; k2 < LQ; k2 += gridDim.x * blockDim.x) {
+        cx<T> a[4] = {col[k2], col[LQ + k2], col[2 * LQ + k2], col[3 * LQ + k2]};
+        Dft<T, 4>::run(a);
+        const T sgn = ((ku + k2) & 1) ? (T)-0.5 : (T)0.5;     // N/4 is even: kv and k2 have one parity
+#pragma unroll
+        for (int k1 = 0; k1 < 4; ++k1) {
+            const int kvs = (k2 + k1 * LQ + N / 2) & (N - 1);
+            if (kvs < rmin || kvs > rmax) continue;
+            const cx<T> val = mk<T>(sgn * a[k1].x, sgn * a[k1].y);
+            if (single) { sown[kvs] = val; } else { own[kvs].a = val; if (ku > 0) prev[kvs].b = val; }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
 // Standalone sweep (image written to memory) and the u-major -> paper-layout transpose.
 // ------------------------------------------------------------------------------------------
 template <typename T>

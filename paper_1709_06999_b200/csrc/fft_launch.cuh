@@ -107,6 +107,39 @@ int launch_col_x2(gal_plan* p, int batch, const int* ext, cudaStream_t st) {
     return GAL_OK;
 }
 
+// nxy = 16384: row pass as two interleaved transforms, column transform four-step through global memory.
+template <typename T>
+int launch_fft_16384(gal_plan* p, const T* image, const SweepParams* sw, int batch, const int* ext, cudaStream_t st) {
+    using GR = Geom<T, 16, 16, 16, 2>;
+    using GC = Geom<T, 16, 16, 16, 1>;
+    RowParams<T> rp;
+    rp.image = image; rp.spec = (cx<T>*)p->work; rp.tw = (const cx<T>*)p->tw; rp.N = p->nxy;
+    rp.rows_total = batch * p->nxy; rp.ext = ext;
+    if (sw) rp.sweep = *sw; else memset(&rp.sweep, 0, sizeof(rp.sweep));
+    int rc;
+    if (sw) {
+        auto k = row_pass_x2_kernel<T, 16, 16, 16, true>;
+        if ((rc = set_smem(p, k, GR::SMEM))) return rc;
+        GAL_CUDA(p, launch_chain(k, dim3((unsigned)rp.rows_total), dim3(GR::NT), GR::SMEM, st, rp));
+    } else {
+        auto k = row_pass_x2_kernel<T, 16, 16, 16, false>;
+        if ((rc = set_smem(p, k, GR::SMEM))) return rc;
+        GAL_CUDA(p, launch_chain(k, dim3((unsigned)rp.rows_total), dim3(GR::NT), GR::SMEM, st, rp));
+    }
+    p->launches++;
+    if (p->t_split) GAL_CUDA(p, cudaEventRecord(p->t_split[2], st));
+    ColParams<T> cp;
+    cp.work = (const cx<T>*)p->work; cp.pair = (NodePair<T>*)p->spec; cp.tw = (const cx<T>*)p->tw; cp.N = p->nxy;
+    cp.cols_total = (long long)batch * (p->nxy / 2 + 1); cp.ext = ext;
+    auto ks = col_sub_kernel<T, 16, 16, 16>;
+    if ((rc = set_smem(p, ks, GC::SMEM))) return rc;
+    GAL_CUDA(p, launch_chain(ks, dim3((unsigned)(4 * cp.cols_total)), dim3(GC::NT), GC::SMEM, st, cp, (cx<T>*)p->work));
+    GAL_CUDA(p, launch_chain(col_comb4_kernel<T>, dim3(4, (unsigned)cp.cols_total), dim3(256), 0, st, cp));
+    p->launches += 2;
+    GAL_CUDA(p, cudaGetLastError());
+    return GAL_OK;
+}
+
 // Groups per CTA and ring slots of the pipelined row pass: fp64 slots are 66 KB (two groups, three slots);
 // fp32 slots are half that (three groups, five slots).
 #ifndef GAL_ROW_NG64
@@ -156,6 +189,8 @@ int fft2(gal_plan* p, const T* image, const SweepParams* sw, int batch, const in
         case 8192:      // column length 8192 = 2 x 4096: two interleaved transforms + one radix-2 combination
             rc = launch_row<T, 16, 16, 16, 1>(p, image, sw, batch, ext, st); if (rc) return rc;
             return launch_col_x2<T, 16, 16, 16>(p, batch, ext, st);
+        case 16384:
+            return launch_fft_16384<T>(p, image, sw, batch, ext, st);
 #undef RR
 #undef GAL_FFT_CASE
         default:

@@ -69,6 +69,25 @@ bool want_prune(const gal_plan* p, int C, int64_t M) {
     return ext_bytes <= 0.25 * 3.0 * spec_bytes;
 }
 
+// Bound uv set: the extent follows from the radius computed once at bind time, for any PA.  The index of a rotated
+// coordinate is at most r_max / du (+ rounding: two cells of margin); rows are symmetric about N/2.  Uploaded once
+// per (binding, dxy).
+int bound_extent(gal_plan* p, const CallScalars& cs, double dxy, cudaStream_t st) {
+    if (p->b_dxy == dxy) return GAL_OK;
+    const int H = p->nxy / 2;
+    const double imax = p->b_rmax / cs.ix.du;
+    int e3[4] = {H, 0, p->nxy - 1, 0};
+    if (imax + 3.0 < (double)(H - 1)) {
+        const int k = (int)imax + 2;
+        e3[0] = k + 1; e3[1] = H - k - 1; e3[2] = H + k + 1;
+    }
+    GAL_CUDA(p, cudaMemcpyAsync(p->b_ext_dev, e3, sizeof(e3), cudaMemcpyHostToDevice, st));
+    GAL_CUDA(p, cudaStreamSynchronize(st));           // e3 is on the stack; once per (binding, dxy)
+    p->b_ext[0] = e3[0]; p->b_ext[1] = e3[1]; p->b_ext[2] = e3[2];
+    p->b_dxy = dxy;
+    return GAL_OK;
+}
+
 // One whole call: [uv extent] -> row pass -> column pass -> sampling, with (diagnostic mode,
 // gal_plan_timing_enable) a CUDA event between the kernels.
 template <typename T>
@@ -96,21 +115,7 @@ int run_call(gal_plan* p, const T* image, const SweepParams* sw, int C, double d
         p->last_obs = true;
     }
     if (p->prune_mode != 0 && uv_bound) {
-        // bound uv set: the extent follows from the radius computed once at bind time, for any PA.  The index of
-        // a rotated coordinate is at most r_max / du (+ rounding: two cells of margin); rows are symmetric about N/2.
-        if (p->b_dxy != dxy) {
-            const int H = p->nxy / 2;
-            const double imax = p->b_rmax / cs.ix.du;
-            int e3[4] = {H, 0, p->nxy - 1, 0};
-            if (imax + 3.0 < (double)(H - 1)) {
-                const int k = (int)imax + 2;
-                e3[0] = k + 1; e3[1] = H - k - 1; e3[2] = H + k + 1;
-            }
-            GAL_CUDA(p, cudaMemcpyAsync(p->b_ext_dev, e3, sizeof(e3), cudaMemcpyHostToDevice, st));
-            GAL_CUDA(p, cudaStreamSynchronize(st));           // e3 is on the stack; once per (binding, dxy)
-            p->b_ext[0] = e3[0]; p->b_ext[1] = e3[1]; p->b_ext[2] = e3[2];
-            p->b_dxy = dxy;
-        }
+        if ((rc = bound_extent(p, cs, dxy, st))) return rc;
         p->last_bound = true;
         p->last_pruned = false;
         ext = p->b_ext_dev;
@@ -134,6 +139,8 @@ int run_call(gal_plan* p, const T* image, const SweepParams* sw, int C, double d
     if (timed) { GAL_CUDA(p, cudaEventRecord(e[4], st)); p->t_calls++; }
     return GAL_OK;
 }
+
+inline bool aligned_to(const void* q, size_t n) { return ((uintptr_t)q % n) == 0; }
 
 template <typename T> bool prec_ok(const gal_plan* p) { return p && p->bits == (int)(8 * sizeof(T)); }
 
@@ -165,6 +172,8 @@ int do_sample_image(gal_plan* p, const T* image, const SweepParams* sw, int C, d
     if (chi2 && (!chi2_pc && !chi2_tot)) return GAL_ERR_INVALID_ARGUMENT;
     if (chi2 && M > 0 && (!re || !im || !w)) return GAL_ERR_INVALID_ARGUMENT;
     if (!std::isfinite(dRA) || !std::isfinite(dDec) || !std::isfinite(PA)) return GAL_ERR_INVALID_ARGUMENT;
+    // the kernels read the image as complex pairs / 16-byte bulk copies and store visibilities as complex values
+    if ((image && !aligned_to(image, 16)) || (vis && !aligned_to(vis, 2 * sizeof(T)))) return GAL_ERR_INVALID_ARGUMENT;
     if (p->viol_host && *(volatile unsigned int*)p->viol_host) {      // an earlier call found the bound uv set changed
         *(volatile unsigned int*)p->viol_host = 0;
         gal_plan_unbind_obs(p);
@@ -184,6 +193,7 @@ int do_hankel(gal_plan* p, const T* I, int nr, double Rmin, double dR, const T* 
     if (!prec_ok<T>(p) || M < 0 || !sweep_args(p, I, nr, Rmin, dR, 1.0, inc, &sw)) return GAL_ERR_INVALID_ARGUMENT;
     if (!vis && !chi2) return GAL_ERR_INVALID_ARGUMENT;
     if (M > 0 && (!u || !v || (!vis && (!re || !im || !w)))) return GAL_ERR_INVALID_ARGUMENT;
+    if (vis && !aligned_to(vis, 2 * sizeof(T))) return GAL_ERR_INVALID_ARGUMENT;
     if (!std::isfinite(dRA) || !std::isfinite(dDec) || !std::isfinite(PA)) return GAL_ERR_INVALID_ARGUMENT;
     DeviceGuard g(p->device);
     cudaStream_t st = (cudaStream_t)stream;
@@ -211,7 +221,7 @@ int do_sweep(gal_plan* p, const T* I, int nr, double Rmin, double dR, double dxy
 
 template <typename T>
 int do_fft2_shifted(gal_plan* p, const T* image, T* out, void* stream) {
-    if (!prec_ok<T>(p) || !image || !out) return GAL_ERR_INVALID_ARGUMENT;
+    if (!prec_ok<T>(p) || !image || !out || !aligned_to(image, 16) || !aligned_to(out, 2 * sizeof(T))) return GAL_ERR_INVALID_ARGUMENT;
     DeviceGuard g(p->device);
     cudaStream_t st = (cudaStream_t)stream;
     p->last_stream = st;
@@ -230,9 +240,11 @@ int grow(gal_plan* p, void** buf, size_t* have, size_t want) {
 }
 
 // Multi-source composition: one model image, S placements
-// (dRA_s, dDec_s, PA_s, scale_s); V = sum_s scale_s V_s by the linearity of the transform.  One FFT (pruned to
-// the union of the sources' uv extents), then one sampling launch per source that adds into vis; for chi2 the sum
-// goes to a plan-owned buffer and a last kernel compares it with the observations.
+// (dRA_s, dDec_s, PA_s, scale_s); V = sum_s scale_s V_s by the linearity of the transform.  One FFT, pruned to the
+// rotation-invariant extent of the point set (its largest baseline length bounds every placement at once: one
+// radius reduction instead of S extent passes; nothing at all on a bound uv set), then ONE sampling launch that
+// loops the placements inside the per-point routine and, for chi2, compares the sum with the observations in the
+// same kernel.  Lists longer than GAL_MULTI_CHUNK placements go chunk by chunk through vis (chi2: a plan-owned sum).
 template <typename T>
 int do_multi(gal_plan* p, const T* image, double dxy, const T* u, const T* v, const T* re, const T* im, const T* w,
              int64_t M, int S, const double* dRA, const double* dDec, const double* PA, const double* scale, T* vis,
@@ -240,9 +252,17 @@ int do_multi(gal_plan* p, const T* image, double dxy, const T* u, const T* v, co
     if (!prec_ok<T>(p) || !image || !(dxy > 0) || M < 0 || S < 1 || S > 4096 || !dRA || !dDec || !PA) return GAL_ERR_INVALID_ARGUMENT;
     if (!vis && !chi2) return GAL_ERR_INVALID_ARGUMENT;
     if (M > 0 && (!u || !v || (chi2 && (!re || !im || !w)))) return GAL_ERR_INVALID_ARGUMENT;
+    if (!aligned_to(image, 16) || (vis && !aligned_to(vis, 2 * sizeof(T)))) return GAL_ERR_INVALID_ARGUMENT;
     for (int s = 0; s < S; ++s)
         if (!std::isfinite(dRA[s]) || !std::isfinite(dDec[s]) || !std::isfinite(PA[s]) || (scale && !std::isfinite(scale[s])))
             return GAL_ERR_INVALID_ARGUMENT;
+    if (S == 1 && (!scale || scale[0] == 1.0))        // a single placement is the plain call (bit for bit)
+        return do_sample_image<T>(p, image, nullptr, 1, dxy, u, v, re, im, w, M, dRA[0], dDec[0], PA[0], vis, chi2, nullptr, stream);
+    if (p->viol_host && *(volatile unsigned int*)p->viol_host) {
+        *(volatile unsigned int*)p->viol_host = 0;
+        gal_plan_unbind_obs(p);
+        return GAL_ERR_BINDING_VIOLATED;
+    }
     DeviceGuard g(p->device);
     cudaStream_t st = (cudaStream_t)stream;
     p->last_stream = st;
@@ -251,29 +271,46 @@ int do_multi(gal_plan* p, const T* image, double dxy, const T* u, const T* v, co
         if (chi2) GAL_CUDA(p, cudaMemsetAsync(chi2, 0, sizeof(double), st));
         return GAL_OK;
     }
-    T* target = vis;
-    if (!vis) {
-        if ((rc = grow(p, &p->st_vis, &p->st_vis_bytes, (size_t)2 * M * sizeof(T)))) return rc;
-        target = (T*)p->st_vis;
-    }
     if ((rc = reset_call_state(p, st))) return rc;
-    std::vector<CallScalars> cs(S);
-    bool prune = want_prune<T>(p, 1, M * S);
-    for (int s = 0; s < S; ++s) { cs[s] = call_scalars(p, dxy, dRA[s], dDec[s], PA[s]); prune = prune && !cs[s].ix.du_exact_div; }
-    p->last_pruned = prune; p->last_bound = false;
+    const CallScalars cs0 = call_scalars(p, dxy, 0.0, 0.0, 0.0);
+    p->last_bound = false; p->last_obs = false;
+    p->last_pruned = want_prune<T>(p, 1, M);
     const int* ext = p->ext_full;
-    if (prune) {                                      // the atomics of the S launches form the union of the extents
-        for (int s = 0; s < S; ++s) if ((rc = launch_extent<T>(p, 1, cs[s], u, v, M, st))) return rc;
+    const bool uv_bound = p->b_u == (const void*)u && p->b_v == (const void*)v && p->b_M == M && p->b_C == 1;
+    if (uv_bound && !vis && p->o_buf && p->o_src[2] == (const void*)re && p->o_src[3] == (const void*)im &&
+        p->o_src[4] == (const void*)w) {              // bound observation set: the private uv-sorted copy
+        const T* o = (const T*)p->o_buf;
+        u = o; v = o + M; re = o + 2 * M; im = o + 3 * M; w = o + 4 * M;
+        p->last_obs = true;
+    }
+    if (p->prune_mode != 0 && uv_bound) {
+        if ((rc = bound_extent(p, cs0, dxy, st))) return rc;
+        p->last_bound = true; p->last_pruned = false;
+        ext = p->b_ext_dev;
+    } else if (p->last_pruned) {
+        if ((rc = launch_extent_radius<T>(p, u, v, M, cs0.ix.du, st))) return rc;
         ext = p->ext;
     }
     p->cur_ext = ext;
     if ((rc = fft2<T>(p, image, nullptr, 1, ext, st))) return rc;
-    for (int s = 0; s < S; ++s) {
-        cs[s].amp = scale ? scale[s] : 1.0;
-        cs[s].accumulate = s > 0;
-        if ((rc = launch_sample<T>(p, 1, cs[s], u, v, nullptr, nullptr, nullptr, M, target, nullptr, nullptr, st))) return rc;
+    T* sum = vis;
+    if (!vis && S > GAL_MULTI_CHUNK) {                // a long list: the running sum of the chunks
+        if ((rc = grow(p, &p->st_vis, &p->st_vis_bytes, (size_t)2 * M * sizeof(T)))) return rc;
+        sum = (T*)p->st_vis;
     }
-    if (!vis) return launch_chi2_from_vis<T>(p, target, re, im, w, M, chi2, st);
+    for (int s0 = 0; s0 < S; s0 += GAL_MULTI_CHUNK) {
+        PlacementSet ps;
+        ps.S = S - s0 < GAL_MULTI_CHUNK ? S - s0 : GAL_MULTI_CHUNK;
+        ps.init_from_vis = s0 > 0;
+        for (int s = 0; s < ps.S; ++s) {
+            const CallScalars c = call_scalars(p, dxy, dRA[s0 + s], dDec[s0 + s], PA[s0 + s]);
+            ps.pl[s] = Placement{c.ix.cos_PA, c.ix.sin_PA, c.dRA_turns, c.dDec_turns, scale ? scale[s0 + s] : 1.0, c.has_phase, 0};
+        }
+        const bool last = s0 + GAL_MULTI_CHUNK >= S;
+        const bool write_vis = vis || !last;
+        if ((rc = launch_sample_multi<T>(p, cs0.ix, ps, u, v, re, im, w, M, sum, write_vis, write_vis ? nullptr : chi2, last, st)))
+            return rc;
+    }
     return GAL_OK;
 }
 
@@ -383,7 +420,7 @@ int gal_plan_create(gal_plan** out, int nxy, int batch, int precision_bits, int 
     *out = nullptr;
     if (!is_pow2(nxy) || nxy < 8 || batch < 1 || (precision_bits != 64 && precision_bits != 32) || device < 0)
         return GAL_ERR_INVALID_ARGUMENT;
-    if (nxy > 8192) return GAL_ERR_UNSUPPORTED;
+    if (nxy > 16384) return GAL_ERR_UNSUPPORTED;
     gal_plan* p = new (std::nothrow) gal_plan();
     if (!p) return GAL_ERR_ALLOC;
     p->nxy = nxy; p->batch = batch; p->bits = precision_bits; p->device = device;

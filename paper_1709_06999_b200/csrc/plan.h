@@ -122,6 +122,10 @@ template <typename T> int launch_bind_sort(gal_plan* p, const T* u, const T* v, 
                                            int C, double rmax, T* dst, cudaStream_t st);
 template <typename T> int launch_hankel(gal_plan* p, const SweepParams& sw, const CallScalars& cs, const T* u, const T* v, const T* re,
                                         const T* im, const T* w, int64_t M, T* vis, double* chi2, cudaStream_t st);
+template <typename T> int launch_sample_multi(gal_plan* p, const IndexScalars& ix, const PlacementSet& ps, const T* u, const T* v,
+                                              const T* re, const T* im, const T* w, int64_t M, T* vis, bool write_vis,
+                                              double* chi2, bool last, cudaStream_t st);
+template <typename T> int launch_extent_radius(gal_plan* p, const T* u, const T* v, int64_t M, double du, cudaStream_t st);
 template <typename T> int launch_uv_radius(gal_plan* p, const T* u, const T* v, long long total, cudaStream_t st);
 
 }  // namespace galb

@@ -46,6 +46,7 @@ template <typename T> struct SampleParams {
     const int* ext;           // the extent the transform was pruned to: whole plane = single-copy layout (fft.cuh)
     const int* ext_check;     // extent of a bound uv set to verify every point against, or null
     unsigned long long* viol; // [1]: points whose cell lies outside ext_check
+    int rearm;                // 1: the last CTA of this launch re-arms next_state (every launch but the non-final chunks of a long multi-source list)
     unsigned int* viol_flag;  // mapped host memory: set when viol becomes non-zero (sticky, read by the next call)
 };
 
@@ -469,11 +470,13 @@ __device__ __forceinline__ void sample_finish(const SampleParams<T>& p, int c, d
         if (ob) atomicAdd(p.oob, (unsigned long long)ob);
         // the last CTA of the launch re-arms the state of the next call: counter 0, extent = the dead-slot cell
         if (atomicAdd(p.done, 1u) == gridDim.x * gridDim.y - 1) {
-            int* nx = reinterpret_cast<int*>(p.next_state);
-            nx[0] = 0; nx[1] = 0;
-            nx[2] = 1; nx[3] = p.N / 2; nx[4] = p.N / 2 + 1;
-            nx[5] = 0;                                          // its own done ticket
-            nx[6] = 0; nx[7] = 0;                               // and its extent-violation counter
+            if (p.rearm) {
+                int* nx = reinterpret_cast<int*>(p.next_state);
+                nx[0] = 0; nx[1] = 0;
+                nx[2] = 1; nx[3] = p.N / 2; nx[4] = p.N / 2 + 1;
+                nx[5] = 0;                                      // its own done ticket
+                nx[6] = 0; nx[7] = 0;                           // and its extent-violation counter
+            }
             *p.done = 0;
         }
         if (DO_CHI2) {
@@ -643,6 +646,98 @@ __global__ void __launch_bounds__(SampleGeom<T, DO_CHI2>::NT_TMA, GAL_SAMPLE_MIN
         if (extent_is_whole(p.ext, p.N)) consume(std::false_type{}); else consume(std::true_type{});
     }
     sample_finish<T, DO_CHI2>(p, c, cx_.acc, cx_.oob, cx_.viol);
+}
+
+// ------------------------------------------------------------------------------------------
+// Multi-source composition in ONE launch ("summing up the visibilities of each single source ...
+// applying a different complex phase"): V(u, v) = sum_s amp_s V_s(u, v; PA_s, dRA_s, dDec_s)
+// of ONE model spectrum.  The per-point arrays are read once, the S placements are looped inside the per-point
+// routine (each one re-rotates the point and gathers its own cell), the sum is compared with the observations
+// in the same kernel: no read-modify-write of vis, no scratch buffer, no second kernel.  One thread per point,
+// plain loads (any alignment); the placements travel in the kernel parameter block.
+// ------------------------------------------------------------------------------------------
+template <typename T, bool PAIR>
+__device__ __forceinline__ void multi_point(const SampleParams<T>& p, const PlacementSet& ps, const NodePair<T>* __restrict__ spec,
+                                            double u, double v, double& vr, double& vi, unsigned int& oob) {
+    const int N = p.N;
+    for (int s = 0; s < ps.S; ++s) {
+        const Placement& pl = ps.pl[s];
+        IndexScalars ix = p.ix;
+        ix.cos_PA = pl.cos_PA; ix.sin_PA = pl.sin_PA;
+        const PointIndex q = point_index<true>(ix, u, v);
+        double re, im;
+        if (cell_inside(ix, q)) {
+            double fx0, fy0;
+            const int ix0 = floor_small(q.uidx, &fx0), iy0 = floor_small(q.vidx, &fy0);
+            const double tx = __dsub_rn(q.uidx, fx0), ty = __dsub_rn(q.vidx, fy0);
+            const int off = ix0 * N + iy0;
+            cx<T> g00, g01, g10, g11;                                         // g[row][column]
+            if (PAIR) {
+                const NodePair<T> e0 = load_pair(spec + off), e1 = load_pair(spec + off + 1);
+                g00 = e0.a; g01 = e0.b; g10 = e1.a; g11 = e1.b;
+            } else {
+                const cx<T>* __restrict__ sg = reinterpret_cast<const cx<T>*>(spec);
+                g00 = __ldg(sg + off); g10 = __ldg(sg + off + 1); g01 = __ldg(sg + off + N); g11 = __ldg(sg + off + N + 1);
+            }
+            const double r0r = fma(tx, (double)g01.x - (double)g00.x, (double)g00.x), r0i = fma(tx, (double)g01.y - (double)g00.y, (double)g00.y);
+            const double r1r = fma(tx, (double)g11.x - (double)g10.x, (double)g10.x), r1i = fma(tx, (double)g11.y - (double)g10.y, (double)g10.y);
+            re = fma(ty, r1r - r0r, r0r);
+            im = fma(ty, r1i - r0i, r0i);
+        } else {                                                              // reading A6
+            if (q.uidx > ix.fH || q.vidx < 0.0 || q.vidx > ix.fN1) ++oob;
+            const cx<double> g = wrapped_cell<T, PAIR>(spec, N, q.uidx, q.vidx);
+            re = g.x; im = g.y;
+        }
+        if (q.uneg) im = -im;
+        if (pl.has_phase) {
+            int qd;
+            const double a = quarter_reduce(fma(q.urot, pl.dRA_turns, q.vrot * pl.dDec_turns), &qd);
+            double sn, co;
+            sincos_quarter(a, qd, &sn, &co);
+            const double t = re * co - im * sn;
+            im = re * sn + im * co;
+            re = t;
+        }
+        vr = fma(pl.amp, re, vr);
+        vi = fma(pl.amp, im, vi);
+    }
+}
+
+template <typename T, bool WRITE_VIS, bool DO_CHI2>
+__global__ void __launch_bounds__(256) sample_multi_kernel(const SampleParams<T> p, const PlacementSet ps) {
+    pdl_wait();
+    const bool single = extent_is_whole(p.ext, p.N);
+    double acc = 0.0;
+    unsigned int oob = 0;
+    cx<T>* vis = reinterpret_cast<cx<T>*>(p.vis);
+    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < p.M; k += (long long)gridDim.x * blockDim.x) {
+        const double u = (double)__ldcs(p.u + k), v = (double)__ldcs(p.v + k);
+        double vr = 0.0, vi = 0.0;
+        if (ps.init_from_vis) { const cx<T> old = vis[k]; vr = (double)old.x; vi = (double)old.y; }
+        if (single) multi_point<T, false>(p, ps, p.spec, u, v, vr, vi, oob);
+        else multi_point<T, true>(p, ps, p.spec, u, v, vr, vi, oob);
+        if (WRITE_VIS) vis[k] = mk<T>((T)vr, (T)vi);
+        if (DO_CHI2) {                                                        // PAPER.md:718 (Eq. 10)
+            const double dr = vr - (double)__ldcs(p.re_obs + k), di = vi - (double)__ldcs(p.im_obs + k);
+            acc = fma(fma(dr, dr, di * di), (double)__ldcs(p.w + k), acc);
+        }
+    }
+    sample_finish<T, DO_CHI2>(p, 0, acc, oob, 0u);
+}
+
+// Extent of a point set under ANY rotation, from its largest baseline length (uv_radius_kernel): the index of a
+// rotated coordinate is at most r_max / du, two cells of margin for the rounding of the listing's arithmetic;
+// rows are symmetric about N/2.  One thread.
+static __global__ void extent_from_radius_kernel(const unsigned long long* __restrict__ r2max_bits, double du, int N, int* ext) {
+    pdl_wait();
+    const double imax = sqrt(__longlong_as_double((long long)*r2max_bits)) * (1.0 + 1e-12) / du;
+    const int H = N / 2;
+    int e0 = H, e1 = 0, e2 = N - 1;
+    if (imax + 3.0 < (double)(H - 1)) {
+        const int k = (int)imax + 2;
+        e0 = k + 1; e1 = H - k - 1; e2 = H + k + 1;
+    }
+    ext[0] = e0; ext[1] = e1; ext[2] = e2;
 }
 
 // chi2 of visibilities that are already in memory (multi-source composition: the sum over the sources has to be

@@ -65,6 +65,7 @@ int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T
     sp.next_state = (unsigned long long*)((char*)p->call_state + 32 * (p->cur ^ 1));
     sp.viol = (unsigned long long*)((char*)p->oob + 24);
     sp.ext = p->cur_ext;
+    sp.rearm = 1;
     sp.ext_check = (p->last_bound && !p->last_obs && p->b_ext[0] < p->nxy / 2) ? p->b_ext_dev : nullptr;
     sp.viol_flag = p->viol_dev;
     // one CTA works through tiles blockIdx.x, blockIdx.x + gridDim.x, ...: a whole number of CTAs per SM
@@ -99,7 +100,7 @@ int launch_chi2_from_vis(gal_plan* p, const T* vis, const T* re, const T* im, co
     sp.partials = p->partials; sp.tickets = p->tickets; sp.chi2_per_channel = chi2; sp.chi2_total = nullptr;
     sp.oob = p->oob; sp.done = (unsigned int*)((char*)p->oob + 20);
     sp.next_state = (unsigned long long*)((char*)p->call_state + 32 * (p->cur ^ 1));
-    sp.viol = (unsigned long long*)((char*)p->oob + 24); sp.ext_check = nullptr;
+    sp.viol = (unsigned long long*)((char*)p->oob + 24); sp.ext_check = nullptr; sp.rearm = 1;
     long long blocks = (M + 1023) / 1024;
     if (blocks > p->max_gx) blocks = p->max_gx;
     GAL_CUDA(p, launch_chain(chi2_from_vis_kernel<T>, dim3((unsigned)blocks), dim3(256), 0, st, sp));
@@ -159,6 +160,40 @@ int launch_bind_sort(gal_plan* p, const T* u, const T* v, const T* re, const T* 
     return GAL_OK;
 }
 
+// Multi-source sampling, one launch per chunk of GAL_MULTI_CHUNK placements (sample.cuh: sample_multi_kernel).
+template <typename T>
+int launch_sample_multi(gal_plan* p, const IndexScalars& ix, const PlacementSet& ps, const T* u, const T* v, const T* re,
+                        const T* im, const T* w, int64_t M, T* vis, bool write_vis, double* chi2, bool last, cudaStream_t st) {
+    SampleParams<T> sp = {};
+    sp.spec = (const NodePair<T>*)p->spec;
+    sp.N = p->nxy; sp.M = M; sp.u = u; sp.v = v; sp.re_obs = re; sp.im_obs = im; sp.w = w; sp.vis = vis; sp.ix = ix;
+    sp.partials = p->partials; sp.tickets = p->tickets; sp.chi2_per_channel = chi2; sp.chi2_total = nullptr;
+    sp.oob = p->oob; sp.done = (unsigned int*)((char*)p->oob + 20);
+    sp.next_state = (unsigned long long*)((char*)p->call_state + 32 * (p->cur ^ 1));
+    sp.viol = (unsigned long long*)((char*)p->oob + 24); sp.ext = p->cur_ext; sp.ext_check = nullptr; sp.viol_flag = p->viol_dev; sp.rearm = last;
+    long long blocks = (M + 255) / 256;
+    const long long cap = (long long)p->sm_count * 6 < p->max_gx ? (long long)p->sm_count * 6 : p->max_gx;
+    if (blocks > cap) blocks = cap;
+    if (write_vis) GAL_CUDA(p, launch_chain(sample_multi_kernel<T, true, false>, dim3((unsigned)blocks), dim3(256), 0, st, sp, ps));
+    else GAL_CUDA(p, launch_chain(sample_multi_kernel<T, false, true>, dim3((unsigned)blocks), dim3(256), 0, st, sp, ps));
+    p->launches++;
+    GAL_CUDA(p, cudaGetLastError());
+    p->next_armed = last;
+    return GAL_OK;
+}
+
+// Rotation-invariant extent on the device: radius reduction, then one thread turns it into {kumax, rmin, rmax}.
+template <typename T>
+int launch_extent_radius(gal_plan* p, const T* u, const T* v, int64_t M, double du, cudaStream_t st) {
+    GAL_CUDA(p, cudaMemsetAsync(p->b_r2, 0, 8, st));
+    int rc = launch_uv_radius<T>(p, u, v, (long long)M, st);
+    if (rc) return rc;
+    extent_from_radius_kernel<<<1, 1, 0, st>>>(p->b_r2, du, p->nxy, p->ext);
+    p->launches++;
+    GAL_CUDA(p, cudaGetLastError());
+    return GAL_OK;
+}
+
 // Direct Hankel evaluation (hankel.cuh): one warp per point, eight warps per CTA.
 template <typename T>
 int launch_hankel(gal_plan* p, const SweepParams& sw, const CallScalars& cs, const T* u, const T* v, const T* re, const T* im,
@@ -172,7 +207,7 @@ int launch_hankel(gal_plan* p, const SweepParams& sw, const CallScalars& cs, con
     sp.partials = p->partials; sp.tickets = p->tickets; sp.chi2_per_channel = chi2; sp.chi2_total = nullptr;
     sp.oob = p->oob; sp.done = (unsigned int*)((char*)p->oob + 20);
     sp.next_state = (unsigned long long*)((char*)p->call_state + 32 * (p->cur ^ 1));
-    sp.viol = (unsigned long long*)((char*)p->oob + 24); sp.ext_check = nullptr; sp.viol_flag = p->viol_dev;
+    sp.viol = (unsigned long long*)((char*)p->oob + 24); sp.ext_check = nullptr; sp.viol_flag = p->viol_dev; sp.rearm = 1;
     long long blocks = (M + 7) / 8;
     if (blocks > p->max_gx) blocks = p->max_gx;
     if (vis) GAL_CUDA(p, launch_chain(hankel_kernel<T, true, false>, dim3((unsigned)blocks), dim3(256), 0, st, h, sp));
@@ -193,6 +228,9 @@ int launch_hankel(gal_plan* p, const SweepParams& sw, const CallScalars& cs, con
                                      cudaStream_t);                                                                    \
     template int launch_hankel<T>(gal_plan*, const SweepParams&, const CallScalars&, const T*, const T*, const T*, const T*, \
                                   const T*, int64_t, T*, double*, cudaStream_t);                                       \
+    template int launch_sample_multi<T>(gal_plan*, const IndexScalars&, const PlacementSet&, const T*, const T*, const T*, \
+                                        const T*, const T*, int64_t, T*, bool, double*, bool, cudaStream_t);           \
+    template int launch_extent_radius<T>(gal_plan*, const T*, const T*, int64_t, double, cudaStream_t);                \
     template int launch_uv_radius<T>(gal_plan*, const T*, const T*, long long, cudaStream_t);
 
 }  // namespace galb

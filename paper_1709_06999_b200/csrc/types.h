@@ -29,4 +29,16 @@ struct CallScalars {
     int accumulate = 0;
 };
 
+// One placement of a multi-source call: rotation, offsets in turns (rotated), flux factor.
+struct Placement {
+    double cos_PA, sin_PA, dRA_turns, dDec_turns, amp;
+    int has_phase, pad;
+};
+constexpr int GAL_MULTI_CHUNK = 16;          // placements per launch (they travel in the kernel parameter block)
+struct PlacementSet {
+    Placement pl[GAL_MULTI_CHUNK];
+    int S;
+    int init_from_vis;                       // start from the sum already in vis (later chunks of a long list)
+};
+
 }  // namespace galb

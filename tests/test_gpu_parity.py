@@ -47,7 +47,7 @@ def threads(orc):
 # ---------------------------------------------------------------------------------------------
 # S2+S3+S4: the transform alone, every supported size (several tiles, both FFT code paths)
 # ---------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("n", [8, 16, 32, 64, 128, 256, 512, 1024, 2048, 4096, 8192])
+@pytest.mark.parametrize("n", [8, 16, 32, 64, 128, 256, 512, 1024, 2048, 4096, 8192, 16384])
 def test_fft2_shifted_matches_oracle_f64(g, orc, n):
     rng = np.random.default_rng(n)
     img = rng.standard_normal((n, n))
@@ -58,7 +58,7 @@ def test_fft2_shifted_matches_oracle_f64(g, orc, n):
     assert np.abs(out - ref).max() <= 1e-12 * np.abs(ref).max()
 
 
-@pytest.mark.parametrize("n", [8, 64, 512, 4096, 8192])
+@pytest.mark.parametrize("n", [8, 64, 512, 4096, 8192, 16384])
 def test_fft2_shifted_matches_oracle_f32(g, orc, n):
     rng = np.random.default_rng(n + 1)
     img = rng.random((n, n)).astype(np.float32)
@@ -617,6 +617,47 @@ def test_multi_source_with_out_of_grid_points(g, orc):
         assert abs(chi2 - ref_chi2) <= TOL_CHI2_F64 * abs(ref_chi2)
 
 
+def test_multi_source_single_launch_long_lists_and_bound_set(g, orc):
+    """The S placements are looped inside ONE sampling launch: launch accounting, a list longer
+    than one chunk of placements (sum carried through vis / a plan-owned sum for chi2), and chi2 on a bound
+    observation set."""
+    w = W.config(2, nxy=512, M=60_007)
+    plan = g.Plan(w.nxy)
+    img, u, v, re, im, wt = (dev(a) for a in (w.image, w.u, w.v, w.re_obs, w.im_obs, w.w))
+    rng = np.random.default_rng(3)
+    mk = lambda S: [(float(a), float(b), float(c), float(d)) for a, b, c, d in
+                    zip(rng.uniform(-3e-7, 3e-7, S), rng.uniform(-3e-7, 3e-7, S), rng.uniform(0, 3.1, S), rng.uniform(0.1, 1.0, S))]
+    for S in (4, 16, 17, 37):
+        places = mk(S)
+        ref, roob = 0.0, 0
+        for dRA, dDec, PA, sc in places:
+            vs, o = orc.sampleImage(w.image, w.dxy, w.u, w.v, PA, dRA, dDec, nthreads=threads(orc), return_oob=True)
+            ref, roob = ref + sc * vs, roob + o
+        ref_chi2 = orc.chi2(ref, w.re_obs, w.im_obs, w.w)
+        n0 = plan.launch_count()
+        vis = plan.sampleImageMulti(img, w.dxy, u, v, places).cpu().numpy()
+        nchunks = (S + 15) // 16
+        assert plan.launch_count() - n0 == 4 + nchunks          # radius, extent, row, column + one launch per chunk
+        assert plan.last_oob_count() == roob
+        assert rel_err(vis, ref) <= TOL_VIS_F64
+        chi2 = float(plan.chi2ImageMulti(img, w.dxy, u, v, re, im, wt, places).cpu()[0])
+        assert abs(chi2 - ref_chi2) <= TOL_CHI2_F64 * abs(ref_chi2)
+    # bound observation set: no extent kernels at all, the private sorted copy is sampled
+    plan.bind_obs(u, v, re, im, wt)
+    n0 = plan.launch_count()
+    b = float(plan.chi2ImageMulti(img, w.dxy, u, v, re, im, wt, places).cpu()[0])
+    assert plan.launch_count() - n0 == 2 + nchunks
+    assert abs(b - ref_chi2) <= TOL_CHI2_F64 * abs(ref_chi2)
+    vis_b = plan.sampleImageMulti(img, w.dxy, u, v, places).cpu().numpy()     # caller's order
+    assert rel_err(vis_b, ref) <= TOL_VIS_F64
+    plan.unbind_obs()
+    # a following plain call finds its per-call state re-armed
+    c = float(plan.chi2Image(img, w.dxy, u, v, re, im, wt, w.dRA, w.dDec, w.PA).cpu()[0])
+    rv, ro = orc.sampleImage(w.image, w.dxy, w.u, w.v, w.PA, w.dRA, w.dDec, nthreads=threads(orc), return_oob=True)
+    r = orc.chi2(rv, w.re_obs, w.im_obs, w.w)
+    assert abs(c - r) <= TOL_CHI2_F64 * abs(r) and plan.last_oob_count() == ro
+
+
 def test_per_call_state_across_calls(g, orc):
     """The out-of-grid counter and the uv extent belong to ONE call: the two device copies of that state are used
     alternately and re-armed by the sampler of the call before (or by an explicit copy after an M = 0 call)."""
@@ -680,7 +721,7 @@ def test_empty_single_and_ragged_M(g, orc):
 
 
 def test_smallest_and_largest_nxy_end_to_end(g, orc):
-    for n, M in ((8, 100), (4096, 1000), (8192, 50_001)):
+    for n, M in ((8, 100), (4096, 1000), (8192, 50_001), (16384, 50_001)):
         rng = np.random.default_rng(n)
         dxy = 0.01 * ARCSEC
         du = 1.0 / (n * dxy)
@@ -706,7 +747,7 @@ def test_error_codes(g):
     assert lib.gal_plan_create(ctypes.byref(h), 100, 1, 64, 0) == -1        # not a power of two
     assert lib.gal_plan_create(ctypes.byref(h), 256, 0, 64, 0) == -1        # batch < 1
     assert lib.gal_plan_create(ctypes.byref(h), 256, 1, 16, 0) == -1        # precision
-    assert lib.gal_plan_create(ctypes.byref(h), 16384, 1, 64, 0) == -4      # unsupported size
+    assert lib.gal_plan_create(ctypes.byref(h), 32768, 1, 64, 0) == -4      # unsupported size
     assert lib.gal_plan_create(None, 256, 1, 64, 0) == -1
     plan = g.Plan(64)
     img = torch.zeros(64, 64, dtype=torch.float64, device="cuda")
@@ -720,6 +761,16 @@ def test_error_codes(g):
     assert bad(1, None) == -1 and bad(3, None) == -1 and bad(7, None) == -1 and bad(12, None) == -1
     assert bad(2, 0.0) == -1 and bad(2, -1.0) == -1 and bad(8, -5) == -1 and bad(9, float("nan")) == -1
     assert lib.gal_chi2_image_f32(*ok) == -1                                 # plan precision mismatch
+    # an image or a visibility buffer at an odd element offset is refused, not faulted on
+    big = torch.zeros(64 * 64 + 1, dtype=torch.float64, device="cuda")
+    assert bad(1, big.data_ptr() + 8) == -1
+    vis = torch.zeros(2 * 10 + 1, dtype=torch.float64, device="cuda")
+    sa = lib.gal_sample_image_f64
+    assert sa(plan._h, img.data_ptr(), 1e-7, x.data_ptr(), x.data_ptr(), 10, 0.0, 0.0, 0.0, vis.data_ptr(), None) == 0
+    assert sa(plan._h, img.data_ptr(), 1e-7, x.data_ptr(), x.data_ptr(), 10, 0.0, 0.0, 0.0, vis.data_ptr() + 8, None) == -1
+    spec = torch.zeros(2 * 64 * 33 + 1, dtype=torch.float64, device="cuda")
+    assert lib.gal_fft2_shifted_f64(plan._h, img.data_ptr(), spec.data_ptr() + 8, None) == -1
+    assert lib.gal_fft2_shifted_f64(plan._h, big.data_ptr() + 8, spec.data_ptr(), None) == -1
     prof = torch.ones(10, dtype=torch.float64, device="cuda")
     sw = lib.gal_sweep_f64
     assert sw(plan._h, prof.data_ptr(), 10, 0.0, 1e-7, 1e-7, 0.0, img.data_ptr(), None) == 0
