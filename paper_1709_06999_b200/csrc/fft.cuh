@@ -379,9 +379,14 @@ __device__ __forceinline__ void group_barrier(int id, int nthreads) {
 }
 __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
-template <typename T, int R1, int R2, int R3, int F, int NG, int NS, bool SWEEP>
-__global__ void __launch_bounds__(RowGeom<T, R1, R2, R3, F>::GT * NG + 32, 1)
+// Where step 1 takes its input from: the TMA ring (persistent CTAs, one per SM), plain global loads (one row block
+// per CTA, several CTAs per SM: no producer warp, no ring), or the swept profile.
+enum RowLoad { ROW_TMA = 0, ROW_DIRECT = 1, ROW_SWEEP = 2 };
+
+template <typename T, int R1, int R2, int R3, int F, int NG, int NS, int MODE>
+__global__ void __launch_bounds__(RowGeom<T, R1, R2, R3, F>::GT * NG + (MODE == ROW_TMA ? 32 : 0), MODE == ROW_TMA ? 1 : 2)
 row_pipe_kernel(const RowParams<T> p) {
+    constexpr bool SWEEP = MODE != ROW_TMA;          // "no ring": inputs do not come through the mbarrier pipeline
     using G = RowGeom<T, R1, R2, R3, F>;
     constexpr int L = G::L, TPF = G::TPF, GT = G::GT, P1 = G::P1, REGION = G::REGION;
     constexpr int N2 = R2 * R3, H1 = R1 / 2, NPAIR = R1 * R2 / 2;
@@ -391,14 +396,16 @@ row_pipe_kernel(const RowParams<T> p) {
     const int tid = threadIdx.x, lane = tid & 31;
     const int N = p.N;
     const long long nblk = p.rows_total / F;                 // F divides nxy: a block never straddles two images
-    if (tid == 0) {
-        for (int s = 0; s < NS; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, GT / 32); }
-        mbar_fence_init();
+    if (MODE == ROW_TMA) {
+        if (tid == 0) {
+            for (int s = 0; s < NS; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, GT / 32); }
+            mbar_fence_init();
+        }
+        __syncthreads();
     }
-    __syncthreads();
 
-    if (tid >= NG * GT) {                                    // ---- producer warp ----
-        if (!SWEEP && lane == 0) {
+    if (MODE == ROW_TMA && tid >= NG * GT) {                 // ---- producer warp ----
+        if (lane == 0) {
             const uint64_t pol = l2_policy_evict_first();
             const uint32_t row_bytes = (uint32_t)N * sizeof(T);
             uint32_t slot = 0, parity = 1;                   // a fresh mbarrier lets a wait on parity 1 through
@@ -437,13 +444,17 @@ row_pipe_kernel(const RowParams<T> p) {
         // step 1: DFT_R1 over n1, twiddle W_L^(n2 k1), n2 = t
         {
             cx<T> a[R1];
-            if (SWEEP) {
+            if (MODE == ROW_SWEEP) {
                 const int i = (int)(row % N);
 #pragma unroll
                 for (int n1 = 0; n1 < R1; ++n1) {
                     const int n = N2 * n1 + t;
                     a[n1] = mk<T>((T)sweep_pixel<T>(p.sweep, N, i, 2 * n), (T)sweep_pixel<T>(p.sweep, N, i, 2 * n + 1));
                 }
+            } else if (MODE == ROW_DIRECT) {
+                const cx<T>* z = reinterpret_cast<const cx<T>*>(p.image + row * (long long)N);
+#pragma unroll
+                for (int n1 = 0; n1 < R1; ++n1) a[n1] = __ldcs(z + N2 * n1 + t);
             } else {
                 mbar_wait(full0 + 8 * slot, par);
 #pragma unroll

@@ -38,9 +38,10 @@ int launch_row(gal_plan* p, const T* image, const SweepParams* sw, int batch, co
     return GAL_OK;
 }
 
-// Pipelined row pass (fft.cuh: row_pipe_kernel): persistent grid, one CTA per SM.
+// Row pass with lane-interleaved rows and the register untangle (fft.cuh: row_pipe_kernel).  tma: persistent grid,
+// one CTA per SM, NG groups and a ring of NS slots; otherwise one row block per CTA and plain loads (or the sweep).
 template <typename T, int R1, int R2, int R3, int F, int NG, int NS>
-int launch_row_pipe(gal_plan* p, const T* image, const SweepParams* sw, int batch, const int* ext, cudaStream_t st) {
+int launch_row_pipe(gal_plan* p, const T* image, const SweepParams* sw, int batch, const int* ext, bool tma, cudaStream_t st) {
     using G = RowGeom<T, R1, R2, R3, F>;
     static_assert(NS >= NG, "one slot per group at least");
     RowParams<T> rp;
@@ -52,17 +53,18 @@ int launch_row_pipe(gal_plan* p, const T* image, const SweepParams* sw, int batc
     rp.ext = ext;
     if (sw) rp.sweep = *sw; else memset(&rp.sweep, 0, sizeof(rp.sweep));
     const long long nblk = rp.rows_total / F;
-    const unsigned grid = (unsigned)(nblk < p->sm_count ? nblk : p->sm_count);
-    const size_t smem = (size_t)NS * G::SLOT_BYTES + 16 * NS;
-    const dim3 block(G::GT * NG + 32);
-    if (sw) {
-        auto k = row_pipe_kernel<T, R1, R2, R3, F, NG, NS, true>;
+    if (!sw && tma) {
+        const unsigned grid = (unsigned)(nblk < p->sm_count ? nblk : p->sm_count);
+        const size_t smem = (size_t)NS * G::SLOT_BYTES + 16 * NS;
+        auto k = row_pipe_kernel<T, R1, R2, R3, F, NG, NS, ROW_TMA>;
         int rc = set_smem(p, k, smem); if (rc) return rc;
-        GAL_CUDA(p, launch_chain(k, dim3(grid), block, smem, st, rp));
+        GAL_CUDA(p, launch_chain(k, dim3(grid), dim3(G::GT * NG + 32), smem, st, rp));
     } else {
-        auto k = row_pipe_kernel<T, R1, R2, R3, F, NG, NS, false>;
+        const size_t smem = (size_t)G::SLOT_BYTES;
+        if (sw) return GAL_ERR_UNSUPPORTED;          // *Profile calls take the plain kernel's sweep loader
+        auto k = row_pipe_kernel<T, R1, R2, R3, F, 1, 1, ROW_DIRECT>;
         int rc = set_smem(p, k, smem); if (rc) return rc;
-        GAL_CUDA(p, launch_chain(k, dim3(grid), block, smem, st, rp));
+        GAL_CUDA(p, launch_chain(k, dim3((unsigned)nblk), dim3(G::GT), smem, st, rp));
     }
     p->launches++;
     GAL_CUDA(p, cudaGetLastError());
@@ -155,8 +157,16 @@ int launch_fft_16384(gal_plan* p, const T* image, const SweepParams* sw, int bat
 #define GAL_ROW_NS32 5
 #endif
 template <typename T> struct RowPipeCfg;
-template <> struct RowPipeCfg<double> { static constexpr int NG = GAL_ROW_NG64, NS = GAL_ROW_NS64; };
-template <> struct RowPipeCfg<float> { static constexpr int NG = GAL_ROW_NG32, NS = GAL_ROW_NS32; };
+// default_mode: which row kernel a size takes when GAL_ROW_PIPE does not say (measured on B200):
+// 0 = plain kernel, 1 = lane-interleaved rows + register untangle with plain loads, 2 = its persistent TMA-ring form.
+template <> struct RowPipeCfg<double> {
+    static constexpr int NG = GAL_ROW_NG64, NS = GAL_ROW_NS64;
+    static int default_mode(int nxy) { return nxy == 4096 ? 1 : 0; }
+};
+template <> struct RowPipeCfg<float> {
+    static constexpr int NG = GAL_ROW_NG32, NS = GAL_ROW_NS32;
+    static int default_mode(int nxy) { return nxy >= 2048 ? 2 : 0; }
+};
 
 // Radix plans.  Row FFT length is nxy/2, column FFT length is nxy.
 template <typename T>
@@ -177,11 +187,13 @@ int fft2(gal_plan* p, const T* image, const SweepParams* sw, int batch, const in
         GAL_FFT_CASE(512, RR(16, 16, 1, 8), RR(8, 8, 8, 4))
         // nxy >= 1024: the pipelined row pass (row_mode 0 keeps the plain one, for comparison)
 #define GAL_FFT_CASE_PIPE(NXY, ROW, PIPE, COL)                                   \
-    case NXY:                                                                    \
-        rc = p->row_mode ? launch_row_pipe<T, PIPE, RowPipeCfg<T>::NG, RowPipeCfg<T>::NS>(p, image, sw, batch, ext, st) \
-                         : launch_row<T, ROW>(p, image, sw, batch, ext, st);     \
+    case NXY: {                                                                  \
+        const int mode = sw ? 0 : (p->row_mode >= 0 ? p->row_mode : RowPipeCfg<T>::default_mode(NXY)); \
+        rc = mode ? launch_row_pipe<T, PIPE, RowPipeCfg<T>::NG, RowPipeCfg<T>::NS>(p, image, sw, batch, ext, mode == 2, st) \
+                  : launch_row<T, ROW>(p, image, sw, batch, ext, st);            \
         if (rc) return rc;                                                       \
-        return launch_col<T, COL>(p, batch, ext, st);
+        return launch_col<T, COL>(p, batch, ext, st);                            \
+    }
         GAL_FFT_CASE_PIPE(1024, RR(8, 8, 8, 4), RR(16, 8, 4, 8), RR(16, 8, 8, 4))
         GAL_FFT_CASE_PIPE(2048, RR(16, 8, 8, 4), RR(16, 8, 8, 4), RR(16, 16, 8, 2))
         GAL_FFT_CASE_PIPE(4096, RR(16, 16, 8, 2), RR(16, 16, 8, 2), RR(16, 16, 16, 1))

@@ -424,7 +424,7 @@ int gal_plan_create(gal_plan** out, int nxy, int batch, int precision_bits, int 
     gal_plan* p = new (std::nothrow) gal_plan();
     if (!p) return GAL_ERR_ALLOC;
     p->nxy = nxy; p->batch = batch; p->bits = precision_bits; p->device = device;
-    if (const char* e = getenv("GAL_ROW_PIPE")) p->row_mode = atoi(e) != 0;    // diagnostic switch
+    if (const char* e = getenv("GAL_ROW_PIPE")) p->row_mode = atoi(e);    // diagnostic switch
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || device >= ndev) { delete p; return GAL_ERR_CUDA; }
     DeviceGuard g(device);

@@ -30,7 +30,7 @@ struct gal_plan {
     int cur = 0;                         // copy used by the most recent call
     bool next_armed = false;             // the other copy has been / will be re-armed by that call's sampler
     int prune_mode = 1;                  // 0 never, 1 auto, 2 always
-    int row_mode = 0;                    // 1: pipelined row pass where built (nxy 1024..4096); 0: the plain one (GAL_ROW_PIPE=0)
+    int row_mode = -1;                   // nxy 1024..4096: -1 per-size default, 0 plain row pass, 1 register-untangle kernel with plain loads, 2 its persistent TMA form (GAL_ROW_PIPE)
     bool last_pruned = false;            // did the most recent call compute a uv extent?
     // bound uv set (gal_plan_bind_uv): addresses, size, the rotation-invariant radius, and the extent derived
     // from it for the pixel size seen last (device copy used by the FFT passes and checked by the sampler)

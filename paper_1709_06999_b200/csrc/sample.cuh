@@ -46,6 +46,7 @@ template <typename T> struct SampleParams {
     const int* ext;           // the extent the transform was pruned to: whole plane = single-copy layout (fft.cuh)
     const int* ext_check;     // extent of a bound uv set to verify every point against, or null
     unsigned long long* viol; // [1]: points whose cell lies outside ext_check
+    int direct;               // 1: every thread gathers its own cell (uv-sorted points of a bound observation set)
     int rearm;                // 1: the last CTA of this launch re-arms next_state (every launch but the non-final chunks of a long multi-source list)
     unsigned int* viol_flag;  // mapped host memory: set when viol becomes non-zero (sticky, read by the next call)
 };
@@ -341,6 +342,36 @@ template <typename T> struct SampleCtx {
     int ck_kumax, ck_rmin, ck_rmax;   // that extent ({N, 0, N}: nothing to check)
 };
 
+// Everything after the interpolation of one point: sign for u' < 0, phase, store / chi2 term.
+template <typename T, bool WRITE_VIS, bool DO_CHI2>
+__device__ __forceinline__ void point_tail(const SampleParams<T>& p, SampleCtx<T>& cx_, T ReInt, T ImInt, bool uneg, double turns,
+                                           long long k, long long M, int c, T re_obs, T im_obs, T w) {
+    using R = T;
+    if (uneg) ImInt = -ImInt;
+    R vr = ReInt, vi = ImInt;
+    if (p.has_phase) {
+        int qd;
+        const double a = quarter_reduce(turns, &qd);
+        R sn, co;
+        sincos_quarter((R)a, qd, &sn, &co);
+        vr = ReInt * co - ImInt * sn;
+        vi = ReInt * sn + ImInt * co;
+    }
+    if (p.amp != 1.0) { vr *= (R)p.amp; vi *= (R)p.amp; }
+    if (WRITE_VIS) {
+        if (k < M) {
+            cx<T>* dst = reinterpret_cast<cx<T>*>(p.vis) + c * M + k;
+            if (p.accumulate) { const cx<T> old = *dst; vr += old.x; vi += old.y; }
+            __stcs(dst, mk<T>(vr, vi));
+        }
+    }
+    if (DO_CHI2) {                                          // PAPER.md:718 (Eq. 10); w = 0 for dead slots
+        const R dr = vr - re_obs;
+        const R di = vi - im_obs;
+        cx_.acc += (double)(fma(dr, dr, di * di) * w);
+    }
+}
+
 // U points of one thread: rotate, index, gather, interpolate, phase, chi2 / store.
 //   ld(a, j): value a (0 = u, 1 = v, 2 = re_obs, 3 = im_obs, 4 = w) of this thread's j-th point;
 //             points past the end read as u = v = 0 with weight 0 (cell (0, N/2), always inside).
@@ -416,30 +447,60 @@ __device__ __forceinline__ void sample_points(const SampleParams<T>& p, SampleCt
             ReInt = (R)g.x;
             ImInt = (R)g.y;
         }
-        if (uneg[j]) ImInt = -ImInt;
-        R vr = ReInt, vi = ImInt;
-        if (p.has_phase) {
-            int qd;
-            const double a = quarter_reduce(turns[j], &qd);
-            R sn, co;
-            sincos_quarter((R)a, qd, &sn, &co);
-            vr = ReInt * co - ImInt * sn;
-            vi = ReInt * sn + ImInt * co;
+        point_tail<T, WRITE_VIS, DO_CHI2>(p, cx_, ReInt, ImInt, uneg[j], turns[j], kpt(j), M, c, ld(2, j), ld(3, j), ld(4, j));
+    }
+}
+
+// The same U points with every thread gathering its OWN cell (two entries of the pair layout / four values of the
+// single-copy layout), no lane pairing: fewer instructions (no shuffles, no selects) but one L1 line per lane and
+// load instead of one per lane pair.  Taken for a bound observation set (gal_plan_bind_obs), whose uv-sorted
+// order makes the lanes of a warp share their lines; in time-major order it loses to the lane-pair gather.
+template <typename T, bool WRITE_VIS, bool DO_CHI2, bool EXACT, int U, bool PAIR, typename LD, typename KP>
+__device__ __forceinline__ void sample_points_direct(const SampleParams<T>& p, SampleCtx<T>& cx_, LD ld, KP kpt, long long M,
+                                                     int c) {
+    const int N = cx_.N;
+    const NodePair<T>* __restrict__ spec = cx_.spec;
+    using R = T;
+    R tx[U], ty[U];
+    double turns[U];
+    bool uneg[U], inside[U];
+    cx<T> g00[U], g01[U], g10[U], g11[U];                   // g[row kvs + 0/1][column ku + 0/1]
+#pragma unroll
+    for (int j = 0; j < U; ++j) {
+        const PointIndex q = point_index<EXACT>(p.ix, (double)ld(0, j), (double)ld(1, j));
+        inside[j] = cell_inside(p.ix, q);
+        uneg[j] = q.uneg;
+        double fx0, fy0;
+        const int ix0 = floor_small(inside[j] ? q.uidx : 0.0, &fx0), iy0 = floor_small(inside[j] ? q.vidx : 0.0, &fy0);
+        tx[j] = (R)__dsub_rn(q.uidx, fx0);
+        ty[j] = (R)__dsub_rn(q.vidx, fy0);
+        turns[j] = fma(q.urot, p.dRA_turns, q.vrot * p.dDec_turns);
+        const int off = ix0 * N + iy0;
+        if (ix0 + 1 > cx_.ck_kumax || iy0 < cx_.ck_rmin || iy0 + 1 > cx_.ck_rmax || (!inside[j] && cx_.ck_kumax < N)) ++cx_.viol;
+        if (PAIR) {
+            const NodePair<T> e0 = load_pair(spec + off), e1 = load_pair(spec + off + 1);
+            g00[j] = e0.a; g01[j] = e0.b; g10[j] = e1.a; g11[j] = e1.b;
+        } else {
+            const cx<T>* __restrict__ sg = reinterpret_cast<const cx<T>*>(spec);
+            g00[j] = __ldg(sg + off); g10[j] = __ldg(sg + off + 1);
+            g01[j] = __ldg(sg + off + N); g11[j] = __ldg(sg + off + N + 1);
         }
-        if (p.amp != 1.0) { vr *= (R)p.amp; vi *= (R)p.amp; }   // multi-source composition only
-        if (WRITE_VIS) {
-            const long long k = kpt(j);
-            if (k < M) {
-                cx<T>* dst = reinterpret_cast<cx<T>*>(p.vis) + c * M + k;
-                if (p.accumulate) { const cx<T> old = *dst; vr += old.x; vi += old.y; }
-                __stcs(dst, mk<T>(vr, vi));
-            }
+    }
+#pragma unroll
+    for (int j = 0; j < U; ++j) {
+        // along u in both rows, then along v
+        const R r0_re = fma(tx[j], g01[j].x - g00[j].x, g00[j].x), r0_im = fma(tx[j], g01[j].y - g00[j].y, g00[j].y);
+        const R r1_re = fma(tx[j], g11[j].x - g10[j].x, g10[j].x), r1_im = fma(tx[j], g11[j].y - g10[j].y, g10[j].y);
+        R ReInt = fma(ty[j], r1_re - r0_re, r0_re);
+        R ImInt = fma(ty[j], r1_im - r0_im, r0_im);
+        if (!inside[j]) {           // rare: the cell leaves the half-plane grid (reading A6)
+            const PointIndex q = point_index<EXACT>(p.ix, (double)ld(0, j), (double)ld(1, j));
+            if (q.uidx > p.ix.fH || q.vidx < 0.0 || q.vidx > p.ix.fN1) ++cx_.oob;
+            const cx<double> g = wrapped_cell<T, PAIR>(spec, N, q.uidx, q.vidx);
+            ReInt = (R)g.x;
+            ImInt = (R)g.y;
         }
-        if (DO_CHI2) {                                      // PAPER.md:718 (Eq. 10); w = 0 for dead slots
-            const R dr = vr - ld(2, j);
-            const R di = vi - ld(3, j);
-            cx_.acc += (double)(fma(dr, dr, di * di) * ld(4, j));
-        }
+        point_tail<T, WRITE_VIS, DO_CHI2>(p, cx_, ReInt, ImInt, uneg[j], turns[j], kpt(j), M, c, ld(2, j), ld(3, j), ld(4, j));
     }
 }
 
@@ -626,8 +687,9 @@ __global__ void __launch_bounds__(SampleGeom<T, DO_CHI2>::NT_TMA, GAL_SAMPLE_MIN
             }
         }
     } else {                                                 // ---- consumers ----
-        auto consume = [&](auto pair_tag) {                  // the loop, once per spectrum layout
+        auto consume = [&](auto pair_tag, auto direct_tag) { // the loop, once per spectrum layout and gather scheme
             constexpr bool PAIR = decltype(pair_tag)::value;
+            constexpr bool DIRECT = decltype(direct_tag)::value;
             uint32_t stage = 0, parity = 0;
             int tile = blockIdx.x;
             for (; tile < nfull; tile += gridDim.x) {
@@ -635,7 +697,8 @@ __global__ void __launch_bounds__(SampleGeom<T, DO_CHI2>::NT_TMA, GAL_SAMPLE_MIN
                 const T* st = reinterpret_cast<const T*>(sample_smem + stage * G::STAGE_BYTES) + tid;
                 auto ld = [&](int a, int j) -> T { return st[a * TILE + j * 256]; };
                 auto kpt = [&](int j) -> long long { return (long long)tile * TILE + j * 256 + tid; };
-                sample_points<T, WRITE_VIS, DO_CHI2, false, U, PAIR>(p, cx_, ld, kpt, M, c);
+                if (DIRECT) sample_points_direct<T, WRITE_VIS, DO_CHI2, false, U, PAIR>(p, cx_, ld, kpt, M, c);
+                else sample_points<T, WRITE_VIS, DO_CHI2, false, U, PAIR>(p, cx_, ld, kpt, M, c);
                 __syncwarp();                                // every lane has read its last value of this stage
                 if (lane == 0) mbar_arrive(empty0 + 8 * stage);
                 if (++stage == S) { stage = 0; parity ^= 1u; }
@@ -643,7 +706,12 @@ __global__ void __launch_bounds__(SampleGeom<T, DO_CHI2>::NT_TMA, GAL_SAMPLE_MIN
             if (tile == nfull && (long long)nfull * TILE < M)    // the ragged last tile falls to this CTA
                 sample_tile_plain<T, WRITE_VIS, DO_CHI2, false, PAIR>(p, cx_, nfull, M, c);
         };
-        if (extent_is_whole(p.ext, p.N)) consume(std::false_type{}); else consume(std::true_type{});
+        const bool whole = extent_is_whole(p.ext, p.N);
+        if (DO_CHI2 && p.direct) {                           // (a bound observation set is a chi2 matter)
+            if (whole) consume(std::false_type{}, std::true_type{}); else consume(std::true_type{}, std::true_type{});
+        } else {
+            if (whole) consume(std::false_type{}, std::false_type{}); else consume(std::true_type{}, std::false_type{});
+        }
     }
     sample_finish<T, DO_CHI2>(p, c, cx_.acc, cx_.oob, cx_.viol);
 }

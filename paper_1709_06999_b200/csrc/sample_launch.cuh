@@ -66,6 +66,7 @@ int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T
     sp.viol = (unsigned long long*)((char*)p->oob + 24);
     sp.ext = p->cur_ext;
     sp.rearm = 1;
+    sp.direct = p->last_obs ? 1 : 0;
     sp.ext_check = (p->last_bound && !p->last_obs && p->b_ext[0] < p->nxy / 2) ? p->b_ext_dev : nullptr;
     sp.viol_flag = p->viol_dev;
     // one CTA works through tiles blockIdx.x, blockIdx.x + gridDim.x, ...: a whole number of CTAs per SM
