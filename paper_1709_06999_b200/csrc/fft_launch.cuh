@@ -34,7 +34,7 @@ int launch_row(gal_plan* p, const T* image, const SweepParams* sw, int batch, co
     }
     p->launches++;
     GAL_CUDA(p, cudaGetLastError());
-    if (p->t_split) GAL_CUDA(p, cudaEventRecord(p->t_split[2], st));
+    if (p->tmark(2, st)) return GAL_ERR_CUDA;
     return GAL_OK;
 }
 
@@ -68,7 +68,7 @@ int launch_row_pipe(gal_plan* p, const T* image, const SweepParams* sw, int batc
     }
     p->launches++;
     GAL_CUDA(p, cudaGetLastError());
-    if (p->t_split) GAL_CUDA(p, cudaEventRecord(p->t_split[2], st));
+    if (p->tmark(2, st)) return GAL_ERR_CUDA;
     return GAL_OK;
 }
 
@@ -129,7 +129,7 @@ int launch_fft_16384(gal_plan* p, const T* image, const SweepParams* sw, int bat
         GAL_CUDA(p, launch_chain(k, dim3((unsigned)rp.rows_total), dim3(GR::NT), GR::SMEM, st, rp));
     }
     p->launches++;
-    if (p->t_split) GAL_CUDA(p, cudaEventRecord(p->t_split[2], st));
+    if (p->tmark(2, st)) return GAL_ERR_CUDA;
     ColParams<T> cp;
     cp.work = (const cx<T>*)p->work; cp.pair = (NodePair<T>*)p->spec; cp.tw = (const cx<T>*)p->tw; cp.N = p->nxy;
     cp.cols_total = (long long)batch * (p->nxy / 2 + 1); cp.ext = ext;

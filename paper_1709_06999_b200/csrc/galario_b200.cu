@@ -65,8 +65,11 @@ bool want_prune(const gal_plan* p, int C, int64_t M) {
     if (p->prune_mode == 0 || M <= 0) return false;
     if (p->prune_mode == 2) return true;
     const double ext_bytes = 2.0 * sizeof(T) * (double)M * C;
-    const double spec_bytes = 2.0 * sizeof(T) * (double)(p->nxy / 2 + 1) * p->nxy * C;
-    return ext_bytes <= 0.25 * 3.0 * spec_bytes;
+    const double spec_one = 2.0 * sizeof(T) * (double)(p->nxy / 2 + 1) * p->nxy;
+    // a spectrum of a few MB is transformed in a few microseconds out of the L2: the extra launch cannot pay
+    // (cfg 0 / 1 / 4: the uv-extent kernel was 15-20 % of the call and mostly found "whole plane")
+    if (spec_one < 16e6) return false;
+    return ext_bytes <= 0.25 * 3.0 * spec_one * C;
 }
 
 // Bound uv set: the extent follows from the radius computed once at bind time, for any PA.  The index of a rotated
@@ -88,18 +91,27 @@ int bound_extent(gal_plan* p, const CallScalars& cs, double dxy, cudaStream_t st
     return GAL_OK;
 }
 
-// One whole call: [uv extent] -> row pass -> column pass -> sampling, with (diagnostic mode,
-// gal_plan_timing_enable) a CUDA event between the kernels.
+// Channels per chunk of a batched call.  The kernels of one chunk run back to back (row pass, column pass,
+// sampling) on the SAME part of the plan's workspace, so that a chunk's intermediates could stay in the 126 MB L2.
+// Measured on B200 at cfg 4 (128 x 1024^2): 1330 us unchunked, 1564 / 1802 / 2205 / 3811 us with 8 / 4 / 2 / 1
+// channels per chunk — launches of a few channels are latency-bound (about 10 us per kernel whatever it moves), so
+// the default is ONE chunk; GAL_BATCH_CHUNK keeps the experiment reproducible.
+int batch_chunk(const gal_plan* p, int C) {
+    if (C <= 1 || p->batch_chunk <= 0) return C;
+    return p->batch_chunk < C ? p->batch_chunk : C;
+}
+
+// One whole call: [uv extent] -> per chunk of channels { row pass -> column pass -> sampling }, with (diagnostic
+// mode, gal_plan_timing_enable) a CUDA event after every kernel.
 template <typename T>
 int run_call(gal_plan* p, const T* image, const SweepParams* sw, int C, double dxy, const T* u, const T* v,
              const T* re, const T* im, const T* w, int64_t M, double dRA, double dDec, double PA, T* vis,
              double* chi2_pc, double* chi2_tot, cudaStream_t st) {
     const CallScalars cs = call_scalars(p, dxy, dRA, dDec, PA);
-    const bool timed = p->t_calls < p->t_max_calls;
-    cudaEvent_t* e = timed ? &p->tev[(size_t)5 * p->t_calls] : nullptr;
+    p->t_on = p->t_calls < p->t_max_calls;
     int rc;
     if ((rc = reset_call_state(p, st))) return rc;
-    if (timed) GAL_CUDA(p, cudaEventRecord(e[0], st));
+    if (p->tmark(0, st)) return GAL_ERR_CUDA;
     const int* ext = p->ext_full;
     p->last_pruned = want_prune<T>(p, C, M) && !cs.ix.du_exact_div;   // the extent kernel only has the division shortcut
     p->last_bound = false;
@@ -124,19 +136,24 @@ int run_call(gal_plan* p, const T* image, const SweepParams* sw, int C, double d
         if ((rc = launch_extent<T>(p, C, cs, u, v, M, st))) return rc;
         ext = p->ext;
     }
-    if (timed) GAL_CUDA(p, cudaEventRecord(e[1], st));
+    if (p->tmark(1, st)) return GAL_ERR_CUDA;
     p->cur_ext = ext;
-    if (M > 0) {                                      // no points: nothing to transform for
-        p->t_split = e;
-        rc = fft2<T>(p, image, sw, C, ext, st);
-        p->t_split = nullptr;
-        if (rc) return rc;
-    } else if (timed) {
-        GAL_CUDA(p, cudaEventRecord(e[2], st));
+    if (M == 0) return launch_sample<T>(p, C, cs, u, v, re, im, w, M, vis, chi2_pc, chi2_tot, true, st);
+    const int G = batch_chunk(p, C);
+    const size_t n2 = (size_t)p->nxy * p->nxy;
+    for (int c0 = 0; c0 < C; c0 += G) {
+        const int g = C - c0 < G ? C - c0 : G;
+        const bool last = c0 + g >= C;
+        const size_t o = (size_t)c0 * M;
+        if ((rc = fft2<T>(p, image ? image + c0 * n2 : nullptr, sw, g, ext, st))) return rc;
+        if (p->tmark(3, st)) return GAL_ERR_CUDA;
+        if ((rc = launch_sample<T>(p, g, cs, u + o, v + o, re ? re + o : nullptr, im ? im + o : nullptr, w ? w + o : nullptr, M,
+                                   vis ? vis + 2 * o : nullptr, chi2_pc ? chi2_pc + c0 : nullptr, G >= C ? chi2_tot : nullptr, last, st)))
+            return rc;
+        if (p->tmark(4, st)) return GAL_ERR_CUDA;
     }
-    if (timed) GAL_CUDA(p, cudaEventRecord(e[3], st));
-    if ((rc = launch_sample<T>(p, C, cs, u, v, re, im, w, M, vis, chi2_pc, chi2_tot, st))) return rc;
-    if (timed) { GAL_CUDA(p, cudaEventRecord(e[4], st)); p->t_calls++; }
+    if (G < C && chi2_tot && (rc = launch_sum_channels<T>(p, chi2_pc, C, chi2_tot, st))) return rc;
+    if (p->t_on) { p->t_calls++; p->t_on = false; }
     return GAL_OK;
 }
 
@@ -424,7 +441,8 @@ int gal_plan_create(gal_plan** out, int nxy, int batch, int precision_bits, int 
     gal_plan* p = new (std::nothrow) gal_plan();
     if (!p) return GAL_ERR_ALLOC;
     p->nxy = nxy; p->batch = batch; p->bits = precision_bits; p->device = device;
-    if (const char* e = getenv("GAL_ROW_PIPE")) p->row_mode = atoi(e);    // diagnostic switch
+    if (const char* e = getenv("GAL_ROW_PIPE")) p->row_mode = atoi(e);
+    if (const char* e = getenv("GAL_BATCH_CHUNK")) p->batch_chunk = atoi(e);     // diagnostic: channels per chunk (0 = automatic)    // diagnostic switch
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || device >= ndev) { delete p; return GAL_ERR_CUDA; }
     DeviceGuard g(device);
@@ -488,7 +506,7 @@ int gal_plan_destroy(gal_plan* p) {
     if (!p) return GAL_ERR_INVALID_ARGUMENT;
     DeviceGuard g(p->device);
     cudaFree(p->spec); cudaFree(p->work); cudaFree(p->tw); cudaFree(p->partials); cudaFree(p->tickets);
-    for (cudaEvent_t e : p->tev) cudaEventDestroy(e);
+    for (auto& m : p->tev) cudaEventDestroy(m.ev);
     cudaFree(p->o_buf); if (p->viol_host) cudaFreeHost(p->viol_host);
     cudaFree(p->call_state); cudaFree(p->call_init); cudaFree(p->ext_full); cudaFree(p->b_ext_dev); cudaFree(p->b_r2); cudaFree(p->st_vis); cudaFree(p->st_image); cudaFree(p->st_pts); cudaFree(p->st_out); cudaFree(p->st_chi2);
     delete p;
@@ -498,12 +516,10 @@ int gal_plan_destroy(gal_plan* p) {
 int gal_plan_timing_enable(gal_plan* p, int max_calls) {
     if (!p || max_calls < 0 || max_calls > (1 << 20)) return GAL_ERR_INVALID_ARGUMENT;
     DeviceGuard g(p->device);
-    for (cudaEvent_t e : p->tev) cudaEventDestroy(e);
+    for (auto& m : p->tev) cudaEventDestroy(m.ev);
     p->tev.clear();
     p->t_calls = 0;
-    p->t_max_calls = 0;
-    p->tev.resize((size_t)5 * max_calls);
-    for (auto& e : p->tev) GAL_CUDA(p, cudaEventCreate(&e));
+    p->t_on = false;
     p->t_max_calls = max_calls;
     return GAL_OK;
 }
@@ -512,14 +528,13 @@ int gal_plan_timing_read(gal_plan* p, double* ms_per_kernel, int64_t* calls) {
     if (!p || !ms_per_kernel) return GAL_ERR_INVALID_ARGUMENT;
     DeviceGuard g(p->device);
     double acc[4] = {0, 0, 0, 0};
-    for (int c = 0; c < p->t_calls; ++c) {
-        cudaEvent_t* e = &p->tev[(size_t)5 * c];
-        GAL_CUDA(p, cudaEventSynchronize(e[4]));
-        for (int k = 0; k < 4; ++k) {
-            float ms = 0;
-            GAL_CUDA(p, cudaEventElapsedTime(&ms, e[k], e[k + 1]));
-            acc[k] += ms;
-        }
+    for (size_t i = 1; i < p->tev.size(); ++i) {
+        const gal_plan::Mark &a = p->tev[i - 1], &b = p->tev[i];
+        if (a.call != b.call || b.what < 1 || b.what > 4) continue;
+        GAL_CUDA(p, cudaEventSynchronize(b.ev));
+        float ms = 0;
+        GAL_CUDA(p, cudaEventElapsedTime(&ms, a.ev, b.ev));
+        acc[b.what - 1] += ms;
     }
     for (int k = 0; k < 4; ++k) ms_per_kernel[k] = p->t_calls ? acc[k] / p->t_calls : 0.0;
     if (calls) *calls = p->t_calls;

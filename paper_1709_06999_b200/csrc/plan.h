@@ -30,6 +30,7 @@ struct gal_plan {
     int cur = 0;                         // copy used by the most recent call
     bool next_armed = false;             // the other copy has been / will be re-armed by that call's sampler
     int prune_mode = 1;                  // 0 never, 1 auto, 2 always
+    int batch_chunk = 0;                 // channels per chunk of a batched call (0: all in one chunk; GAL_BATCH_CHUNK, see galario_b200.cu batch_chunk)
     int row_mode = -1;                   // nxy 1024..4096: -1 per-size default, 0 plain row pass, 1 register-untangle kernel with plain loads, 2 its persistent TMA form (GAL_ROW_PIPE)
     bool last_pruned = false;            // did the most recent call compute a uv extent?
     // bound uv set (gal_plan_bind_uv): addresses, size, the rotation-invariant radius, and the extent derived
@@ -62,10 +63,21 @@ struct gal_plan {
     void* st_pts = nullptr;   size_t st_pts_bytes = 0;
     void* st_out = nullptr;   size_t st_out_bytes = 0;
     double* st_chi2 = nullptr;
-    // optional per-kernel timing (gal_plan_timing_enable): 5 events per call
-    std::vector<cudaEvent_t> tev;
+    // optional per-kernel timing (gal_plan_timing_enable): an event after every kernel of the recorded calls, each
+    // tagged with what ended there (0 call start, 1 uv extent, 2 row pass, 3 column pass, 4 sampling)
+    struct Mark { cudaEvent_t ev; int what; int call; };
+    std::vector<Mark> tev;
     int t_max_calls = 0, t_calls = 0;
-    cudaEvent_t* t_split = nullptr;  // when set, the row launcher records t_split[2] after its kernel
+    bool t_on = false;               // the call being issued is recorded
+    int tmark(int what, cudaStream_t st) {
+        if (!t_on) return 0;
+        Mark m; m.what = what; m.call = t_calls;
+        cudaError_t e = cudaEventCreate(&m.ev);
+        if (e == cudaSuccess) e = cudaEventRecord(m.ev, st);
+        if (e != cudaSuccess) { last_cuda = (int)e; return -3; }
+        tev.push_back(m);
+        return 0;
+    }
 };
 
 namespace galb {
@@ -114,7 +126,8 @@ template <typename T> int launch_sweep(gal_plan* p, const SweepParams& sw, T* ou
 template <typename T> int launch_transpose(gal_plan* p, T* out, cudaStream_t st);
 template <typename T> int launch_extent(gal_plan* p, int C, const CallScalars& cs, const T* u, const T* v, int64_t M, cudaStream_t st);
 template <typename T> int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T* v, const T* re, const T* im,
-                                        const T* w, int64_t M, T* vis, double* chi2_pc, double* chi2_tot, cudaStream_t st);
+                                        const T* w, int64_t M, T* vis, double* chi2_pc, double* chi2_tot, bool last, cudaStream_t st);
+template <typename T> int launch_sum_channels(gal_plan* p, const double* chi2_pc, int C, double* chi2_tot, cudaStream_t st);
 template <typename T> int launch_chi2_from_vis(gal_plan* p, const T* vis, const T* re, const T* im, const T* w, int64_t M,
                                                double* chi2, cudaStream_t st);
 // bind_obs: sort channel by channel, write the five sorted arrays to dst = [5][C][M]

@@ -808,6 +808,14 @@ static __global__ void extent_from_radius_kernel(const unsigned long long* __res
     ext[0] = e0; ext[1] = e1; ext[2] = e2;
 }
 
+// total of a chunked batch: chi2_total = sum of the per-channel values in channel order (reading A17); one thread
+static __global__ void sum_channels_kernel(const double* __restrict__ chi2_pc, int C, double* __restrict__ chi2_tot) {
+    pdl_wait();
+    double t = 0.0;
+    for (int i = 0; i < C; ++i) t += chi2_pc[i];
+    *chi2_tot = t;
+}
+
 // chi2 of visibilities that are already in memory (multi-source composition: the sum over the sources has to be
 // complete before it is compared with the observations).  Same deterministic reduction as the sampler.
 template <typename T>

@@ -41,7 +41,7 @@ int launch_sample_kernel(gal_plan* p, const SampleParams<T>& sp, dim3 grid, bool
 
 template <typename T>
 int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T* v, const T* re, const T* im,
-                  const T* w, int64_t M, T* vis, double* chi2_pc, double* chi2_tot, cudaStream_t st) {
+                  const T* w, int64_t M, T* vis, double* chi2_pc, double* chi2_tot, bool last, cudaStream_t st) {
     const bool do_chi2 = (vis == nullptr);
     if (M == 0) {
         if (chi2_pc) GAL_CUDA(p, cudaMemsetAsync(chi2_pc, 0, sizeof(double) * C, st));
@@ -65,7 +65,7 @@ int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T
     sp.next_state = (unsigned long long*)((char*)p->call_state + 32 * (p->cur ^ 1));
     sp.viol = (unsigned long long*)((char*)p->oob + 24);
     sp.ext = p->cur_ext;
-    sp.rearm = 1;
+    sp.rearm = last;
     sp.direct = p->last_obs ? 1 : 0;
     sp.ext_check = (p->last_bound && !p->last_obs && p->b_ext[0] < p->nxy / 2) ? p->b_ext_dev : nullptr;
     sp.viol_flag = p->viol_dev;
@@ -76,7 +76,7 @@ int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T
     // batched: CTAs are placed channel by channel (blockIdx.x fastest); an eighth of the resident CTAs per
     // channel keeps about eight channels' spectra (not dozens) competing for the L2 at any time and gives every
     // CTA enough tiles to amortise its prologue and reduction (measured at cfg 4: 2: 573, 4: 481, 8: 420 us)
-    if (C > 1) cap = (cap + 7) / 8;
+    if (C > 1) cap = (cap + (C < 8 ? C : 8) - 1) / (C < 8 ? C : 8);
     if (cap > p->max_gx) cap = p->max_gx;
     long long gx = ntiles < cap ? ntiles : cap;
     if (gx < 1) gx = 1;
@@ -89,7 +89,7 @@ int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T
     if (rc) return rc;
     p->launches++;
     GAL_CUDA(p, cudaGetLastError());
-    p->next_armed = true;                 // the last CTA of this launch re-arms the other copy of the call state
+    p->next_armed = last;                 // the last CTA of a call's last launch re-arms the other copy of the call state
     return GAL_OK;
 }
 
@@ -195,6 +195,14 @@ int launch_extent_radius(gal_plan* p, const T* u, const T* v, int64_t M, double 
     return GAL_OK;
 }
 
+template <typename T>
+int launch_sum_channels(gal_plan* p, const double* chi2_pc, int C, double* chi2_tot, cudaStream_t st) {
+    GAL_CUDA(p, launch_chain(sum_channels_kernel, dim3(1), dim3(1), 0, st, chi2_pc, C, chi2_tot));
+    p->launches++;
+    GAL_CUDA(p, cudaGetLastError());
+    return GAL_OK;
+}
+
 // Direct Hankel evaluation (hankel.cuh): one warp per point, eight warps per CTA.
 template <typename T>
 int launch_hankel(gal_plan* p, const SweepParams& sw, const CallScalars& cs, const T* u, const T* v, const T* re, const T* im,
@@ -222,7 +230,7 @@ int launch_hankel(gal_plan* p, const SweepParams& sw, const CallScalars& cs, con
 #define GAL_INSTANTIATE_SAMPLE(T)                                                                                      \
     template int launch_extent<T>(gal_plan*, int, const CallScalars&, const T*, const T*, int64_t, cudaStream_t);      \
     template int launch_sample<T>(gal_plan*, int, const CallScalars&, const T*, const T*, const T*, const T*, const T*, \
-                                  int64_t, T*, double*, double*, cudaStream_t);                                        \
+                                  int64_t, T*, double*, double*, bool, cudaStream_t);                                  \
     template int launch_chi2_from_vis<T>(gal_plan*, const T*, const T*, const T*, const T*, int64_t, double*,          \
                                          cudaStream_t);                                                                \
     template int launch_bind_sort<T>(gal_plan*, const T*, const T*, const T*, const T*, const T*, int64_t, int, double, T*, \
@@ -232,6 +240,7 @@ int launch_hankel(gal_plan* p, const SweepParams& sw, const CallScalars& cs, con
     template int launch_sample_multi<T>(gal_plan*, const IndexScalars&, const PlacementSet&, const T*, const T*, const T*, \
                                         const T*, const T*, int64_t, T*, bool, double*, bool, cudaStream_t);           \
     template int launch_extent_radius<T>(gal_plan*, const T*, const T*, int64_t, double, cudaStream_t);                \
+    template int launch_sum_channels<T>(gal_plan*, const double*, int, double*, cudaStream_t);                         \
     template int launch_uv_radius<T>(gal_plan*, const T*, const T*, long long, cudaStream_t);
 
 }  // namespace galb

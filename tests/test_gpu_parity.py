@@ -623,6 +623,7 @@ def test_multi_source_single_launch_long_lists_and_bound_set(g, orc):
     observation set."""
     w = W.config(2, nxy=512, M=60_007)
     plan = g.Plan(w.nxy)
+    plan.set_pruning(2)                 # (automatic mode does not prune a spectrum this small)
     img, u, v, re, im, wt = (dev(a) for a in (w.image, w.u, w.v, w.re_obs, w.im_obs, w.w))
     rng = np.random.default_rng(3)
     mk = lambda S: [(float(a), float(b), float(c), float(d)) for a, b, c, d in
@@ -663,6 +664,7 @@ def test_per_call_state_across_calls(g, orc):
     alternately and re-armed by the sampler of the call before (or by an explicit copy after an M = 0 call)."""
     w = W.config(0)
     plan = g.Plan(w.nxy)
+    plan.set_pruning(2)                 # always compute the extent (automatic mode skips it for a spectrum this small)
     t = dev
     _, ref_oob = orc.sampleImage(w.image, w.dxy, w.u, w.v, w.PA, w.dRA, w.dDec, return_oob=True)
     assert ref_oob > 0
