@@ -238,6 +238,16 @@ def measure_case(g, torch, dev, peak, name, w, dtype, entry, prune, steps, warmu
             prof = up(w.profile)
             out = torch.empty(1, dtype=torch.float64, device=dev)
             fn = lambda: plan.chi2Profile(prof, w.Rmin, w.dR, w.dxy, u, v, re, im, wt, w.dRA, w.dDec, w.PA, w.inc, out=out)
+        elif entry == "chi2ProfileHankel":              # Eq. 25 directly: no image, no transform
+            prof = up(w.profile)
+            out = torch.empty(1, dtype=torch.float64, device=dev)
+            fn = lambda: plan.chi2ProfileHankel(prof, w.Rmin, w.dR, u, v, re, im, wt, w.dRA, w.dDec, w.PA, w.inc, out=out)
+        elif entry.startswith("chi2ImageMulti"):        # S placements of one model in one sampling launch
+            S = int(entry[len("chi2ImageMulti"):])
+            image = up(w.image)
+            out = torch.empty(1, dtype=torch.float64, device=dev)
+            pl = [(w.dRA * (1 + 0.1 * s), w.dDec * (1 - 0.1 * s), w.PA + 0.05 * s, 1.0 / S) for s in range(S)]
+            fn = lambda: plan.chi2ImageMulti(image, w.dxy, u, v, re, im, wt, pl, out=out)
         elif entry == "chi2ImageBatch":
             image = up(w.image)
             out = torch.empty(C + 1, dtype=torch.float64, device=dev)
@@ -263,52 +273,74 @@ def measure_case(g, torch, dev, peak, name, w, dtype, entry, prune, steps, warmu
            "method_bytes_this_extent": Bp["step"], "frac": Bp["step"] / (ms * 1e-3) / 1e9 / peak,
            "kernels_us": {k: round(1e3 * t, 2) for k, t in kms.items() if t > 0},
            "kernels_frac": {k: round(Bp[k] / (t * 1e-3) / 1e9 / peak, 3) for k, t in kms.items() if t > 0 and Bp[k] > 0}}
+    if entry == "chi2ProfileHankel":
+        # no image, no transform: M * nr Bessel evaluations, FP64-ALU bound.  One evaluation is
+        # about 45 FP64 instructions; the pipe issues 148 SMs x 64 lanes per clock.
+        nr = len(w.profile)
+        for k in ("method_bytes_whole_plane", "frac_whole_plane_bytes", "method_bytes_this_extent", "frac", "uv_extent", "pruned"):
+            row.pop(k)
+        row.update({"bound": "alu", "j0_evaluations": w.M * nr, "j0_evaluations_per_s": w.M * nr / (ms * 1e-3),
+                    "fp64_pipe_frac_at_45_instr": 45.0 * w.M * nr / (ms * 1e-3) / (148 * 64 * 1.965e9)})
     del plan
     torch.cuda.empty_cache()
     return row
 
 
-def measure_other(g, torch, dev, peak, w3, args):
-    """Every other BASELINE.json config, the whole-plane path, fp32, sampleImage and nxy = 8192, measured in this
-    run with the headline's method.  Workloads are the seeded generators' full sizes."""
+def measure_other(g, torch, dev, peak, w3, args, only=None):
+    """Every other BASELINE.json config, the whole-plane path, fp32, sampleImage, nxy = 8192 and 16384, measured in
+    this run with the headline's method.  Workloads are the seeded generators' full sizes, built
+    when their case runs.  `only`: run the cases whose name contains this string (`--case`, used for ncu captures)."""
     import workloads
     rows = []
     S, Wm = args.other_steps, 5
+    cache = {}
 
-    def add(*a, **k):
+    def wl(key):
+        if key not in cache:
+            cache.clear()                              # one big workload in host memory at a time
+            if key == "3":
+                cache[key] = w3 if w3 is not None else workloads.config(3)
+            elif key == "3f":
+                cache[key] = (w3 if w3 is not None else workloads.config(3)).as_f32()
+            elif key in ("8192", "16384"):
+                # SURVEY 8(f) row 4: a seeded random image, the cfg-2 uv set scaled to the same pixel indices
+                # (16384 is the paper's largest size, PAPER.md:428, 621: 810 ms per chi2Image on a GTX 1060 with
+                # M = 1e6, copies included; context only)
+                n = int(key)
+                w2 = workloads.config(2)
+                rng = np.random.default_rng(n)
+                cache[key] = workloads.Workload(f"n{n}", "chi2Image", n, w2.dxy * 2048 / n, w2.u, w2.v, w2.re_obs, w2.im_obs,
+                                                w2.w, w2.dRA, w2.dDec, w2.PA, image=rng.random((n, n)))
+            else:
+                cache[key] = workloads.config(int(key))
+        return cache[key]
+
+    def add(name, key, *a, **k):
+        if only is not None and only not in name:
+            return
         try:
-            rows.append(measure_case(g, torch, dev, peak, *a, steps=S, warmup=Wm, **k))
+            rows.append(measure_case(g, torch, dev, peak, name, wl(key), *a, steps=S, warmup=Wm, **k))
         except Exception as exc:                       # a failing case is reported, not hidden
-            rows.append({"case": a[0], "error": repr(exc)})
+            rows.append({"case": name, "error": repr(exc)})
 
     f64, f32 = torch.float64, torch.float32
-    add("cfg3 f64 chi2Image, whole plane (prune 0)", w3, f64, "chi2Image", 0)
-    add("cfg3 f64 chi2Image, bound observations", w3, f64, "chi2Image", 1, bind=True)
-    add("cfg3 f64 sampleImage", w3, f64, "sampleImage", 1)
-    w3f = w3.as_f32()
-    add("cfg3 f32 chi2Image", w3f, f32, "chi2Image", 1)
-    add("cfg3 f32 sampleImage", w3f, f32, "sampleImage", 1)
-    add("cfg3 f32 chi2Image, whole plane (prune 0)", w3f, f32, "chi2Image", 0)
-    del w3f
-    w2 = workloads.config(2)
-    add("cfg2 f64 chi2Image", w2, f64, "chi2Image", 1)
-    # nxy = 8192 (SURVEY 8(f) row 4): a seeded random image, the cfg-2 uv set scaled to the same pixel indices
-    rng = np.random.default_rng(8192)
-    w8 = workloads.Workload("n8192", "chi2Image", 8192, w2.dxy * 2048 / 8192, w2.u, w2.v, w2.re_obs, w2.im_obs, w2.w,
-                            w2.dRA, w2.dDec, w2.PA, image=rng.random((8192, 8192)))
-    add("nxy=8192 f64 chi2Image (cfg-2 uv set, random image)", w8, f64, "chi2Image", 1)
-    del w8
-    # nxy = 16384, the paper's largest size (PAPER.md:428, 621: 810 ms per chi2Image on a GTX 1060 with M = 1e6,
-    # copies included; context only)
-    w16 = workloads.Workload("n16384", "chi2Image", 16384, w2.dxy * 2048 / 16384, w2.u, w2.v, w2.re_obs, w2.im_obs,
-                             w2.w, w2.dRA, w2.dDec, w2.PA, image=rng.random((16384, 16384)))
-    add("nxy=16384 f64 chi2Image (cfg-2 uv set, random image)", w16, f64, "chi2Image", 1)
-    del w16, w2
-    add("cfg1 f64 chi2Profile", workloads.config(1), f64, "chi2Profile", 1)
-    add("cfg0 f64 chi2Image", workloads.config(0), f64, "chi2Image", 1)
-    w4 = workloads.config(4)
-    add("cfg4 f64 chi2ImageBatch (128 channels)", w4, f64, "chi2ImageBatch", 1)
-    add("cfg4 f64 chi2ImageBatch (128 channels), bound observations", w4, f64, "chi2ImageBatch", 1, bind=True)
+    add("cfg3 f64 chi2Image (automatic pruning)", "3", f64, "chi2Image", 1)
+    add("cfg3 f64 chi2Image, whole plane (prune 0)", "3", f64, "chi2Image", 0)
+    add("cfg3 f64 chi2Image, bound observations", "3", f64, "chi2Image", 1, bind=True)
+    add("cfg3 f64 sampleImage", "3", f64, "sampleImage", 1)
+    add("cfg3 f32 chi2Image (automatic pruning)", "3f", f32, "chi2Image", 1)
+    add("cfg3 f32 sampleImage", "3f", f32, "sampleImage", 1)
+    add("cfg3 f32 chi2Image, whole plane (prune 0)", "3f", f32, "chi2Image", 0)
+    add("cfg3 f32 chi2Image, bound observations", "3f", f32, "chi2Image", 1, bind=True)
+    add("cfg2 f64 chi2Image", "2", f64, "chi2Image", 1)
+    add("nxy=8192 f64 chi2Image (cfg-2 uv set, random image)", "8192", f64, "chi2Image", 1)
+    add("nxy=16384 f64 chi2Image (cfg-2 uv set, random image)", "16384", f64, "chi2Image", 1)
+    add("cfg1 f64 chi2Profile", "1", f64, "chi2Profile", 1)
+    add("cfg1 f64 chi2Profile by the direct Hankel transform (Eq. 25)", "1", f64, "chi2ProfileHankel", 1)
+    add("cfg2 f64 chi2ImageMulti, 4 placements in one sampling launch", "2", f64, "chi2ImageMulti4", 1)
+    add("cfg0 f64 chi2Image", "0", f64, "chi2Image", 1)
+    add("cfg4 f64 chi2ImageBatch (128 channels)", "4", f64, "chi2ImageBatch", 1)
+    add("cfg4 f64 chi2ImageBatch (128 channels), bound observations", "4", f64, "chi2ImageBatch", 1, bind=True)
     return rows
 
 
@@ -322,6 +354,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-other", action="store_true", help="skip the `other` block (every other config and path)")
     ap.add_argument("--other-steps", type=int, default=50)
+    ap.add_argument("--case", default=None,
+                    help="run only the `other` cases whose name contains this string and print them (no headline, no "
+                         "e2e, no oracle): the command the ncu captures under profiles/ were taken with")
     ap.add_argument("--prune", type=int, default=1, choices=[0, 1, 2],
                     help="gal_plan_set_pruning mode: 0 never, 1 automatic (library default), 2 always")
     args = ap.parse_args()
@@ -345,6 +380,14 @@ def main():
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
+
+    if args.case is not None:              # a selection of the `other` cases alone (profiling runs)
+        if rank == 0:
+            peak, _ = measured_peaks()
+            print(json.dumps({"cases": measure_other(g, torch, dev, peak, None, args, only=args.case)}))
+        if world > 1:
+            torch.distributed.destroy_process_group()
+        return
 
     w = workloads.config(3)               # every rank: the same seeded replica
     esz = 8
