@@ -79,7 +79,7 @@ def ncu_traffic(kernel: str):
         try:
             with open(path) as f:
                 for row in csv.DictReader(f):
-                    if row["kernel"].startswith(kernel):
+                    if row["kernel"] == kernel or row["kernel"].startswith(kernel + "_kernel"):
                         best = int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
         except (OSError, ValueError, KeyError):
             continue

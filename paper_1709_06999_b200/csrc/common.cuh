@@ -83,6 +83,13 @@ __device__ __forceinline__ void tma_load_1d(uint32_t dst, const void* src, uint3
         ::"r"(dst), "l"(src), "r"(bytes), "r"(mb), "l"(pol) : "memory");
 }
 
+// Ask the L2 to fetch `bytes` (a multiple of 16, 16-byte aligned) from global memory: no destination, no completion
+// to wait for.  One thread prefetches what a LATER CTA of the grid will read, so that CTA's loads find it in the
+// L2 (about 250 clocks) instead of in HBM (a microsecond and more under load).
+__device__ __forceinline__ void l2_prefetch_bulk(const void* src, uint32_t bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+}
+
 __device__ __forceinline__ void mbar_arrive(uint32_t mb) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(mb) : "memory");
 }

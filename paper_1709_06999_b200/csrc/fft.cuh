@@ -262,8 +262,19 @@ template <typename T> struct RowParams {
     int N;
     int rows_total;        // batch * N
     const int* ext;        // {largest column ku needed, first row kvs, last row kvs} (sample.cuh, uv extent)
+    int pf_blocks;         // > 0: CTA b asks the L2 for the image rows of CTA b + pf_blocks (the CTAs resident at once)
     SweepParams sweep;
 };
+
+// CTA `blk` of a grid of row blocks (rows_per_block rows each) prefetches the rows of block blk + pf_blocks into the
+// L2.  The image is an input of the call, not a product of the kernel before in the chain, so this runs before the
+// programmatic dependency is waited for.
+template <typename T>
+__device__ __forceinline__ void prefetch_row_block(const RowParams<T>& p, long long blk, int rows_per_block) {
+    if (p.pf_blocks <= 0 || threadIdx.x >= rows_per_block) return;
+    const long long row = (blk + p.pf_blocks) * rows_per_block + threadIdx.x;
+    if (row < p.rows_total) l2_prefetch_bulk(p.image + row * (long long)p.N, (uint32_t)(p.N * sizeof(T)));
+}
 
 template <typename T, int R1, int R2, int R3, int F, bool SWEEP>
 __global__ void __launch_bounds__(Geom<T, R1, R2, R3, F>::NT)
@@ -279,6 +290,7 @@ row_pass_kernel(const RowParams<T> p) {
     const long long row = row0 + f;
     const bool valid = row < p.rows_total;
     cx<T>* S = smem + f * G::REGION;
+    if (!SWEEP) prefetch_row_block(p, blockIdx.x, F);
     pdl_wait();
 
     if (SWEEP) {
@@ -384,7 +396,8 @@ __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.p
 enum RowLoad { ROW_TMA = 0, ROW_DIRECT = 1, ROW_SWEEP = 2 };
 
 template <typename T, int R1, int R2, int R3, int F, int NG, int NS, int MODE>
-__global__ void __launch_bounds__(RowGeom<T, R1, R2, R3, F>::GT * NG + (MODE == ROW_TMA ? 32 : 0), MODE == ROW_TMA ? 1 : 2)
+__global__ void __launch_bounds__(RowGeom<T, R1, R2, R3, F>::GT * NG + (MODE == ROW_TMA ? 32 : 0),
+                                  MODE == ROW_TMA ? 1 : cmax(2, 512 / (RowGeom<T, R1, R2, R3, F>::GT * NG)))
 row_pipe_kernel(const RowParams<T> p) {
     constexpr bool SWEEP = MODE != ROW_TMA;          // "no ring": inputs do not come through the mbarrier pipeline
     using G = RowGeom<T, R1, R2, R3, F>;
@@ -427,6 +440,7 @@ row_pipe_kernel(const RowParams<T> p) {
     const int g = tid / GT, gtid = tid % GT;
     const int t = gtid / F, f = gtid % F;
     const int bar_id = 1 + g;
+    if (MODE == ROW_DIRECT) prefetch_row_block(p, blockIdx.x, F);
     pdl_wait();
     const int kumax = __ldg(p.ext);
     const int NU = N / 2 + 1;
@@ -568,6 +582,7 @@ template <typename T> struct ColParams {
     int N;
     long long cols_total;  // batch * (N/2+1)
     const int* ext;        // as RowParams::ext
+    int pf_groups;         // > 0: CTA b asks the L2 for the columns of CTA b + pf_groups (whole-plane transforms only)
 };
 
 template <typename T, int R1, int R2, int R3, int F>
@@ -585,6 +600,12 @@ col_pass_kernel(const ColParams<T> p) {
     const int kumax = __ldg(p.ext), rmin = __ldg(p.ext + 1), rmax = __ldg(p.ext + 2);
     const bool single = extent_is_whole_plane(p.ext, L);
     cx<T>* S = smem + f * G::REGION;
+    // whole plane: the row-transformed image comes back from HBM (a pruned one is still in the L2): ask the L2 for
+    // the columns of the CTA that will take this one's place
+    if (single && p.pf_groups > 0 && tid < F) {
+        const long long gg = ((long long)blockIdx.x + p.pf_groups) * F + tid;
+        if (gg < p.cols_total) l2_prefetch_bulk(p.work + gg * (long long)L, (uint32_t)(L * sizeof(cx<T>)));
+    }
     {
         const long long grp = blockIdx.x;                   // one group of F columns per CTA
         const long long g = grp * F + f;
@@ -765,6 +786,7 @@ row_pass_x2_kernel(const RowParams<T> p) {
     const int N = p.N;
     const long long row = blockIdx.x;
     cx<T>* S = smem + f * G::REGION;
+    if (!SWEEP) prefetch_row_block(p, blockIdx.x, 1);
     pdl_wait();
     if (SWEEP) {
         const int i = (int)(row % N);

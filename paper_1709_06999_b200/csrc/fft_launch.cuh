@@ -21,6 +21,7 @@ int launch_row(gal_plan* p, const T* image, const SweepParams* sw, int batch, co
     rp.N = p->nxy;
     rp.rows_total = batch * p->nxy;
     rp.ext = ext;
+    rp.pf_blocks = 0;
     if (sw) rp.sweep = *sw; else memset(&rp.sweep, 0, sizeof(rp.sweep));
     const unsigned grid = (unsigned)((rp.rows_total + F - 1) / F);
     if (sw) {
@@ -30,6 +31,7 @@ int launch_row(gal_plan* p, const T* image, const SweepParams* sw, int batch, co
     } else {
         auto k = row_pass_kernel<T, R1, R2, R3, F, false>;
         int rc = set_smem(p, k, G::SMEM); if (rc) return rc;
+        rp.pf_blocks = resident_ctas(p, k, G::NT, G::SMEM);
         GAL_CUDA(p, launch_chain(k, dim3(grid), dim3(G::NT), G::SMEM, st, rp));
     }
     p->launches++;
@@ -51,6 +53,7 @@ int launch_row_pipe(gal_plan* p, const T* image, const SweepParams* sw, int batc
     rp.N = p->nxy;
     rp.rows_total = batch * p->nxy;
     rp.ext = ext;
+    rp.pf_blocks = 0;
     if (sw) rp.sweep = *sw; else memset(&rp.sweep, 0, sizeof(rp.sweep));
     const long long nblk = rp.rows_total / F;
     if (!sw && tma) {
@@ -64,6 +67,7 @@ int launch_row_pipe(gal_plan* p, const T* image, const SweepParams* sw, int batc
         if (sw) return GAL_ERR_UNSUPPORTED;          // *Profile calls take the plain kernel's sweep loader
         auto k = row_pipe_kernel<T, R1, R2, R3, F, 1, 1, ROW_DIRECT>;
         int rc = set_smem(p, k, smem); if (rc) return rc;
+        rp.pf_blocks = resident_ctas(p, k, G::GT, smem);
         GAL_CUDA(p, launch_chain(k, dim3((unsigned)nblk), dim3(G::GT), smem, st, rp));
     }
     p->launches++;
@@ -85,6 +89,7 @@ int launch_col(gal_plan* p, int batch, const int* ext, cudaStream_t st) {
     const unsigned grid = (unsigned)((cp.cols_total + F - 1) / F);
     auto k = col_pass_kernel<T, R1, R2, R3, F>;
     int rc = set_smem(p, k, G::SMEM); if (rc) return rc;
+    cp.pf_groups = resident_ctas(p, k, G::NT, G::SMEM);
     GAL_CUDA(p, launch_chain(k, dim3(grid), dim3(G::NT), G::SMEM, st, cp));
     p->launches++;
     GAL_CUDA(p, cudaGetLastError());
@@ -101,6 +106,7 @@ int launch_col_x2(gal_plan* p, int batch, const int* ext, cudaStream_t st) {
     cp.N = p->nxy;
     cp.cols_total = (long long)batch * (p->nxy / 2 + 1);
     cp.ext = ext;
+    cp.pf_groups = 0;
     auto k = col_pass_x2_kernel<T, R1, R2, R3>;
     int rc = set_smem(p, k, G::SMEM); if (rc) return rc;
     GAL_CUDA(p, launch_chain(k, dim3((unsigned)cp.cols_total), dim3(G::NT), G::SMEM, st, cp));
@@ -116,7 +122,7 @@ int launch_fft_16384(gal_plan* p, const T* image, const SweepParams* sw, int bat
     using GC = Geom<T, 16, 16, 16, 1>;
     RowParams<T> rp;
     rp.image = image; rp.spec = (cx<T>*)p->work; rp.tw = (const cx<T>*)p->tw; rp.N = p->nxy;
-    rp.rows_total = batch * p->nxy; rp.ext = ext;
+    rp.rows_total = batch * p->nxy; rp.ext = ext; rp.pf_blocks = 0;
     if (sw) rp.sweep = *sw; else memset(&rp.sweep, 0, sizeof(rp.sweep));
     int rc;
     if (sw) {
@@ -126,13 +132,14 @@ int launch_fft_16384(gal_plan* p, const T* image, const SweepParams* sw, int bat
     } else {
         auto k = row_pass_x2_kernel<T, 16, 16, 16, false>;
         if ((rc = set_smem(p, k, GR::SMEM))) return rc;
+        rp.pf_blocks = resident_ctas(p, k, GR::NT, GR::SMEM);
         GAL_CUDA(p, launch_chain(k, dim3((unsigned)rp.rows_total), dim3(GR::NT), GR::SMEM, st, rp));
     }
     p->launches++;
     if (p->tmark(2, st)) return GAL_ERR_CUDA;
     ColParams<T> cp;
     cp.work = (const cx<T>*)p->work; cp.pair = (NodePair<T>*)p->spec; cp.tw = (const cx<T>*)p->tw; cp.N = p->nxy;
-    cp.cols_total = (long long)batch * (p->nxy / 2 + 1); cp.ext = ext;
+    cp.cols_total = (long long)batch * (p->nxy / 2 + 1); cp.ext = ext; cp.pf_groups = 0;
     auto ks = col_sub_kernel<T, 16, 16, 16>;
     if ((rc = set_smem(p, ks, GC::SMEM))) return rc;
     GAL_CUDA(p, launch_chain(ks, dim3((unsigned)(4 * cp.cols_total)), dim3(GC::NT), GC::SMEM, st, cp, (cx<T>*)p->work));
@@ -196,8 +203,21 @@ int fft2(gal_plan* p, const T* image, const SweepParams* sw, int batch, const in
     }
         GAL_FFT_CASE_PIPE(1024, RR(8, 8, 8, 4), RR(16, 8, 4, 8), RR(16, 8, 8, 4))
         GAL_FFT_CASE_PIPE(2048, RR(16, 8, 8, 4), RR(16, 8, 8, 4), RR(16, 16, 8, 2))
-        GAL_FFT_CASE_PIPE(4096, RR(16, 16, 8, 2), RR(16, 16, 8, 2), RR(16, 16, 16, 1))
 #undef GAL_FFT_CASE_PIPE
+        case 4096: {
+            int mode = sw ? 0 : (p->row_mode >= 0 ? p->row_mode : RowPipeCfg<T>::default_mode(4096));
+            // A transform pruned to a part of the half plane leaves a row-transformed image of a few tens of MB,
+            // which stays in the L2: there ONE row per CTA (barriers over four warps instead of eight, a tail half
+            // as long; 16-byte stores that the L2 merges) is faster, 46.5 against 51.3 us at cfg 3.  Written out to
+            // HBM (whole plane) the half-sector stores cost a factor of two (147 against 68 us), so the choice
+            // follows the extent the plan expects (plan.h row_small).  Mode 3 forces it (diagnostic).
+            if (mode == 1 && p->row_small && sizeof(T) == 8) mode = 3;
+            if (mode == 3) rc = launch_row_pipe<T, 16, 16, 8, 1, 1, 1>(p, image, sw, batch, ext, false, st);
+            else if (mode) rc = launch_row_pipe<T, 16, 16, 8, 2, RowPipeCfg<T>::NG, RowPipeCfg<T>::NS>(p, image, sw, batch, ext, mode == 2, st);
+            else rc = launch_row<T, 16, 16, 8, 2>(p, image, sw, batch, ext, st);
+            if (rc) return rc;
+            return launch_col<T, 16, 16, 16, 1>(p, batch, ext, st);
+        }
         case 8192:      // column length 8192 = 2 x 4096: two interleaved transforms + one radix-2 combination
             rc = launch_row<T, 16, 16, 16, 1>(p, image, sw, batch, ext, st); if (rc) return rc;
             return launch_col_x2<T, 16, 16, 16>(p, batch, ext, st);

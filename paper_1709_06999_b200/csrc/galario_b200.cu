@@ -138,6 +138,8 @@ int run_call(gal_plan* p, const T* image, const SweepParams* sw, int C, double d
     }
     if (p->tmark(1, st)) return GAL_ERR_CUDA;
     p->cur_ext = ext;
+    p->row_small = p->last_bound ? p->b_ext[0] < p->nxy / 2
+                                 : (p->last_pruned && ((volatile unsigned int*)p->viol_host)[1] == 2u);
     if (M == 0) return launch_sample<T>(p, C, cs, u, v, re, im, w, M, vis, chi2_pc, chi2_tot, true, st);
     const int G = batch_chunk(p, C);
     const size_t n2 = (size_t)p->nxy * p->nxy;
@@ -242,6 +244,7 @@ int do_fft2_shifted(gal_plan* p, const T* image, T* out, void* stream) {
     DeviceGuard g(p->device);
     cudaStream_t st = (cudaStream_t)stream;
     p->last_stream = st;
+    p->row_small = false;                                  // whole plane
     int rc = fft2<T>(p, image, nullptr, 1, p->ext_full, st);
     if (rc) return rc;
     return launch_transpose<T>(p, out, st);
@@ -309,6 +312,7 @@ int do_multi(gal_plan* p, const T* image, double dxy, const T* u, const T* v, co
         ext = p->ext;
     }
     p->cur_ext = ext;
+    p->row_small = p->last_bound ? p->b_ext[0] < p->nxy / 2 : p->last_pruned;   // (the radius extent is pruned unless the data violate Eq. 19)
     if ((rc = fft2<T>(p, image, nullptr, 1, ext, st))) return rc;
     T* sum = vis;
     if (!vis && S > GAL_MULTI_CHUNK) {                // a long list: the running sum of the chunks
@@ -463,8 +467,8 @@ int gal_plan_create(gal_plan** out, int nxy, int batch, int precision_bits, int 
     if ((e = cudaMalloc((void**)&p->ext_full, 16)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     if ((e = cudaMalloc((void**)&p->b_ext_dev, 16)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     if ((e = cudaMalloc((void**)&p->b_r2, 8)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
-    if ((e = cudaHostAlloc((void**)&p->viol_host, sizeof(unsigned int), cudaHostAllocMapped)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
-    *p->viol_host = 0;
+    if ((e = cudaHostAlloc((void**)&p->viol_host, 2 * sizeof(unsigned int), cudaHostAllocMapped)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
+    p->viol_host[0] = 0; p->viol_host[1] = 0;          // [1]: extent hint (plan.h row_small)
     if ((e = cudaHostGetDevicePointer((void**)&p->viol_dev, p->viol_host, 0)) != cudaSuccess) return fail(GAL_ERR_CUDA, e);
     p->oob = (unsigned long long*)p->call_state;
     p->ext = (int*)((char*)p->call_state + 8);

@@ -4,6 +4,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <cstdlib>
+#include <map>
 #include <set>
 #include <vector>
 
@@ -51,8 +53,13 @@ struct gal_plan {
     // set (from the device, plain store to mapped host memory) by a sampler that found a point outside the extent
     // of a bound uv set: the promise was broken; the next call returns GAL_ERR_BINDING_VIOLATED
     unsigned int* viol_host = nullptr; unsigned int* viol_dev = nullptr;
+    // viol_host[1] = extent hint, written by the last CTA of every sampling launch: 1 = that call's transform covered
+    // the whole half plane, 2 = it was pruned.  The host reads it WITHOUT synchronising when it picks the row-pass
+    // variant of the next call (a stale value costs time, never correctness): row_small = "expect a pruned extent".
+    bool row_small = false;
     void* st_vis = nullptr; size_t st_vis_bytes = 0; // summed visibilities of a chi2 multi-source call
     std::set<const void*> smem_set;      // kernels whose dynamic shared-memory limit has been raised
+    std::map<const void*, int> resident; // kernel -> CTAs resident on the whole GPU at once (occupancy x SM count)
     int max_gx = 0;
     size_t owned_bytes = 0;
     int last_cuda = 0;
@@ -103,6 +110,19 @@ template <typename K> inline int set_smem(gal_plan* p, K kernel, size_t bytes) {
         p->smem_set.insert((const void*)kernel);
     }
     return GAL_OK;
+}
+
+// CTAs of `kernel` resident on the GPU at once: the distance (in blocks) at which a CTA of an FFT pass prefetches
+// into the L2 for a later one.  GAL_ROW_PF scales it (0 switches the prefetch off; diagnostic).
+template <typename K> inline int resident_ctas(gal_plan* p, K kernel, int threads, size_t smem) {
+    auto it = p->resident.find((const void*)kernel);
+    if (it != p->resident.end()) return it->second;
+    int per_sm = 1;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
+    static const double mul = getenv("GAL_ROW_PF") ? atof(getenv("GAL_ROW_PF")) : 1.0;
+    const int r = (int)(per_sm * p->sm_count * mul);
+    p->resident[(const void*)kernel] = r;
+    return r;
 }
 
 // Programmatic dependent launch: the kernels of one call form a chain on the stream; each is launched with

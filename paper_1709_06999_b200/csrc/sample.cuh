@@ -49,6 +49,7 @@ template <typename T> struct SampleParams {
     int direct;               // 1: every thread gathers its own cell (uv-sorted points of a bound observation set)
     int rearm;                // 1: the last CTA of this launch re-arms next_state (every launch but the non-final chunks of a long multi-source list)
     unsigned int* viol_flag;  // mapped host memory: set when viol becomes non-zero (sticky, read by the next call)
+    unsigned int* ext_hint;   // mapped host memory or null: 1 = this call's extent was the whole plane, 2 = pruned (plan.h)
 };
 
 // Which layout did the column pass write?  Same rule as fft.cuh: extent_is_whole_plane.
@@ -539,6 +540,7 @@ __device__ __forceinline__ void sample_finish(const SampleParams<T>& p, int c, d
                 nx[6] = 0; nx[7] = 0;                           // and its extent-violation counter
             }
             *p.done = 0;
+            if (p.ext_hint && p.ext) *(volatile unsigned int*)p.ext_hint = extent_is_whole(p.ext, p.N) ? 1u : 2u;
         }
         if (DO_CHI2) {
             p.partials[(long long)c * gridDim.x + blockIdx.x] = s;

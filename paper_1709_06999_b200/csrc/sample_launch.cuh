@@ -69,6 +69,7 @@ int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T
     sp.direct = p->last_obs ? 1 : 0;
     sp.ext_check = (p->last_bound && !p->last_obs && p->b_ext[0] < p->nxy / 2) ? p->b_ext_dev : nullptr;
     sp.viol_flag = p->viol_dev;
+    sp.ext_hint = p->viol_dev + 1;
     // one CTA works through tiles blockIdx.x, blockIdx.x + gridDim.x, ...: a whole number of CTAs per SM
     const int tile = SampleGeom<T, true>::TILE;
     const long long ntiles = (M + tile - 1) / tile;
