@@ -266,6 +266,10 @@ def measure_case(g, torch, dev, peak, name, w, dtype, entry, prune, steps, warmu
     whole = (w.nxy // 2, 0, w.nxy - 1)
     B = algorithmic_bytes(w.nxy, w.M, esz, entry, None, C)
     Bp = algorithmic_bytes(w.nxy, w.M, esz, entry, extent, C) if extent != whole else B
+    if kms.get("row_pass", 0) <= 0 < kms.get("col_pass", 0):       # nxy = 256 / 1024: both passes in one fused launch
+        kms = {"uv_extent": kms["uv_extent"], "fft_fused": kms["col_pass"], "sample": kms["sample"]}
+        B, Bp = dict(B), dict(Bp)
+        B["fft_fused"], Bp["fft_fused"] = B["row_pass"] + B["col_pass"], Bp["row_pass"] + Bp["col_pass"]
     row = {"case": name, "entry": entry, "dtype": "f64" if esz == 8 else "f32", "nxy": w.nxy, "M": w.M, "C": C,
            "prune_mode": prune, "bound_obs": bool(bind), "us_per_call": 1e3 * ms, "uv_extent": list(extent),
            "pruned": extent != whole,

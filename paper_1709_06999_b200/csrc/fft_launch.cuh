@@ -202,7 +202,16 @@ int fft2(gal_plan* p, const T* image, const SweepParams* sw, int batch, const in
         return launch_col<T, COL>(p, batch, ext, st);                            \
     }
         GAL_FFT_CASE_PIPE(1024, RR(8, 8, 8, 4), RR(16, 8, 4, 8), RR(16, 8, 8, 4))
-        GAL_FFT_CASE_PIPE(2048, RR(16, 8, 8, 4), RR(16, 8, 8, 4), RR(16, 16, 8, 2))
+        case 2048: {
+            const int mode = sw ? 0 : (p->row_mode >= 0 ? p->row_mode : RowPipeCfg<T>::default_mode(2048));
+            if (mode == 4) rc = launch_row<T, 16, 8, 8, 2>(p, image, sw, batch, ext, st);          // experiments: fewer rows per CTA
+            else if (mode == 5) rc = launch_row<T, 16, 8, 8, 1>(p, image, sw, batch, ext, st);
+            else if (mode == 3) rc = launch_row_pipe<T, 16, 8, 8, 1, 1, 1>(p, image, sw, batch, ext, false, st);
+            else if (mode) rc = launch_row_pipe<T, 16, 8, 8, 4, RowPipeCfg<T>::NG, RowPipeCfg<T>::NS>(p, image, sw, batch, ext, mode == 2, st);
+            else rc = launch_row<T, 16, 8, 8, 4>(p, image, sw, batch, ext, st);
+            if (rc) return rc;
+            return launch_col<T, 16, 16, 8, 2>(p, batch, ext, st);
+        }
 #undef GAL_FFT_CASE_PIPE
         case 4096: {
             int mode = sw ? 0 : (p->row_mode >= 0 ? p->row_mode : RowPipeCfg<T>::default_mode(4096));
