@@ -394,10 +394,13 @@ __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.p
 // Where step 1 takes its input from: the TMA ring (persistent CTAs, one per SM), plain global loads (one row block
 // per CTA, several CTAs per SM: no producer warp, no ring), or the swept profile.
 enum RowLoad { ROW_TMA = 0, ROW_DIRECT = 1, ROW_SWEEP = 2 };
+#ifndef GAL_ROW_F1_MINB
+#define GAL_ROW_F1_MINB 4            // resident CTAs per SM the one-row-per-CTA form (128 threads) is compiled for
+#endif
 
 template <typename T, int R1, int R2, int R3, int F, int NG, int NS, int MODE>
 __global__ void __launch_bounds__(RowGeom<T, R1, R2, R3, F>::GT * NG + (MODE == ROW_TMA ? 32 : 0),
-                                  MODE == ROW_TMA ? 1 : cmax(2, 512 / (RowGeom<T, R1, R2, R3, F>::GT * NG)))
+                                  MODE == ROW_TMA ? 1 : (RowGeom<T, R1, R2, R3, F>::GT * NG == 128 ? GAL_ROW_F1_MINB : cmax(2, 512 / (RowGeom<T, R1, R2, R3, F>::GT * NG))))
 row_pipe_kernel(const RowParams<T> p) {
     constexpr bool SWEEP = MODE != ROW_TMA;          // "no ring": inputs do not come through the mbarrier pipeline
     using G = RowGeom<T, R1, R2, R3, F>;

@@ -168,7 +168,7 @@ template <typename T> struct RowPipeCfg;
 // 0 = plain kernel, 1 = lane-interleaved rows + register untangle with plain loads, 2 = its persistent TMA-ring form.
 template <> struct RowPipeCfg<double> {
     static constexpr int NG = GAL_ROW_NG64, NS = GAL_ROW_NS64;
-    static int default_mode(int nxy) { return nxy == 4096 ? 1 : 0; }
+    static int default_mode(int nxy) { return nxy >= 2048 ? 1 : 0; }   // (2048: as fast as the plain kernel, and the same arithmetic as its one-row form)
 };
 template <> struct RowPipeCfg<float> {
     static constexpr int NG = GAL_ROW_NG32, NS = GAL_ROW_NS32;
@@ -203,10 +203,10 @@ int fft2(gal_plan* p, const T* image, const SweepParams* sw, int batch, const in
     }
         GAL_FFT_CASE_PIPE(1024, RR(8, 8, 8, 4), RR(16, 8, 4, 8), RR(16, 8, 8, 4))
         case 2048: {
-            const int mode = sw ? 0 : (p->row_mode >= 0 ? p->row_mode : RowPipeCfg<T>::default_mode(2048));
-            if (mode == 4) rc = launch_row<T, 16, 8, 8, 2>(p, image, sw, batch, ext, st);          // experiments: fewer rows per CTA
-            else if (mode == 5) rc = launch_row<T, 16, 8, 8, 1>(p, image, sw, batch, ext, st);
-            else if (mode == 3) rc = launch_row_pipe<T, 16, 8, 8, 1, 1, 1>(p, image, sw, batch, ext, false, st);
+            int mode = sw ? 0 : (p->row_mode >= 0 ? p->row_mode : RowPipeCfg<T>::default_mode(2048));
+            // as at 4096 (below): one row per CTA where the plan expects a pruned extent (cfg 2: row pass 20.8 -> 18.7 us)
+            if (mode == 1 && p->row_small && sizeof(T) == 8) mode = 3;
+            if (mode == 3) rc = launch_row_pipe<T, 16, 8, 8, 1, 1, 1>(p, image, sw, batch, ext, false, st);
             else if (mode) rc = launch_row_pipe<T, 16, 8, 8, 4, RowPipeCfg<T>::NG, RowPipeCfg<T>::NS>(p, image, sw, batch, ext, mode == 2, st);
             else rc = launch_row<T, 16, 8, 8, 4>(p, image, sw, batch, ext, st);
             if (rc) return rc;

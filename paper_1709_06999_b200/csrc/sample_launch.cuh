@@ -1,5 +1,6 @@
 // sample_launch.cuh — launch geometry of the per-point kernels; included by sample_f64.cu / sample_f32.cu.
 #pragma once
+#include <cstdlib>
 #include "plan.h"
 #include "sample.cuh"
 #include "sort.cuh"
@@ -77,7 +78,8 @@ int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T
     // batched: CTAs are placed channel by channel (blockIdx.x fastest); an eighth of the resident CTAs per
     // channel keeps about eight channels' spectra (not dozens) competing for the L2 at any time and gives every
     // CTA enough tiles to amortise its prologue and reduction (measured at cfg 4: 2: 573, 4: 481, 8: 420 us)
-    if (C > 1) cap = (cap + (C < 8 ? C : 8) - 1) / (C < 8 ? C : 8);
+    static const int conc = getenv("GAL_BATCH_CONC") ? atoi(getenv("GAL_BATCH_CONC")) : 8;     // channels in flight (diagnostic)
+    if (C > 1) cap = (cap + (C < conc ? C : conc) - 1) / (C < conc ? C : conc);
     if (cap > p->max_gx) cap = p->max_gx;
     long long gx = ntiles < cap ? ntiles : cap;
     if (gx < 1) gx = 1;

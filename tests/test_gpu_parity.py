@@ -683,6 +683,33 @@ def test_per_call_state_across_calls(g, orc):
             assert plan.last_oob_count() == 0
 
 
+@pytest.mark.parametrize("nxy", [2048, 4096])
+def test_row_pass_variant_follows_the_expected_extent(g, nxy):
+    """At nxy = 2048 / 4096 (fp64) the plan picks the row-pass form from the extent it EXPECTS — a hint the sampler of
+    the call before leaves in mapped host memory, read without synchronising: several rows per CTA (whole sectors)
+    for a whole-plane transform, one row per CTA when the row-transformed image stays in the L2.  Both forms do the
+    same arithmetic: whatever the history of a plan, its results equal, bit for bit, those of a plan that never
+    prunes (which always takes the first form)."""
+    w = W.config(2, nxy=nxy, M=100_003)
+    image = dev(w.image)
+    ref_plan = g.Plan(nxy)
+    ref_plan.set_pruning(0)
+    plan = g.Plan(nxy)
+    obs = (dev(w.re_obs), dev(w.im_obs), dev(w.w))
+    for scale in (1.0, 1.0, 1.0, 9.0, 9.0, 1.0, 1.0):        # in-grid (pruned), then wrapping (whole plane), then back
+        u, v = dev(w.u * scale), dev(w.v * scale)
+        a = plan.chi2Image(image, w.dxy, u, v, *obs, w.dRA, w.dDec, w.PA)
+        b = ref_plan.chi2Image(image, w.dxy, u, v, *obs, w.dRA, w.dDec, w.PA)
+        torch.cuda.synchronize()                             # (the hint of this call is in host memory now)
+        assert torch.equal(a, b), scale
+        va = plan.sampleImage(image, w.dxy, u, v, w.PA, w.dRA, w.dDec)
+        vb = ref_plan.sampleImage(image, w.dxy, u, v, w.PA, w.dRA, w.dDec)
+        torch.cuda.synchronize()
+        assert torch.equal(va, vb), scale
+        whole = plan.last_uv_extent() == (nxy // 2, 0, nxy - 1)
+        assert whole == (scale > 1.0)
+
+
 # ---------------------------------------------------------------------------------------------
 # edge cases
 # ---------------------------------------------------------------------------------------------
