@@ -83,7 +83,10 @@ __device__ __forceinline__ PointIndex point_index(const IndexScalars& s, double 
     q.uidx = div_by<EXACT>(fabs(q.urot), s);
     q.uneg = q.urot < 0.0;
     const double vq = div_by<EXACT>(q.vrot, s);
-    q.vidx = q.uneg ? __dsub_rn(s.fH, vq) : __dadd_rn(s.fH, vq);
+    // N/2 - v'/du where u' < 0 is N/2 + (-(v'/du)) bit for bit: flip the sign bit instead of selecting
+    // (the comparison decides, not the sign bit of u': -0.0 takes the non-negative branch, reading A8)
+    const double vs = __hiloint2double(__double2hiint(vq) ^ (q.uneg ? (int)0x80000000 : 0), __double2loint(vq));
+    q.vidx = __dadd_rn(s.fH, vs);
     return q;
 }
 // the interpolation cell lies fully inside the stored half-plane grid
@@ -107,17 +110,14 @@ static __constant__ double SINCOS_COEF[16] = {
     6755399441055744.0 /* 1.5 * 2^52: keeps negative k in range */, 1.57079632679489661923, 4503599627370496.0 /* 2^52 */, 0.0};
 
 //
-// floor of 0 <= x < 2^31 as a double (*fl) and as an int (return): x + 2^52 rounds x to an integer in the
-// low mantissa bits; one compare fixes round-to-nearest into round-down.  fl is exactly floor(x), so the
-// fractional weight x - fl is bit-identical to the listing's.  (Only used for cells inside the grid.)
+// floor of 0 <= x < 2^31 as a double (*fl) and as an int (return): x + 2^52 in round-down mode leaves floor(x) in
+// the low mantissa bits.  fl is exactly floor(x), so the fractional weight x - fl is bit-identical to the
+// listing's.  (Values outside that range give a meaningless result, never a trap: callers discard it.)
 __device__ __forceinline__ int floor_small(double x, double* fl) {
     const double MAGIC = SINCOS_COEF[14];                // 2^52 (constant-bank operand)
-    const double t = __dadd_rn(x, MAGIC);
-    double r = __dsub_rn(t, MAGIC);                      // rint(x)
-    int i = __double2loint(t);
-    if (r > x) { r = __dsub_rn(r, 1.0); i -= 1; }
-    *fl = r;
-    return i;
+    const double t = __dadd_rd(x, MAGIC);                // rounded towards -inf: exactly floor(x) + 2^52, no fix-up
+    *fl = __dsub_rn(t, MAGIC);
+    return __double2loint(t);
 }
 
 // sin and cos of 2 pi t for t in turns, |t| < 2^49.  k = rint(4 t) from the same mantissa trick (exact), the
@@ -404,12 +404,12 @@ __device__ __forceinline__ void sample_points(const SampleParams<T>& p, SampleCt
         inside[j] = cell_inside(p.ix, q);
         uneg[j] = q.uneg;
         double fx0, fy0;
-        const int ix0 = floor_small(inside[j] ? q.uidx : 0.0, &fx0), iy0 = floor_small(inside[j] ? q.vidx : 0.0, &fy0);
+        const int ix0 = floor_small(q.uidx, &fx0), iy0 = floor_small(q.vidx, &fy0);      // (meaningless outside the grid)
         tx[j] = (R)__dsub_rn(q.uidx, fx0);               // (outside the grid the rare path below redoes this)
         ty[j] = (R)__dsub_rn(q.vidx, fy0);
         // theta / 2 pi in turns (exact range reduction in quarter_reduce)
         turns[j] = fma(q.urot, p.dRA_turns, q.vrot * p.dDec_turns);
-        const int off = ix0 * N + iy0;                   // 0 outside
+        const int off = inside[j] ? ix0 * N + iy0 : 0;   // outside the grid: any valid entry (the rare path below redoes the point)
         if (ix0 + 1 > cx_.ck_kumax || iy0 < cx_.ck_rmin || iy0 + 1 > cx_.ck_rmax || (!inside[j] && cx_.ck_kumax < N)) ++cx_.viol;
         const int off_partner = __shfl_xor_sync(0xffffffffu, off, 1);
         const int ia = (odd ? off_partner : off) + odd, ib = (odd ? off : off_partner) + odd;
@@ -472,11 +472,11 @@ __device__ __forceinline__ void sample_points_direct(const SampleParams<T>& p, S
         inside[j] = cell_inside(p.ix, q);
         uneg[j] = q.uneg;
         double fx0, fy0;
-        const int ix0 = floor_small(inside[j] ? q.uidx : 0.0, &fx0), iy0 = floor_small(inside[j] ? q.vidx : 0.0, &fy0);
+        const int ix0 = floor_small(q.uidx, &fx0), iy0 = floor_small(q.vidx, &fy0);      // (meaningless outside the grid)
         tx[j] = (R)__dsub_rn(q.uidx, fx0);
         ty[j] = (R)__dsub_rn(q.vidx, fy0);
         turns[j] = fma(q.urot, p.dRA_turns, q.vrot * p.dDec_turns);
-        const int off = ix0 * N + iy0;
+        const int off = inside[j] ? ix0 * N + iy0 : 0;
         if (ix0 + 1 > cx_.ck_kumax || iy0 < cx_.ck_rmin || iy0 + 1 > cx_.ck_rmax || (!inside[j] && cx_.ck_kumax < N)) ++cx_.viol;
         if (PAIR) {
             const NodePair<T> e0 = load_pair(spec + off), e1 = load_pair(spec + off + 1);
