@@ -841,6 +841,90 @@ row_pass_x2_kernel(const RowParams<T> p) {
     }
 }
 
+// The same row, split over a CLUSTER of two CTAs (nxy = 16384): CTA r of the pair transforms the samples 2 m + r
+// of the packed sequence (one 4096-point transform, 256 threads, 70 KB: two CTAs of different rows fit an SM, so one
+// row's load overlaps another row's arithmetic — the one-CTA form holds a whole SM and serialises them).  After a
+// cluster barrier each CTA forms the outputs X[k] of its parity of k; the radix-2 combination and the untangle read
+// E from the even CTA and O from the odd one, the partner's through distributed shared memory (`mapa` +
+// `ld.shared::cluster`): four 16-byte reads per output, a few hundred outputs per row when the transform is pruned.
+__device__ __forceinline__ uint32_t cluster_rank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ void cluster_barrier() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ uint32_t map_to_rank(uint32_t saddr, uint32_t rank) {
+    uint32_t r; asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(rank)); return r;
+}
+__device__ __forceinline__ double2 ld_cluster(uint32_t addr, double) {
+    double2 v; asm volatile("ld.shared::cluster.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr) : "memory"); return v;
+}
+__device__ __forceinline__ float2 ld_cluster(uint32_t addr, float) {
+    float2 v; asm volatile("ld.shared::cluster.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr) : "memory"); return v;
+}
+
+template <typename T, int R1, int R2, int R3, bool SWEEP>
+__global__ void __launch_bounds__(Geom<T, R1, R2, R3, 1>::NT, 2)
+row_pass_c2_kernel(const RowParams<T> p) {
+    using G = Geom<T, R1, R2, R3, 1>;
+    constexpr int LH = G::L;                   // = N / 4: length of this CTA's transform
+    constexpr int L = 2 * LH;                  // = N / 2: length of the packed complex row
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cx<T>* S = reinterpret_cast<cx<T>*>(smem_raw);
+    const int t = threadIdx.x;
+    const int N = p.N;
+    const uint32_t r = cluster_rank();
+    const long long row = blockIdx.x >> 1;
+    if (!SWEEP && r == 0) prefetch_row_block(p, row, 1);
+    pdl_wait();
+    if (SWEEP) {
+        const int i = (int)(row % N);
+        fft_steps12<T, R1, R2, R3, G::TPF>(S, t, p.tw, 4, [&](int m) -> cx<T> {
+            const int n = 2 * m + (int)r;
+            return mk<T>((T)sweep_pixel<T>(p.sweep, N, i, 2 * n), (T)sweep_pixel<T>(p.sweep, N, i, 2 * n + 1));
+        });
+    } else {
+        const cx<T>* z = reinterpret_cast<const cx<T>*>(p.image + row * (long long)N);
+        fft_steps12<T, R1, R2, R3, G::TPF>(S, t, p.tw, 4, [&](int m) -> cx<T> { return __ldcs(z + 2 * m + (int)r); });
+    }
+    if (R3 > 1) {                              // step 3, in place
+        for (int it = t; it < R1 * R2; it += G::TPF) {
+            const int k1 = it % R1, c = it / R1;
+            cx<T>* base = S + k1 * G::P1 + c * R3;
+            cx<T> a[R3];
+#pragma unroll
+            for (int b = 0; b < R3; ++b) a[b] = base[b];
+            Dft<T, R3>::run(a);
+#pragma unroll
+            for (int d = 0; d < R3; ++d) base[d] = a[d];
+        }
+    }
+    cluster_barrier();                         // both halves complete and visible across the pair
+    const uint32_t mine = smem_u32(S), theirs = map_to_rank(mine, r ^ 1u);
+    const uint32_t sE = r == 0 ? mine : theirs, sO = r == 0 ? theirs : mine;
+    // Z[k] = E[k] + W_L^k O[k] (k < L/2), Z[k + L/2] = E[k] - W_L^k O[k]
+    auto Z = [&](int k) -> cx<T> {
+        const int a = k < LH ? k : k - LH;
+        const uint32_t off = (uint32_t)(G::zaddr(a) * sizeof(cx<T>));
+        const cx<T> E = ld_cluster(sE + off, T()), O = ld_cluster(sO + off, T());
+        const cx<T> WO = cmul(__ldg(p.tw + 2 * a), O);
+        return k < LH ? cadd(E, WO) : csub(E, WO);
+    };
+    const int NU = N / 2 + 1;
+    const int i = (int)(row % N);
+    const int pos = (i & 3) * (N >> 2) + (i >> 2);           // decimated by four for the column transform
+    cx<T>* out = p.spec + (row / N) * (long long)NU * N + pos;
+    const int kumax = __ldg(p.ext);
+    const int kend = kumax < L / 2 ? kumax : L / 2;
+    for (int k = 2 * t + (int)r; k <= kend; k += 2 * G::NT) {   // this CTA: k of its own parity; untangle as row_pass_x2
+        const cx<T> zk = Z(k), zm = Z((L - k) % L);
+        const cx<T> E = mk<T>(zk.x + zm.x, zk.y - zm.y);
+        const cx<T> O = mk<T>(zk.y + zm.y, zm.x - zk.x);
+        const cx<T> WO = cmul(__ldg(p.tw + k), O);
+        out[(long long)k * N] = cadd(E, WO);
+        if (L - k <= kumax) { cx<T> xm = csub(E, WO); xm.y = -xm.y; out[(long long)(L - k) * N] = xm; }
+    }
+    cluster_barrier();                         // the partner may still be reading this CTA's shared memory
+}
+
 // One quarter column (n1 = blockIdx.x & 3) per CTA: DFT_{N/4} in place, then times W_N^(n1 k2).
 template <typename T, int R1, int R2, int R3>
 __global__ void __launch_bounds__(Geom<T, R1, R2, R3, 1>::NT)

@@ -125,7 +125,21 @@ int launch_fft_16384(gal_plan* p, const T* image, const SweepParams* sw, int bat
     rp.rows_total = batch * p->nxy; rp.ext = ext; rp.pf_blocks = 0;
     if (sw) rp.sweep = *sw; else memset(&rp.sweep, 0, sizeof(rp.sweep));
     int rc;
-    if (sw) {
+    static const bool one_cta = getenv("GAL_ROW_X2_ONE_CTA") != nullptr;     // diagnostic: the one-CTA-per-row form
+    if (!one_cta) {
+        // a cluster of two CTAs per row (fft.cuh: row_pass_c2_kernel)
+        const unsigned grid = 2u * (unsigned)rp.rows_total;
+        if (sw) {
+            auto k = row_pass_c2_kernel<T, 16, 16, 16, true>;
+            if ((rc = set_smem(p, k, GC::SMEM))) return rc;
+            GAL_CUDA(p, launch_chain_cluster(k, dim3(grid), dim3(GC::NT), GC::SMEM, 2u, st, rp));
+        } else {
+            auto k = row_pass_c2_kernel<T, 16, 16, 16, false>;
+            if ((rc = set_smem(p, k, GC::SMEM))) return rc;
+            rp.pf_blocks = resident_ctas(p, k, GC::NT, GC::SMEM) / 2;        // (in rows)
+            GAL_CUDA(p, launch_chain_cluster(k, dim3(grid), dim3(GC::NT), GC::SMEM, 2u, st, rp));
+        }
+    } else if (sw) {
         auto k = row_pass_x2_kernel<T, 16, 16, 16, true>;
         if ((rc = set_smem(p, k, GR::SMEM))) return rc;
         GAL_CUDA(p, launch_chain(k, dim3((unsigned)rp.rows_total), dim3(GR::NT), GR::SMEM, st, rp));
