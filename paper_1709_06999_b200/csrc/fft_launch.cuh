@@ -215,7 +215,17 @@ int fft2(gal_plan* p, const T* image, const SweepParams* sw, int batch, const in
         if (rc) return rc;                                                       \
         return launch_col<T, COL>(p, batch, ext, st);                            \
     }
-        GAL_FFT_CASE_PIPE(1024, RR(8, 8, 8, 4), RR(16, 8, 4, 8), RR(16, 8, 8, 4))
+        case 1024: {
+            const int mode = sw ? 0 : (p->row_mode >= 0 ? p->row_mode : RowPipeCfg<T>::default_mode(1024));
+            // rows: eight per CTA when the batch fills the GPU several times over (cfg 4: 417 -> 406 us), else four
+            const bool many = (long long)batch * 1024 / 8 >= 4LL * p->sm_count;
+            rc = mode ? launch_row_pipe<T, 16, 8, 4, 8, RowPipeCfg<T>::NG, RowPipeCfg<T>::NS>(p, image, sw, batch, ext, mode == 2, st)
+                      : many ? launch_row<T, 8, 8, 8, 8>(p, image, sw, batch, ext, st)
+                             : launch_row<T, 8, 8, 8, 4>(p, image, sw, batch, ext, st);
+            if (rc) return rc;
+            // columns: two per CTA (128 threads, five CTAs per SM) instead of four: cfg 4 column pass 422 -> 357 us
+            return launch_col<T, 16, 8, 8, 2>(p, batch, ext, st);
+        }
         case 2048: {
             int mode = sw ? 0 : (p->row_mode >= 0 ? p->row_mode : RowPipeCfg<T>::default_mode(2048));
             // as at 4096 (below): one row per CTA where the plan expects a pruned extent (cfg 2: row pass 20.8 -> 18.7 us)
