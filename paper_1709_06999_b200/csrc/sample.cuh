@@ -304,12 +304,15 @@ __global__ void __launch_bounds__(256, 4) uv_extent_kernel(const ExtentParams p,
 #ifndef GAL_SAMPLE_MINB
 #define GAL_SAMPLE_MINB 2
 #endif
+#ifndef GAL_SAMPLE_NT
+#define GAL_SAMPLE_NT 256            // consumer threads per CTA
+#endif
 
 // The unit of work is a tile of 256*U consecutive points; CTA b takes tiles b, b + gridDim.x, ...; thread t
 // of the 256 consumer threads takes points t, t + 256, ... of the tile.
 template <typename T, bool DO_CHI2> struct SampleGeom {
     static constexpr int U = GAL_SAMPLE_U;
-    static constexpr int NT = 256, NW = NT / 32;                    // consumer threads / warps
+    static constexpr int NT = GAL_SAMPLE_NT, NW = NT / 32;         // consumer threads / warps
     static constexpr int NT_TMA = NT + 32;                          // + one producer warp (TMA kernel)
     static constexpr int TILE = NT * U;
     static constexpr int NARR = DO_CHI2 ? 5 : 2;
@@ -598,12 +601,12 @@ __device__ __forceinline__ void sample_tile_plain(const SampleParams<T>& p, Samp
     const T* __restrict__ g3 = DO_CHI2 ? p.im_obs + c * M : nullptr;
     const T* __restrict__ g4 = DO_CHI2 ? p.w + c * M : nullptr;
     auto ld = [&](int a, int j) -> T {
-        const long long k = k0 + j * 256;
+        const long long k = k0 + j * GAL_SAMPLE_NT;
         if (k >= M) return (T)0;
         const T* g = a == 0 ? g0 : a == 1 ? g1 : a == 2 ? g2 : a == 3 ? g3 : g4;
         return __ldcs(g + k);
     };
-    auto kpt = [&](int j) -> long long { return k0 + j * 256; };
+    auto kpt = [&](int j) -> long long { return k0 + j * GAL_SAMPLE_NT; };
     sample_points<T, WRITE_VIS, DO_CHI2, EXACT, U, PAIR>(p, cx_, ld, kpt, M, c);
 }
 
@@ -626,7 +629,7 @@ __device__ __forceinline__ SampleCtx<T> sample_ctx(const SampleParams<T>& p, int
 
 // General kernel (256 threads): any alignment, any du (takes the true division when the shortcut is not valid).
 template <typename T, bool WRITE_VIS, bool DO_CHI2>
-__global__ void __launch_bounds__(256, GAL_SAMPLE_MINB) sample_kernel_plain(const SampleParams<T> p) {
+__global__ void __launch_bounds__(GAL_SAMPLE_NT, GAL_SAMPLE_MINB) sample_kernel_plain(const SampleParams<T> p) {
     using G = SampleGeom<T, DO_CHI2>;
     const int c = blockIdx.y;
     const long long M = p.M;
@@ -697,8 +700,8 @@ __global__ void __launch_bounds__(SampleGeom<T, DO_CHI2>::NT_TMA, GAL_SAMPLE_MIN
             for (; tile < nfull; tile += gridDim.x) {
                 mbar_wait(full0 + 8 * stage, parity);
                 const T* st = reinterpret_cast<const T*>(sample_smem + stage * G::STAGE_BYTES) + tid;
-                auto ld = [&](int a, int j) -> T { return st[a * TILE + j * 256]; };
-                auto kpt = [&](int j) -> long long { return (long long)tile * TILE + j * 256 + tid; };
+                auto ld = [&](int a, int j) -> T { return st[a * TILE + j * GAL_SAMPLE_NT]; };
+                auto kpt = [&](int j) -> long long { return (long long)tile * TILE + j * GAL_SAMPLE_NT + tid; };
                 if (DIRECT) sample_points_direct<T, WRITE_VIS, DO_CHI2, false, U, PAIR>(p, cx_, ld, kpt, M, c);
                 else sample_points<T, WRITE_VIS, DO_CHI2, false, U, PAIR>(p, cx_, ld, kpt, M, c);
                 __syncwarp();                                // every lane has read its last value of this stage
