@@ -295,6 +295,9 @@ __global__ void __launch_bounds__(256, 4) uv_extent_kernel(const ExtentParams p,
 
 // Points per thread and tile (U), stages of the shared-memory ring, resident CTAs per SM the register
 // budget is set for.
+#ifndef GAL_SAMPLE_U32
+#define GAL_SAMPLE_U32 2             // points per thread and tile in fp32
+#endif
 #ifndef GAL_SAMPLE_U
 #define GAL_SAMPLE_U 2
 #endif
@@ -311,7 +314,7 @@ __global__ void __launch_bounds__(256, 4) uv_extent_kernel(const ExtentParams p,
 // The unit of work is a tile of 256*U consecutive points; CTA b takes tiles b, b + gridDim.x, ...; thread t
 // of the 256 consumer threads takes points t, t + 256, ... of the tile.
 template <typename T, bool DO_CHI2> struct SampleGeom {
-    static constexpr int U = GAL_SAMPLE_U;
+    static constexpr int U = sizeof(T) == 4 ? GAL_SAMPLE_U32 : GAL_SAMPLE_U;
     static constexpr int NT = GAL_SAMPLE_NT, NW = NT / 32;         // consumer threads / warps
     static constexpr int NT_TMA = NT + 32;                          // + one producer warp (TMA kernel)
     static constexpr int TILE = NT * U;
