@@ -276,22 +276,19 @@ __device__ __forceinline__ void prefetch_row_block(const RowParams<T>& p, long l
     if (row < p.rows_total) l2_prefetch_bulk(p.image + row * (long long)p.N, (uint32_t)(p.N * sizeof(T)));
 }
 
+// One block of F image rows (block index vb): transform, untangle, transposed write.  Shared by the row-pass kernel
+// (one block per CTA) and the conditional second pass of a call (redo_kernel).
 template <typename T, int R1, int R2, int R3, int F, bool SWEEP>
-__global__ void __launch_bounds__(Geom<T, R1, R2, R3, F>::NT)
-row_pass_kernel(const RowParams<T> p) {
+__device__ __forceinline__ void row_block(const RowParams<T>& p, const long long vb, cx<T>* smem) {
     using G = Geom<T, R1, R2, R3, F>;
     constexpr int L = G::L;                    // = N / 2
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    cx<T>* smem = reinterpret_cast<cx<T>*>(smem_raw);
     const int tid = threadIdx.x;
     const int f = tid / G::TPF, t = tid % G::TPF;
     const int N = p.N;
-    const long long row0 = (long long)blockIdx.x * F;
+    const long long row0 = vb * F;
     const long long row = row0 + f;
     const bool valid = row < p.rows_total;
     cx<T>* S = smem + f * G::REGION;
-    if (!SWEEP) prefetch_row_block(p, blockIdx.x, F);
-    pdl_wait();
 
     if (SWEEP) {
         const int i = (int)(row % N);
@@ -345,6 +342,15 @@ row_pass_kernel(const RowParams<T> p) {
         out[(long long)k * N + ff] = xk;
         if (L - k <= kumax) out[(long long)(L - k) * N + ff] = xm;
     }
+}
+
+template <typename T, int R1, int R2, int R3, int F, bool SWEEP>
+__global__ void __launch_bounds__(Geom<T, R1, R2, R3, F>::NT)
+row_pass_kernel(const RowParams<T> p) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    if (!SWEEP) prefetch_row_block(p, blockIdx.x, F);
+    pdl_wait();
+    row_block<T, R1, R2, R3, F, SWEEP>(p, blockIdx.x, reinterpret_cast<cx<T>*>(smem_raw));
 }
 
 // ------------------------------------------------------------------------------------------
@@ -588,36 +594,27 @@ template <typename T> struct ColParams {
     int pf_groups;         // > 0: CTA b asks the L2 for the columns of CTA b + pf_groups (whole-plane transforms only)
 };
 
+// One group of F adjacent columns, g0 .. g0 + F - 1 of the u-major work array: transform, sign / row folds, write
+// the sampled spectrum.  Shared by the column-pass kernel and the conditional second pass of a call (redo_kernel).
 template <typename T, int R1, int R2, int R3, int F>
-__global__ void __launch_bounds__(Geom<T, R1, R2, R3, F>::NT)
-col_pass_kernel(const ColParams<T> p) {
+__device__ __forceinline__ void col_block(const ColParams<T>& p, const long long g0, cx<T>* smem) {
     using G = Geom<T, R1, R2, R3, F>;
     constexpr int L = G::L;                    // = N
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    cx<T>* smem = reinterpret_cast<cx<T>*>(smem_raw);
     const int tid = threadIdx.x;
     const int f = tid / G::TPF, t = tid % G::TPF;
     const int NU = L / 2 + 1;
-    pdl_wait();
     // uv extent: columns beyond kumax are skipped, rows outside [rmin, rmax] are not written
     const int kumax = __ldg(p.ext), rmin = __ldg(p.ext + 1), rmax = __ldg(p.ext + 2);
     const bool single = extent_is_whole_plane(p.ext, L);
     cx<T>* S = smem + f * G::REGION;
-    // whole plane: the row-transformed image comes back from HBM (a pruned one is still in the L2): ask the L2 for
-    // the columns of the CTA that will take this one's place
-    if (single && p.pf_groups > 0 && tid < F) {
-        const long long gg = ((long long)blockIdx.x + p.pf_groups) * F + tid;
-        if (gg < p.cols_total) l2_prefetch_bulk(p.work + gg * (long long)L, (uint32_t)(L * sizeof(cx<T>)));
-    }
     {
-        const long long grp = blockIdx.x;                   // one group of F columns per CTA
-        const long long g = grp * F + f;
+        const long long g = g0 + f;
         const int ku = (int)(g % NU);
         {
             bool any = false;
 #pragma unroll
             for (int ff = 0; ff < F; ++ff) {
-                const long long gg = grp * F + ff;
+                const long long gg = g0 + ff;
                 any = any || (gg < p.cols_total && (int)(gg % NU) <= kumax);
             }
             if (!any) return;
@@ -678,7 +675,6 @@ col_pass_kernel(const ColParams<T> p) {
                 for (int d = 0; d < R3; ++d) base[d] = mk<T>(sgn * a[d].x, sgn * a[d].y);
             }
             __syncthreads();
-            const long long g0 = grp * F;
             for (int idx = tid; idx < F * L; idx += G::NT) {
                 const int ff = idx / L, kvs = idx % L;
                 const long long gg = g0 + ff;
@@ -700,6 +696,21 @@ col_pass_kernel(const ColParams<T> p) {
             }
         }
     }
+}
+
+template <typename T, int R1, int R2, int R3, int F>
+__global__ void __launch_bounds__(Geom<T, R1, R2, R3, F>::NT)
+col_pass_kernel(const ColParams<T> p) {
+    constexpr int L = Geom<T, R1, R2, R3, F>::L;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    pdl_wait();
+    // whole plane: the row-transformed image comes back from HBM (a pruned one is still in the L2): ask the L2 for
+    // the columns of the CTA that will take this one's place
+    if (p.pf_groups > 0 && threadIdx.x < F && extent_is_whole_plane(p.ext, L)) {
+        const long long gg = ((long long)blockIdx.x + p.pf_groups) * F + threadIdx.x;
+        if (gg < p.cols_total) l2_prefetch_bulk(p.work + gg * (long long)L, (uint32_t)(L * sizeof(cx<T>)));
+    }
+    col_block<T, R1, R2, R3, F>(p, (long long)blockIdx.x * F, reinterpret_cast<cx<T>*>(smem_raw));   // one group of F columns per CTA
 }
 
 // ------------------------------------------------------------------------------------------

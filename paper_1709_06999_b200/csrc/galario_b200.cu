@@ -21,6 +21,7 @@ extern "C" int gal_plan_unbind_obs(gal_plan* p);
 namespace {
 
 inline bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+inline bool aligned_to(const void* q, size_t n) { return ((uintptr_t)q % n) == 0; }
 
 // ---------------------------------------------------------------------------------------------
 // per-call scalars, uv extent, sampling launcher
@@ -132,14 +133,26 @@ int run_call(gal_plan* p, const T* image, const SweepParams* sw, int C, double d
         p->last_pruned = false;
         ext = p->b_ext_dev;
     }
-    if (p->last_pruned) {
+    // speculative extent (plan.h): possible where this call would otherwise run the uv-extent kernel; an image call on
+    // 16-byte aligned arrays (the sampler's TMA form) at a size the conditional second pass is built for
+    const bool all16 = aligned_to(u, 16) && aligned_to(v, 16) && (vis || (aligned_to(re, 16) && aligned_to(im, 16) && aligned_to(w, 16)));
+    const bool can_spec = p->last_pruned && p->prune_mode == 1 && C == 1 && M > 0 && image && !sw && !p->spec_off && all16 &&
+                          (p->nxy == 2048 || p->nxy == 4096) &&
+                          (2.0 * sizeof(T) * (double)M >= p->spec_min_bytes);   // (a short extent pass costs no more than the conditional launch)
+    const bool speculate = can_spec && p->spec_valid && p->spec_dxy == dxy && p->spec_stream == st;
+    p->last_spec = speculate;
+    p->spec_mode = speculate ? 2 : (can_spec ? 1 : 0);
+    if (speculate) {
+        p->last_pruned = false;
+        ext = p->spec_E(p->spec_par);
+    } else if (p->last_pruned) {
         if ((rc = launch_extent<T>(p, C, cs, u, v, M, st))) return rc;
         ext = p->ext;
     }
     if (p->tmark(1, st)) return GAL_ERR_CUDA;
     p->cur_ext = ext;
     p->row_small = p->last_bound ? p->b_ext[0] < p->nxy / 2
-                                 : (p->last_pruned && ((volatile unsigned int*)p->viol_host)[1] == 2u);
+                                 : ((p->last_pruned || speculate) && ((volatile unsigned int*)p->viol_host)[1] == 2u);
     if (M == 0) return launch_sample<T>(p, C, cs, u, v, re, im, w, M, vis, chi2_pc, chi2_tot, true, st);
     const int G = batch_chunk(p, C);
     const size_t n2 = (size_t)p->nxy * p->nxy;
@@ -152,14 +165,19 @@ int run_call(gal_plan* p, const T* image, const SweepParams* sw, int C, double d
         if ((rc = launch_sample<T>(p, g, cs, u + o, v + o, re ? re + o : nullptr, im ? im + o : nullptr, w ? w + o : nullptr, M,
                                    vis ? vis + 2 * o : nullptr, chi2_pc ? chi2_pc + c0 : nullptr, G >= C ? chi2_tot : nullptr, last, st)))
             return rc;
+        // speculative call: the conditional second pass (it leaves at once unless the sampler found a point outside)
+        if (speculate && (rc = launch_redo<T>(p, image, cs, u, v, re, im, w, M, vis, chi2_pc, chi2_tot, st))) return rc;
         if (p->tmark(4, st)) return GAL_ERR_CUDA;
+    }
+    if (p->spec_mode != 0) {                   // the sampler has derived (will have, in stream order) the next extent
+        p->spec_par ^= 1;
+        p->spec_valid = true; p->spec_dxy = dxy; p->spec_stream = st;
+        p->spec_mode = 0;
     }
     if (G < C && chi2_tot && (rc = launch_sum_channels<T>(p, chi2_pc, C, chi2_tot, st))) return rc;
     if (p->t_on) { p->t_calls++; p->t_on = false; }
     return GAL_OK;
 }
-
-inline bool aligned_to(const void* q, size_t n) { return ((uintptr_t)q % n) == 0; }
 
 template <typename T> bool prec_ok(const gal_plan* p) { return p && p->bits == (int)(8 * sizeof(T)); }
 
@@ -223,7 +241,7 @@ int do_hankel(gal_plan* p, const T* I, int nr, double Rmin, double dR, const T* 
     }
     int rc;
     if ((rc = reset_call_state(p, st))) return rc;
-    p->last_pruned = false; p->last_bound = false; p->last_obs = false;
+    p->last_pruned = false; p->last_bound = false; p->last_obs = false; p->last_spec = false; p->spec_mode = 0;
     const CallScalars cs = call_scalars(p, 1.0 / p->nxy, dRA, dDec, PA);      // only the rotation and the phase are used
     return launch_hankel<T>(p, sw, cs, u, v, re, im, w, M, vis, vis ? nullptr : chi2, st);
 }
@@ -293,7 +311,7 @@ int do_multi(gal_plan* p, const T* image, double dxy, const T* u, const T* v, co
     }
     if ((rc = reset_call_state(p, st))) return rc;
     const CallScalars cs0 = call_scalars(p, dxy, 0.0, 0.0, 0.0);
-    p->last_bound = false; p->last_obs = false;
+    p->last_bound = false; p->last_obs = false; p->last_spec = false; p->spec_mode = 0;
     p->last_pruned = want_prune<T>(p, 1, M);
     const int* ext = p->ext_full;
     const bool uv_bound = p->b_u == (const void*)u && p->b_v == (const void*)v && p->b_M == M && p->b_C == 1;
@@ -467,6 +485,10 @@ int gal_plan_create(gal_plan** out, int nxy, int batch, int precision_bits, int 
     if ((e = cudaMalloc((void**)&p->ext_full, 16)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     if ((e = cudaMalloc((void**)&p->b_ext_dev, 16)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     if ((e = cudaMalloc((void**)&p->b_r2, 8)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
+    if ((e = cudaMalloc(&p->spec_state, 64)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
+    if ((e = cudaMemset(p->spec_state, 0, 64)) != cudaSuccess) return fail(GAL_ERR_CUDA, e);
+    p->spec_off = getenv("GAL_NO_SPEC") != nullptr;
+    if (const char* e2 = getenv("GAL_SPEC_MIN_BYTES")) p->spec_min_bytes = atof(e2);      // diagnostic / tests
     if ((e = cudaHostAlloc((void**)&p->viol_host, 2 * sizeof(unsigned int), cudaHostAllocMapped)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     p->viol_host[0] = 0; p->viol_host[1] = 0;          // [1]: extent hint (plan.h row_small)
     if ((e = cudaHostGetDevicePointer((void**)&p->viol_dev, p->viol_host, 0)) != cudaSuccess) return fail(GAL_ERR_CUDA, e);
@@ -512,7 +534,7 @@ int gal_plan_destroy(gal_plan* p) {
     cudaFree(p->spec); cudaFree(p->work); cudaFree(p->tw); cudaFree(p->partials); cudaFree(p->tickets);
     for (auto& m : p->tev) cudaEventDestroy(m.ev);
     cudaFree(p->o_buf); if (p->viol_host) cudaFreeHost(p->viol_host);
-    cudaFree(p->call_state); cudaFree(p->call_init); cudaFree(p->ext_full); cudaFree(p->b_ext_dev); cudaFree(p->b_r2); cudaFree(p->st_vis); cudaFree(p->st_image); cudaFree(p->st_pts); cudaFree(p->st_out); cudaFree(p->st_chi2);
+    cudaFree(p->call_state); cudaFree(p->call_init); cudaFree(p->ext_full); cudaFree(p->b_ext_dev); cudaFree(p->b_r2); cudaFree(p->spec_state); cudaFree(p->st_vis); cudaFree(p->st_image); cudaFree(p->st_pts); cudaFree(p->st_out); cudaFree(p->st_chi2);
     delete p;
     return GAL_OK;
 }
@@ -556,6 +578,7 @@ int gal_last_uv_extent(gal_plan* p, int* extent) {
     DeviceGuard g(p->device);
     GAL_CUDA(p, cudaStreamSynchronize(p->last_stream));
     if (p->last_bound) { extent[0] = p->b_ext[0]; extent[1] = p->b_ext[1]; extent[2] = p->b_ext[2]; return GAL_OK; }
+    if (p->last_spec) { GAL_CUDA(p, cudaMemcpy(extent, p->spec_used(), 3 * sizeof(int), cudaMemcpyDeviceToHost)); return GAL_OK; }
     GAL_CUDA(p, cudaMemcpy(extent, p->last_pruned ? p->ext : p->ext_full, 3 * sizeof(int), cudaMemcpyDeviceToHost));
     return GAL_OK;
 }

@@ -57,6 +57,26 @@ struct gal_plan {
     // the whole half plane, 2 = it was pruned.  The host reads it WITHOUT synchronising when it picks the row-pass
     // variant of the next call (a stale value costs time, never correctness): row_small = "expect a pruned extent".
     bool row_small = false;
+    // Speculative extent (automatic pruning mode, one image per call, unbound uv, nxy 2048 / 4096): instead of a
+    // uv-extent kernel in front of every call, the transform is pruned to the extent the previous call's sampler
+    // derived from the largest baseline length of its points (rotation-invariant); the sampler verifies every point
+    // against it and derives the extent for the next call; if a point lay outside, ONE conditional kernel (redo.cuh:
+    // it leaves at once unless the device flag `redo` is set) repeats transform and sampling on the new extent.
+    // No host synchronisation, results unchanged.
+    // spec_state (device, 64 B): [0] u64 r2max | [8] int E[2][4] | [40] u32 redo | [44] int used_ext[3] | [56] u32 bar[2]
+    void* spec_state = nullptr;
+    int spec_par = 0;                    // E[spec_par] is the extent the next speculative call transforms
+    bool spec_valid = false;             // E[spec_par] has been (will have been, in stream order) written ...
+    double spec_dxy = 0.0;               // ... for this pixel size
+    cudaStream_t spec_stream = nullptr;  // ... on this stream
+    int spec_mode = 0;                   // the launch being issued: 0 none, 1 derive only, 2 verify + derive
+    bool spec_off = false;               // GAL_NO_SPEC (diagnostic)
+    double spec_min_bytes = 32e6;        // speculate only where the uv-extent pass would read at least this much (cfg 2, 16 MB: 42.0 against 44.5 us)
+    bool last_spec = false;              // the most recent call speculated
+    int* spec_E(int par) const { return (int*)((char*)spec_state + 8 + 16 * par); }
+    unsigned int* spec_redo() const { return (unsigned int*)((char*)spec_state + 40); }
+    int* spec_used() const { return (int*)((char*)spec_state + 44); }
+    unsigned int* spec_bar() const { return (unsigned int*)((char*)spec_state + 56); }
     void* st_vis = nullptr; size_t st_vis_bytes = 0; // summed visibilities of a chi2 multi-source call
     std::set<const void*> smem_set;      // kernels whose dynamic shared-memory limit has been raised
     std::map<const void*, int> resident; // kernel -> CTAs resident on the whole GPU at once (occupancy x SM count)
@@ -162,6 +182,10 @@ template <typename T> int launch_transpose(gal_plan* p, T* out, cudaStream_t st)
 template <typename T> int launch_extent(gal_plan* p, int C, const CallScalars& cs, const T* u, const T* v, int64_t M, cudaStream_t st);
 template <typename T> int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T* v, const T* re, const T* im,
                                         const T* w, int64_t M, T* vis, double* chi2_pc, double* chi2_tot, bool last, cudaStream_t st);
+// conditional second pass of a speculative call: one persistent kernel (row pass, column pass, sampling behind grid
+// barriers) on the extent E[spec_par ^ 1]; it does nothing unless the sampler before it raised the redo flag
+template <typename T> int launch_redo(gal_plan* p, const T* image, const CallScalars& cs, const T* u, const T* v, const T* re,
+                                      const T* im, const T* w, int64_t M, T* vis, double* chi2_pc, double* chi2_tot, cudaStream_t st);
 template <typename T> int launch_sum_channels(gal_plan* p, const double* chi2_pc, int C, double* chi2_tot, cudaStream_t st);
 template <typename T> int launch_chi2_from_vis(gal_plan* p, const T* vis, const T* re, const T* im, const T* w, int64_t M,
                                                double* chi2, cudaStream_t st);

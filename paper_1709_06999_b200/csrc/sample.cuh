@@ -50,6 +50,16 @@ template <typename T> struct SampleParams {
     int rearm;                // 1: the last CTA of this launch re-arms next_state (every launch but the non-final chunks of a long multi-source list)
     unsigned int* viol_flag;  // mapped host memory: set when viol becomes non-zero (sticky, read by the next call)
     unsigned int* ext_hint;   // mapped host memory or null: 1 = this call's extent was the whole plane, 2 = pruned (plan.h)
+    // Speculative extent (galario_b200.cu: run_call; the SPEC instantiation of the TMA kernel).  The transform of this
+    // call was pruned to the extent the PREVIOUS call derived; this kernel verifies every point against it (ext_check,
+    // viol), reduces max(u^2 + v^2) of ITS points as a by-product of the pass it makes over u and v anyway, and its
+    // last CTA turns that into the extent for the next call (spec_out) and raises `redo` if a point lay outside: the
+    // conditional second pass (fft.cuh / sample.cuh: redo_kernel, which leaves at once otherwise) then repeats
+    // transform and sampling on spec_out, which covers every point by construction.
+    unsigned long long* r2max;    // atomicMax of the bit pattern of u^2 + v^2 (SPEC only)
+    int* spec_out;                // [3] not null: the last CTA writes the extent derived from r2max here and re-arms r2max
+    unsigned int* redo;           // raised by the last CTA when viol != 0
+    int* used_ext;                // [3] the extent the final result was computed with (gal_last_uv_extent)
 };
 
 // Which layout did the column pass write?  Same rule as fft.cuh: extent_is_whole_plane.
@@ -347,6 +357,7 @@ template <typename T> struct SampleCtx {
     unsigned int oob;      // points of this thread beyond the half-plane grid
     unsigned int viol;     // points of this thread outside the extent of the bound uv set
     int ck_kumax, ck_rmin, ck_rmax;   // that extent ({N, 0, N}: nothing to check)
+    double r2;             // largest u^2 + v^2 of this thread's points (SPEC)
 };
 
 // Everything after the interpolation of one point: sign for u' < 0, phase, store / chi2 term.
@@ -393,7 +404,7 @@ __device__ __forceinline__ void point_tail(const SampleParams<T>& p, SampleCtx<T
 // single-copy layout and 126 for one 16-byte load per node and lane).  Each lane then interpolates its row
 // along u for both cells, one shuffle hands the row the partner needs across, and the owner finishes its
 // own point.
-template <typename T, bool WRITE_VIS, bool DO_CHI2, bool EXACT, int U, bool PAIR, typename LD, typename KP>
+template <typename T, bool WRITE_VIS, bool DO_CHI2, bool EXACT, int U, bool PAIR, bool SPEC = false, typename LD, typename KP>
 __device__ __forceinline__ void sample_points(const SampleParams<T>& p, SampleCtx<T>& cx_, LD ld, KP kpt, long long M,
                                               int c) {
     const int N = cx_.N, odd = cx_.odd;
@@ -406,6 +417,7 @@ __device__ __forceinline__ void sample_points(const SampleParams<T>& p, SampleCt
 #pragma unroll
     for (int j = 0; j < U; ++j) {
         const PointIndex q = point_index<EXACT>(p.ix, (double)ld(0, j), (double)ld(1, j));
+        if (SPEC) cx_.r2 = fmax(cx_.r2, fma(q.urot, q.urot, q.vrot * q.vrot));               // = u^2 + v^2 up to rounding (margin in the verdict)
         // bilinear interpolation
         inside[j] = cell_inside(p.ix, q);
         uneg[j] = q.uneg;
@@ -515,10 +527,18 @@ __device__ __forceinline__ void sample_points_direct(const SampleParams<T>& p, S
 // no floating-point atomics.  Also adds this CTA's out-of-grid count.
 template <typename T, bool DO_CHI2>
 __device__ __forceinline__ void sample_finish(const SampleParams<T>& p, int c, double acc, unsigned int oob,
-                                              unsigned int viol) {
-    if (p.ext_check) {                                       // rare: a bound uv set is being verified
+                                              unsigned int viol, double r2 = 0.0) {
+    if (p.ext_check) {                                       // a bound uv set or a speculative extent is being verified
         viol = __reduce_add_sync(0xffffffffu, viol);
-        if ((threadIdx.x & 31) == 0 && viol) { atomicAdd(p.viol, (unsigned long long)viol); *(volatile unsigned int*)p.viol_flag = 1u; }
+        if ((threadIdx.x & 31) == 0 && viol) {
+            atomicAdd(p.viol, (unsigned long long)viol);
+            if (p.viol_flag) *(volatile unsigned int*)p.viol_flag = 1u;
+        }
+    }
+    if (p.spec_out) {                                        // bit patterns of non-negative doubles order like integers
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) r2 = fmax(r2, __shfl_xor_sync(0xffffffffu, r2, o));
+        if ((threadIdx.x & 31) == 0) atomicMax(p.r2max, (unsigned long long)__double_as_longlong(r2));
     }
     __shared__ double wsum[32];
     __shared__ unsigned int woob[32];
@@ -536,8 +556,27 @@ __device__ __forceinline__ void sample_finish(const SampleParams<T>& p, int c, d
         unsigned int ob = 0;
         for (int i = 0; i < (int)(blockDim.x >> 5); ++i) { s += wsum[i]; ob += woob[i]; }
         if (ob) atomicAdd(p.oob, (unsigned long long)ob);
+        if (p.spec_out) __threadfence();                        // this CTA's atomics before its ticket
         // the last CTA of the launch re-arms the state of the next call: counter 0, extent = the dead-slot cell
         if (atomicAdd(p.done, 1u) == gridDim.x * gridDim.y - 1) {
+            if (p.spec_out) {                                   // speculative extent: by-product and verdict (SampleParams)
+                __threadfence();
+                const unsigned long long bits = atomicExch(p.r2max, 0ull);          // read and re-arm
+                const double imax = sqrt(__longlong_as_double((long long)bits)) * (1.0 + 1e-12) / p.ix.du;
+                const int H = p.N / 2;
+                int e0 = H, e1 = 0, e2 = p.N - 1;               // as extent_from_radius_kernel: two cells of margin
+                if (imax + 3.0 < (double)(H - 1)) {
+                    const int k = (int)imax + 2;
+                    e0 = k + 1; e1 = H - k - 1; e2 = H + k + 1;
+                }
+                p.spec_out[0] = e0; p.spec_out[1] = e1; p.spec_out[2] = e2;
+                // (a whole-plane extent covers every point, wrapped ones too: it cannot fail)
+                const bool failed = p.ext_check && !extent_is_whole(p.ext_check, p.N) && atomicAdd(p.viol, 0ull) != 0ull;
+                if (failed) { *p.redo = 1u; atomicExch(p.oob, 0ull); }              // the second pass counts again
+                p.used_ext[0] = failed ? e0 : __ldg(p.ext);
+                p.used_ext[1] = failed ? e1 : __ldg(p.ext + 1);
+                p.used_ext[2] = failed ? e2 : __ldg(p.ext + 2);
+            }
             if (p.rearm) {
                 int* nx = reinterpret_cast<int*>(p.next_state);
                 nx[0] = 0; nx[1] = 0;
@@ -593,7 +632,7 @@ __device__ __forceinline__ void sample_finish(const SampleParams<T>& p, int c, d
 }
 
 // One tile by plain (guarded) loads straight from global memory.
-template <typename T, bool WRITE_VIS, bool DO_CHI2, bool EXACT, bool PAIR>
+template <typename T, bool WRITE_VIS, bool DO_CHI2, bool EXACT, bool PAIR, bool SPEC = false>
 __device__ __forceinline__ void sample_tile_plain(const SampleParams<T>& p, SampleCtx<T>& cx_, long long tile, long long M,
                                                   int c) {
     constexpr int U = SampleGeom<T, DO_CHI2>::U, TILE = SampleGeom<T, DO_CHI2>::TILE;
@@ -610,7 +649,7 @@ __device__ __forceinline__ void sample_tile_plain(const SampleParams<T>& p, Samp
         return __ldcs(g + k);
     };
     auto kpt = [&](int j) -> long long { return k0 + j * GAL_SAMPLE_NT; };
-    sample_points<T, WRITE_VIS, DO_CHI2, EXACT, U, PAIR>(p, cx_, ld, kpt, M, c);
+    sample_points<T, WRITE_VIS, DO_CHI2, EXACT, U, PAIR, SPEC>(p, cx_, ld, kpt, M, c);
 }
 
 template <typename T>
@@ -625,6 +664,7 @@ __device__ __forceinline__ SampleCtx<T> sample_ctx(const SampleParams<T>& p, int
     cx_.acc = 0.0;
     cx_.oob = 0;
     cx_.viol = 0;
+    cx_.r2 = 0.0;
     cx_.ck_kumax = p.N; cx_.ck_rmin = 0; cx_.ck_rmax = p.N;
     if (p.ext_check) { cx_.ck_kumax = __ldg(p.ext_check); cx_.ck_rmin = __ldg(p.ext_check + 1); cx_.ck_rmax = __ldg(p.ext_check + 2); }
     return cx_;
@@ -656,7 +696,7 @@ __global__ void __launch_bounds__(GAL_SAMPLE_NT, GAL_SAMPLE_MINB) sample_kernel_
 // `full`, work, and release the stage.  No block-wide barrier in the loop: a consumer warp only ever waits
 // for data, the producer runs up to S tiles ahead.  The ragged last tile (if any) is read with plain loads
 // by the CTA whose turn it would have been.
-template <typename T, bool WRITE_VIS, bool DO_CHI2>
+template <typename T, bool WRITE_VIS, bool DO_CHI2, bool SPEC = false>
 __global__ void __launch_bounds__(SampleGeom<T, DO_CHI2>::NT_TMA, GAL_SAMPLE_MINB) sample_kernel_tma(const SampleParams<T> p) {
     using G = SampleGeom<T, DO_CHI2>;
     constexpr int U = G::U, TILE = G::TILE, S = G::S;
@@ -706,22 +746,22 @@ __global__ void __launch_bounds__(SampleGeom<T, DO_CHI2>::NT_TMA, GAL_SAMPLE_MIN
                 auto ld = [&](int a, int j) -> T { return st[a * TILE + j * GAL_SAMPLE_NT]; };
                 auto kpt = [&](int j) -> long long { return (long long)tile * TILE + j * GAL_SAMPLE_NT + tid; };
                 if (DIRECT) sample_points_direct<T, WRITE_VIS, DO_CHI2, false, U, PAIR>(p, cx_, ld, kpt, M, c);
-                else sample_points<T, WRITE_VIS, DO_CHI2, false, U, PAIR>(p, cx_, ld, kpt, M, c);
+                else sample_points<T, WRITE_VIS, DO_CHI2, false, U, PAIR, SPEC>(p, cx_, ld, kpt, M, c);
                 __syncwarp();                                // every lane has read its last value of this stage
                 if (lane == 0) mbar_arrive(empty0 + 8 * stage);
                 if (++stage == S) { stage = 0; parity ^= 1u; }
             }
             if (tile == nfull && (long long)nfull * TILE < M)    // the ragged last tile falls to this CTA
-                sample_tile_plain<T, WRITE_VIS, DO_CHI2, false, PAIR>(p, cx_, nfull, M, c);
+                sample_tile_plain<T, WRITE_VIS, DO_CHI2, false, PAIR, SPEC>(p, cx_, nfull, M, c);
         };
         const bool whole = extent_is_whole(p.ext, p.N);
-        if (DO_CHI2 && p.direct) {                           // (a bound observation set is a chi2 matter)
+        if (!SPEC && DO_CHI2 && p.direct) {                  // (a bound observation set is a chi2 matter)
             if (whole) consume(std::false_type{}, std::true_type{}); else consume(std::true_type{}, std::true_type{});
         } else {
             if (whole) consume(std::false_type{}, std::false_type{}); else consume(std::true_type{}, std::false_type{});
         }
     }
-    sample_finish<T, DO_CHI2>(p, c, cx_.acc, cx_.oob, cx_.viol);
+    sample_finish<T, DO_CHI2>(p, c, cx_.acc, cx_.oob, cx_.viol, cx_.r2);
 }
 
 // ------------------------------------------------------------------------------------------

@@ -40,15 +40,11 @@ int launch_sample_kernel(gal_plan* p, const SampleParams<T>& sp, dim3 grid, bool
     return GAL_OK;
 }
 
+// The parameter block of a sampling launch on the plan's current call state (shared with the conditional second
+// pass, redo.cuh).
 template <typename T>
-int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T* v, const T* re, const T* im,
-                  const T* w, int64_t M, T* vis, double* chi2_pc, double* chi2_tot, bool last, cudaStream_t st) {
-    const bool do_chi2 = (vis == nullptr);
-    if (M == 0) {
-        if (chi2_pc) GAL_CUDA(p, cudaMemsetAsync(chi2_pc, 0, sizeof(double) * C, st));
-        if (chi2_tot) GAL_CUDA(p, cudaMemsetAsync(chi2_tot, 0, sizeof(double), st));
-        return GAL_OK;
-    }
+SampleParams<T> make_sample_params(gal_plan* p, const CallScalars& cs, const T* u, const T* v, const T* re, const T* im, const T* w,
+                                   int64_t M, T* vis, double* chi2_pc, double* chi2_tot, bool last) {
     SampleParams<T> sp;
     sp.spec = (const NodePair<T>*)p->spec;
     sp.N = p->nxy;
@@ -71,6 +67,27 @@ int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T
     sp.ext_check = (p->last_bound && !p->last_obs && p->b_ext[0] < p->nxy / 2) ? p->b_ext_dev : nullptr;
     sp.viol_flag = p->viol_dev;
     sp.ext_hint = p->viol_dev + 1;
+    sp.r2max = nullptr; sp.spec_out = nullptr; sp.redo = p->spec_redo(); sp.used_ext = p->spec_used();
+    return sp;
+}
+
+template <typename T>
+int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T* v, const T* re, const T* im,
+                  const T* w, int64_t M, T* vis, double* chi2_pc, double* chi2_tot, bool last, cudaStream_t st) {
+    const bool do_chi2 = (vis == nullptr);
+    if (M == 0) {
+        if (chi2_pc) GAL_CUDA(p, cudaMemsetAsync(chi2_pc, 0, sizeof(double) * C, st));
+        if (chi2_tot) GAL_CUDA(p, cudaMemsetAsync(chi2_tot, 0, sizeof(double), st));
+        return GAL_OK;
+    }
+    SampleParams<T> sp = make_sample_params<T>(p, cs, u, v, re, im, w, M, vis, chi2_pc, chi2_tot, last);
+    // speculative extent (plan.h spec_mode): 1 = derive the next call's extent, 2 = verify this call's and derive
+    const bool spec = p->spec_mode == 1 || p->spec_mode == 2;
+    if (spec) {
+        sp.r2max = (unsigned long long*)p->spec_state;
+        sp.spec_out = p->spec_E(p->spec_par ^ 1);
+        if (p->spec_mode == 2) { sp.ext_check = p->cur_ext; sp.viol_flag = nullptr; }
+    }
     // one CTA works through tiles blockIdx.x, blockIdx.x + gridDim.x, ...: a whole number of CTAs per SM
     const int tile = SampleGeom<T, true>::TILE;
     const long long ntiles = (M + tile - 1) / tile;
@@ -87,8 +104,24 @@ int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T
     // the TMA path needs 16-byte aligned tiles in every channel (and a du fit for the division shortcut)
     bool tma = !cs.ix.du_exact_div && aligned16(u) && aligned16(v) && (C == 1 || ((size_t)M * sizeof(T)) % 16 == 0);
     if (do_chi2) tma = tma && aligned16(re) && aligned16(im) && aligned16(w);
-    int rc = do_chi2 ? launch_sample_kernel<T, false, true>(p, sp, grid, tma, st)
+    int rc;
+    if (spec) {                                   // (run_call only speculates on aligned arrays: the TMA kernel)
+        using G = SampleGeom<T, true>;
+        if (!tma) return GAL_ERR_INVALID_ARGUMENT;
+        if (do_chi2) {
+            auto k = sample_kernel_tma<T, false, true, true>;
+            if ((rc = set_smem(p, k, SampleGeom<T, true>::SMEM))) return rc;
+            GAL_CUDA(p, launch_chain(k, grid, dim3(G::NT_TMA), SampleGeom<T, true>::SMEM, st, sp));
+        } else {
+            auto k = sample_kernel_tma<T, true, false, true>;
+            if ((rc = set_smem(p, k, SampleGeom<T, false>::SMEM))) return rc;
+            GAL_CUDA(p, launch_chain(k, grid, dim3(G::NT_TMA), SampleGeom<T, false>::SMEM, st, sp));
+        }
+        rc = GAL_OK;
+    } else {
+        rc = do_chi2 ? launch_sample_kernel<T, false, true>(p, sp, grid, tma, st)
                      : launch_sample_kernel<T, true, false>(p, sp, grid, tma, st);
+    }
     if (rc) return rc;
     p->launches++;
     GAL_CUDA(p, cudaGetLastError());

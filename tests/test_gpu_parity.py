@@ -683,6 +683,76 @@ def test_per_call_state_across_calls(g, orc):
             assert plan.last_oob_count() == 0
 
 
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+def test_speculative_extent_and_its_second_pass(g, orc, dtype):
+    """Automatic pruning, unbound uv, nxy = 2048 / 4096: from the second call on the transform is pruned to the extent
+    the call before derived from its points' largest baseline (no uv-extent kernel), every point is verified against
+    it, and a call whose points reach further repeats itself on the device (one conditional kernel).  Whatever the
+    history, every result equals the one of a plan that never prunes — bit for bit, except for a repeated call, whose
+    row pass is the plain kernel's (last bits of the transform) — and the out-of-grid count is the oracle's."""
+    w = W.config(2, nxy=2048, M=300_007)
+    f32 = dtype == torch.float32
+    if f32:
+        w = w.as_f32()
+    fresh = g.Plan(w.nxy, 1, dtype)
+    fresh.set_pruning(0)
+    import os
+    os.environ["GAL_SPEC_MIN_BYTES"] = "0"              # (read at plan creation: speculate at this test's size too)
+    try:
+        plan = g.Plan(w.nxy, 1, dtype)                  # prune mode 1 (default)
+    finally:
+        del os.environ["GAL_SPEC_MIN_BYTES"]
+    image = dev(w.image)
+    N = w.nxy
+
+    def both(scale, PA, dRA, what, repeated=False):
+        u, v = dev(w.u * scale), dev(w.v * scale)
+        n0 = plan.launch_count()
+        if what == "chi2":
+            args = (image, w.dxy, u, v, dev(w.re_obs), dev(w.im_obs), dev(w.w), dRA, w.dDec, PA)
+            a, b = plan.chi2Image(*args).cpu().numpy(), fresh.chi2Image(*args).cpu().numpy()
+        else:
+            a = plan.sampleImage(image, w.dxy, u, v, PA, dRA, w.dDec).cpu().numpy()
+            b = fresh.sampleImage(image, w.dxy, u, v, PA, dRA, w.dDec).cpu().numpy()
+        if repeated:
+            tol = 1e-5 if f32 else 1e-11
+            assert np.abs(a - b).max() <= tol * np.abs(b).max(), (scale, PA, what)
+        else:
+            assert np.array_equal(a, b), (scale, PA, what)
+        assert plan.last_oob_count() == fresh.last_oob_count()
+        return plan.last_uv_extent(), plan.launch_count() - n0
+
+    e1, n1 = both(1.0, w.PA, w.dRA, "chi2")             # uv-extent kernel: the exact extent
+    e2, n2 = both(1.0, w.PA, w.dRA, "chi2")             # speculates on the radius extent of call 1: symmetric, a superset
+    assert n1 == 4 and n2 == 4                          # (extent, row, column, sampling) / (row, column, sampling, conditional)
+    assert e2[0] >= e1[0] and e2[1] <= e1[1] and e2[2] >= e1[2] and e2[0] < N // 2
+    assert e2[1] + e2[2] == N
+    e3, _ = both(1.0, w.PA + 0.7, 2 * w.dRA, "sample")  # any rotation stays inside the radius extent
+    assert e3 == e2
+    e4, _ = both(1.6, w.PA, w.dRA, "chi2", repeated=True)     # longer baselines: verification fails, second pass on the new extent
+    assert e4[0] > e2[0] and e4[1] < e2[1]
+    e5, _ = both(1.0, w.PA - 0.3, w.dRA, "sample")      # shorter again: speculates on call 4's (larger) extent, no second pass
+    assert e5 == e4
+    e6, _ = both(1.0, w.PA, w.dRA, "chi2")              # and back to the extent of the data
+    assert e6 == e2
+    # points beyond the grid: the derived extent is the whole plane, results and counts still equal
+    e7, _ = both(8.0, w.PA, w.dRA, "chi2", repeated=True)
+    assert e7 == (N // 2, 0, N - 1) and plan.last_oob_count() > 0
+    e8, _ = both(8.0, w.PA, w.dRA, "sample")
+    assert e8 == (N // 2, 0, N - 1)
+    e9, _ = both(1.0, w.PA, w.dRA, "chi2")              # whole-plane speculation can not fail
+    assert e9 == (N // 2, 0, N - 1)
+    assert both(1.0, w.PA, w.dRA, "chi2")[0] == e2
+    both(1.7, w.PA, w.dRA, "sample", repeated=True)     # a repeated sampleImage
+    # against the oracle once, on the state this history has left behind (a repeated call)
+    f = lambda a: np.asarray(a, dtype=np.float64)
+    us, vs = (w.u * 1.9).astype(w.u.dtype), (w.v * 1.9).astype(w.v.dtype)
+    ref = orc.chi2Image(f(w.image), w.dxy, f(us), f(vs), f(w.re_obs), f(w.im_obs), f(w.w), w.dRA, w.dDec, w.PA)
+    got = float(plan.chi2Image(image, w.dxy, dev(us), dev(vs), dev(w.re_obs), dev(w.im_obs), dev(w.w),
+                               w.dRA, w.dDec, w.PA).cpu()[0])
+    assert abs(got - ref) <= (TOL_CHI2_F32 if f32 else TOL_CHI2_F64) * abs(ref)
+
+
 @pytest.mark.parametrize("nxy", [2048, 4096])
 def test_row_pass_variant_follows_the_expected_extent(g, nxy):
     """At nxy = 2048 / 4096 (fp64) the plan picks the row-pass form from the extent it EXPECTS — a hint the sampler of
@@ -694,7 +764,12 @@ def test_row_pass_variant_follows_the_expected_extent(g, nxy):
     image = dev(w.image)
     ref_plan = g.Plan(nxy)
     ref_plan.set_pruning(0)
-    plan = g.Plan(nxy)
+    import os
+    os.environ["GAL_NO_SPEC"] = "1"                          # (read at plan creation: this test is about the row-pass forms,
+    try:                                                     #  the speculative extent has its own, above)
+        plan = g.Plan(nxy)
+    finally:
+        del os.environ["GAL_NO_SPEC"]
     obs = (dev(w.re_obs), dev(w.im_obs), dev(w.w))
     for scale in (1.0, 1.0, 1.0, 9.0, 9.0, 1.0, 1.0):        # in-grid (pruned), then wrapping (whole plane), then back
         u, v = dev(w.u * scale), dev(w.v * scale)
