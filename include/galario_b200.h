@@ -82,7 +82,13 @@ int64_t gal_plan_launch_count(const gal_plan* plan);
  * {largest column ku, first and last shifted row kvs} with the sampler's own index arithmetic, and the FFT
  * passes neither form nor write what lies outside it.  mode 0 = never, 1 = automatic (default: prune when
  * re-reading u and v costs less than a quarter of the three spectrum passes it can save), 2 = always.
- * A point whose cell leaves the grid (reading A6) makes the extent the whole half plane. */
+ * A point whose cell leaves the grid (reading A6) makes the extent the whole half plane.
+ * In mode 1, image calls at nxy = 2048 / 4096 on 16-byte aligned arrays of 32 MB of (u, v) or more do not run the
+ * uv-extent kernel from the second call on: the transform is pruned to the extent the call before derived from the
+ * largest baseline length of ITS points (valid for any PA), the sampling kernel verifies every point of this call
+ * against it, and if a point lies outside, the call repeats itself on the device on the extent of its own points
+ * (one conditional kernel, no host synchronisation).  Results do not depend on this: a repeated call may differ
+ * from an unrepeated one in the last bits of the transform only.  Mode 2 always computes the exact extent. */
 int gal_plan_set_pruning(gal_plan* plan, int mode);
 /* extent[3] (host) = {kumax, kvs_min, kvs_max} used by the most recent sample/chi2 call (the whole half plane
  * {nxy/2, 0, nxy-1} if that call did not prune).  Synchronises the stream of that call. */
