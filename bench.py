@@ -165,6 +165,9 @@ def base_config(w, precision):
     return {"workload": "BASELINE.json configs[3]: chi2Image, 500 elliptical Gaussians (total 1 Jy), nxy=4096, "
                         "dxy=0.0015 arcsec, M=5e6 ALMA-like tracks (50 antennas, 16 km, 0.87 mm), log-normal weights",
             "entry": "chi2Image", "nxy": w.nxy, "M": w.M, "precision": precision, "seed": w.meta.get("seed"),
+            "pruning": "library default (automatic): transform pruned to the part of the half plane the uv points can reach; "
+                       "from the second call on the extent is the one the previous call derived, verified per point "
+                       "(speculative extent, DESIGN.md section 5); unbound observations",
             "l2": "inputs+workspace per step (image 134 MB + spectrum 134 MB + 200 MB of per-point arrays) exceed "
                   "the 126 MB L2; no explicit flush"}
 
