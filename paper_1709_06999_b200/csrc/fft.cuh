@@ -581,7 +581,11 @@ row_pipe_kernel(const RowParams<T> p) {
 // spectrum volumes and the gather pays three sectors per point instead of two.  Both layouts live in the same
 // plan buffer; the column pass and the sampler take the decision from the same device-resident extent.
 __device__ __forceinline__ bool extent_is_whole_plane(const int* ext, int N) {
+#ifdef GAL_FORCE_PAIR
+    return false;
+#else
     return __ldg(ext) >= N / 2 && __ldg(ext + 1) <= 0 && __ldg(ext + 2) >= N - 1;
+#endif
 }
 
 template <typename T> struct ColParams {

@@ -61,7 +61,7 @@ redo_kernel(const RowParams<T> rp, const ColParams<T> cp, const SampleParams<T> 
     // ---- sampling (S5-S8): plain loads, any alignment
     SampleCtx<T> cx_ = sample_ctx(sp, 0);
     const long long ntiles = (sp.M + SampleGeom<T, DO_CHI2>::TILE - 1) / SampleGeom<T, DO_CHI2>::TILE;
-    if (extent_is_whole(sp.ext, sp.N)) {
+    if (layout_single(sp.ext, sp.N)) {
         for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x)
             sample_tile_plain<T, WRITE_VIS, DO_CHI2, true, false>(sp, cx_, tile, sp.M, 0);
     } else {

@@ -66,6 +66,14 @@ template <typename T> struct SampleParams {
 __device__ __forceinline__ bool extent_is_whole(const int* ext, int N) {
     return __ldg(ext) >= N / 2 && __ldg(ext + 1) <= 0 && __ldg(ext + 2) >= N - 1;
 }
+// ... and which layout the column pass wrote (fft.cuh: layout_is_single, the same rule)
+__device__ __forceinline__ bool layout_single(const int* ext, int N) {
+#ifdef GAL_FORCE_PAIR
+    return false;
+#else
+    return extent_is_whole(ext, N);
+#endif
+}
 
 // Correctly rounded a / b from r = RN(1/b) (Markstein): q0 = RN(a r); rem = a - q0 b (exact in an
 // FMA); q = RN(q0 + rem r).  Bit-identical to __ddiv_rn for the operand ranges met here (finite,
@@ -658,7 +666,7 @@ __device__ __forceinline__ SampleCtx<T> sample_ctx(const SampleParams<T>& p, int
     cx_.N = p.N;
     // channel c of the batch: [N/2+1][N] entries, column pairs or (whole-plane extent) single values
     const long long plane = (long long)c * (p.N / 2 + 1) * p.N;
-    cx_.spec = extent_is_whole(p.ext, p.N) ? reinterpret_cast<const NodePair<T>*>(reinterpret_cast<const cx<T>*>(p.spec) + plane)
+    cx_.spec = layout_single(p.ext, p.N) ? reinterpret_cast<const NodePair<T>*>(reinterpret_cast<const cx<T>*>(p.spec) + plane)
                                            : p.spec + plane;
     cx_.odd = threadIdx.x & 1;
     cx_.acc = 0.0;
@@ -679,7 +687,7 @@ __global__ void __launch_bounds__(GAL_SAMPLE_NT, GAL_SAMPLE_MINB) sample_kernel_
     SampleCtx<T> cx_ = sample_ctx(p, c);
     pdl_wait();
     const long long ntiles = (M + G::TILE - 1) / G::TILE;
-    if (extent_is_whole(p.ext, p.N)) {
+    if (layout_single(p.ext, p.N)) {
         for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x)
             sample_tile_plain<T, WRITE_VIS, DO_CHI2, true, false>(p, cx_, tile, M, c);
     } else {
@@ -754,7 +762,7 @@ __global__ void __launch_bounds__(SampleGeom<T, DO_CHI2>::NT_TMA, GAL_SAMPLE_MIN
             if (tile == nfull && (long long)nfull * TILE < M)    // the ragged last tile falls to this CTA
                 sample_tile_plain<T, WRITE_VIS, DO_CHI2, false, PAIR, SPEC>(p, cx_, nfull, M, c);
         };
-        const bool whole = extent_is_whole(p.ext, p.N);
+        const bool whole = layout_single(p.ext, p.N);
         if (!SPEC && DO_CHI2 && p.direct) {                  // (a bound observation set is a chi2 matter)
             if (whole) consume(std::false_type{}, std::true_type{}); else consume(std::true_type{}, std::true_type{});
         } else {
@@ -822,7 +830,7 @@ __device__ __forceinline__ void multi_point(const SampleParams<T>& p, const Plac
 template <typename T, bool WRITE_VIS, bool DO_CHI2>
 __global__ void __launch_bounds__(256) sample_multi_kernel(const SampleParams<T> p, const PlacementSet ps) {
     pdl_wait();
-    const bool single = extent_is_whole(p.ext, p.N);
+    const bool single = layout_single(p.ext, p.N);
     double acc = 0.0;
     unsigned int oob = 0;
     cx<T>* vis = reinterpret_cast<cx<T>*>(p.vis);
