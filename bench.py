@@ -505,12 +505,38 @@ def main():
            "d2h_bytes_per_step": 8, "steps": args.e2e_steps, "ms_per_step": e2e_ms / args.e2e_steps,
            "api": "gal_chi2_image_host_f64 (pinned host buffers in, chi2 to a host double out)",
            "matches_device_path": bool(e2e_chi2 == chi2_val)}
-    del himg, hu, hv, hre, him, hw
+    # the fit loop the library is made for: the observations stay on the device, every step brings a
+    # new MODEL IMAGE from the host (pinned) and takes chi2 back.  Reported beside `e2e`, not instead of it.
+    img_dev = torch.empty_like(image)
+    hout = torch.empty(1, dtype=torch.float64).pin_memory()
+
+    def istep():
+        img_dev.copy_(himg, non_blocking=True)
+        plan.chi2Image(img_dev, w.dxy, u, v, re, im, wt, w.dRA, w.dDec, w.PA, out=out)
+        hout.copy_(out, non_blocking=True)
+
+    for _ in range(3):
+        istep()
+    barrier()
+    g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    g0.record()
+    for _ in range(args.e2e_steps):
+        istep()
+    g1.record()
+    barrier()
+    img_ms = max_over_ranks(g0.elapsed_time(g1), world, dev)
+    e2e_image_only = {"value": world * args.e2e_steps / (img_ms * 1e-3), "unit": UNIT,
+                      "h2d_bytes_per_step": himg.numel() * himg.element_size(), "d2h_bytes_per_step": 8,
+                      "steps": args.e2e_steps, "ms_per_step": img_ms / args.e2e_steps,
+                      "what": "observations resident on the device, the model image copied from pinned host memory and chi2 "
+                              "copied back every step (torch copies + gal_chi2_image_f64)",
+                      "matches_device_path": bool(float(hout[0]) == chi2_val)}
+    del himg, hu, hv, hre, him, hw, img_dev
 
     result = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-        "data": "synthetic", "config": base_config(w, "f64"), "clocks": clk.summary(), "e2e": e2e,
+        "data": "synthetic", "config": base_config(w, "f64"), "clocks": clk.summary(), "e2e": e2e, "e2e_image_only": e2e_image_only,
         "gpu_launches": int(launches), "roofline": roofline, "step_roofline": step_roofline, "kernels": kernels,
         "visibilities_per_s": value * w.M, "chi2": chi2_val, "multi_gpu": "replicas only", "bound_obs": bound_obs,
         "paper_context": "GTX 1060, M=1e6, PCIe copies included: chi2Image 4096^2 = 59 ms (PAPER.md:619); not like for like",
