@@ -107,7 +107,8 @@ def get_image_size(u, v, PB: float = 0.0, f_min: float = 5.0, f_max: float = 2.5
 
 
 def _stream() -> int:
-    return torch.cuda.current_stream().cuda_stream
+    # (the raw handle of torch's current stream; small calls are bound by the host's issue rate, so the cheap accessor)
+    return torch._C._cuda_getCurrentRawStream(torch.cuda.current_device())
 
 
 class Plan:
@@ -122,6 +123,7 @@ class Plan:
         self._sfx = "f64" if dtype == torch.float64 else "f32"
         self._cdtype = torch.complex128 if dtype == torch.float64 else torch.complex64
         self._lib = load_library()
+        self._fns = {}
         h = _vp()
         _check(self._lib.gal_plan_create(ctypes.byref(h), self.nxy, self.batch, 64 if dtype == torch.float64 else 32,
                                          self.device), "gal_plan_create")
@@ -135,13 +137,16 @@ class Plan:
 
     # -- helpers ---------------------------------------------------------------------------
     def _fn(self, name):
-        return getattr(self._lib, f"gal_{name}_{self._sfx}")
+        f = self._fns.get(name)
+        if f is None:
+            f = self._fns[name] = getattr(self._lib, f"gal_{name}_{self._sfx}")
+        return f
 
     def _dev(self, t: torch.Tensor, what: str, numel: Optional[int] = None) -> int:
         if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == self.dtype and t.is_contiguous()):
             raise GalarioError(f"{what} must be a contiguous CUDA tensor of dtype {self.dtype}")
-        if t.device.index != self.device:
-            raise GalarioError(f"{what} lives on cuda:{t.device.index}, the plan on cuda:{self.device}")
+        if t.get_device() != self.device:
+            raise GalarioError(f"{what} lives on cuda:{t.get_device()}, the plan on cuda:{self.device}")
         if numel is not None and t.numel() != numel:
             raise GalarioError(f"{what} has {t.numel()} elements, expected {numel}")
         return t.data_ptr()
