@@ -92,10 +92,11 @@ int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T
     const int tile = SampleGeom<T, true>::TILE;
     const long long ntiles = (M + tile - 1) / tile;
     long long cap = (long long)p->sm_count * GAL_SAMPLE_MINB;
-    // batched: CTAs are placed channel by channel (blockIdx.x fastest); an eighth of the resident CTAs per
-    // channel keeps about eight channels' spectra (not dozens) competing for the L2 at any time and gives every
-    // CTA enough tiles to amortise its prologue and reduction (measured at cfg 4: 2: 573, 4: 481, 8: 420 us)
-    static const int conc = getenv("GAL_BATCH_CONC") ? atoi(getenv("GAL_BATCH_CONC")) : 8;     // channels in flight (diagnostic)
+    // batched: CTAs are placed channel by channel (blockIdx.x fastest); a twelfth of the resident CTAs per
+    // channel keeps about twelve channels' spectra (not dozens) competing for the L2 at any time and gives every
+    // CTA enough tiles to amortise its prologue and reduction (measured at cfg 4, bound observations: 4: 437,
+    // 8: 396, 12: 384, 16: 385 us)
+    static const int conc = getenv("GAL_BATCH_CONC") ? atoi(getenv("GAL_BATCH_CONC")) : 12;     // channels in flight (diagnostic)
     if (C > 1) cap = (cap + (C < conc ? C : conc) - 1) / (C < conc ? C : conc);
     if (cap > p->max_gx) cap = p->max_gx;
     long long gx = ntiles < cap ? ntiles : cap;
