@@ -56,6 +56,7 @@ extern "C" {
 #define GAL_ERR_CUDA (-3)             /* a CUDA call failed; see gal_last_cuda_error() */
 #define GAL_ERR_UNSUPPORTED (-4)      /* a power-of-two nxy above 16384; M >= 2^32 in gal_plan_bind_obs */
 #define GAL_ERR_BINDING_VIOLATED (-5) /* an earlier call found a bound (u, v) set changed: that call's results are invalid; the binding is dropped */
+#define GAL_ERR_TOO_LARGE (-6)        /* gal_chi2_profile_hankel_noalloc_f64 only: M > GAL_NOALLOC_MAX_POINTS, its fixed scratch cannot hold the partial sums */
 
 typedef struct gal_plan gal_plan;
 
@@ -271,6 +272,54 @@ int gal_chi2_profile_host_f64(gal_plan* plan, const double* I, int nr, double Rm
                               const double* u, const double* v, const double* re_obs, const double* im_obs,
                               const double* w, int64_t M, double dRA, double dDec, double PA, double inc,
                               double* chi2_out, void* stream);
+
+/* ---- chi2Profile WITHOUT A PLAN AND WITHOUT ANY ALLOCATION (direct Hankel transform, Eq. 25 and Eq. 10:
+ *      PAPER.md:366-368, 194-198, 718; same mathematics and same arguments as gal_chi2_profile_hankel_f64).
+ *
+ *      Why it exists.  Every other call needs a gal_plan, and gal_plan_create takes its workspace with cudaMalloc.
+ *      That rules the library out for two kinds of caller: (1) code that runs inside a fixed device-memory budget —
+ *      an application that partitions the GPU once at start-up and hands each component its slice, a memory-capped
+ *      MPS client, a GPU already filled by the rest of the fit — where one more cudaMalloc fails or eats memory
+ *      promised to somebody else; (2) latency-critical loops, because cudaMalloc / cudaFree synchronise the whole
+ *      device and serialise on the driver's allocator lock.  This entry point never calls cudaMalloc, cudaFree,
+ *      cudaMallocAsync or an allocating library routine, at set-up or later.
+ *
+ *      How.  Its reduction scratch (one double per CTA of 128 points, one ticket counter) is a file-scope
+ *      `static __device__` array of gal_noalloc_scratch_bytes() = 65 792 bytes (64 KiB + 256 B), part of the
+ *      library image: every GPU that loads the library holds it until the process exits, whether this call is
+ *      used or not.  The array's size fixes the limit: M <= GAL_NOALLOC_MAX_POINTS (1 048 576 = 8192 CTAs x 128
+ *      points); a larger M returns GAL_ERR_TOO_LARGE and launches nothing (split the set — chi2 is a sum over
+ *      points — or use a plan).  nr is not limited.
+ *
+ *      Arguments.  `device`: the CUDA device the pointers live on (0 <= device < 64); it is made current for
+ *      the duration of the call and the previous device restored.  I[nr], u, v, re_obs, im_obs, w [M]: DEVICE
+ *      arrays of doubles, owned by the caller, never modified, any alignment.  chi2_out: DEVICE double[1].
+ *      `stream`: cudaStream_t as void* (NULL = legacy default stream); the call is asynchronous on it and never
+ *      synchronises the host.  M == 0 is valid (chi2 = 0).  Errors: GAL_ERR_INVALID_ARGUMENT as for
+ *      gal_chi2_profile_hankel_f64 (null pointer, nr < 2, dR <= 0, |inc| >= pi/2, M < 0, non-finite scalars, bad
+ *      device); GAL_ERR_TOO_LARGE; GAL_ERR_CUDA with the cudaError_t in gal_noalloc_last_cuda_error().
+ *
+ *      First call on a device.  It looks up the device address of the scratch array (cudaGetSymbolAddress, once
+ *      per device, cached) and thereby loads this library's device code on that GPU.  Make one call — M = 1 will
+ *      do — during start-up, before any stream capture begins and before the time-critical part of the program.
+ *
+ *      Shared state.  All calls on one GPU use the same array.  The ticket is zeroed on `stream` in front of every
+ *      launch and every partial sum is written before it is read, so nothing leaks from one call into the next;
+ *      the array simply keeps the last call's partial sums.  Calls that may OVERLAP on the same GPU (two streams,
+ *      two threads) race on it and return wrong sums: keep them on one stream or order them with events.
+ *
+ *      Result.  Per-point arithmetic identical to gal_chi2_profile_hankel_f64; the sum runs over fixed 128-point
+ *      tiles in tile order, so the value is bit-reproducible from run to run and across GPU models, and agrees
+ *      with the plan-based call to rounding (a few ulp; the tests allow 1e-12 relative). ---- */
+#define GAL_NOALLOC_MAX_POINTS 1048576
+int gal_chi2_profile_hankel_noalloc_f64(int device, const double* I, int nr, double Rmin, double dR, const double* u,
+                                        const double* v, const double* re_obs, const double* im_obs, const double* w,
+                                        int64_t M, double dRA, double dDec, double PA, double inc, double* chi2_out,
+                                        void* stream);
+/* Bytes of the static scratch array each GPU holds for the call above (65 792). */
+size_t gal_noalloc_scratch_bytes(void);
+/* cudaError_t of the most recent failing CUDA call made by gal_chi2_profile_hankel_noalloc_f64 (0 if none). */
+int gal_noalloc_last_cuda_error(void);
 
 #ifdef __cplusplus
 }

@@ -12,7 +12,9 @@ Paper-style calls (PAPER.md:82-113, 650, 723)::
     chi2 = chi2Image(image, dxy, u, v, re_obs, im_obs, w, dRA, dDec, PA)   # 1-element CUDA tensor
 """
 from .binding import (Plan, GalarioError, library_path, load_library, sampleImage, chi2Image, sampleProfile,
-                      chi2Profile, sweep, chi2ImageBatch, fft2_shifted, get_plan, get_image_size)
+                      chi2Profile, sweep, chi2ImageBatch, fft2_shifted, get_plan, get_image_size,
+                      chi2ProfileHankelNoAlloc, NOALLOC_MAX_POINTS)
 
 __all__ = ["Plan", "GalarioError", "library_path", "load_library", "sampleImage", "chi2Image", "sampleProfile",
-           "chi2Profile", "sweep", "chi2ImageBatch", "fft2_shifted", "get_plan", "get_image_size"]
+           "chi2Profile", "sweep", "chi2ImageBatch", "fft2_shifted", "get_plan", "get_image_size",
+           "chi2ProfileHankelNoAlloc", "NOALLOC_MAX_POINTS"]

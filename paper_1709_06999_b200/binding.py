@@ -82,6 +82,9 @@ def load_library() -> ctypes.CDLL:
         lib.gal_sample_image_host_f64.argtypes = [_vp, _vp, _d, _vp, _vp, _i64, _d, _d, _d, _vp, _vp]
         lib.gal_chi2_profile_host_f64.argtypes = [_vp, _vp, _i, _d, _d, _d, _vp, _vp, _vp, _vp, _vp, _i64, _d, _d, _d,
                                                   _d, _vp, _vp]
+        lib.gal_chi2_profile_hankel_noalloc_f64.argtypes = [_i, _vp, _i, _d, _d, _vp, _vp, _vp, _vp, _vp, _i64, _d, _d,
+                                                            _d, _d, _vp, _vp]
+        lib.gal_noalloc_scratch_bytes.restype = ctypes.c_size_t
         _lib = lib
     return _lib
 
@@ -104,6 +107,52 @@ def get_image_size(u, v, PB: float = 0.0, f_min: float = 5.0, f_max: float = 2.5
                                              float(f_max), ctypes.addressof(n), ctypes.addressof(d)),
            "gal_get_image_size")
     return n.value, d.value
+
+
+NOALLOC_MAX_POINTS = 1 << 20          # GAL_NOALLOC_MAX_POINTS of the header
+
+
+def chi2ProfileHankelNoAlloc(I, Rmin, dR, u, v, re_obs, im_obs, w, out, dRA=0.0, dDec=0.0, PA=0.0, inc=0.0):
+    """chi2Profile by the direct Hankel transform (Eq. 25) for callers that may not allocate device memory.
+
+    Every other call of this package goes through a ``Plan``, and creating a plan calls ``cudaMalloc``.  A program
+    that lives inside a fixed device-memory budget (its host application split the GPU up at start-up, it runs as a
+    memory-capped MPS client, the GPU is already full) or that cannot tolerate the device-wide synchronisation of
+    ``cudaMalloc`` in its inner loop uses this function instead: no plan, no allocation of any kind — neither in the
+    library nor here, which is why ``out`` (a 1-element float64 CUDA tensor for the result) is a required argument
+    and is returned as it is.  The reduction scratch is a 65 792-byte static array inside the library that every GPU
+    holds until the process exits; its size limits the call to ``NOALLOC_MAX_POINTS`` = 1 048 576 points (more
+    raises ``GalarioError``; split the set and add the results).
+
+    All tensors are contiguous float64 CUDA tensors on one device.  The call is asynchronous on torch's current
+    stream.  The first call on each GPU also looks up the scratch array's device address and loads the library's
+    device code there: make one small call at start-up, before capturing any stream and before the time-critical
+    part.  All calls on a GPU share the one array — calls that may overlap (several streams or threads) race and
+    return wrong sums; keep them on one stream."""
+    lib = load_library()
+    if not torch.cuda.is_available():
+        raise GalarioError("no CUDA device: the galario-b200 path has no CPU fallback")
+    dev = None
+    M = u.numel() if isinstance(u, torch.Tensor) else -1
+    for t, what, n in ((I, "I", None), (u, "u", M), (v, "v", M), (re_obs, "re_obs", M), (im_obs, "im_obs", M), (w, "w", M),
+                       (out, "out", 1)):
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+            raise GalarioError(f"{what} must be a contiguous float64 CUDA tensor")
+        if n is not None and t.numel() != n:
+            raise GalarioError(f"{what} has {t.numel()} elements, expected {n}")
+        dev = t.get_device() if dev is None else dev
+        if t.get_device() != dev:
+            raise GalarioError(f"{what} lives on cuda:{t.get_device()}, I on cuda:{dev}")
+    if dev != torch.cuda.current_device():
+        raise GalarioError(f"the tensors live on cuda:{dev} but torch's current device (whose stream is used) is "
+                           f"cuda:{torch.cuda.current_device()}")
+    rc = lib.gal_chi2_profile_hankel_noalloc_f64(dev, I.data_ptr(), I.numel(), Rmin, dR, u.data_ptr(), v.data_ptr(),
+                                                 re_obs.data_ptr(), im_obs.data_ptr(), w.data_ptr(), M, dRA, dDec, PA,
+                                                 inc, out.data_ptr(), _stream())
+    if rc != 0:
+        extra = f" (cudaError {lib.gal_noalloc_last_cuda_error()})" if rc == -3 else ""
+        raise GalarioError(f"gal_chi2_profile_hankel_noalloc_f64: {lib.gal_strerror(rc).decode()}{extra}")
+    return out
 
 
 def _stream() -> int:

@@ -450,6 +450,7 @@ const char* gal_strerror(int code) {
         case GAL_ERR_CUDA: return "CUDA error (see gal_last_cuda_error)";
         case GAL_ERR_UNSUPPORTED: return "unsupported size";
         case GAL_ERR_BINDING_VIOLATED: return "a bound (u, v) set changed after gal_plan_bind_uv / gal_plan_bind_obs";
+        case GAL_ERR_TOO_LARGE: return "M exceeds GAL_NOALLOC_MAX_POINTS (1048576): the fixed scratch of the no-allocation entry point cannot hold more partial sums";
         default: return "unknown error";
     }
 }
