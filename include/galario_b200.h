@@ -8,7 +8,7 @@
  *     -> phase ramp for (dRA, dDec)
  *     -> weighted chi-square against observed visibilities                  (Eq. 10, 718)
  * The executable definition followed is the paper's Appendix D listing;
- * the readings taken where it is silent or garbled are listed in DESIGN.md (A1..A17).
+ * the readings taken where it is silent or garbled are listed in DESIGN.md (A1..A20).
  *
  * Conventions
  *   - Every array pointer is a DEVICE pointer unless the function name ends in `_host_*`, in which case
@@ -91,6 +91,19 @@ int64_t gal_plan_launch_count(const gal_plan* plan);
  * (one conditional kernel, no host synchronisation).  Results do not depend on this: a repeated call may differ
  * from an unrepeated one in the last bits of the transform only.  Mode 2 always computes the exact extent. */
 int gal_plan_set_pruning(gal_plan* plan, int mode);
+/* Tuning options of a plan.  The library reads NO environment variable; these are the only switches.  They choose
+ * among kernel forms and launch geometries that compute the same thing (results agree bit for bit, except where a
+ * different row-pass kernel is selected: last bits of the transform), and their defaults are the measured optimum
+ * on B200 — they exist for measurements and for tests that must reach a particular kernel at a small size.
+ * Takes effect from the next call.  GAL_ERR_INVALID_ARGUMENT for an unknown option or a value out of range. */
+#define GAL_OPT_ROW_MODE 1        /* nxy 1024..4096: -1 per-size default, 0 plain row pass, 1 register untangle with plain loads, 2 its persistent TMA-ring form, 3 one row per CTA */
+#define GAL_OPT_BATCH_CHUNK 2     /* channels per chunk of a batched call; 0 (default) = all in one chunk */
+#define GAL_OPT_SPECULATE 3       /* 1 (default) = speculative extent in pruning mode 1 (see above); 0 = always run the uv-extent kernel */
+#define GAL_OPT_SPEC_MIN_BYTES 4  /* smallest volume of (u, v), in bytes, the speculative extent is used for (default 32e6) */
+#define GAL_OPT_BATCH_CONC 5      /* channels in flight in the batched sampler (default 12) */
+#define GAL_OPT_ROW_PREFETCH 6    /* scale of the L2 prefetch distance of the FFT passes (default 1; 0 = no prefetch) */
+#define GAL_OPT_ROW_X2_ONE_CTA 7  /* nxy = 16384: 1 = one CTA per row instead of a cluster of two (default 0) */
+int gal_plan_set_option(gal_plan* plan, int option, double value);
 /* extent[3] (host) = {kumax, kvs_min, kvs_max} used by the most recent sample/chi2 call (the whole half plane
  * {nxy/2, 0, nxy-1} if that call did not prune).  Synchronises the stream of that call. */
 int gal_last_uv_extent(gal_plan* plan, int* extent);

@@ -10,7 +10,7 @@
 // No blocking, no fusion, no reordering.  Every function cites the passage it follows.
 //
 // Readings of the paper where it is silent or garbled are the ones listed in
-// DESIGN.md ("Readings", items A1..A17; they restate SURVEY.md §8(c)).
+// DESIGN.md ("Readings", items A1..A20; they restate SURVEY.md §8(c)).
 //
 // Pins (tests/test_oracle_*.py, run with -m "not gpu"): brute-force sky-coordinate DFT
 // at nxy <= 64, the Appendix-D listing re-run with numpy.fft + scipy, delta-source and

@@ -46,6 +46,7 @@ def load_library() -> ctypes.CDLL:
         lib.gal_plan_timing_read.argtypes = [_vp, _vp, _vp]
         lib.gal_get_image_size.argtypes = [_vp, _vp, _i64, _d, _d, _d, _vp, _vp]
         lib.gal_plan_set_pruning.argtypes = [_vp, _i]
+        lib.gal_plan_set_option.argtypes = [_vp, _i, _d]
         lib.gal_plan_unbind_uv.argtypes = [_vp]
         lib.gal_last_extent_violations.argtypes = [_vp]
         lib.gal_last_extent_violations.restype = _i64
@@ -177,6 +178,8 @@ class Plan:
         _check(self._lib.gal_plan_create(ctypes.byref(h), self.nxy, self.batch, 64 if dtype == torch.float64 else 32,
                                          self.device), "gal_plan_create")
         self._h = h
+        self._bound_uv = None       # tensors of the current gal_plan_bind_uv / gal_plan_bind_obs (kept alive, see bind_uv)
+        self._bound_obs = None
 
     def __del__(self):
         h = getattr(self, "_h", None)
@@ -233,6 +236,15 @@ class Plan:
         """0 = never, 1 = automatic (default), 2 = always: see gal_plan_set_pruning."""
         _check(self._lib.gal_plan_set_pruning(self._h, int(mode)), "gal_plan_set_pruning", self)
 
+    OPTIONS = {"row_mode": 1, "batch_chunk": 2, "speculate": 3, "spec_min_bytes": 4, "batch_conc": 5, "row_prefetch": 6,
+               "row_x2_one_cta": 7}                          # GAL_OPT_* of the header
+
+    def set_option(self, name: str, value) -> None:
+        """Tuning options (gal_plan_set_option): kernel forms / launch geometries, never results."""
+        if name not in self.OPTIONS:
+            raise GalarioError(f"unknown option {name!r}; one of {sorted(self.OPTIONS)}")
+        _check(self._lib.gal_plan_set_option(self._h, self.OPTIONS[name], float(value)), "gal_plan_set_option", self)
+
     @staticmethod
     def _placements(placements):
         """[(dRA, dDec, PA[, scale]), ...] -> four host double arrays."""
@@ -265,23 +277,35 @@ class Plan:
         very tensors skip the per-call uv-extent kernel (gal_plan_bind_uv)."""
         C = 1 if u.dim() == 1 else u.shape[0]
         M = u.shape[-1]
-        _check(self._fn("plan_bind_uv")(self._h, self._dev(u, "u"), self._dev(v, "v"), M, C, _stream()),
+        _check(self._fn("plan_bind_uv")(self._h, self._dev(u, "u"), self._dev(v, "v", u.numel()), M, C, _stream()),
                "gal_plan_bind_uv", self)
+        # The binding is identified by device addresses.  Keep the tensors alive until unbind / rebind: torch's caching
+        # allocator would otherwise hand a freed tensor's address to NEW data, which would then match the old binding.
+        self._bound_uv = (u, v)
+        self._bound_obs = None
 
     def bind_obs(self, u, v, re_obs, im_obs, w) -> None:
         """Promise that the five observation arrays ([M] or [C][M]) keep their contents: later chi2 calls that pass
         these very tensors sample the plan's private, uv-sorted copy (gal_plan_bind_obs)."""
         C = 1 if u.dim() == 1 else u.shape[0]
         M = u.shape[-1]
-        _check(self._fn("plan_bind_obs")(self._h, self._dev(u, "u"), self._dev(v, "v"), self._dev(re_obs, "re_obs"),
-                                         self._dev(im_obs, "im_obs"), self._dev(w, "w"), M, C, _stream()),
+        n = u.numel()
+        _check(self._fn("plan_bind_obs")(self._h, self._dev(u, "u"), self._dev(v, "v", n), self._dev(re_obs, "re_obs", n),
+                                         self._dev(im_obs, "im_obs", n), self._dev(w, "w", n), M, C, _stream()),
                "gal_plan_bind_obs", self)
+        # as bind_uv: the five addresses ARE the binding, so the tensors must not be freed (and their addresses
+        # recycled for other data, which would silently sample the plan's old private copy) while it stands
+        self._bound_uv = (u, v)
+        self._bound_obs = (u, v, re_obs, im_obs, w)
 
     def unbind_obs(self) -> None:
         _check(self._lib.gal_plan_unbind_obs(self._h), "gal_plan_unbind_obs", self)
+        self._bound_obs = None
 
     def unbind_uv(self) -> None:
         _check(self._lib.gal_plan_unbind_uv(self._h), "gal_plan_unbind_uv", self)
+        self._bound_uv = None
+        self._bound_obs = None
 
     def last_extent_violations(self) -> int:
         return int(self._lib.gal_last_extent_violations(self._h))

@@ -325,7 +325,7 @@ __device__ __forceinline__ void row_block(const RowParams<T>& p, const long long
     cx<T>* out = p.spec + b_img * (long long)NU * N + i0;
     const int rows_here = (int)((p.rows_total - row0) < F ? (p.rows_total - row0) : F);
     // columns beyond the uv extent are never sampled: neither formed nor written
-    const int kumax = __ldg(p.ext);
+    const int kumax = __ldcg(p.ext);
     const int kend = kumax < L / 2 ? kumax : L / 2;
     for (int idx = tid; idx < F * (kend + 1); idx += G::NT) {
         const int ff = idx % F, k = idx / F;
@@ -451,7 +451,7 @@ row_pipe_kernel(const RowParams<T> p) {
     const int bar_id = 1 + g;
     if (MODE == ROW_DIRECT) prefetch_row_block(p, blockIdx.x, F);
     pdl_wait();
-    const int kumax = __ldg(p.ext);
+    const int kumax = __ldcg(p.ext);
     const int NU = N / 2 + 1;
     const cx<T>* __restrict__ tw = p.tw;
     // the only table reads of steps 1 and 2: one base twiddle each, W_L^t and W_(R2 R3)^(t mod R3)
@@ -584,7 +584,7 @@ __device__ __forceinline__ bool extent_is_whole_plane(const int* ext, int N) {
 #ifdef GAL_FORCE_PAIR
     return false;
 #else
-    return __ldg(ext) >= N / 2 && __ldg(ext + 1) <= 0 && __ldg(ext + 2) >= N - 1;
+    return __ldcg(ext) >= N / 2 && __ldcg(ext + 1) <= 0 && __ldcg(ext + 2) >= N - 1;
 #endif
 }
 
@@ -608,7 +608,7 @@ __device__ __forceinline__ void col_block(const ColParams<T>& p, const long long
     const int f = tid / G::TPF, t = tid % G::TPF;
     const int NU = L / 2 + 1;
     // uv extent: columns beyond kumax are skipped, rows outside [rmin, rmax] are not written
-    const int kumax = __ldg(p.ext), rmin = __ldg(p.ext + 1), rmax = __ldg(p.ext + 2);
+    const int kumax = __ldcg(p.ext), rmin = __ldcg(p.ext + 1), rmax = __ldcg(p.ext + 2);
     const bool single = extent_is_whole_plane(p.ext, L);
     cx<T>* S = smem + f * G::REGION;
     {
@@ -734,7 +734,7 @@ col_pass_x2_kernel(const ColParams<T> p) {
     const int tid = threadIdx.x;
     const int f = tid / G::TPF, t = tid % G::TPF;
     pdl_wait();
-    const int kumax = __ldg(p.ext), rmin = __ldg(p.ext + 1), rmax = __ldg(p.ext + 2);
+    const int kumax = __ldcg(p.ext), rmin = __ldcg(p.ext + 1), rmax = __ldcg(p.ext + 2);
     const long long g = blockIdx.x;
     const int ku = (int)(g % NU);
     if (ku > kumax) return;
@@ -844,7 +844,7 @@ row_pass_x2_kernel(const RowParams<T> p) {
     const int i = (int)(row % N);
     const int pos = (i & 3) * (N >> 2) + (i >> 2);           // decimated by four for the column transform
     cx<T>* out = p.spec + (row / N) * (long long)NU * N + pos;
-    const int kumax = __ldg(p.ext);
+    const int kumax = __ldcg(p.ext);
     const int kend = kumax < L / 2 ? kumax : L / 2;
     for (int k = tid; k <= kend; k += G::NT) {               // untangle (factor 1/2 folded into the column pass)
         const cx<T> zk = Z(k), zm = Z((L - k) % L);
@@ -927,7 +927,7 @@ row_pass_c2_kernel(const RowParams<T> p) {
     const int i = (int)(row % N);
     const int pos = (i & 3) * (N >> 2) + (i >> 2);           // decimated by four for the column transform
     cx<T>* out = p.spec + (row / N) * (long long)NU * N + pos;
-    const int kumax = __ldg(p.ext);
+    const int kumax = __ldcg(p.ext);
     const int kend = kumax < L / 2 ? kumax : L / 2;
     for (int k = 2 * t + (int)r; k <= kend; k += 2 * G::NT) {   // this CTA: k of its own parity; untangle as row_pass_x2
         const cx<T> zk = Z(k), zm = Z((L - k) % L);
@@ -953,7 +953,7 @@ col_sub_kernel(const ColParams<T> p, cx<T>* __restrict__ work) {
     pdl_wait();
     const long long g = blockIdx.x >> 2;
     const int n1 = blockIdx.x & 3;
-    if ((int)(g % NU) > __ldg(p.ext)) return;
+    if ((int)(g % NU) > __ldcg(p.ext)) return;
     cx<T>* q = work + g * (long long)N + (long long)n1 * LQ;
     fft_steps12<T, R1, R2, R3, G::TPF>(S, t, p.tw, 4, [&](int n) -> cx<T> { return q[n]; });
     for (int it = t; it < R1 * R2; it += G::TPF) {           // step 3 from shared memory, twiddle, straight to memory
@@ -976,7 +976,7 @@ template <typename T>
 __global__ void __launch_bounds__(256) col_comb4_kernel(const ColParams<T> p) {
     const int N = p.N, LQ = N >> 2, NU = N / 2 + 1;
     pdl_wait();
-    const int kumax = __ldg(p.ext), rmin = __ldg(p.ext + 1), rmax = __ldg(p.ext + 2);
+    const int kumax = __ldcg(p.ext), rmin = __ldcg(p.ext + 1), rmax = __ldcg(p.ext + 2);
     const bool single = extent_is_whole_plane(p.ext, N);
     const long long g = blockIdx.y;
     const int ku = (int)(g % NU);

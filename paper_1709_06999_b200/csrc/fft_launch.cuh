@@ -125,7 +125,7 @@ int launch_fft_16384(gal_plan* p, const T* image, const SweepParams* sw, int bat
     rp.rows_total = batch * p->nxy; rp.ext = ext; rp.pf_blocks = 0;
     if (sw) rp.sweep = *sw; else memset(&rp.sweep, 0, sizeof(rp.sweep));
     int rc;
-    static const bool one_cta = getenv("GAL_ROW_X2_ONE_CTA") != nullptr;     // diagnostic: the one-CTA-per-row form
+    const bool one_cta = p->row_x2_one_cta;                  // GAL_OPT_ROW_X2_ONE_CTA: the one-CTA-per-row form
     if (!one_cta) {
         // a cluster of two CTAs per row (fft.cuh: row_pass_c2_kernel)
         const unsigned grid = 2u * (unsigned)rp.rows_total;

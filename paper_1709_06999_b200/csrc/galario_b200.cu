@@ -464,8 +464,6 @@ int gal_plan_create(gal_plan** out, int nxy, int batch, int precision_bits, int 
     gal_plan* p = new (std::nothrow) gal_plan();
     if (!p) return GAL_ERR_ALLOC;
     p->nxy = nxy; p->batch = batch; p->bits = precision_bits; p->device = device;
-    if (const char* e = getenv("GAL_ROW_PIPE")) p->row_mode = atoi(e);
-    if (const char* e = getenv("GAL_BATCH_CHUNK")) p->batch_chunk = atoi(e);     // diagnostic: channels per chunk (0 = automatic)    // diagnostic switch
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || device >= ndev) { delete p; return GAL_ERR_CUDA; }
     DeviceGuard g(device);
@@ -488,8 +486,6 @@ int gal_plan_create(gal_plan** out, int nxy, int batch, int precision_bits, int 
     if ((e = cudaMalloc((void**)&p->b_r2, 8)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     if ((e = cudaMalloc(&p->spec_state, 64)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     if ((e = cudaMemset(p->spec_state, 0, 64)) != cudaSuccess) return fail(GAL_ERR_CUDA, e);
-    p->spec_off = getenv("GAL_NO_SPEC") != nullptr;
-    if (const char* e2 = getenv("GAL_SPEC_MIN_BYTES")) p->spec_min_bytes = atof(e2);      // diagnostic / tests
     if ((e = cudaHostAlloc((void**)&p->viol_host, 2 * sizeof(unsigned int), cudaHostAllocMapped)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     p->viol_host[0] = 0; p->viol_host[1] = 0;          // [1]: extent hint (plan.h row_small)
     if ((e = cudaHostGetDevicePointer((void**)&p->viol_dev, p->viol_host, 0)) != cudaSuccess) return fail(GAL_ERR_CUDA, e);
@@ -571,6 +567,24 @@ int gal_plan_timing_read(gal_plan* p, double* ms_per_kernel, int64_t* calls) {
 int gal_plan_set_pruning(gal_plan* p, int mode) {
     if (!p || mode < 0 || mode > 2) return GAL_ERR_INVALID_ARGUMENT;
     p->prune_mode = mode;
+    return GAL_OK;
+}
+
+// Tuning options of a plan (the library reads no environment variable).  They select among kernels / launch
+// geometries that compute the same thing; no result depends on them beyond the last bits of the transform.
+int gal_plan_set_option(gal_plan* p, int option, double value) {
+    if (!p || !std::isfinite(value)) return GAL_ERR_INVALID_ARGUMENT;
+    const int iv = (int)value;
+    switch (option) {
+        case GAL_OPT_ROW_MODE: if (iv < -1 || iv > 3) return GAL_ERR_INVALID_ARGUMENT; p->row_mode = iv; break;
+        case GAL_OPT_BATCH_CHUNK: if (iv < 0) return GAL_ERR_INVALID_ARGUMENT; p->batch_chunk = iv; break;
+        case GAL_OPT_SPECULATE: p->spec_off = (iv == 0); p->spec_valid = false; break;
+        case GAL_OPT_SPEC_MIN_BYTES: if (value < 0) return GAL_ERR_INVALID_ARGUMENT; p->spec_min_bytes = value; p->spec_valid = false; break;
+        case GAL_OPT_BATCH_CONC: if (iv < 1) return GAL_ERR_INVALID_ARGUMENT; p->batch_conc = iv; break;
+        case GAL_OPT_ROW_PREFETCH: if (value < 0) return GAL_ERR_INVALID_ARGUMENT; p->row_pf = value; p->resident.clear(); break;
+        case GAL_OPT_ROW_X2_ONE_CTA: p->row_x2_one_cta = (iv != 0); break;
+        default: return GAL_ERR_INVALID_ARGUMENT;
+    }
     return GAL_OK;
 }
 

@@ -32,8 +32,12 @@ struct gal_plan {
     int cur = 0;                         // copy used by the most recent call
     bool next_armed = false;             // the other copy has been / will be re-armed by that call's sampler
     int prune_mode = 1;                  // 0 never, 1 auto, 2 always
-    int batch_chunk = 0;                 // channels per chunk of a batched call (0: all in one chunk; GAL_BATCH_CHUNK, see galario_b200.cu batch_chunk)
-    int row_mode = -1;                   // nxy 1024..4096: -1 per-size default, 0 plain row pass, 1 register-untangle kernel with plain loads, 2 its persistent TMA form (GAL_ROW_PIPE)
+    // tuning options (gal_plan_set_option; the defaults are the measured optimum on B200)
+    int batch_chunk = 0;                 // GAL_OPT_BATCH_CHUNK: channels per chunk of a batched call (0: all in one chunk; galario_b200.cu batch_chunk)
+    int row_mode = -1;                   // GAL_OPT_ROW_MODE, nxy 1024..4096: -1 per-size default, 0 plain row pass, 1 register-untangle kernel with plain loads, 2 its persistent TMA form, 3 one row per CTA
+    int batch_conc = 12;                 // GAL_OPT_BATCH_CONC: channels in flight in the batched sampler
+    double row_pf = 1.0;                 // GAL_OPT_ROW_PREFETCH: scale of the L2 prefetch distance of the FFT passes (0 = off)
+    bool row_x2_one_cta = false;         // GAL_OPT_ROW_X2_ONE_CTA: nxy = 16384, one CTA per row instead of a cluster of two
     bool last_pruned = false;            // did the most recent call compute a uv extent?
     // bound uv set (gal_plan_bind_uv): addresses, size, the rotation-invariant radius, and the extent derived
     // from it for the pixel size seen last (device copy used by the FFT passes and checked by the sampler)
@@ -70,7 +74,7 @@ struct gal_plan {
     double spec_dxy = 0.0;               // ... for this pixel size
     cudaStream_t spec_stream = nullptr;  // ... on this stream
     int spec_mode = 0;                   // the launch being issued: 0 none, 1 derive only, 2 verify + derive
-    bool spec_off = false;               // GAL_NO_SPEC (diagnostic)
+    bool spec_off = false;               // GAL_OPT_SPECULATE = 0
     double spec_min_bytes = 32e6;        // speculate only where the uv-extent pass would read at least this much (cfg 2, 16 MB: 42.0 against 44.5 us)
     bool last_spec = false;              // the most recent call speculated
     int* spec_E(int par) const { return (int*)((char*)spec_state + 8 + 16 * par); }
@@ -133,14 +137,13 @@ template <typename K> inline int set_smem(gal_plan* p, K kernel, size_t bytes) {
 }
 
 // CTAs of `kernel` resident on the GPU at once: the distance (in blocks) at which a CTA of an FFT pass prefetches
-// into the L2 for a later one.  GAL_ROW_PF scales it (0 switches the prefetch off; diagnostic).
+// into the L2 for a later one.  GAL_OPT_ROW_PREFETCH scales it (0 switches the prefetch off).
 template <typename K> inline int resident_ctas(gal_plan* p, K kernel, int threads, size_t smem) {
     auto it = p->resident.find((const void*)kernel);
     if (it != p->resident.end()) return it->second;
     int per_sm = 1;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
-    static const double mul = getenv("GAL_ROW_PF") ? atof(getenv("GAL_ROW_PF")) : 1.0;
-    const int r = (int)(per_sm * p->sm_count * mul);
+    const int r = (int)(per_sm * p->sm_count * p->row_pf);
     p->resident[(const void*)kernel] = r;
     return r;
 }

@@ -63,8 +63,11 @@ template <typename T> struct SampleParams {
 };
 
 // Which layout did the column pass write?  Same rule as fft.cuh: extent_is_whole_plane.
+// Extents are produced on the device earlier in the same programmatic-launch chain (uv-extent kernel, the previous
+// call's sampler): they are read only AFTER pdl_wait() and with L2-coherent loads (ld.global.cg), never through the
+// non-coherent path, whose L1 line could predate the producer's store.
 __device__ __forceinline__ bool extent_is_whole(const int* ext, int N) {
-    return __ldg(ext) >= N / 2 && __ldg(ext + 1) <= 0 && __ldg(ext + 2) >= N - 1;
+    return __ldcg(ext) >= N / 2 && __ldcg(ext + 1) <= 0 && __ldcg(ext + 2) >= N - 1;
 }
 // ... and which layout the column pass wrote (fft.cuh: layout_is_single, the same rule)
 __device__ __forceinline__ bool layout_single(const int* ext, int N) {
@@ -581,9 +584,9 @@ __device__ __forceinline__ void sample_finish(const SampleParams<T>& p, int c, d
                 // (a whole-plane extent covers every point, wrapped ones too: it cannot fail)
                 const bool failed = p.ext_check && !extent_is_whole(p.ext_check, p.N) && atomicAdd(p.viol, 0ull) != 0ull;
                 if (failed) { *p.redo = 1u; atomicExch(p.oob, 0ull); }              // the second pass counts again
-                p.used_ext[0] = failed ? e0 : __ldg(p.ext);
-                p.used_ext[1] = failed ? e1 : __ldg(p.ext + 1);
-                p.used_ext[2] = failed ? e2 : __ldg(p.ext + 2);
+                p.used_ext[0] = failed ? e0 : __ldcg(p.ext);
+                p.used_ext[1] = failed ? e1 : __ldcg(p.ext + 1);
+                p.used_ext[2] = failed ? e2 : __ldcg(p.ext + 2);
             }
             if (p.rearm) {
                 int* nx = reinterpret_cast<int*>(p.next_state);
@@ -674,7 +677,7 @@ __device__ __forceinline__ SampleCtx<T> sample_ctx(const SampleParams<T>& p, int
     cx_.viol = 0;
     cx_.r2 = 0.0;
     cx_.ck_kumax = p.N; cx_.ck_rmin = 0; cx_.ck_rmax = p.N;
-    if (p.ext_check) { cx_.ck_kumax = __ldg(p.ext_check); cx_.ck_rmin = __ldg(p.ext_check + 1); cx_.ck_rmax = __ldg(p.ext_check + 2); }
+    if (p.ext_check) { cx_.ck_kumax = __ldcg(p.ext_check); cx_.ck_rmin = __ldcg(p.ext_check + 1); cx_.ck_rmax = __ldcg(p.ext_check + 2); }
     return cx_;
 }
 
@@ -684,8 +687,8 @@ __global__ void __launch_bounds__(GAL_SAMPLE_NT, GAL_SAMPLE_MINB) sample_kernel_
     using G = SampleGeom<T, DO_CHI2>;
     const int c = blockIdx.y;
     const long long M = p.M;
-    SampleCtx<T> cx_ = sample_ctx(p, c);
     pdl_wait();
+    SampleCtx<T> cx_ = sample_ctx(p, c);                     // (reads the extent: after the wait)
     const long long ntiles = (M + G::TILE - 1) / G::TILE;
     if (layout_single(p.ext, p.N)) {
         for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x)
@@ -712,7 +715,6 @@ __global__ void __launch_bounds__(SampleGeom<T, DO_CHI2>::NT_TMA, GAL_SAMPLE_MIN
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int c = blockIdx.y;
     const long long M = p.M;
-    SampleCtx<T> cx_ = sample_ctx(p, c);
     const int nfull = (int)(M / TILE);
     const uint32_t stage0 = smem_u32(sample_smem);
     const uint32_t full0 = stage0 + S * G::STAGE_BYTES, empty0 = full0 + 8 * S;
@@ -722,6 +724,7 @@ __global__ void __launch_bounds__(SampleGeom<T, DO_CHI2>::NT_TMA, GAL_SAMPLE_MIN
     }
     pdl_wait();
     __syncthreads();
+    SampleCtx<T> cx_ = sample_ctx(p, c);                     // (reads the extent: after the wait)
 
     if (wid == G::NW) {
         if (lane == 0) {                                     // ---- producer ----
@@ -897,7 +900,9 @@ __global__ void __launch_bounds__(256) uv_radius_kernel(const T* __restrict__ u,
     double m = 0.0;
     for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < total; k += (long long)gridDim.x * blockDim.x) {
         const double a = (double)__ldcs(u + k), b = (double)__ldcs(v + k);
-        m = fmax(m, fma(a, a, b * b));
+        const double r2 = fma(a, a, b * b);
+        // fmax drops a NaN operand: a NaN coordinate counts as an infinite baseline, which the bind call rejects
+        m = (r2 == r2) ? fmax(m, r2) : __longlong_as_double(0x7ff0000000000000LL);
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));

@@ -96,7 +96,7 @@ int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T
     // channel keeps about twelve channels' spectra (not dozens) competing for the L2 at any time and gives every
     // CTA enough tiles to amortise its prologue and reduction (measured at cfg 4, bound observations: 4: 437,
     // 8: 396, 12: 384, 16: 385 us)
-    static const int conc = getenv("GAL_BATCH_CONC") ? atoi(getenv("GAL_BATCH_CONC")) : 12;     // channels in flight (diagnostic)
+    const int conc = p->batch_conc;                      // channels in flight (GAL_OPT_BATCH_CONC)
     if (C > 1) cap = (cap + (C < conc ? C : conc) - 1) / (C < conc ? C : conc);
     if (cap > p->max_gx) cap = p->max_gx;
     long long gx = ntiles < cap ? ntiles : cap;

@@ -696,12 +696,8 @@ def test_speculative_extent_and_its_second_pass(g, orc, dtype):
         w = w.as_f32()
     fresh = g.Plan(w.nxy, 1, dtype)
     fresh.set_pruning(0)
-    import os
-    os.environ["GAL_SPEC_MIN_BYTES"] = "0"              # (read at plan creation: speculate at this test's size too)
-    try:
-        plan = g.Plan(w.nxy, 1, dtype)                  # prune mode 1 (default)
-    finally:
-        del os.environ["GAL_SPEC_MIN_BYTES"]
+    plan = g.Plan(w.nxy, 1, dtype)                      # prune mode 1 (default)
+    plan.set_option("spec_min_bytes", 0)                # speculate at this test's size too
     image = dev(w.image)
     N = w.nxy
 
@@ -753,6 +749,89 @@ def test_speculative_extent_and_its_second_pass(g, orc, dtype):
     assert abs(got - ref) <= (TOL_CHI2_F32 if f32 else TOL_CHI2_F64) * abs(ref)
 
 
+@pytest.mark.parametrize("nxy,dtype", [(2048, torch.float64), (4096, torch.float64), (2048, torch.float32), (4096, torch.float32)])
+def test_second_pass_of_a_speculative_call_against_the_oracle(g, orc, nxy, dtype):
+    """The conditional second pass (redo.cuh) at BOTH sizes it is built for, incl. the headline's nxy = 4096: after a
+    speculating call on short baselines the uv set grows, the sampler's verification fails and the persistent kernel
+    repeats row pass, column pass and sampling on the device.  Its visibilities and chi2 are compared with the ORACLE
+    at the tolerances of every other parity test (reading A13), with the out-of-grid count and the extent."""
+    f32 = dtype == torch.float32
+    w = W.config(3, nxy=nxy, M=150_001, n_src=40)
+    if f32:
+        w = w.as_f32()
+    f = lambda a: np.asarray(a, dtype=np.float64)
+    plan = g.Plan(nxy, 1, dtype)                             # prune mode 1 (default)
+    plan.set_option("spec_min_bytes", 0)                     # speculate at this test's M too
+    image, obs = dev(w.image), (dev(w.re_obs), dev(w.im_obs), dev(w.w))
+    small = (dev(w.u * 0.5), dev(w.v * 0.5))
+    N = nxy
+
+    def prime():                                             # two calls on the short baselines: the 2nd speculates
+        plan.chi2Image(image, w.dxy, *small, *obs, w.dRA, w.dDec, w.PA)
+        n0 = plan.launch_count()
+        plan.chi2Image(image, w.dxy, *small, *obs, w.dRA, w.dDec, w.PA)
+        assert plan.launch_count() - n0 == 4                 # row, column, sampling, conditional kernel: no extent pass
+        return plan.last_uv_extent()
+
+    for scale, wraps in ((1.0, False), (5.0, True)):         # grown set inside the grid / beyond it (whole plane, A6)
+        us, vs = (w.u * scale).astype(w.u.dtype), (w.v * scale).astype(w.v.dtype)
+        u, v = dev(us), dev(vs)
+        ref, ref_oob = orc.sampleImage(f(w.image), w.dxy, f(us), f(vs), w.PA, w.dRA, w.dDec, return_oob=True,
+                                       nthreads=threads(orc))
+        ref_chi2 = orc.chi2(ref, f(w.re_obs), f(w.im_obs), f(w.w))
+        peak = np.abs(ref).max()
+        # sampleImage through the second pass
+        e_small = prime()
+        vis = plan.sampleImage(image, w.dxy, u, v, w.PA, w.dRA, w.dDec).cpu().numpy()
+        e_big = plan.last_uv_extent()
+        assert e_big[0] > e_small[0] and e_big[1] < e_small[1] and e_big[2] > e_small[2]      # the call did repeat itself
+        assert (e_big == (N // 2, 0, N - 1)) == wraps
+        assert plan.last_oob_count() == ref_oob and (ref_oob > 0) == wraps
+        if f32:
+            assert np.abs(vis - ref).max() <= TOL_VIS_F32 * peak
+        else:
+            assert rel_err(vis, ref) <= TOL_VIS_F64
+        # chi2Image through the second pass
+        prime()
+        chi2 = float(plan.chi2Image(image, w.dxy, u, v, *obs, w.dRA, w.dDec, w.PA).cpu()[0])
+        assert plan.last_uv_extent() == e_big and plan.last_oob_count() == ref_oob
+        assert abs(chi2 - ref_chi2) <= (TOL_CHI2_F32 if f32 else TOL_CHI2_F64) * abs(ref_chi2)
+        # and the call after it speculates on the grown extent: no second pass, same numbers
+        chi2b = float(plan.chi2Image(image, w.dxy, u, v, *obs, w.dRA, w.dDec, w.PA).cpu()[0])
+        assert abs(chi2b - ref_chi2) <= (TOL_CHI2_F32 if f32 else TOL_CHI2_F64) * abs(ref_chi2)
+
+
+def test_batched_calls_back_to_back_read_the_extent_after_the_wait(g):
+    """Small grids, always-prune mode, C > 1, points beyond the grid (so the exact extent is the WHOLE plane and the
+    spectrum takes the single-value layout, while the armed default says 'pair'), many calls issued back to back with
+    no host synchronisation: the kernels of consecutive calls are co-resident through programmatic dependent launch,
+    so a sampler that read the extent before its griddepcontrol.wait would pick the wrong layout / plane offset.
+    Every call must equal the never-pruning plan's result, bit for bit."""
+    w = W.config(4, nxy=128, M=60_000, C=6)
+    u, v = dev(w.u), dev(w.v)                                # at this nxy: far beyond the grid in every channel
+    args = (dev(w.image), w.dxy, u, v, dev(w.re_obs), dev(w.im_obs), dev(w.w), w.dRA, w.dDec, w.PA)
+    ref_plan = g.Plan(w.nxy, 6)
+    ref_plan.set_pruning(0)
+    rper, rtot = ref_plan.chi2ImageBatch(*args)
+    assert ref_plan.last_oob_count() > 0
+    plan = g.Plan(w.nxy, 6)
+    plan.set_pruning(2)
+    outs = [plan.chi2ImageBatch(*args) for _ in range(40)]   # no synchronisation in between
+    torch.cuda.synchronize()
+    assert plan.last_uv_extent() == (w.nxy // 2, 0, w.nxy - 1)
+    for per, tot in outs:
+        assert torch.equal(per, rper) and torch.equal(tot, rtot)
+    # the same with in-grid points in between (pair layout <-> single layout from one call to the next)
+    ui, vi = dev(w.u * 0.08), dev(w.v * 0.08)                # (longest baseline at 49 of 64 cells)
+    argi = (args[0], w.dxy, ui, vi) + args[4:]
+    iper, itot = ref_plan.chi2ImageBatch(*argi)
+    assert ref_plan.last_oob_count() == 0
+    mixed = [plan.chi2ImageBatch(*(args if k % 2 else argi)) for k in range(40)]
+    torch.cuda.synchronize()
+    for k, (per, tot) in enumerate(mixed):
+        assert torch.equal(per, rper if k % 2 else iper) and torch.equal(tot, rtot if k % 2 else itot), k
+
+
 @pytest.mark.parametrize("nxy", [2048, 4096])
 def test_row_pass_variant_follows_the_expected_extent(g, nxy):
     """At nxy = 2048 / 4096 (fp64) the plan picks the row-pass form from the extent it EXPECTS — a hint the sampler of
@@ -764,12 +843,9 @@ def test_row_pass_variant_follows_the_expected_extent(g, nxy):
     image = dev(w.image)
     ref_plan = g.Plan(nxy)
     ref_plan.set_pruning(0)
-    import os
-    os.environ["GAL_NO_SPEC"] = "1"                          # (read at plan creation: this test is about the row-pass forms,
-    try:                                                     #  the speculative extent has its own, above)
-        plan = g.Plan(nxy)
-    finally:
-        del os.environ["GAL_NO_SPEC"]
+    plan = g.Plan(nxy)
+    plan.set_option("speculate", 0)                          # this test is about the row-pass forms (the speculative
+                                                             # extent has its own, above)
     obs = (dev(w.re_obs), dev(w.im_obs), dev(w.w))
     for scale in (1.0, 1.0, 1.0, 9.0, 9.0, 1.0, 1.0):        # in-grid (pruned), then wrapping (whole plane), then back
         u, v = dev(w.u * scale), dev(w.v * scale)
