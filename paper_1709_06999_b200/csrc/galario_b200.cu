@@ -484,8 +484,8 @@ int gal_plan_create(gal_plan** out, int nxy, int batch, int precision_bits, int 
     if ((e = cudaMalloc((void**)&p->ext_full, 16)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     if ((e = cudaMalloc((void**)&p->b_ext_dev, 16)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     if ((e = cudaMalloc((void**)&p->b_r2, 8)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
-    if ((e = cudaMalloc(&p->spec_state, 64)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
-    if ((e = cudaMemset(p->spec_state, 0, 64)) != cudaSuccess) return fail(GAL_ERR_CUDA, e);
+    if ((e = cudaMalloc(&p->spec_state, 128)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
+    if ((e = cudaMemset(p->spec_state, 0, 128)) != cudaSuccess) return fail(GAL_ERR_CUDA, e);
     if ((e = cudaHostAlloc((void**)&p->viol_host, 2 * sizeof(unsigned int), cudaHostAllocMapped)) != cudaSuccess) return fail(GAL_ERR_ALLOC, e);
     p->viol_host[0] = 0; p->viol_host[1] = 0;          // [1]: extent hint (plan.h row_small)
     if ((e = cudaHostGetDevicePointer((void**)&p->viol_dev, p->viol_host, 0)) != cudaSuccess) return fail(GAL_ERR_CUDA, e);

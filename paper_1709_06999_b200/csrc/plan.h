@@ -67,7 +67,7 @@ struct gal_plan {
     // against it and derives the extent for the next call; if a point lay outside, ONE conditional kernel (redo.cuh:
     // it leaves at once unless the device flag `redo` is set) repeats transform and sampling on the new extent.
     // No host synchronisation, results unchanged.
-    // spec_state (device, 64 B): [0] u64 r2max | [8] int E[2][4] | [40] u32 redo | [44] int used_ext[3] | [56] u32 bar[2]
+    // spec_state (device, 128 B): [0] u64 r2max | [8] int E[2][4] | [40] u32 redo | [44] int used_ext[3] | [64] u32 ctr[5] (redo.cuh)
     void* spec_state = nullptr;
     int spec_par = 0;                    // E[spec_par] is the extent the next speculative call transforms
     bool spec_valid = false;             // E[spec_par] has been (will have been, in stream order) written ...
@@ -80,7 +80,7 @@ struct gal_plan {
     int* spec_E(int par) const { return (int*)((char*)spec_state + 8 + 16 * par); }
     unsigned int* spec_redo() const { return (unsigned int*)((char*)spec_state + 40); }
     int* spec_used() const { return (int*)((char*)spec_state + 44); }
-    unsigned int* spec_bar() const { return (unsigned int*)((char*)spec_state + 56); }
+    unsigned int* spec_ctr() const { return (unsigned int*)((char*)spec_state + 64); }
     void* st_vis = nullptr; size_t st_vis_bytes = 0; // summed visibilities of a chi2 multi-source call
     std::set<const void*> smem_set;      // kernels whose dynamic shared-memory limit has been raised
     std::map<const void*, int> resident; // kernel -> CTAs resident on the whole GPU at once (occupancy x SM count)

@@ -801,6 +801,45 @@ def test_second_pass_of_a_speculative_call_against_the_oracle(g, orc, nxy, dtype
         assert abs(chi2b - ref_chi2) <= (TOL_CHI2_F32 if f32 else TOL_CHI2_F64) * abs(ref_chi2)
 
 
+def test_second_passes_of_two_plans_under_contention(g):
+    """The second pass is one persistent kernel with grid barriers, so all of its CTAs must be resident together.  It is
+    launched cooperatively: two plans on two streams that BOTH repeat a call at the same moment — each grid wants every
+    SM — and a third stream that keeps the SMs busy with long direct-Hankel launches must all finish (a plain launch
+    could place part of each grid and spin for ever), with the results of a never-pruning plan."""
+    w = W.config(3, nxy=2048, M=150_001, n_src=40)
+    image, obs = dev(w.image), (dev(w.re_obs), dev(w.im_obs), dev(w.w))
+    small, big = (dev(w.u * 0.5), dev(w.v * 0.5)), (dev(w.u), dev(w.v))
+    fresh = g.Plan(w.nxy)
+    fresh.set_pruning(0)
+    ref_small = float(fresh.chi2Image(image, w.dxy, *small, *obs, w.dRA, w.dDec, w.PA).cpu()[0])
+    ref_big = float(fresh.chi2Image(image, w.dxy, *big, *obs, w.dRA, w.dDec, w.PA).cpu()[0])
+    plans = [g.Plan(w.nxy), g.Plan(w.nxy)]
+    for p in plans:
+        p.set_option("spec_min_bytes", 0)
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    filler_stream, filler_plan = torch.cuda.Stream(), g.Plan(64)
+    w1 = W.config(1, nxy=256, M=60_000, nr=2000)
+    fill = [dev(a) for a in (w1.profile, w1.u, w1.v, w1.re_obs, w1.im_obs, w1.w)]
+    torch.cuda.synchronize()
+    outs = ([], [])
+    for it in range(8):
+        with torch.cuda.stream(filler_stream):               # some milliseconds of CTAs on every SM
+            filler_plan.chi2ProfileHankel(fill[0], w1.Rmin, w1.dR, *fill[1:], 0.0, 0.0, w1.PA, w1.inc)
+        for p, st, o in zip(plans, streams, outs):
+            with torch.cuda.stream(st):                      # small, small (speculates), big (verification fails: second pass)
+                a = p.chi2Image(image, w.dxy, *small, *obs, w.dRA, w.dDec, w.PA)
+                b = p.chi2Image(image, w.dxy, *small, *obs, w.dRA, w.dDec, w.PA)
+                c = p.chi2Image(image, w.dxy, *big, *obs, w.dRA, w.dDec, w.PA)
+                o.append((a, b, c))
+    torch.cuda.synchronize()
+    for o in outs:
+        for a, b, c in o:
+            for got, ref in ((a, ref_small), (b, ref_small), (c, ref_big)):
+                assert abs(float(got[0]) - ref) <= TOL_CHI2_F64 * abs(ref)
+    for p in plans:
+        assert p.last_uv_extent()[0] < w.nxy // 2 and p.last_oob_count() == 0
+
+
 def test_batched_calls_back_to_back_read_the_extent_after_the_wait(g):
     """Small grids, always-prune mode, C > 1, points beyond the grid (so the exact extent is the WHOLE plane and the
     spectrum takes the single-value layout, while the armed default says 'pair'), many calls issued back to back with
