@@ -61,6 +61,23 @@ def algorithmic_bytes(nxy: int, M: int, esz: int, entry: str = "chi2Image", exte
     return out
 
 
+# FP64 FMA rate measured on this box by gal_measure_fp64_fma_peak at the start of the run (TFLOP/s, 2 flop per DFMA);
+# the ALU fractions below divide by it.  None until main() has measured it.
+FP64_PEAK_TFLOPS = None
+
+# Warp-level FP64 instructions (DADD + DMUL + DFMA: one issue slot of the FP64 pipe each) per launch of the three
+# kernels of the headline call on its pruned extent, from the instruction mix of profiles/r2_stalls.md (c3:
+# executed warp instructions x the FP64 share of the mix; the shares are rounded to 1 %, so these are +-3 %).
+FP64_WARP_INSTR_CFG3 = {"row_pass": 19362880 * 0.64, "col_pass": 5298719 * 0.59, "sample": 31638068 * 0.34}
+
+
+def alu_frac(warp_instr: float, ms: float):
+    """Fraction of the measured FP64 pipe rate: lane-instructions per second over DFMA lanes per second."""
+    if not FP64_PEAK_TFLOPS or ms <= 0:
+        return None
+    return warp_instr * 32.0 / (ms * 1e-3) / (FP64_PEAK_TFLOPS * 1e12 / 2.0)
+
+
 def measured_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -282,12 +299,14 @@ def measure_case(g, torch, dev, peak, name, w, dtype, entry, prune, steps, warmu
            "kernels_frac": {k: round(Bp[k] / (t * 1e-3) / 1e9 / peak, 3) for k, t in kms.items() if t > 0 and Bp[k] > 0}}
     if entry == "chi2ProfileHankel":
         # no image, no transform: M * nr Bessel evaluations, FP64-ALU bound.  One evaluation is
-        # about 45 FP64 instructions; the pipe issues 148 SMs x 64 lanes per clock.
+        # about 45 FP64 instructions (hand count of hankel.cuh's inner loop); the pipe rate is the one measured on this box.
         nr = len(w.profile)
         for k in ("method_bytes_whole_plane", "frac_whole_plane_bytes", "method_bytes_this_extent", "frac", "uv_extent", "pruned"):
             row.pop(k)
+        lanes_per_s = FP64_PEAK_TFLOPS * 1e12 / 2.0 if FP64_PEAK_TFLOPS else None      # measured DFMA lanes per second
         row.update({"bound": "alu", "j0_evaluations": w.M * nr, "j0_evaluations_per_s": w.M * nr / (ms * 1e-3),
-                    "fp64_pipe_frac_at_45_instr": 45.0 * w.M * nr / (ms * 1e-3) / (148 * 64 * 1.965e9)})
+                    "fp64_tflops_measured": FP64_PEAK_TFLOPS,
+                    "fp64_pipe_frac_at_45_instr": 45.0 * w.M * nr / (ms * 1e-3) / lanes_per_s if lanes_per_s else None})
     del plan
     torch.cuda.empty_cache()
     return row
@@ -410,17 +429,22 @@ def main():
             torch.distributed.barrier()
         torch.cuda.synchronize()
 
+    global FP64_PEAK_TFLOPS
+    # the clock is sampled over the whole GPU-busy part of the headline (FP64 peak, warm-up, timed loop, per-kernel
+    # timing, bound-observation loop): the timed loop alone lasts 2-3 ms, one or two samples
+    clk = ClockSampler(local_rank)
+    clk.__enter__()
+    FP64_PEAK_TFLOPS, fp64_peak_ms = g.measure_fp64_peak(local_rank)
     for _ in range(args.warmup):
         step()
     barrier()
     l0 = plan.launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    with ClockSampler(local_rank) as clk:
-        e0.record()
-        for _ in range(args.steps):
-            step()
-        e1.record()
-        barrier()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
     ms_total = max_over_ranks(e0.elapsed_time(e1), world, dev)
     launches = plan.launch_count() - l0
     chi2_val = float(out.cpu()[0])
@@ -442,7 +466,8 @@ def main():
             continue
         gbs = Bk[name] / (ms * 1e-3) / 1e9
         kernels.append({"kernel": name, "ms": ms, "algorithmic_bytes": Bk[name], "achieved_gbs": gbs,
-                        "frac": gbs / peak, "share_of_step": ms / ms_sum})
+                        "frac": gbs / peak, "share_of_step": ms / ms_sum,
+                        "alu_frac": alu_frac(FP64_WARP_INSTR_CFG3[name], ms) if (pruned and name in FP64_WARP_INSTR_CFG3) else None})
     dom = max(kernels, key=lambda k: k["ms"])
     roofline = {"bound": "hbm", "kernel": dom["kernel"], "achieved": dom["achieved_gbs"], "peak": peak, "unit": "GB/s",
                 "frac": dom["frac"], "traffic": ncu_traffic(dom["kernel"]),
@@ -485,6 +510,7 @@ def main():
                  "kernels_us": {k: round(1e3 * t, 2) for k, t in bkms.items() if t > 0},
                  "kernels_frac": {k: round(Bb[k] / (t * 1e-3) / 1e9 / peak, 3) for k, t in bkms.items() if t > 0 and Bb[k] > 0}}
     plan.unbind_obs()
+    clk.__exit__(None, None, None)
 
     # end to end through the host-pointer C-ABI call: pinned host inputs, H2D + kernels + D2H each step
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
@@ -536,7 +562,11 @@ def main():
     result = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-        "data": "synthetic", "config": base_config(w, "f64"), "clocks": clk.summary(), "e2e": e2e, "e2e_image_only": e2e_image_only,
+        "data": "synthetic", "config": dict(base_config(w, "f64"), uv_extent=list(extent), pruned_transform=pruned,
+                                            method_bytes_this_extent=Bk["step"]),
+        "clocks": clk.summary(), "fp64_tflops_measured": FP64_PEAK_TFLOPS, "fp64_peak_launch_ms": fp64_peak_ms,
+        "fp64_peak_note": "gal_measure_fp64_fma_peak: 8 independent DFMA chains per thread, 8 x 256 threads per SM, best of 5; "
+                          "kernels[].alu_frac = FP64 lane-instructions/s (profiles/r2_stalls.md mix) over this rate", "e2e": e2e, "e2e_image_only": e2e_image_only,
         "gpu_launches": int(launches), "roofline": roofline, "step_roofline": step_roofline, "kernels": kernels,
         "visibilities_per_s": value * w.M, "chi2": chi2_val, "multi_gpu": "replicas only", "bound_obs": bound_obs,
         "paper_context": "GTX 1060, M=1e6, PCIe copies included: chi2Image 4096^2 = 59 ms (PAPER.md:619); not like for like",

@@ -286,6 +286,13 @@ int gal_chi2_profile_host_f64(gal_plan* plan, const double* I, int nr, double Rm
                               const double* w, int64_t M, double dRA, double dDec, double PA, double inc,
                               double* chi2_out, void* stream);
 
+/* ---- measurement helper (not part of the method): the FP64 fused-multiply-add rate of `device`, measured with
+ *      independent DFMA chains on every SM (a few launches of a few ms each, CUDA-event timed, best of five;
+ *      synchronises the device; allocates and frees 8 bytes).  *tflops_out = 2 flop x DFMA/s / 1e12 (host);
+ *      ms_out (host, may be NULL) = duration of the best launch.  bench.py divides the FP64 instruction rate of each
+ *      kernel by this to report an ALU fraction beside the HBM fraction. ---- */
+int gal_measure_fp64_fma_peak(int device, double* tflops_out, double* ms_out);
+
 /* ---- chi2Profile WITHOUT A PLAN AND WITHOUT ANY ALLOCATION (direct Hankel transform, Eq. 25 and Eq. 10:
  *      PAPER.md:366-368, 194-198, 718; same mathematics and same arguments as gal_chi2_profile_hankel_f64).
  *

@@ -13,8 +13,8 @@ Paper-style calls (PAPER.md:82-113, 650, 723)::
 """
 from .binding import (Plan, GalarioError, library_path, load_library, sampleImage, chi2Image, sampleProfile,
                       chi2Profile, sweep, chi2ImageBatch, fft2_shifted, get_plan, get_image_size,
-                      chi2ProfileHankelNoAlloc, NOALLOC_MAX_POINTS)
+                      chi2ProfileHankelNoAlloc, NOALLOC_MAX_POINTS, measure_fp64_peak)
 
 __all__ = ["Plan", "GalarioError", "library_path", "load_library", "sampleImage", "chi2Image", "sampleProfile",
            "chi2Profile", "sweep", "chi2ImageBatch", "fft2_shifted", "get_plan", "get_image_size",
-           "chi2ProfileHankelNoAlloc", "NOALLOC_MAX_POINTS"]
+           "chi2ProfileHankelNoAlloc", "NOALLOC_MAX_POINTS", "measure_fp64_peak"]

@@ -86,6 +86,7 @@ def load_library() -> ctypes.CDLL:
         lib.gal_chi2_profile_hankel_noalloc_f64.argtypes = [_i, _vp, _i, _d, _d, _vp, _vp, _vp, _vp, _vp, _i64, _d, _d,
                                                             _d, _d, _vp, _vp]
         lib.gal_noalloc_scratch_bytes.restype = ctypes.c_size_t
+        lib.gal_measure_fp64_fma_peak.argtypes = [_i, _vp, _vp]
         _lib = lib
     return _lib
 
@@ -108,6 +109,14 @@ def get_image_size(u, v, PB: float = 0.0, f_min: float = 5.0, f_max: float = 2.5
                                              float(f_max), ctypes.addressof(n), ctypes.addressof(d)),
            "gal_get_image_size")
     return n.value, d.value
+
+
+def measure_fp64_peak(device: int = 0):
+    """(TFLOP/s, ms of the best launch): the FP64 FMA rate measured on `device` (gal_measure_fp64_fma_peak)."""
+    tf, ms = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    _check(load_library().gal_measure_fp64_fma_peak(int(device), ctypes.addressof(tf), ctypes.addressof(ms)),
+           "gal_measure_fp64_fma_peak")
+    return tf.value, ms.value
 
 
 NOALLOC_MAX_POINTS = 1 << 20          # GAL_NOALLOC_MAX_POINTS of the header
@@ -254,20 +263,21 @@ class Plan:
     def sampleImageMulti(self, image, dxy, u, v, placements, out=None):
         """sum_s scale_s * sampleImage(image; dRA_s, dDec_s, PA_s): one transform, S placements."""
         M = u.numel()
-        out = torch.empty(M, dtype=self._cdtype, device=u.device) if out is None else out
+        out = self._out(out, M, self._cdtype, u)
         dRA, dDec, PA, sc = self._placements(placements)
-        _check(self._fn("sample_image_multi")(self._h, self._dev(image, "image"), dxy, self._dev(u, "u"),
-                                              self._dev(v, "v"), M, len(dRA), dRA.ctypes.data, dDec.ctypes.data,
+        _check(self._fn("sample_image_multi")(self._h, self._dev(image, "image", self.nxy ** 2), dxy, self._dev(u, "u"),
+                                              self._dev(v, "v", M), M, len(dRA), dRA.ctypes.data, dDec.ctypes.data,
                                               PA.ctypes.data, sc.ctypes.data, out.data_ptr(), _stream()),
                "gal_sample_image_multi", self)
         return out
 
     def chi2ImageMulti(self, image, dxy, u, v, re_obs, im_obs, w, placements, out=None):
-        out = torch.empty(1, dtype=torch.float64, device=u.device) if out is None else out
+        M = u.numel()
+        out = self._out(out, 1, torch.float64, u)
         dRA, dDec, PA, sc = self._placements(placements)
-        _check(self._fn("chi2_image_multi")(self._h, self._dev(image, "image"), dxy, self._dev(u, "u"),
-                                            self._dev(v, "v"), self._dev(re_obs, "re_obs"), self._dev(im_obs, "im_obs"),
-                                            self._dev(w, "w"), u.numel(), len(dRA), dRA.ctypes.data, dDec.ctypes.data,
+        _check(self._fn("chi2_image_multi")(self._h, self._dev(image, "image", self.nxy ** 2), dxy, self._dev(u, "u"),
+                                            self._dev(v, "v", M), self._dev(re_obs, "re_obs", M), self._dev(im_obs, "im_obs", M),
+                                            self._dev(w, "w", M), M, len(dRA), dRA.ctypes.data, dDec.ctypes.data,
                                             PA.ctypes.data, sc.ctypes.data, out.data_ptr(), _stream()),
                "gal_chi2_image_multi", self)
         return out
@@ -366,17 +376,18 @@ class Plan:
     def sampleProfileHankel(self, I, Rmin, dR, u, v, inc=0.0, PA=0.0, dRA=0.0, dDec=0.0, out=None):
         """sampleProfile by the direct Hankel transform of Eq. 25 (no image, no FFT)."""
         M = u.numel()
-        out = torch.empty(M, dtype=self._cdtype, device=u.device) if out is None else out
+        out = self._out(out, M, self._cdtype, u)
         _check(self._fn("sample_profile_hankel")(self._h, self._dev(I, "I"), I.numel(), Rmin, dR, self._dev(u, "u"),
-                                                 self._dev(v, "v"), M, dRA, dDec, PA, inc, out.data_ptr(), _stream()),
+                                                 self._dev(v, "v", M), M, dRA, dDec, PA, inc, out.data_ptr(), _stream()),
                "gal_sample_profile_hankel", self)
         return out
 
     def chi2ProfileHankel(self, I, Rmin, dR, u, v, re_obs, im_obs, w, dRA=0.0, dDec=0.0, PA=0.0, inc=0.0, out=None):
-        out = torch.empty(1, dtype=torch.float64, device=u.device) if out is None else out
+        M = u.numel()
+        out = self._out(out, 1, torch.float64, u)
         _check(self._fn("chi2_profile_hankel")(self._h, self._dev(I, "I"), I.numel(), Rmin, dR, self._dev(u, "u"),
-                                               self._dev(v, "v"), self._dev(re_obs, "re_obs"),
-                                               self._dev(im_obs, "im_obs"), self._dev(w, "w"), u.numel(), dRA, dDec,
+                                               self._dev(v, "v", M), self._dev(re_obs, "re_obs", M),
+                                               self._dev(im_obs, "im_obs", M), self._dev(w, "w", M), M, dRA, dDec,
                                                PA, inc, out.data_ptr(), _stream()), "gal_chi2_profile_hankel", self)
         return out
 

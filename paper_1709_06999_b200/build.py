@@ -34,8 +34,21 @@ def _stale(target: Path, deps) -> bool:
     return not target.exists() or any(target.stat().st_mtime < d.stat().st_mtime for d in deps)
 
 
+STAMP = OBJ / "flags.stamp"
+
+
+def _flags() -> str:
+    """The flag set the objects are compiled with.  It is written next to them: objects from a tuning build
+    (GAL_NVCC_EXTRA=-D...) must never be mistaken for fresh ones by a later default build, or the other way round."""
+    return " ".join(NVCC_FLAGS + os.environ.get("GAL_NVCC_EXTRA", "").split())
+
+
+def _flags_changed() -> bool:
+    return not STAMP.exists() or STAMP.read_text() != _flags()
+
+
 def needs_build() -> bool:
-    return _stale(LIB, sources() + headers())
+    return _flags_changed() or _stale(LIB, sources() + headers())
 
 
 def build(force: bool = False, verbose: bool = False) -> Path:
@@ -46,9 +59,12 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     OBJ.mkdir(exist_ok=True)
     hdrs = headers()
     jobs = []
+    force = force or _flags_changed()                           # other flags than the objects on disk were built with
+    if STAMP.exists():
+        STAMP.unlink()                                          # (rewritten once every object has been compiled)
     for src in sources():
         obj = OBJ / (src.stem + ".o")
-        if force or extra or _stale(obj, [src] + hdrs):
+        if force or _stale(obj, [src] + hdrs):
             jobs.append([nvcc, *NVCC_FLAGS, *extra, *(["-Xptxas", "-v"] if verbose else []), "-c", str(src), "-o", str(obj)])
     with ThreadPoolExecutor(max_workers=min(len(jobs), os.cpu_count() or 1) or 1) as ex:
         for r in ex.map(lambda c: subprocess.run(c, capture_output=not verbose, text=True), jobs):
@@ -59,6 +75,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     subprocess.run([nvcc, "-shared", "-cudart", "static", "-gencode", "arch=compute_100a,code=sm_100a", "-o", str(tmp), *objs],
                    check=True)
     os.replace(tmp, LIB)
+    STAMP.write_text(_flags())
     return LIB
 
 

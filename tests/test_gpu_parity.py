@@ -1033,3 +1033,40 @@ def test_paper_style_module_calls(g, orc):
     c = g.chi2Image(dev(w.image), w.dxy, dev(w.u), dev(w.v), dev(w.re_obs), dev(w.im_obs), dev(w.w), w.dRA, w.dDec, w.PA)
     r = orc.chi2(ref, w.re_obs, w.im_obs, w.w)
     assert abs(float(c.cpu()[0]) - r) <= TOL_CHI2_F64 * abs(r)
+
+
+def test_binding_rejects_short_arrays_and_wrong_outputs(g):
+    """The multi-source and direct-Hankel methods of the binding check what they hand to the C ABI (a short array or a
+    wrong-typed output would be an out-of-bounds device access), and a NaN coordinate cannot be bound."""
+    w = W.config(1, nxy=64, M=500, nr=100)
+    plan = g.Plan(64)
+    img = torch.zeros(64, 64, dtype=torch.float64, device="cuda")
+    prof, u, v, re, im, wt = (dev(a) for a in (w.profile, w.u, w.v, w.re_obs, w.im_obs, w.w))
+    pl = [(0.0, 0.0, 0.0), (1e-7, 0.0, 0.3, 0.5)]
+    bad_out = torch.empty(500, dtype=torch.complex64, device="cuda")
+    for call in (lambda: plan.sampleImageMulti(img, w.dxy, u, v[:-1], pl),
+                 lambda: plan.sampleImageMulti(img, w.dxy, u, v, pl, out=bad_out),
+                 lambda: plan.sampleImageMulti(img[:32], w.dxy, u, v, pl),
+                 lambda: plan.chi2ImageMulti(img, w.dxy, u, v, re, im[:-3], wt, pl),
+                 lambda: plan.chi2ImageMulti(img, w.dxy, u, v, re, im, wt, pl, out=torch.empty(1, device="cuda")),
+                 lambda: plan.sampleProfileHankel(prof, w.Rmin, w.dR, u, v[:10]),
+                 lambda: plan.sampleProfileHankel(prof, w.Rmin, w.dR, u, v, out=bad_out),
+                 lambda: plan.chi2ProfileHankel(prof, w.Rmin, w.dR, u, v, re, im, wt[:-1]),
+                 lambda: plan.chi2ProfileHankel(prof, w.Rmin, w.dR, u, v, re, im, wt, out=torch.empty(2, dtype=torch.float64, device="cuda")),
+                 lambda: plan.bind_uv(u, v[:-1])):
+        with pytest.raises(g.GalarioError):
+            call()
+    assert plan.sampleImageMulti(img, w.dxy, u, v, pl).shape == (500,)       # and the good calls still go through
+    un = u.clone()
+    un[17] = float("nan")
+    with pytest.raises(g.GalarioError):
+        plan.bind_uv(un, v)                                  # the radius reduction must not drop a NaN
+    with pytest.raises(g.GalarioError):
+        plan.bind_obs(u, un, re, im, wt)
+    plan.bind_uv(u, v)
+    plan.unbind_uv()
+    plan.set_option("batch_conc", 4)
+    with pytest.raises(g.GalarioError):
+        plan.set_option("no_such_option", 1)
+    with pytest.raises(g.GalarioError):
+        plan.set_option("row_mode", 9)
