@@ -190,8 +190,6 @@ template <typename T> int launch_sample(gal_plan* p, int C, const CallScalars& c
 template <typename T> int launch_redo(gal_plan* p, const T* image, const CallScalars& cs, const T* u, const T* v, const T* re,
                                       const T* im, const T* w, int64_t M, T* vis, double* chi2_pc, double* chi2_tot, cudaStream_t st);
 template <typename T> int launch_sum_channels(gal_plan* p, const double* chi2_pc, int C, double* chi2_tot, cudaStream_t st);
-template <typename T> int launch_chi2_from_vis(gal_plan* p, const T* vis, const T* re, const T* im, const T* w, int64_t M,
-                                               double* chi2, cudaStream_t st);
 // bind_obs: sort channel by channel, write the five sorted arrays to dst = [5][C][M]
 template <typename T> int launch_bind_sort(gal_plan* p, const T* u, const T* v, const T* re, const T* im, const T* w, int64_t M,
                                            int C, double rmax, T* dst, cudaStream_t st);

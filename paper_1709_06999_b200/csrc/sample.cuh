@@ -785,7 +785,8 @@ __global__ void __launch_bounds__(SampleGeom<T, DO_CHI2>::NT_TMA, GAL_SAMPLE_MIN
 // ------------------------------------------------------------------------------------------
 template <typename T, bool PAIR>
 __device__ __forceinline__ void multi_point(const SampleParams<T>& p, const PlacementSet& ps, const NodePair<T>* __restrict__ spec,
-                                            double u, double v, double& vr, double& vi, unsigned int& oob) {
+                                            double u, double v, double& vr, double& vi, unsigned int& oob,
+                                            int ck_kumax, int ck_rmin, int ck_rmax, unsigned int& viol) {
     const int N = p.N;
     for (int s = 0; s < ps.S; ++s) {
         const Placement& pl = ps.pl[s];
@@ -798,6 +799,7 @@ __device__ __forceinline__ void multi_point(const SampleParams<T>& p, const Plac
             const int ix0 = floor_small(q.uidx, &fx0), iy0 = floor_small(q.vidx, &fy0);
             const double tx = __dsub_rn(q.uidx, fx0), ty = __dsub_rn(q.vidx, fy0);
             const int off = ix0 * N + iy0;
+            if (ix0 + 1 > ck_kumax || iy0 < ck_rmin || iy0 + 1 > ck_rmax) ++viol;   // outside the extent the transform was pruned to
             cx<T> g00, g01, g10, g11;                                         // g[row][column]
             if (PAIR) {
                 const NodePair<T> e0 = load_pair(spec + off), e1 = load_pair(spec + off + 1);
@@ -812,6 +814,7 @@ __device__ __forceinline__ void multi_point(const SampleParams<T>& p, const Plac
             im = fma(ty, r1i - r0i, r0i);
         } else {                                                              // reading A6
             if (q.uidx > ix.fH || q.vidx < 0.0 || q.vidx > ix.fN1) ++oob;
+            if (ck_kumax < N) ++viol;                                         // (a wrapped cell needs the whole plane)
             const cx<double> g = wrapped_cell<T, PAIR>(spec, N, q.uidx, q.vidx);
             re = g.x; im = g.y;
         }
@@ -834,22 +837,25 @@ template <typename T, bool WRITE_VIS, bool DO_CHI2>
 __global__ void __launch_bounds__(256) sample_multi_kernel(const SampleParams<T> p, const PlacementSet ps) {
     pdl_wait();
     const bool single = layout_single(p.ext, p.N);
+    // a bound uv set (gal_plan_bind_uv): every cell is verified against the extent the transform was pruned to
+    int ck_kumax = p.N, ck_rmin = 0, ck_rmax = p.N;
+    if (p.ext_check) { ck_kumax = __ldcg(p.ext_check); ck_rmin = __ldcg(p.ext_check + 1); ck_rmax = __ldcg(p.ext_check + 2); }
     double acc = 0.0;
-    unsigned int oob = 0;
+    unsigned int oob = 0, viol = 0;
     cx<T>* vis = reinterpret_cast<cx<T>*>(p.vis);
     for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < p.M; k += (long long)gridDim.x * blockDim.x) {
         const double u = (double)__ldcs(p.u + k), v = (double)__ldcs(p.v + k);
         double vr = 0.0, vi = 0.0;
         if (ps.init_from_vis) { const cx<T> old = vis[k]; vr = (double)old.x; vi = (double)old.y; }
-        if (single) multi_point<T, false>(p, ps, p.spec, u, v, vr, vi, oob);
-        else multi_point<T, true>(p, ps, p.spec, u, v, vr, vi, oob);
+        if (single) multi_point<T, false>(p, ps, p.spec, u, v, vr, vi, oob, ck_kumax, ck_rmin, ck_rmax, viol);
+        else multi_point<T, true>(p, ps, p.spec, u, v, vr, vi, oob, ck_kumax, ck_rmin, ck_rmax, viol);
         if (WRITE_VIS) vis[k] = mk<T>((T)vr, (T)vi);
         if (DO_CHI2) {                                                        // PAPER.md:718 (Eq. 10)
             const double dr = vr - (double)__ldcs(p.re_obs + k), di = vi - (double)__ldcs(p.im_obs + k);
             acc = fma(fma(dr, dr, di * di), (double)__ldcs(p.w + k), acc);
         }
     }
-    sample_finish<T, DO_CHI2>(p, 0, acc, oob, 0u);
+    sample_finish<T, DO_CHI2>(p, 0, acc, oob, viol);
 }
 
 // Extent of a point set under ANY rotation, from its largest baseline length (uv_radius_kernel): the index of a
@@ -873,23 +879,6 @@ static __global__ void sum_channels_kernel(const double* __restrict__ chi2_pc, i
     double t = 0.0;
     for (int i = 0; i < C; ++i) t += chi2_pc[i];
     *chi2_tot = t;
-}
-
-// chi2 of visibilities that are already in memory (multi-source composition: the sum over the sources has to be
-// complete before it is compared with the observations).  Same deterministic reduction as the sampler.
-template <typename T>
-__global__ void __launch_bounds__(256) chi2_from_vis_kernel(const SampleParams<T> p) {
-    pdl_wait();
-    const cx<T>* vis = reinterpret_cast<const cx<T>*>(p.vis);
-    double acc = 0.0;
-    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < p.M; k += (long long)gridDim.x * blockDim.x) {
-        const cx<T> vv = __ldcs(vis + k);
-        const double dr = (double)vv.x - (double)__ldcs(p.re_obs + k), di = (double)vv.y - (double)__ldcs(p.im_obs + k);
-        acc = fma(fma(dr, dr, di * di), (double)__ldcs(p.w + k), acc);
-    }
-    SampleParams<T> q = p;
-    q.ext_check = nullptr;
-    sample_finish<T, true>(q, 0, acc, 0u, 0u);
 }
 
 // max over the points of u^2 + v^2 (bit pattern of a non-negative double orders like an integer): the

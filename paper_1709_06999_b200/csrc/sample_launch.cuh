@@ -131,23 +131,6 @@ int launch_sample(gal_plan* p, int C, const CallScalars& cs, const T* u, const T
 }
 
 template <typename T>
-int launch_chi2_from_vis(gal_plan* p, const T* vis, const T* re, const T* im, const T* w, int64_t M, double* chi2,
-                         cudaStream_t st) {
-    SampleParams<T> sp = {};
-    sp.N = p->nxy; sp.M = M; sp.vis = const_cast<T*>(vis); sp.re_obs = re; sp.im_obs = im; sp.w = w;
-    sp.partials = p->partials; sp.tickets = p->tickets; sp.chi2_per_channel = chi2; sp.chi2_total = nullptr;
-    sp.oob = p->oob; sp.done = (unsigned int*)((char*)p->oob + 20);
-    sp.next_state = (unsigned long long*)((char*)p->call_state + 32 * (p->cur ^ 1));
-    sp.viol = (unsigned long long*)((char*)p->oob + 24); sp.ext_check = nullptr; sp.rearm = 1;
-    long long blocks = (M + 1023) / 1024;
-    if (blocks > p->max_gx) blocks = p->max_gx;
-    GAL_CUDA(p, launch_chain(chi2_from_vis_kernel<T>, dim3((unsigned)blocks), dim3(256), 0, st, sp));
-    p->launches++;
-    GAL_CUDA(p, cudaGetLastError());
-    return GAL_OK;
-}
-
-template <typename T>
 int launch_uv_radius(gal_plan* p, const T* u, const T* v, long long total, cudaStream_t st) {
     long long blocks = (total + 1023) / 1024;
     if (blocks > (long long)p->sm_count * 8) blocks = (long long)p->sm_count * 8;
@@ -208,7 +191,11 @@ int launch_sample_multi(gal_plan* p, const IndexScalars& ix, const PlacementSet&
     sp.partials = p->partials; sp.tickets = p->tickets; sp.chi2_per_channel = chi2; sp.chi2_total = nullptr;
     sp.oob = p->oob; sp.done = (unsigned int*)((char*)p->oob + 20);
     sp.next_state = (unsigned long long*)((char*)p->call_state + 32 * (p->cur ^ 1));
-    sp.viol = (unsigned long long*)((char*)p->oob + 24); sp.ext = p->cur_ext; sp.ext_check = nullptr; sp.viol_flag = p->viol_dev; sp.rearm = last;
+    sp.viol = (unsigned long long*)((char*)p->oob + 24); sp.ext = p->cur_ext; sp.viol_flag = p->viol_dev; sp.rearm = last;
+    // as make_sample_params: a bound uv set pruned below the whole plane is verified point by point (a changed set
+    // raises GAL_ERR_BINDING_VIOLATED on the next call); the last CTA leaves the row-pass hint for the next call
+    sp.ext_check = (p->last_bound && !p->last_obs && p->b_ext[0] < p->nxy / 2) ? p->b_ext_dev : nullptr;
+    sp.ext_hint = p->viol_dev + 1;
     long long blocks = (M + 255) / 256;
     const long long cap = (long long)p->sm_count * 6 < p->max_gx ? (long long)p->sm_count * 6 : p->max_gx;
     if (blocks > cap) blocks = cap;
@@ -268,8 +255,6 @@ int launch_hankel(gal_plan* p, const SweepParams& sw, const CallScalars& cs, con
     template int launch_extent<T>(gal_plan*, int, const CallScalars&, const T*, const T*, int64_t, cudaStream_t);      \
     template int launch_sample<T>(gal_plan*, int, const CallScalars&, const T*, const T*, const T*, const T*, const T*, \
                                   int64_t, T*, double*, double*, bool, cudaStream_t);                                  \
-    template int launch_chi2_from_vis<T>(gal_plan*, const T*, const T*, const T*, const T*, int64_t, double*,          \
-                                         cudaStream_t);                                                                \
     template int launch_bind_sort<T>(gal_plan*, const T*, const T*, const T*, const T*, const T*, int64_t, int, double, T*, \
                                      cudaStream_t);                                                                    \
     template int launch_hankel<T>(gal_plan*, const SweepParams&, const CallScalars&, const T*, const T*, const T*, const T*, \

@@ -489,6 +489,19 @@ def test_bound_uv_set(g):
     bound.unbind_uv()
     c = bound.sampleImage(img, w.dxy, u, v, w.PA, w.dRA, w.dDec)
     assert torch.equal(c, free.sampleImage(img, w.dxy, u, v, w.PA, w.dRA, w.dDec))
+    # the multi-source call verifies a bound set too: same results while the promise holds, reported when it breaks
+    pl = [(w.dRA, w.dDec, w.PA), (-2 * w.dRA, w.dDec, 0.4, 0.3)]
+    u.copy_(dev(w.u))                                        # (back to the original baselines)
+    bound.bind_uv(u, v)
+    m = bound.sampleImageMulti(img, w.dxy, u, v, pl)
+    assert bound.last_extent_violations() == 0 and bound.last_uv_extent()[0] < w.nxy // 2
+    assert torch.equal(m, free.sampleImageMulti(img, w.dxy, u, v, pl))
+    u.mul_(1.4)
+    bound.sampleImageMulti(img, w.dxy, u, v, pl)
+    assert bound.last_extent_violations() > 0
+    with pytest.raises(g.GalarioError, match="bound"):
+        bound.sampleImageMulti(img, w.dxy, u, v, pl)
+    assert torch.equal(bound.sampleImageMulti(img, w.dxy, u, v, pl), free.sampleImageMulti(img, w.dxy, u, v, pl))
 
 
 @pytest.mark.parametrize("idx,kw,dtype", [(2, dict(nxy=1024, M=200_003), torch.float64),
