@@ -281,10 +281,22 @@ int gal_chi2_image_host_f32(gal_plan* plan, const float* image, double dxy, cons
                             double dDec, double PA, double* chi2_out, void* stream);
 int gal_sample_image_host_f64(gal_plan* plan, const double* image, double dxy, const double* u, const double* v,
                               int64_t M, double dRA, double dDec, double PA, double* vis_out, void* stream);
+int gal_sample_image_host_f32(gal_plan* plan, const float* image, double dxy, const float* u, const float* v,
+                              int64_t M, double dRA, double dDec, double PA, float* vis_out, void* stream);
 int gal_chi2_profile_host_f64(gal_plan* plan, const double* I, int nr, double Rmin, double dR, double dxy,
                               const double* u, const double* v, const double* re_obs, const double* im_obs,
                               const double* w, int64_t M, double dRA, double dDec, double PA, double inc,
                               double* chi2_out, void* stream);
+int gal_chi2_profile_host_f32(gal_plan* plan, const float* I, int nr, double Rmin, double dR, double dxy,
+                              const float* u, const float* v, const float* re_obs, const float* im_obs,
+                              const float* w, int64_t M, double dRA, double dDec, double PA, double inc,
+                              double* chi2_out, void* stream);
+int gal_sample_profile_host_f64(gal_plan* plan, const double* I, int nr, double Rmin, double dR, double dxy,
+                                const double* u, const double* v, int64_t M, double dRA, double dDec, double PA,
+                                double inc, double* vis_out, void* stream);
+int gal_sample_profile_host_f32(gal_plan* plan, const float* I, int nr, double Rmin, double dR, double dxy,
+                                const float* u, const float* v, int64_t M, double dRA, double dDec, double PA,
+                                double inc, float* vis_out, void* stream);
 
 /* ---- measurement helper (not part of the method): the FP64 fused-multiply-add rate of `device`, measured with
  *      independent DFMA chains on every SM (a few launches of a few ms each, CUDA-event timed, best of five;

@@ -175,6 +175,26 @@ def chi2ImageBatch(images, dxy, u, v, re_obs, im_obs, w, dRA=0.0, dDec=0.0, PA=0
     return (per, tot.value, oob.value) if return_oob else (per, tot.value)
 
 
+def chi2ImageSets(image, dxy, u, v, re_obs, im_obs, w, dRA=0.0, dDec=0.0, PA=0.0, nthreads: int = 1,
+                  return_oob: bool = False):
+    """K observation sets against ONE model image ("fit simultaneously several observations"; SURVEY.md
+    8(f) row 3): u, v, re_obs, im_obs, w are [K][M]; the result is chi2Image of the image with every set in turn, and
+    their sum in set order.  Written out as exactly that loop.  Returns (chi2[K], total[, out-of-grid points])."""
+    u, v, re_obs, im_obs, w = _f64(u), _f64(v), _f64(re_obs), _f64(im_obs), _f64(w)
+    K = u.shape[0]
+    per = np.empty(K, dtype=np.float64)
+    oob = 0
+    for k in range(K):
+        if return_oob:
+            _, n = sampleImage(image, dxy, u[k], v[k], PA, dRA, dDec, return_oob=True, nthreads=nthreads)
+            oob += n
+        per[k] = chi2Image(image, dxy, u[k], v[k], re_obs[k], im_obs[k], w[k], dRA, dDec, PA, nthreads=nthreads)
+    tot = 0.0
+    for k in range(K):
+        tot += per[k]
+    return (per, tot, oob) if return_oob else (per, tot)
+
+
 def sampleProfileHankel(I, Rmin, dR, u, v, inc=0.0, PA=0.0, dRA=0.0, dDec=0.0, nthreads: int = 1):
     """Direct Hankel-transform evaluation of Eq. 25 on the profile grid; no image, no FFT."""
     I, u, v = _f64(I), _f64(u), _f64(v)

@@ -80,9 +80,12 @@ def load_library() -> ctypes.CDLL:
                                                                     _vp, _vp]
             getattr(lib, f"gal_chi2_image_multi_{s}").argtypes = [_vp, _vp, _d, _vp, _vp, _vp, _vp, _vp, _i64, _i, _vp,
                                                                   _vp, _vp, _vp, _vp, _vp]
-        lib.gal_sample_image_host_f64.argtypes = [_vp, _vp, _d, _vp, _vp, _i64, _d, _d, _d, _vp, _vp]
-        lib.gal_chi2_profile_host_f64.argtypes = [_vp, _vp, _i, _d, _d, _d, _vp, _vp, _vp, _vp, _vp, _i64, _d, _d, _d,
-                                                  _d, _vp, _vp]
+        for s in ("f64", "f32"):
+            getattr(lib, f"gal_sample_image_host_{s}").argtypes = [_vp, _vp, _d, _vp, _vp, _i64, _d, _d, _d, _vp, _vp]
+            getattr(lib, f"gal_chi2_profile_host_{s}").argtypes = [_vp, _vp, _i, _d, _d, _d, _vp, _vp, _vp, _vp, _vp, _i64,
+                                                                   _d, _d, _d, _d, _vp, _vp]
+            getattr(lib, f"gal_sample_profile_host_{s}").argtypes = [_vp, _vp, _i, _d, _d, _d, _vp, _vp, _i64, _d, _d, _d,
+                                                                     _d, _vp, _vp]
         lib.gal_chi2_profile_hankel_noalloc_f64.argtypes = [_i, _vp, _i, _d, _d, _vp, _vp, _vp, _vp, _vp, _i64, _d, _d,
                                                             _d, _d, _vp, _vp]
         lib.gal_noalloc_scratch_bytes.restype = ctypes.c_size_t
@@ -418,11 +421,19 @@ class Plan:
                                            dRA, dDec, PA, ctypes.addressof(out), _stream()), "gal_chi2_image_host", self)
         return out.value
 
+    def _host_n(self, a, what, n=None):
+        """Host array -> address, with its length checked (a short array would be an out-of-bounds host read)."""
+        p = self._host(a, what)
+        size = a.size if isinstance(a, np.ndarray) else a.numel()
+        if n is not None and size != n:
+            raise GalarioError(f"{what} has {size} elements, expected {n}")
+        return p
+
     def sampleImage_host(self, image, dxy, u, v, PA=0.0, dRA=0.0, dDec=0.0) -> np.ndarray:
         M = u.size if isinstance(u, np.ndarray) else u.numel()
-        out = np.empty(M, dtype=np.complex128)
-        _check(self._lib.gal_sample_image_host_f64(self._h, self._host(image, "image"), dxy, self._host(u, "u"),
-                                                   self._host(v, "v"), M, dRA, dDec, PA, out.ctypes.data, _stream()),
+        out = np.empty(M, dtype=np.complex128 if self.dtype == torch.float64 else np.complex64)
+        _check(self._fn("sample_image_host")(self._h, self._host_n(image, "image", self.nxy ** 2), dxy, self._host(u, "u"),
+                                             self._host_n(v, "v", M), M, dRA, dDec, PA, out.ctypes.data, _stream()),
                "gal_sample_image_host", self)
         return out
 
@@ -430,11 +441,20 @@ class Plan:
         out = ctypes.c_double(0.0)
         n = I.size if isinstance(I, np.ndarray) else I.numel()
         M = u.size if isinstance(u, np.ndarray) else u.numel()
-        _check(self._lib.gal_chi2_profile_host_f64(self._h, self._host(I, "I"), n, Rmin, dR, dxy, self._host(u, "u"),
-                                                   self._host(v, "v"), self._host(re_obs, "re_obs"),
-                                                   self._host(im_obs, "im_obs"), self._host(w, "w"), M, dRA, dDec, PA,
-                                                   inc, ctypes.addressof(out), _stream()), "gal_chi2_profile_host", self)
+        _check(self._fn("chi2_profile_host")(self._h, self._host(I, "I"), n, Rmin, dR, dxy, self._host(u, "u"),
+                                             self._host_n(v, "v", M), self._host_n(re_obs, "re_obs", M),
+                                             self._host_n(im_obs, "im_obs", M), self._host_n(w, "w", M), M, dRA, dDec, PA,
+                                             inc, ctypes.addressof(out), _stream()), "gal_chi2_profile_host", self)
         return out.value
+
+    def sampleProfile_host(self, I, Rmin, dR, dxy, u, v, inc=0.0, PA=0.0, dRA=0.0, dDec=0.0) -> np.ndarray:
+        n = I.size if isinstance(I, np.ndarray) else I.numel()
+        M = u.size if isinstance(u, np.ndarray) else u.numel()
+        out = np.empty(M, dtype=np.complex128 if self.dtype == torch.float64 else np.complex64)
+        _check(self._fn("sample_profile_host")(self._h, self._host(I, "I"), n, Rmin, dR, dxy, self._host(u, "u"),
+                                               self._host_n(v, "v", M), M, dRA, dDec, PA, inc, out.ctypes.data, _stream()),
+               "gal_sample_profile_host", self)
+        return out
 
 
 # -- module-level calls in the paper's style, with a plan cache -------------------------------------

@@ -742,24 +742,29 @@ int64_t gal_last_oob_count(gal_plan* p) {
         if (!image || !chi2) return GAL_ERR_INVALID_ARGUMENT;                                                         \
         return do_host_call<T>(p, image, nullptr, 0, 0, 0, 0, dxy, u, v, re, im, w, M, dRA, dDec, PA, nullptr, chi2,  \
                                stream);                                                                               \
+    }                                                                                                                 \
+    int gal_sample_image_host_##SFX(gal_plan* p, const T* image, double dxy, const T* u, const T* v, int64_t M,       \
+                                    double dRA, double dDec, double PA, T* vis, void* stream) {                       \
+        if (!image || !vis) return GAL_ERR_INVALID_ARGUMENT;                                                          \
+        return do_host_call<T>(p, image, nullptr, 0, 0, 0, 0, dxy, u, v, nullptr, nullptr, nullptr, M, dRA, dDec, PA, \
+                               vis, nullptr, stream);                                                                 \
+    }                                                                                                                 \
+    int gal_chi2_profile_host_##SFX(gal_plan* p, const T* I, int nr, double Rmin, double dR, double dxy, const T* u,  \
+                                    const T* v, const T* re, const T* im, const T* w, int64_t M, double dRA,          \
+                                    double dDec, double PA, double inc, double* chi2, void* stream) {                 \
+        if (!I || !chi2 || nr < 2) return GAL_ERR_INVALID_ARGUMENT;                                                   \
+        return do_host_call<T>(p, nullptr, I, nr, Rmin, dR, inc, dxy, u, v, re, im, w, M, dRA, dDec, PA, nullptr,     \
+                               chi2, stream);                                                                         \
+    }                                                                                                                 \
+    int gal_sample_profile_host_##SFX(gal_plan* p, const T* I, int nr, double Rmin, double dR, double dxy,            \
+                                      const T* u, const T* v, int64_t M, double dRA, double dDec, double PA,          \
+                                      double inc, T* vis, void* stream) {                                             \
+        if (!I || !vis || nr < 2) return GAL_ERR_INVALID_ARGUMENT;                                                    \
+        return do_host_call<T>(p, nullptr, I, nr, Rmin, dR, inc, dxy, u, v, nullptr, nullptr, nullptr, M, dRA, dDec,  \
+                               PA, vis, nullptr, stream);                                                             \
     }
 
 GAL_DEFINE_PRECISION(f64, double)
 GAL_DEFINE_PRECISION(f32, float)
-
-int gal_sample_image_host_f64(gal_plan* p, const double* image, double dxy, const double* u, const double* v,
-                              int64_t M, double dRA, double dDec, double PA, double* vis, void* stream) {
-    if (!image || !vis) return GAL_ERR_INVALID_ARGUMENT;
-    return do_host_call<double>(p, image, nullptr, 0, 0, 0, 0, dxy, u, v, nullptr, nullptr, nullptr, M, dRA, dDec, PA,
-                                vis, nullptr, stream);
-}
-
-int gal_chi2_profile_host_f64(gal_plan* p, const double* I, int nr, double Rmin, double dR, double dxy,
-                              const double* u, const double* v, const double* re, const double* im, const double* w,
-                              int64_t M, double dRA, double dDec, double PA, double inc, double* chi2, void* stream) {
-    if (!I || !chi2 || nr < 2) return GAL_ERR_INVALID_ARGUMENT;
-    return do_host_call<double>(p, nullptr, I, nr, Rmin, dR, inc, dxy, u, v, re, im, w, M, dRA, dDec, PA, nullptr,
-                                chi2, stream);
-}
 
 }  // extern "C"

@@ -1036,6 +1036,25 @@ def test_host_pointer_calls_match_device_calls(g, orc):
     r = orc.chi2Profile(w1.profile, w1.Rmin, w1.dR, w1.nxy, w1.dxy, w1.u, w1.v, w1.re_obs, w1.im_obs, w1.w, 0.0, 0.0,
                         w1.PA, w1.inc)
     assert abs(ch - r) <= TOL_CHI2_F64 * abs(r)
+    vp_host = p1.sampleProfile_host(w1.profile, w1.Rmin, w1.dR, w1.dxy, w1.u, w1.v, w1.inc, w1.PA, 1e-7, -2e-7)
+    vp_dev = p1.sampleProfile(dev(w1.profile), w1.Rmin, w1.dR, w1.dxy, dev(w1.u), dev(w1.v), w1.inc, w1.PA, 1e-7, -2e-7)
+    assert np.array_equal(vp_host, vp_dev.cpu().numpy())
+    with pytest.raises(g.GalarioError):
+        p1.sampleProfile_host(w1.profile, w1.Rmin, w1.dR, w1.dxy, w1.u, w1.v[:-1])
+    # the single-precision library offers the same calls
+    wf, w1f = w.as_f32(), w1.as_f32()
+    q, q1 = g.Plan(w.nxy, 1, torch.float32), g.Plan(w1.nxy, 1, torch.float32)
+    vh = q.sampleImage_host(wf.image, w.dxy, wf.u, wf.v, w.PA, w.dRA, w.dDec)
+    vd = q.sampleImage(dev(wf.image), w.dxy, dev(wf.u), dev(wf.v), w.PA, w.dRA, w.dDec).cpu().numpy()
+    assert vh.dtype == np.complex64 and np.array_equal(vh, vd)
+    ch32 = q1.chi2Profile_host(w1f.profile, w1.Rmin, w1.dR, w1.dxy, w1f.u, w1f.v, w1f.re_obs, w1f.im_obs, w1f.w, 0.0, 0.0,
+                               w1.PA, w1.inc)
+    cd32 = float(q1.chi2Profile(dev(w1f.profile), w1.Rmin, w1.dR, w1.dxy, dev(w1f.u), dev(w1f.v), dev(w1f.re_obs),
+                                dev(w1f.im_obs), dev(w1f.w), 0.0, 0.0, w1.PA, w1.inc).cpu()[0])
+    assert ch32 == cd32 and abs(ch32 - r) <= TOL_CHI2_F32 * abs(r)
+    vph = q1.sampleProfile_host(w1f.profile, w1.Rmin, w1.dR, w1.dxy, w1f.u, w1f.v, w1.inc, w1.PA)
+    vpd = q1.sampleProfile(dev(w1f.profile), w1.Rmin, w1.dR, w1.dxy, dev(w1f.u), dev(w1f.v), w1.inc, w1.PA).cpu().numpy()
+    assert np.array_equal(vph, vpd)
 
 
 def test_paper_style_module_calls(g, orc):

@@ -409,6 +409,32 @@ def test_batch_is_a_loop_over_channels(orc):
     assert tot == pytest.approx(per.sum(), rel=1e-15)
 
 
+def test_observation_sets_against_one_image_closed_form(orc):
+    """chi2ImageSets pinned by a closed form, not by itself: a point source of flux F at the phase centre has a
+    constant spectrum, which bilinear interpolation reproduces exactly, so V = F exp(2 pi i (u dRA + v dDec)) at
+    every point and chi2 of set k is a plain numpy sum over THAT set's arrays.  The sets differ in
+    length scale, observations and weights, so a mixed-up set index (u of one set with the weights of another, a
+    total that skips a set) fails."""
+    rng = np.random.default_rng(5)
+    K, n, M, dxy, F = 4, 32, 300, 0.05 * ARCSEC, 2.5
+    img = np.zeros((n, n))
+    img[n // 2, n // 2] = F
+    du = 1.0 / (n * dxy)
+    scale = np.array([0.1, 0.2, 0.3, 0.4])[:, None]
+    u, v = rng.uniform(-n, n, (K, M)) * du * scale, rng.uniform(-n, n, (K, M)) * du * scale
+    ro, io, w = rng.standard_normal((K, M)), rng.standard_normal((K, M)), rng.random((K, M)) * np.arange(1, K + 1)[:, None]
+    dRA, dDec = 0.31 * ARCSEC, -0.17 * ARCSEC
+    per, tot = orc.chi2ImageSets(img, dxy, u, v, ro, io, w, dRA, dDec, 0.0)
+    V = F * np.exp(2j * np.pi * (u * dRA + v * dDec))
+    ref = (w * ((V.real - ro) ** 2 + (V.imag - io) ** 2)).sum(axis=1)
+    assert per.shape == (K,) and np.allclose(per, ref, rtol=1e-11, atol=0)
+    assert tot == pytest.approx(ref.sum(), rel=1e-11)
+    assert len(set(np.round(per, 6))) == K                   # the sets really are different problems
+    # with the out-of-grid count: the sum over the sets
+    per2, tot2, oob = orc.chi2ImageSets(img, dxy, u * 8, v * 8, ro, io, w, dRA, dDec, 0.0, return_oob=True)
+    assert oob == sum(orc.sampleImage(img, dxy, u[k] * 8, v[k] * 8, 0.0, dRA, dDec, return_oob=True)[1] for k in range(K)) > 0
+
+
 # ---------------------------------------------------------------------------------------
 # H1: direct Hankel evaluation of Eq. 25 (PAPER.md:366-368) — oracle.sampleProfileHankel / chi2ProfileHankel
 # ---------------------------------------------------------------------------------------
