@@ -245,7 +245,8 @@ def measure_case(g, torch, dev, peak, name, w, dtype, entry, prune, steps, warmu
     up = lambda a: torch.as_tensor(np.ascontiguousarray(a), device=dev)
     esz = 8 if dtype == torch.float64 else 4
     C = w.image.shape[0] if entry == "chi2ImageBatch" else 1
-    plan = g.Plan(w.nxy, C, dtype, dev.index)
+    K = int(entry[len("chi2ImageSets"):]) if entry.startswith("chi2ImageSets") else 0     # observation sets of one image
+    plan = g.Plan(w.nxy, max(C, K), dtype, dev.index)
     plan.set_pruning(prune)
     u, v = up(w.u), up(w.v)
     if entry == "sampleImage":
@@ -268,6 +269,12 @@ def measure_case(g, torch, dev, peak, name, w, dtype, entry, prune, steps, warmu
             out = torch.empty(1, dtype=torch.float64, device=dev)
             pl = [(w.dRA * (1 + 0.1 * s), w.dDec * (1 - 0.1 * s), w.PA + 0.05 * s, 1.0 / S) for s in range(S)]
             fn = lambda: plan.chi2ImageMulti(image, w.dxy, u, v, re, im, wt, pl, out=out)
+        elif K:                                         # K observation sets against one image: one transform, K samplings
+            image = up(w.image)
+            stack = lambda a, sc=None: torch.stack([torch.roll(a, 1009 * k) * ((1.0 - 0.1 * k) if sc else 1.0) for k in range(K)]).contiguous()
+            us, vs, res, ims, wts = stack(u, True), stack(v, True), stack(re), stack(im), stack(wt)
+            out = torch.empty(K + 1, dtype=torch.float64, device=dev)
+            fn = lambda: plan.chi2ImageSets(image, w.dxy, us, vs, res, ims, wts, w.dRA, w.dDec, w.PA, out=out)
         elif entry == "chi2ImageBatch":
             image = up(w.image)
             out = torch.empty(C + 1, dtype=torch.float64, device=dev)
@@ -286,6 +293,11 @@ def measure_case(g, torch, dev, peak, name, w, dtype, entry, prune, steps, warmu
     whole = (w.nxy // 2, 0, w.nxy - 1)
     B = algorithmic_bytes(w.nxy, w.M, esz, entry, None, C)
     Bp = algorithmic_bytes(w.nxy, w.M, esz, entry, extent, C) if extent != whole else B
+    if K:                                               # the per-point arrays of the K - 1 further sets
+        B, Bp = dict(B), dict(Bp)
+        for d in (B, Bp):
+            d["step"] += (K - 1) * d["sample"]
+            d["sample"] *= K
     if kms.get("row_pass", 0) <= 0 < kms.get("col_pass", 0):       # nxy = 256 / 1024: both passes in one fused launch
         kms = {"uv_extent": kms["uv_extent"], "fft_fused": kms["col_pass"], "sample": kms["sample"]}
         B, Bp = dict(B), dict(Bp)
@@ -364,6 +376,7 @@ def measure_other(g, torch, dev, peak, w3, args, only=None):
     add("cfg1 f64 chi2Profile", "1", f64, "chi2Profile", 1)
     add("cfg1 f64 chi2Profile by the direct Hankel transform (Eq. 25)", "1", f64, "chi2ProfileHankel", 1)
     add("cfg2 f64 chi2ImageMulti, 4 placements in one sampling launch", "2", f64, "chi2ImageMulti4", 1)
+    add("cfg2 f64 chi2ImageSets, 4 observation sets against one image in one call", "2", f64, "chi2ImageSets4", 1)
     add("cfg0 f64 chi2Image", "0", f64, "chi2Image", 1)
     add("cfg4 f64 chi2ImageBatch (128 channels)", "4", f64, "chi2ImageBatch", 1)
     add("cfg4 f64 chi2ImageBatch (128 channels), bound observations", "4", f64, "chi2ImageBatch", 1, bind=True)

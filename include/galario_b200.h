@@ -249,6 +249,22 @@ int gal_chi2_image_batch_f32(gal_plan* plan, const float* images, int C, double 
                              int64_t M, double dRA, double dDec, double PA, double* chi2_per_channel,
                              double* chi2_total, void* stream);
 
+/* ---- K observation sets against ONE model image in one call ("fit simultaneously several observations";
+ *      PAPER.md:212, second alternative): chi2_per_set[k] = chi2Image(image; set k), for
+ *      K <= plan batch sets of M points each sharing (dxy, dRA, dDec, PA).  ONE transform of the image — pruned, when
+ *      pruning is on, to the union of the sets' uv extents — then one sampling launch whose grid.y runs over the sets,
+ *      all reading the one spectrum: K sets cost one FFT + K samplings, not K calls.  image [nxy][nxy]; u, v, re_obs,
+ *      im_obs, w each [K][M] (device); chi2_per_set[K] and chi2_total[1] (device, double; chi2_total may be NULL; it
+ *      is the sum in set order).  K is limited by the plan's batch because the reduction scratch is sized by it (the
+ *      plan's spectrum workspace for batch > 1 is not used by this call).  Sets of different lengths: pad the
+ *      shorter ones with points of weight 0 at u = v = 0.  gal_last_oob_count() is summed over the sets. ---- */
+int gal_chi2_image_sets_f64(gal_plan* plan, const double* image, int K, double dxy, const double* u, const double* v,
+                            const double* re_obs, const double* im_obs, const double* w, int64_t M, double dRA,
+                            double dDec, double PA, double* chi2_per_set, double* chi2_total, void* stream);
+int gal_chi2_image_sets_f32(gal_plan* plan, const float* image, int K, double dxy, const float* u, const float* v,
+                            const float* re_obs, const float* im_obs, const float* w, int64_t M, double dRA,
+                            double dDec, double PA, double* chi2_per_set, double* chi2_total, void* stream);
+
 /* ---- multi-source composition ("summing up the visibilities of each single source ... applying a
  *      different complex phase"): one model image placed S times,
  *        V(u, v) = sum_s scale[s] * sampleImage(image; dRA[s], dDec[s], PA[s])(u, v),

@@ -71,6 +71,9 @@ def load_library() -> ctypes.CDLL:
             getattr(lib, f"gal_chi2_image_batch_{s}").argtypes = [_vp, _vp, _i, _d, _vp, _vp, _vp, _vp, _vp, _i64, _d,
                                                                   _d, _d, _vp, _vp, _vp]
         for s in ("f64", "f32"):
+            getattr(lib, f"gal_chi2_image_sets_{s}").argtypes = [_vp, _vp, _i, _d, _vp, _vp, _vp, _vp, _vp, _i64, _d, _d,
+                                                                 _d, _vp, _vp, _vp]
+        for s in ("f64", "f32"):
             getattr(lib, f"gal_sample_profile_hankel_{s}").argtypes = [_vp, _vp, _i, _d, _d, _vp, _vp, _i64, _d, _d, _d, _d,
                                                                        _vp, _vp]
             getattr(lib, f"gal_chi2_profile_hankel_{s}").argtypes = [_vp, _vp, _i, _d, _d, _vp, _vp, _vp, _vp, _vp, _i64,
@@ -404,6 +407,20 @@ class Plan:
                                             self._dev(w, "w", n), M, dRA, dDec, PA, out.data_ptr(),
                                             out.data_ptr() + 8 * C, _stream()), "gal_chi2_image_batch", self)
         return out[:C], out[C:]
+
+    def chi2ImageSets(self, image, dxy, u, v, re_obs, im_obs, w, dRA=0.0, dDec=0.0, PA=0.0, out=None):
+        """K observation sets ([K][M] tensors, K <= the plan's batch) against ONE image: one transform, one sampling
+        launch over the sets (gal_chi2_image_sets).  Returns (chi2_per_set[K], chi2_total[1])."""
+        if u.dim() != 2:
+            raise GalarioError("u, v, re_obs, im_obs, w must be [K][M]")
+        K, M = u.shape
+        n = K * M
+        out = self._out(out, K + 1, torch.float64, u)
+        _check(self._fn("chi2_image_sets")(self._h, self._dev(image, "image", self.nxy ** 2), K, dxy, self._dev(u, "u"),
+                                           self._dev(v, "v", n), self._dev(re_obs, "re_obs", n),
+                                           self._dev(im_obs, "im_obs", n), self._dev(w, "w", n), M, dRA, dDec, PA,
+                                           out.data_ptr(), out.data_ptr() + 8 * K, _stream()), "gal_chi2_image_sets", self)
+        return out[:K], out[K:]
 
     # -- host-pointer calls (numpy / CPU tensors in, Python float or numpy out) ------------------
     def _host(self, a, what):

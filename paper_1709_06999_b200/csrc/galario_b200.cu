@@ -62,7 +62,8 @@ int reset_call_state(gal_plan* p, cudaStream_t st) {
 // Should this call compute the uv extent and prune the transform?  The extent pass re-reads u and v
 // (2 sizeof(T) M bytes per channel); pruning can save up to three passes over the spectrum.
 template <typename T>
-bool want_prune(const gal_plan* p, int C, int64_t M) {
+bool want_prune(const gal_plan* p, int C, int64_t M, int n_spec = 0) {
+    if (n_spec <= 0) n_spec = C;                 // spectra transformed by the call (1 for K observation sets of one image)
     if (p->prune_mode == 0 || M <= 0) return false;
     if (p->prune_mode == 2) return true;
     const double ext_bytes = 2.0 * sizeof(T) * (double)M * C;
@@ -70,7 +71,7 @@ bool want_prune(const gal_plan* p, int C, int64_t M) {
     // a spectrum of a few MB is transformed in a few microseconds out of the L2: the extra launch cannot pay
     // (cfg 0 / 1 / 4: the uv-extent kernel was 15-20 % of the call and mostly found "whole plane")
     if (spec_one < 16e6) return false;
-    return ext_bytes <= 0.25 * 3.0 * spec_one * C;
+    return ext_bytes <= 0.25 * 3.0 * spec_one * n_spec;
 }
 
 // Bound uv set: the extent follows from the radius computed once at bind time, for any PA.  The index of a rotated
@@ -114,7 +115,7 @@ int run_call(gal_plan* p, const T* image, const SweepParams* sw, int C, double d
     if ((rc = reset_call_state(p, st))) return rc;
     if (p->tmark(0, st)) return GAL_ERR_CUDA;
     const int* ext = p->ext_full;
-    p->last_pruned = want_prune<T>(p, C, M) && !cs.ix.du_exact_div;   // the extent kernel only has the division shortcut
+    p->last_pruned = want_prune<T>(p, C, M, p->shared_spec ? 1 : C) && !cs.ix.du_exact_div;   // the extent kernel only has the division shortcut
     p->last_bound = false;
     p->last_obs = false;
     const bool uv_bound = M > 0 && p->b_u == (const void*)u && p->b_v == (const void*)v && p->b_M == M && p->b_C == C;
@@ -154,13 +155,13 @@ int run_call(gal_plan* p, const T* image, const SweepParams* sw, int C, double d
     p->row_small = p->last_bound ? p->b_ext[0] < p->nxy / 2
                                  : ((p->last_pruned || speculate) && ((volatile unsigned int*)p->viol_host)[1] == 2u);
     if (M == 0) return launch_sample<T>(p, C, cs, u, v, re, im, w, M, vis, chi2_pc, chi2_tot, true, st);
-    const int G = batch_chunk(p, C);
+    const int G = p->shared_spec ? C : batch_chunk(p, C);      // (one image, one transform: nothing to chunk)
     const size_t n2 = (size_t)p->nxy * p->nxy;
     for (int c0 = 0; c0 < C; c0 += G) {
         const int g = C - c0 < G ? C - c0 : G;
         const bool last = c0 + g >= C;
         const size_t o = (size_t)c0 * M;
-        if ((rc = fft2<T>(p, image ? image + c0 * n2 : nullptr, sw, g, ext, st))) return rc;
+        if ((rc = fft2<T>(p, image ? image + (p->shared_spec ? 0 : c0 * n2) : nullptr, sw, p->shared_spec ? 1 : g, ext, st))) return rc;
         if (p->tmark(3, st)) return GAL_ERR_CUDA;
         if ((rc = launch_sample<T>(p, g, cs, u + o, v + o, re ? re + o : nullptr, im ? im + o : nullptr, w ? w + o : nullptr, M,
                                    vis ? vis + 2 * o : nullptr, chi2_pc ? chi2_pc + c0 : nullptr, G >= C ? chi2_tot : nullptr, last, st)))
@@ -721,6 +722,16 @@ int64_t gal_last_oob_count(gal_plan* p) {
         if (!p || !images || !chi2_pc || C < 1) return GAL_ERR_INVALID_ARGUMENT;                                      \
         return do_sample_image<T>(p, images, nullptr, C, dxy, u, v, re, im, w, M, dRA, dDec, PA, nullptr, chi2_pc,    \
                                   chi2_tot, stream);                                                                  \
+    }                                                                                                                 \
+    int gal_chi2_image_sets_##SFX(gal_plan* p, const T* image, int K, double dxy, const T* u, const T* v,             \
+                                  const T* re, const T* im, const T* w, int64_t M, double dRA, double dDec,           \
+                                  double PA, double* chi2_ps, double* chi2_tot, void* stream) {                       \
+        if (!p || !image || !chi2_ps || K < 1) return GAL_ERR_INVALID_ARGUMENT;                                       \
+        p->shared_spec = true;                                                                                        \
+        const int rc = do_sample_image<T>(p, image, nullptr, K, dxy, u, v, re, im, w, M, dRA, dDec, PA, nullptr,      \
+                                          chi2_ps, chi2_tot, stream);                                                 \
+        p->shared_spec = false;                                                                                       \
+        return rc;                                                                                                    \
     }                                                                                                                 \
     int gal_sample_image_multi_##SFX(gal_plan* p, const T* image, double dxy, const T* u, const T* v, int64_t M,      \
                                      int S, const double* dRA, const double* dDec, const double* PA,                  \

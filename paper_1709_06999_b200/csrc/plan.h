@@ -77,6 +77,7 @@ struct gal_plan {
     bool spec_off = false;               // GAL_OPT_SPECULATE = 0
     double spec_min_bytes = 32e6;        // speculate only where the uv-extent pass would read at least this much (cfg 2, 16 MB: 42.0 against 44.5 us)
     bool last_spec = false;              // the most recent call speculated
+    bool shared_spec = false;            // the call being issued samples ONE spectrum with every channel (gal_chi2_image_sets)
     int* spec_E(int par) const { return (int*)((char*)spec_state + 8 + 16 * par); }
     unsigned int* spec_redo() const { return (unsigned int*)((char*)spec_state + 40); }
     int* spec_used() const { return (int*)((char*)spec_state + 44); }

@@ -47,6 +47,7 @@ template <typename T> struct SampleParams {
     const int* ext_check;     // extent of a bound uv set to verify every point against, or null
     unsigned long long* viol; // [1]: points whose cell lies outside ext_check
     int direct;               // 1: every thread gathers its own cell (uv-sorted points of a bound observation set)
+    int shared_spec;          // 1: every channel (blockIdx.y) samples the ONE spectrum at spec (K observation sets against one image)
     int rearm;                // 1: the last CTA of this launch re-arms next_state (every launch but the non-final chunks of a long multi-source list)
     unsigned int* viol_flag;  // mapped host memory: set when viol becomes non-zero (sticky, read by the next call)
     unsigned int* ext_hint;   // mapped host memory or null: 1 = this call's extent was the whole plane, 2 = pruned (plan.h)
@@ -668,7 +669,7 @@ __device__ __forceinline__ SampleCtx<T> sample_ctx(const SampleParams<T>& p, int
     SampleCtx<T> cx_;
     cx_.N = p.N;
     // channel c of the batch: [N/2+1][N] entries, column pairs or (whole-plane extent) single values
-    const long long plane = (long long)c * (p.N / 2 + 1) * p.N;
+    const long long plane = p.shared_spec ? 0ll : (long long)c * (p.N / 2 + 1) * p.N;
     cx_.spec = layout_single(p.ext, p.N) ? reinterpret_cast<const NodePair<T>*>(reinterpret_cast<const cx<T>*>(p.spec) + plane)
                                            : p.spec + plane;
     cx_.odd = threadIdx.x & 1;

@@ -64,6 +64,7 @@ SampleParams<T> make_sample_params(gal_plan* p, const CallScalars& cs, const T* 
     sp.ext = p->cur_ext;
     sp.rearm = last;
     sp.direct = p->last_obs ? 1 : 0;
+    sp.shared_spec = p->shared_spec ? 1 : 0;
     sp.ext_check = (p->last_bound && !p->last_obs && p->b_ext[0] < p->nxy / 2) ? p->b_ext_dev : nullptr;
     sp.viol_flag = p->viol_dev;
     sp.ext_hint = p->viol_dev + 1;

@@ -1102,3 +1102,47 @@ def test_binding_rejects_short_arrays_and_wrong_outputs(g):
         plan.set_option("no_such_option", 1)
     with pytest.raises(g.GalarioError):
         plan.set_option("row_mode", 9)
+
+
+# ---------------------------------------------------------------------------------------------
+# K observation sets against one model image in one call (second alternative)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype,M", [(torch.float64, 40_004), (torch.float64, 40_003), (torch.float32, 40_004)])
+def test_observation_sets_against_one_image(g, orc, dtype, M):
+    """gal_chi2_image_sets: ONE transform, grid.y over the sets.  Every set's chi2, the total, the out-of-grid count
+    against the oracle's loop over chi2Image; sets of different reach (one of them beyond the grid), data and weights;
+    16-byte aligned rows (TMA path, M = 40 004) and ragged ones (plain loads); pruned to the union of the extents."""
+    f32 = dtype == torch.float32
+    w = W.config(3, nxy=1024, M=M, n_src=40)
+    if f32:
+        w = w.as_f32()
+    tol = TOL_CHI2_F32 if f32 else TOL_CHI2_F64
+    f = lambda a: np.asarray(a, dtype=np.float64)
+    K = 4
+    for scales, mode in (((0.9, 0.7, 0.5, 0.3), 2), ((1.0, 0.5, 3.0, 0.7), 1), ((0.9, 0.7, 0.5, 0.3), 0)):
+        st = lambda a, sc=False: np.ascontiguousarray(np.stack(
+            [np.roll(a, 997 * k) * (a.dtype.type(scales[k]) if sc else a.dtype.type(1)) for k in range(K)]))
+        u, v, ro, io, wt = st(w.u, True), st(w.v, True), st(w.re_obs), st(w.im_obs), st(w.w)
+        wt = np.ascontiguousarray(wt * np.arange(1, K + 1, dtype=wt.dtype)[:, None])
+        plan = g.Plan(w.nxy, K, dtype)
+        plan.set_pruning(mode)
+        n0 = plan.launch_count()
+        per, tot = plan.chi2ImageSets(dev(w.image), w.dxy, dev(u), dev(v), dev(ro), dev(io), dev(wt), w.dRA, w.dDec, w.PA)
+        per, tot = per.cpu().numpy(), float(tot.cpu()[0])
+        assert plan.launch_count() - n0 <= 4                  # [extent,] one transform (1-2 kernels), ONE sampling launch
+        rper, rtot, roob = orc.chi2ImageSets(f(w.image), w.dxy, f(u), f(v), f(ro), f(io), f(wt), w.dRA, w.dDec, w.PA,
+                                             nthreads=threads(orc), return_oob=True)
+        assert (np.abs(per - rper) <= tol * np.abs(rper)).all(), (scales, mode)
+        assert abs(tot - rtot) <= tol * abs(rtot)
+        assert plan.last_oob_count() == roob and (roob > 0) == (max(scales) > 0.95)   # (longest baseline: 548 of 512 cells)
+        ext = plan.last_uv_extent()
+        if mode == 2:
+            assert ext[0] < w.nxy // 2                        # pruned to the union of the sets' extents
+        # each set alone through the single-set call: the same numbers to rounding (other partial-sum grouping)
+        one = g.Plan(w.nxy, 1, dtype)
+        for k in (0, K - 1):
+            c = float(one.chi2Image(dev(w.image), w.dxy, dev(u[k]), dev(v[k]), dev(ro[k]), dev(io[k]), dev(wt[k]),
+                                    w.dRA, w.dDec, w.PA).cpu()[0])
+            assert abs(c - per[k]) <= (1e-5 if f32 else 1e-12) * abs(c)
+    with pytest.raises(g.GalarioError):
+        g.Plan(w.nxy, 2, dtype).chi2ImageSets(dev(w.image), w.dxy, dev(u), dev(v), dev(ro), dev(io), dev(wt))   # K > plan batch
