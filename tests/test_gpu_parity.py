@@ -1146,3 +1146,51 @@ def test_observation_sets_against_one_image(g, orc, dtype, M):
             assert abs(c - per[k]) <= (1e-5 if f32 else 1e-12) * abs(c)
     with pytest.raises(g.GalarioError):
         g.Plan(w.nxy, 2, dtype).chi2ImageSets(dev(w.image), w.dxy, dev(u), dev(v), dev(ro), dev(io), dev(wt))   # K > plan batch
+
+
+def test_two_hundred_mixed_calls_on_one_plan_against_the_oracle(g, orc):
+    """Stand-in for the sanitizer pass this pool does not allow: 200 calls on ONE plan in a
+    seeded random order — chi2Image and sampleImage, six uv sets of two lengths (ragged and 16-byte aligned) and four
+    reaches (so the speculative extent shrinks, grows, fails and repeats itself on the device, and wraps to the whole
+    plane), bound observation sets coming and going — issued in bursts of 20 without host synchronisation, every
+    result compared with the oracle's for that uv set.  State leaking from one call into the next (tickets, the
+    alternating call state, extents, the second pass's counters) would show as a wrong number."""
+    w = W.config(3, nxy=2048, M=120_000, n_src=40)
+    f = lambda a: np.asarray(a, dtype=np.float64)
+    image = dev(w.image)
+    variants = []
+    for M, scale in ((120_000, 1.0), (50_001, 0.5), (120_000, 1.8), (50_001, 2.5), (120_000, 0.3), (50_001, 1.0)):
+        u, v = w.u[:M] * scale, w.v[:M] * scale
+        ro, io, wt = w.re_obs[:M], w.im_obs[:M], w.w[:M]
+        vis, oob = orc.sampleImage(f(w.image), w.dxy, u, v, w.PA, w.dRA, w.dDec, return_oob=True, nthreads=threads(orc))
+        variants.append(dict(d=[dev(a) for a in (u, v, ro, io, wt)], vis=vis, chi2=orc.chi2(vis, ro, io, wt), oob=oob))
+    assert any(x["oob"] > 0 for x in variants) and any(x["oob"] == 0 for x in variants)
+    plan = g.Plan(w.nxy)
+    plan.set_option("spec_min_bytes", 0)
+    rng = np.random.default_rng(2024)
+    n_calls, n_bound = 0, 0
+    for burst in range(10):
+        issued = []
+        bind_k = int(rng.integers(len(variants))) if burst % 3 == 2 else None
+        if bind_k is not None:
+            plan.bind_obs(*variants[bind_k]["d"])
+        for _ in range(20):
+            k = int(rng.integers(len(variants)))
+            x = variants[k]
+            if rng.random() < 0.3:
+                issued.append((k, "vis", plan.sampleImage(image, w.dxy, x["d"][0], x["d"][1], w.PA, w.dRA, w.dDec)))
+            else:
+                issued.append((k, "chi2", plan.chi2Image(image, w.dxy, *x["d"], w.dRA, w.dDec, w.PA)))
+                n_bound += bind_k == k
+            n_calls += 1
+        torch.cuda.synchronize()
+        assert plan.last_oob_count() == variants[issued[-1][0]]["oob"]
+        for k, what, out in issued:
+            x = variants[k]
+            if what == "vis":
+                assert rel_err(out.cpu().numpy(), x["vis"]) <= TOL_VIS_F64, (burst, k)
+            else:
+                assert abs(float(out.cpu()[0]) - x["chi2"]) <= TOL_CHI2_F64 * abs(x["chi2"]), (burst, k)
+        if bind_k is not None:
+            plan.unbind_obs()
+    assert n_calls == 200 and n_bound > 0
